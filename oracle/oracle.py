@@ -1,0 +1,270 @@
+"""ctypes wrapper of the CPU ORACLE (oracle/gateau_oracle.cpp).
+
+TEST INFRASTRUCTURE, NOT THE PRODUCT: imported only by tests/, __graft_entry__.smoke()
+and bench.py's cpu_baseline / --impl reference legs.  Nothing here touches the CUDA
+path; it marshals a `Workload` (the shared seeded inputs) into the oracle's own struct.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from pathlib import Path
+
+import numpy as np
+
+_HERE = Path(__file__).resolve().parent
+_SRC = _HERE / "gateau_oracle.cpp"
+_LIB = _HERE / "libgateau_oracle.so"
+
+CXXFLAGS = ["-O2", "-std=c++17", "-fopenmp", "-ffp-contract=off", "-fno-fast-math",
+            "-Wall", "-Wextra", "-shared", "-fPIC"]
+
+
+def build(force: bool = False) -> Path:
+    """Compile the oracle with g++ (building the checker is not using it)."""
+    hdr = _HERE / "gateau_oracle.h"
+    stale = (not _LIB.exists() or _LIB.stat().st_mtime < _SRC.stat().st_mtime
+             or _LIB.stat().st_mtime < hdr.stat().st_mtime)
+    if force or stale:
+        tmp = _LIB.with_suffix(f".so.tmp{os.getpid()}")
+        subprocess.check_call(["g++", *CXXFLAGS, str(_SRC), "-o", str(tmp)])
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+class GoStage(C.Structure):
+    _fields_ = [("eta_nu", C.c_void_p), ("eta_scalar", C.c_double), ("T_K", C.c_double),
+                ("couple_atmosphere", C.c_int32)]
+
+
+class GoConfig(C.Structure):
+    _fields_ = [
+        ("n_freq", C.c_int32), ("nu0_hz", C.c_double), ("dnu_hz", C.c_double),
+        ("n_samples", C.c_int64), ("f_sample_hz", C.c_double),
+        ("az_rad", C.c_void_p), ("el_rad", C.c_void_p), ("el0_rad", C.c_double),
+        ("n_spaxel", C.c_int32), ("daz_rad", C.c_void_p), ("del_rad", C.c_void_p),
+        ("cube", C.c_void_p), ("n_az", C.c_int32), ("n_el", C.c_int32),
+        ("az_min_rad", C.c_double), ("daz_grid_rad", C.c_double),
+        ("el_min_rad", C.c_double), ("del_grid_rad", C.c_double),
+        ("eta_front_nu", C.c_void_p), ("T_cmb_K", C.c_double),
+        ("screen", C.c_void_p), ("nx", C.c_int32), ("ny", C.c_int32),
+        ("dx_m", C.c_double), ("dy_m", C.c_double), ("h_column_m", C.c_double),
+        ("wind_mps", C.c_double), ("pwv0_a_mm", C.c_double), ("pwv0_b_mm_per_s", C.c_double),
+        ("atm_lut", C.c_void_p), ("n_pwv", C.c_int32), ("n_nu_lut", C.c_int32),
+        ("lut_nu0_hz", C.c_double), ("lut_dnu_hz", C.c_double), ("lut_pwv0_mm", C.c_double),
+        ("lut_dpwv_mm", C.c_double), ("T_atm_K", C.c_double),
+        ("n_stage", C.c_int32), ("stages", C.c_void_p),
+        ("n_chan", C.c_int32), ("filt", C.c_void_p),
+        ("f_center_hz", C.c_void_p), ("dnu_eff_hz", C.c_void_p),
+        ("seed", C.c_uint64), ("photon_noise", C.c_int32), ("pink_noise", C.c_int32),
+        ("pink_A", C.c_void_p), ("pink_alpha", C.c_void_p),
+        ("pink_n_stage", C.c_int32), ("pink_f_corner_hz", C.c_void_p),
+    ]
+
+
+GEOREC_DTYPE = np.dtype([
+    ("n", "<i8"), ("iu0", "<i4"), ("iv0", "<i4"), ("ju", "<i4"), ("jv", "<i4"), ("ip", "<i4"),
+    ("pad_", "<i4"), ("fu", "<f8"), ("fv", "<f8"), ("gu", "<f8"), ("gv", "<f8"), ("fp", "<f8"),
+    ("pwv_mm", "<f8"), ("csc", "<f8")])
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    global _lib
+    if _lib is None:
+        build()
+        L = C.CDLL(str(_LIB))
+        L.go_planck.restype = C.c_double
+        L.go_planck.argtypes = [C.c_double, C.c_double]
+        L.go_uniform.restype = C.c_double
+        L.go_uniform.argtypes = [C.c_uint32]
+        L.go_photon_sigma.restype = C.c_double
+        L.go_photon_sigma.argtypes = [C.c_double] * 4
+        L.go_philox4x32_10.restype = None
+        L.go_normals4.restype = None
+        L.go_normals4.argtypes = [C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint32, C.c_void_p]
+        for name in ("go_geometry", "go_row_spectrum", "go_simulate", "go_simulate_rows",
+                     "go_pink_series", "go_num_threads"):
+            getattr(L, name).restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _f32(a):
+    return np.ascontiguousarray(a, dtype=np.float32)
+
+
+class Oracle:
+    """The oracle bound to one Workload.  Keeps the marshalled arrays alive."""
+
+    def __init__(self, w):
+        self.w = w
+        self.L = lib()
+        k = self._keep = {}
+        c = self.cfg = GoConfig()
+
+        def ptr(name, arr):
+            k[name] = arr
+            return arr.ctypes.data
+
+        c.n_freq, c.nu0_hz, c.dnu_hz = w.n_freq, w.nu0_hz, w.dnu_hz
+        c.n_samples, c.f_sample_hz = w.n_samples, w.f_sample_hz
+        c.az_rad, c.el_rad, c.el0_rad = ptr("az", _f64(w.az_rad)), ptr("el", _f64(w.el_rad)), w.el0_rad
+        c.n_spaxel = w.n_spaxel
+        c.daz_rad, c.del_rad = ptr("daz", _f64(w.daz_rad)), ptr("del", _f64(w.del_rad))
+        if w.cube is not None:
+            cube = _f32(w.cube)
+            c.cube, c.n_el, c.n_az = ptr("cube", cube), cube.shape[0], cube.shape[1]
+            assert cube.shape[2] == w.n_freq
+        else:
+            c.cube, c.n_el, c.n_az = None, 0, 0
+        c.az_min_rad, c.daz_grid_rad = w.az_min_rad, w.daz_grid_rad
+        c.el_min_rad, c.del_grid_rad = w.el_min_rad, w.del_grid_rad
+        c.eta_front_nu = ptr("front", _f32(w.eta_front_nu)) if w.eta_front_nu is not None else None
+        c.T_cmb_K = w.T_cmb_K
+        scr = _f32(w.screen)
+        c.screen, c.ny, c.nx = ptr("screen", scr), scr.shape[0], scr.shape[1]
+        c.dx_m, c.dy_m, c.h_column_m, c.wind_mps = w.dx_m, w.dy_m, w.h_column_m, w.wind_mps
+        c.pwv0_a_mm, c.pwv0_b_mm_per_s = w.pwv0_a_mm, w.pwv0_b_mm_per_s
+        lut = _f32(w.atm_lut)
+        c.atm_lut, c.n_pwv, c.n_nu_lut = ptr("lut", lut), lut.shape[0], lut.shape[1]
+        c.lut_nu0_hz, c.lut_dnu_hz = w.lut_nu0_hz, w.lut_dnu_hz
+        c.lut_pwv0_mm, c.lut_dpwv_mm, c.T_atm_K = w.lut_pwv0_mm, w.lut_dpwv_mm, w.T_atm_K
+        st = (GoStage * max(len(w.stages), 1))()
+        for i, s in enumerate(w.stages):
+            if np.ndim(s.eta) == 0:
+                st[i].eta_nu, st[i].eta_scalar = None, float(s.eta)
+            else:
+                st[i].eta_nu, st[i].eta_scalar = ptr(f"stage{i}", _f32(s.eta)), 0.0
+            st[i].T_K, st[i].couple_atmosphere = float(s.T_K), int(bool(s.couple_atmosphere))
+        k["stages"] = st
+        c.n_stage, c.stages = len(w.stages), C.cast(st, C.c_void_p)
+        filt = _f32(w.filt)
+        assert filt.shape == (w.n_chan, w.n_freq)
+        c.n_chan, c.filt = filt.shape[0], ptr("filt", filt)
+        c.f_center_hz = ptr("fc", _f64(w.f_center_hz))
+        c.dnu_eff_hz = ptr("dnueff", _f64(w.dnu_eff_hz)) if w.dnu_eff_hz is not None else None
+        c.seed, c.photon_noise, c.pink_noise = int(w.seed), int(w.photon_noise), int(w.pink_noise)
+        if w.pink_noise:
+            c.pink_A, c.pink_alpha = ptr("pA", _f64(w.pink_A)), ptr("palpha", _f64(w.pink_alpha))
+            fcn = _f64(w.pink_f_corner_hz)
+            c.pink_n_stage, c.pink_f_corner_hz = fcn.size, ptr("pfc", fcn)
+        else:
+            c.pink_A = c.pink_alpha = c.pink_f_corner_hz = None
+            c.pink_n_stage = 0
+
+    def _chk(self, rc, what):
+        if rc != 0:
+            raise RuntimeError(f"oracle {what} failed with code {rc}")
+
+    # ---- the path ----
+    def geometry(self, t_begin=0, t_count=None):
+        t_count = self.w.n_samples - t_begin if t_count is None else t_count
+        out = np.zeros(t_count * self.w.n_spaxel, dtype=GEOREC_DTYPE)
+        self._chk(self.L.go_geometry(C.byref(self.cfg), C.c_int64(t_begin), C.c_int64(t_count),
+                                     C.c_void_p(out.ctypes.data)), "geometry")
+        return out.reshape(t_count, self.w.n_spaxel)
+
+    def row_spectrum(self, n, spaxel, intermediates=False):
+        P = np.zeros(self.w.n_freq)
+        eta = np.zeros(self.w.n_freq)
+        S = np.zeros(self.w.n_freq)
+        self._chk(self.L.go_row_spectrum(C.byref(self.cfg), C.c_int64(n), C.c_int32(spaxel),
+                                         C.c_void_p(P.ctypes.data), C.c_void_p(eta.ctypes.data),
+                                         C.c_void_p(S.ctypes.data)), "row_spectrum")
+        return (P, eta, S) if intermediates else P
+
+    def simulate(self, t_begin=0, t_count=None, want=("tod",)):
+        """Returns a dict with the requested arrays among tod, pkid, pwv (float64)."""
+        w = self.w
+        t_count = w.n_samples - t_begin if t_count is None else t_count
+        out = {}
+        if "tod" in want:
+            out["tod"] = np.zeros((t_count, w.n_spaxel, w.n_chan))
+        if "pkid" in want:
+            out["pkid"] = np.zeros((t_count, w.n_spaxel, w.n_chan))
+        if "pwv" in want:
+            out["pwv"] = np.zeros((t_count, w.n_spaxel))
+        p = lambda key: C.c_void_p(out[key].ctypes.data) if key in out else None
+        self._chk(self.L.go_simulate(C.byref(self.cfg), C.c_int64(t_begin), C.c_int64(t_count),
+                                     p("tod"), p("pkid"), p("pwv")), "simulate")
+        return out
+
+    def simulate_rows(self, t_idx, s_idx, noise=False):
+        t_idx = np.ascontiguousarray(t_idx, dtype=np.int64)
+        s_idx = np.ascontiguousarray(s_idx, dtype=np.int32)
+        pk = np.zeros((t_idx.size, self.w.n_chan))
+        wn = np.zeros((t_idx.size, self.w.n_chan)) if noise else None
+        self._chk(self.L.go_simulate_rows(C.byref(self.cfg), C.c_int64(t_idx.size),
+                                          C.c_void_p(t_idx.ctypes.data), C.c_void_p(s_idx.ctypes.data),
+                                          C.c_void_p(pk.ctypes.data),
+                                          C.c_void_p(wn.ctypes.data) if noise else None), "simulate_rows")
+        return (pk, wn) if noise else pk
+
+    def pink_series(self, s_idx, c_idx, t_begin, t_count):
+        s_idx = np.ascontiguousarray(s_idx, dtype=np.int32)
+        c_idx = np.ascontiguousarray(c_idx, dtype=np.int32)
+        out = np.zeros((s_idx.size, t_count))
+        self._chk(self.L.go_pink_series(C.byref(self.cfg), C.c_int64(s_idx.size),
+                                        C.c_void_p(s_idx.ctypes.data), C.c_void_p(c_idx.ctypes.data),
+                                        C.c_int64(t_begin), C.c_int64(t_count),
+                                        C.c_void_p(out.ctypes.data)), "pink_series")
+        return out
+
+    def dnu_eff(self):
+        out = np.zeros(self.w.n_chan)
+        self.L.go_dnu_eff(C.byref(self.cfg), C.c_void_p(out.ctypes.data))
+        return out
+
+    def pink_coeffs(self, spaxel, chan):
+        J = self.cfg.pink_n_stage
+        phi, g = np.zeros(J), np.zeros(J)
+        self.L.go_pink_coeffs(C.byref(self.cfg), C.c_int32(spaxel), C.c_int32(chan),
+                              C.c_void_p(phi.ctypes.data), C.c_void_p(g.ctypes.data))
+        return phi, g
+
+
+# ---- elementary pieces ----
+def planck(nu_hz, T_K):
+    return lib().go_planck(float(nu_hz), float(T_K))
+
+
+def philox4x32_10(ctr, key):
+    c = (C.c_uint32 * 4)(*[int(x) & 0xffffffff for x in ctr])
+    k = (C.c_uint32 * 2)(*[int(x) & 0xffffffff for x in key])
+    o = (C.c_uint32 * 4)()
+    lib().go_philox4x32_10(c, k, o)
+    return [int(x) for x in o]
+
+
+def uniform01(w):
+    return lib().go_uniform(int(w) & 0xffffffff)
+
+
+def normals4(seed, c0, c1, c2, c3):
+    z = np.zeros(4)
+    lib().go_normals4(int(seed), int(c0) & 0xffffffff, int(c1), int(c2), int(c3), C.c_void_p(z.ctypes.data))
+    return z
+
+
+def normals_bulk(seed, c0_begin, count, c1=0, c2=0, c3=0):
+    z = np.zeros((count, 4))
+    f = lib().go_normals_bulk
+    f.restype = None
+    f(C.c_uint64(int(seed)), C.c_uint32(int(c0_begin)), C.c_int64(count), C.c_uint32(c1),
+      C.c_uint32(c2), C.c_uint32(c3), C.c_void_p(z.ctypes.data))
+    return z
+
+
+def photon_sigma(P_W, f_center_hz, dnu_eff_hz, f_sample_hz):
+    return lib().go_photon_sigma(float(P_W), float(f_center_hz), float(dnu_eff_hz), float(f_sample_hz))
+
+
+def num_threads():
+    return lib().go_num_threads()

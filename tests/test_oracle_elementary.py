@@ -1,0 +1,185 @@
+"""Pins for the oracle's elementary pieces: each is checked against something other than
+the oracle itself (closed forms, the vendor's Philox, distribution tests, exact PSDs)."""
+import math
+import shutil
+import subprocess
+from pathlib import Path
+
+import numpy as np
+import pytest
+from scipy import signal, stats
+
+from oracle import oracle as O
+from paper_2604_23305_b200 import workloads as W
+
+H, KB = 6.62607015e-34, 1.380649e-23
+GOLDEN = Path(__file__).resolve().parent / "golden"
+
+
+# ---------------------------------------------------------------- P^JN
+def test_planck_rayleigh_jeans_limit():
+    # h nu << k T:  B = k T (1 - x/2 + x^2/12 - ...)
+    nu, T = 1e9, 300.0
+    x = H * nu / (KB * T)
+    assert O.planck(nu, T) == pytest.approx(KB * T * (1 - x / 2 + x * x / 12), rel=1e-14)
+
+
+def test_planck_wien_tail_and_zero():
+    nu, T = 400e9, 2.0          # x ~ 9.6
+    x = H * nu / (KB * T)
+    # exact form via exp; and the Wien tail B -> h nu e^-x within e^-x relative
+    assert O.planck(nu, T) == pytest.approx(H * nu / (math.exp(x) - 1.0), rel=1e-13)
+    assert O.planck(nu, T) == pytest.approx(H * nu * math.exp(-x), rel=2 * math.exp(-x))
+    assert O.planck(nu, 0.0) == 0.0
+    assert O.planck(300e9, 273.0) == pytest.approx(3.5697e-21, rel=1e-3)   # ~ k T (1 - x/2)
+
+
+def test_planck_monotone_in_T():
+    v = [O.planck(350e9, T) for T in (2.725, 4.0, 77.0, 273.0, 290.0)]
+    assert all(a < b for a, b in zip(v, v[1:]))
+
+
+# ---------------------------------------------------------------- Philox4x32-10
+@pytest.mark.skipif(shutil.which("nvcc") is None, reason="needs nvcc for the vendor header")
+def test_philox_matches_curand_host_implementation(tmp_path):
+    """Known answers from NVIDIA's curand_philox4x32_x.h compiled for the host."""
+    exe = tmp_path / "curand_philox_host"
+    subprocess.check_call(["nvcc", "-O1", "-Wno-deprecated-gpu-targets", "-o", str(exe),
+                           str(GOLDEN / "curand_philox_host.cu")])
+    rng = np.random.default_rng(11)
+    cases = [[0] * 6, [0xffffffff] * 6, [1, 0, 0, 0, 0, 0], [0, 0, 0, 0, 1, 0], [0, 0, 0, 1, 0, 0]]
+    cases += [list(map(int, rng.integers(0, 2 ** 32, 6))) for _ in range(200)]
+    inp = "\n".join(" ".join(f"{v:x}" for v in c) for c in cases) + "\n"
+    out = subprocess.run([str(exe)], input=inp, capture_output=True, text=True, check=True).stdout
+    ref = [[int(t, 16) for t in line.split()] for line in out.strip().splitlines()]
+    assert len(ref) == len(cases)
+    for c, r in zip(cases, ref):
+        assert O.philox4x32_10(c[:4], c[4:]) == r
+
+
+def test_philox_is_a_bijection_on_a_small_slice():
+    outs = {tuple(O.philox4x32_10([i, 0, 0, 0], [5, 6])) for i in range(2000)}
+    assert len(outs) == 2000
+
+
+def test_uniform_is_open_interval_and_fp32_exact():
+    for w in (0, 1, 511, 512, 2 ** 31, 2 ** 32 - 1):
+        u = O.uniform01(w)
+        assert 0.0 < u < 1.0
+        assert float(np.float32(u)) == u                 # exactly representable in binary32
+    assert O.uniform01(0) == 0.5 / 2 ** 23
+    assert O.uniform01(2 ** 32 - 1) == 1.0 - 0.5 / 2 ** 23
+
+
+def test_normals_box_muller_definition():
+    seed, ctr = 0x1234567890abcdef, (7, 3, 5, 1)
+    w = O.philox4x32_10(ctr, [seed & 0xffffffff, seed >> 32])
+    u = [((x >> 9) + 0.5) / 2 ** 23 for x in w]
+    z = O.normals4(seed, *ctr)
+    r0, r1 = math.sqrt(-2 * math.log(u[0])), math.sqrt(-2 * math.log(u[2]))
+    exp = [r0 * math.cos(2 * math.pi * u[1]), r0 * math.sin(2 * math.pi * u[1]),
+           r1 * math.cos(2 * math.pi * u[3]), r1 * math.sin(2 * math.pi * u[3])]
+    np.testing.assert_allclose(z, exp, rtol=1e-13, atol=1e-15)
+
+
+def test_normals_distribution():
+    z = O.normals_bulk(seed=42, c0_begin=0, count=500_000, c1=1, c2=2, c3=0).ravel()   # 2e6 draws
+    n = z.size
+    assert abs(z.mean()) < 4 / math.sqrt(n)
+    assert abs(z.var() - 1) < 4 * math.sqrt(2 / n)
+    assert abs(stats.kurtosis(z)) < 4 * math.sqrt(24 / n)
+    assert abs(stats.skew(z)) < 4 * math.sqrt(6 / n)
+    assert stats.kstest(z[:200_000], "norm").pvalue > 1e-3
+    assert np.abs(z).max() <= math.sqrt(2 * 24 * math.log(2)) + 1e-9        # U >= 2^-24
+    # the four outputs of a block are uncorrelated
+    c = np.corrcoef(z.reshape(-1, 4).T)
+    assert np.abs(c - np.eye(4)).max() < 5 / math.sqrt(n / 4)
+
+
+# ---------------------------------------------------------------- photon noise (Eq. 17-19)
+def test_photon_sigma_formula_and_limits():
+    P, fc, dn, fs = 1.3e-13, 300e9, 1.9e9, 160.0
+    s = O.photon_sigma(P, fc, dn, fs)
+    assert s == pytest.approx(math.sqrt((2 * H * fc * P + 2 * P * P / dn) * fs / 2), rel=1e-14)
+    # shot-noise limit (P -> 0): sigma^2 -> h f P f_s ; bunching limit: sigma -> P sqrt(f_s/dnu)
+    assert O.photon_sigma(1e-22, fc, dn, fs) ** 2 == pytest.approx(H * fc * 1e-22 * fs, rel=1e-5)
+    assert O.photon_sigma(1e-6, fc, dn, fs) == pytest.approx(1e-6 * math.sqrt(fs / dn), rel=1e-5)
+    assert O.photon_sigma(0.0, fc, dn, fs) == 0.0
+
+
+def test_dnu_eff_default_is_lorentzian_equivalent_width():
+    # an isolated Lorentzian on a wide fine grid: (int F)^2 / int F^2 = pi f / R
+    f0, R = 300e9, 500.0
+    nu = np.linspace(f0 - 150e9, f0 + 150e9, 60001)
+    w = W.random_workload(1, n_chan=1, n_freq=nu.size)
+    w = w.replace(nu0_hz=float(nu[0]), dnu_hz=float(nu[1] - nu[0]),
+                  filt=W.lorentzian_filterbank(nu, np.array([f0]), R), f_center_hz=np.array([f0]),
+                  eta_front_nu=None, cube=None,
+                  stages=[], lut_nu0_hz=float(nu[0]) - 1e9,
+                  lut_dnu_hz=(nu[-1] - nu[0] + 2e9) / (w.atm_lut.shape[1] - 1))
+    d = O.Oracle(w).dnu_eff()[0]
+    assert d == pytest.approx(math.pi * f0 / R, rel=1e-2)
+
+
+# ---------------------------------------------------------------- AR(1) cascade pink noise
+def _pink_workload(J=4, n_samples=1 << 15, n_chan=64):
+    w = W.random_workload(3, n_samples=8, n_spaxel=1, n_chan=n_chan, pink_noise=True, J=J)
+    n = w.n_spaxel * w.n_chan
+    return w.replace(n_samples=n_samples, az_rad=np.zeros(n_samples), el_rad=np.zeros(n_samples),
+                     pink_A=np.full(n, 2.5e-34), pink_alpha=np.full(n, 1.0))
+
+
+def test_pink_coefficients_closed_form():
+    w = _pink_workload()
+    phi, g = O.Oracle(w).pink_coeffs(0, 5)
+    fj = w.pink_f_corner_hz
+    np.testing.assert_allclose(phi, np.exp(-2 * np.pi * fj / w.f_sample_hz), rtol=1e-15)
+    # alpha = 1: g_j^2 = A ln(10)
+    np.testing.assert_allclose(g ** 2, 2.5e-34 * math.log(10.0) * np.ones(4), rtol=1e-12)
+
+
+def test_pink_stage_statistics_and_psd():
+    """Unit-variance stationary stages: total variance = sum g_j^2; Welch PSD averaged over
+    detectors matches the exact discrete-time AR(1) sum, and follows A/f mid-band."""
+    w = _pink_workload()
+    o = O.Oracle(w)
+    nd = w.n_chan
+    x = o.pink_series(np.zeros(nd, np.int32), np.arange(nd, dtype=np.int32), 0, w.n_samples)
+    phi, g = o.pink_coeffs(0, 0)
+    var_exact = float(np.sum(g ** 2))
+    # slow stages decorrelate slowly: compare the ensemble variance at fixed times
+    v = x[:, ::4096].var(axis=0).mean()
+    assert v == pytest.approx(var_exact, rel=0.25)
+    fs = w.f_sample_hz
+    f, pxx = signal.welch(x, fs=fs, nperseg=4096, axis=1)
+    pxx = pxx.mean(axis=0)
+    exact = sum(gj ** 2 * (2 / fs) * (1 - p * p) / (1 - 2 * p * np.cos(2 * np.pi * f / fs) + p * p)
+                for gj, p in zip(g, phi))
+    band = (f > 0.2) & (f < 60)
+    n_avg = nd * (w.n_samples // 2048 - 1)
+    assert np.abs(pxx[band] / exact[band] - 1).max() < 6 / math.sqrt(n_avg) + 0.03
+    # stated approximation of A f^-alpha: holds between the lowest and the highest corner
+    # (0.002-2 Hz here); above the top corner the cascade rolls off as f^-2 (R18)
+    mid = (f > 0.04) & (f < 2.0)
+    ratio = exact[mid] / (2.5e-34 / f[mid])
+    assert 0.85 < ratio.min() and ratio.max() < 1.1
+
+
+def test_pink_lag1_autocorrelation_single_stage():
+    w = _pink_workload(J=1, n_samples=1 << 14, n_chan=32)
+    o = O.Oracle(w)
+    x = o.pink_series(np.zeros(32, np.int32), np.arange(32, dtype=np.int32), 0, w.n_samples)
+    phi, g = o.pink_coeffs(0, 0)
+    r1 = np.mean(x[:, 1:] * x[:, :-1]) / np.mean(x * x)
+    assert r1 == pytest.approx(phi[0], abs=0.01)
+    assert np.mean(x * x) == pytest.approx(g[0] ** 2, rel=0.05)
+
+
+def test_pink_series_windows_are_consistent():
+    """A window starting at t_begin equals the same samples of a run from 0 (chunk seams)."""
+    w = _pink_workload(n_samples=600, n_chan=4)
+    o = O.Oracle(w)
+    s, c = np.zeros(4, np.int32), np.arange(4, dtype=np.int32)
+    full = o.pink_series(s, c, 0, 600)
+    part = o.pink_series(s, c, 217, 300)
+    assert np.array_equal(full[:, 217:517], part)
