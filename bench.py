@@ -1,0 +1,322 @@
+#!/usr/bin/env python
+"""bench.py -- detector-samples/s of the gateau hot path on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C4] [--variant default|fp32|tensor]
+    python bench.py --impl reference ...      # the CPU oracle, timed on the host cores
+
+One "step" = one pass of the whole hot path (geometry -> fused generator/contraction/photon
+noise -> pink noise) over the full workload (default: BASELINE.json configs[3], the 61-spaxel
+IFU config the metric and the roofline target are quoted on; it fits one GPU).  `value` is
+timed with inputs and outputs resident in HBM; `e2e` runs the public API from HOST buffers
+(pinned H2D of the inputs, gt_plan_create, gt_simulate streaming the TOD into pinned host
+memory) inside the timed region.  With N > 1 (torchrun) every rank simulates an independent
+observation (seed + rank) of the same config: weak scaling, no data-path collective.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+sys.path.insert(0, str(ROOT))
+
+METRIC = "detector-samples/s"
+UNIT = "detector-samples/s"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="C4")
+    ap.add_argument("--variant", default="default", choices=["default", "fp32", "tensor"])
+    ap.add_argument("--samples", type=int, default=None, help="shrink n_samples (debug only; marks the line invalid)")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    return ap.parse_args()
+
+
+def workload_config(w, extra=None):
+    cfg = {"workload": f"{w.name}: {w.n_spaxel} spaxel x {w.n_chan} chan x {w.n_samples} samples, "
+                       f"{w.n_freq} freq, {len(w.stages)}-stage cascade, photon={int(w.photon_noise)} pink={int(w.pink_noise)}",
+           "n_spaxel": w.n_spaxel, "n_chan": w.n_chan, "n_freq": w.n_freq, "n_samples": w.n_samples,
+           "cache": "inputs (cube+screen) and the TOD written per step are larger than L2"}
+    if extra:
+        cfg.update(extra)
+    return cfg
+
+
+# ------------------------------------------------------------------------------------------
+# clocks during the timed region (recipe's nvidia-smi line)
+# ------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100", "-i", str(self.index)], stdout=subprocess.PIPE,
+                                         stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[1])); mx.append(float(r[2]))
+                for nm, v in zip(names, r[5:9]):
+                    if v.lower().startswith("active"):
+                        reasons.add(nm)
+            except Exception:
+                pass
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# ------------------------------------------------------------------------------------------
+# CPU oracle legs (cpu_baseline and --impl reference): the only places that execute oracle/
+# ------------------------------------------------------------------------------------------
+def oracle_sample(w, seconds):
+    """Times the oracle, as it stands, on a bounded prefix of the workload (all spaxels and
+    channels, the first n samples), sized for about `seconds` of wall time."""
+    from oracle import oracle as O
+    o = O.Oracle(w)
+    cores = O.num_threads()
+    per_sample = w.n_spaxel * w.n_chan
+    n = max(1, min(w.n_samples, 4096 // max(w.n_spaxel, 1)))
+    t0 = time.perf_counter(); o.simulate(0, n, want=("tod",)); dt = time.perf_counter() - t0
+    if dt < 0.5 * seconds:
+        n2 = int(min(w.n_samples, max(n, n * (seconds - dt) / max(dt, 1e-3))))
+        t0 = time.perf_counter(); o.simulate(0, n2, want=("tod",)); dt = time.perf_counter() - t0
+        n = n2
+    return {"value": n * per_sample / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"first {n} samples x {w.n_spaxel} spaxels x {w.n_chan} channels of {w.name} "
+                      f"({n * w.n_spaxel} rows, {dt:.1f} s wall, OpenMP over rows, fp64)"}, n, dt
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_2604_23305_b200 import workloads as W
+    w = W.make_workload(args.workload, n_samples=args.samples)
+    from oracle import oracle as O
+    o = O.Oracle(w)
+    cores = O.num_threads()
+    # size one step at ~ (120 s / (steps + warmup)) of oracle work, from a short calibration
+    n = max(1, 2048 // w.n_spaxel)
+    t0 = time.perf_counter(); o.simulate(0, n, want=("tod",)); dt = time.perf_counter() - t0
+    budget = 120.0 / max(args.steps + args.warmup, 1)
+    n_step = int(max(1, min(w.n_samples, n * budget / max(dt, 1e-3))))
+    for _ in range(args.warmup):
+        o.simulate(0, n_step, want=("tod",))
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        o.simulate(0, n_step, want=("tod",))
+    total = time.perf_counter() - t0
+    units = n_step * w.n_spaxel * w.n_chan * args.steps
+    value = units / total
+    sample = (f"each step = first {n_step} samples x {w.n_spaxel} spaxels x {w.n_chan} channels of {w.name} "
+              f"({n_step * w.n_spaxel} rows), CPU oracle fp64, OpenMP")
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_config(w, {"sample": sample}),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+# ------------------------------------------------------------------------------------------
+# the CUDA path
+# ------------------------------------------------------------------------------------------
+def peaks():
+    f = ROOT / "MEASURED_PEAKS.json"
+    if f.exists():
+        d = json.loads(f.read_text())
+        return d, "measured (MEASURED_PEAKS.json)"
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "sm_max_mhz": 1965.0}, \
+        "fallback (B200_PROFILING.md)"
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2604_23305_b200 import binding as B
+    from paper_2604_23305_b200 import workloads as W
+
+    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the gateau_b200 path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    w = W.make_workload(args.workload, n_samples=args.samples)
+    w = w.replace(seed=w.seed + 1000 * rank)                      # independent observation per rank
+    variant = {"default": B.VARIANT_DEFAULT, "fp32": B.VARIANT_FP32, "tensor": B.VARIANT_TENSOR}[args.variant]
+    plan = B.Plan(w, variant=variant, device=f"cuda:{local}")
+    units = w.detector_samples()
+    tod = torch.empty((w.n_samples, w.n_spaxel, w.n_chan), dtype=torch.float32, device=f"cuda:{local}")
+
+    for _ in range(max(args.warmup, 3)):
+        plan.simulate(out=tod)
+    barrier()
+    sampler = ClockSampler(local); sampler.start()
+    launches0 = plan.launch_count
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    fused_ms, fused_n = 0.0, 0
+    barrier()
+    step_ms = []
+    for k in range(args.steps):
+        ev[k].record()
+        plan.simulate(out=tod)
+        e = torch.cuda.Event(enable_timing=True); e.record(); e.synchronize()
+        step_ms.append(ev[k].elapsed_time(e))
+        ms, n = plan.last_fused_ms(); fused_ms += ms; fused_n += n
+    barrier()
+    total_ms = float(sum(step_ms))
+    launches = plan.launch_count - launches0
+    clocks = sampler.stop()
+    t = torch.tensor([total_ms], dtype=torch.float64, device=f"cuda:{local}")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms = float(t.item())
+    value = world * units * args.steps / (total_ms * 1e-3)
+
+    # ---- roofline of the dominant kernel (the fused kernel) ----
+    pk, pk_src = peaks()
+    flops_per_launch = 2.0 * w.n_chan * w.n_freq * (w.n_samples * w.n_spaxel) / max(fused_n / args.steps, 1)
+    avg_launch_s = fused_ms * 1e-3 / max(fused_n, 1)
+    achieved = flops_per_launch / avg_launch_s / 1e12
+    if plan.variant_name.startswith("tcgen05"):
+        peak = 0.5 * pk["bf16_tflops_sustained"]
+        roof = {"bound": "tensor", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+                "traffic": None, "kernel": "fused_tc_kernel",
+                "peak_source": f"TF32 dense = 0.5 x bf16 sustained, {pk_src}",
+                "issued_tflops": 3 * achieved, "issued_frac": 3 * achieved / peak,
+                "note": "achieved = algorithmic 2*n_chan*n_freq flop/row; the split-TF32 scheme issues 3 MMAs per useful one"}
+    else:
+        mhz = clocks.get("sm_mhz") or pk.get("sm_max_mhz", 1965.0)
+        peak = 148 * 128 * 2 * mhz * 1e6 / 1e12
+        roof = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+                "traffic": None, "kernel": "fused_fp32_kernel",
+                "peak_source": f"FP32 FMA = 148 SM x 128 lanes x 2 x {mhz:.0f} MHz (median SM clock under load)"}
+    roof["fused_ms_per_step"] = fused_ms / args.steps
+    roof["fused_share_of_step"] = fused_ms / total_ms if world == 1 else None
+
+    # ---- end to end through the public API with host buffers ----
+    e2e = None
+    if not args.no_e2e:
+        try:
+            e2e = run_e2e(torch, B, w, variant, local, world, max(1, min(args.steps, 3)), barrier)
+        except Exception as ex:                                   # report, never fake
+            e2e = {"value": None, "unit": UNIT, "error": repr(ex)[:200]}
+
+    plan.destroy()
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cpu, _, _ = oracle_sample(w, args.cpu_seconds)
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": workload_config(w, {"variant": plan_variant_name(args, roof), "parallelism": f"replica x{world}"}),
+                "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roof, "cpu_baseline": cpu}
+        if args.samples:
+            line["invalid"] = "--samples shrinks the workload: debug only"
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def plan_variant_name(args, roof):
+    return "tcgen05-3xtf32" if roof["bound"] == "tensor" else "fp32-ffma"
+
+
+def run_e2e(torch, B, w, variant, local, world, steps, barrier):
+    """Public API from HOST buffers: per step, pinned inputs -> device, gt_plan_create,
+    gt_simulate streaming the TOD into pinned host memory, gt_plan_destroy."""
+    dev = f"cuda:{local}"
+    host = {}
+    for name, arr in (("cube", w.cube), ("screen", w.screen), ("atm_lut", w.atm_lut), ("filt", w.filt)):
+        if arr is not None:
+            host[name] = torch.from_numpy(np.ascontiguousarray(arr, dtype=np.float32)).pin_memory()
+    h2d = sum(t.numel() * 4 for t in host.values()) + 16 * w.n_samples
+    out = torch.empty((w.n_samples, w.n_spaxel, w.n_chan), dtype=torch.float32, pin_memory=True)
+    d2h = out.numel() * 4
+
+    # the workload's large arrays now live in pinned host memory (views of the pinned tensors)
+    wp = w.replace(**{k: v.numpy() for k, v in host.items()})
+
+    def one():
+        # B.Plan copies the pinned arrays to the device (H2D) and creates the plan; simulate streams to `out`
+        p = B.Plan(wp, variant=variant, device=dev)
+        p.simulate(out=out)
+        p.destroy()
+
+    one()                                                        # warm-up (allocators, pinned pages)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        one()
+    torch.cuda.synchronize()
+    dt = time.perf_counter() - t0
+    t = torch.tensor([dt], dtype=torch.float64, device=dev)
+    if world > 1:
+        import torch.distributed as dist
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dt = float(t.item())
+    return {"value": world * w.detector_samples() * steps / dt, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+            "d2h_bytes_per_step": int(d2h), "ms_per_step": 1e3 * dt / steps, "steps": steps,
+            "what": "host arrays -> H2D -> gt_plan_create -> gt_simulate into pinned host TOD (chunked D2H on a side stream) -> gt_plan_destroy"}
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,174 @@
+/*
+ * gateau_b200.h -- C ABI of libgateau_b200.so, the B200 (sm_100a) hot path of the gateau
+ * observation simulator of arXiv 2604.23305.
+ *
+ * The library computes, for every (time sample n, spaxel s), the signal chain of
+ * PAPER.md Sect. 2.4-2.7 (lines 125-229) and writes time-ordered data (TOD):
+ *
+ *   step 0  pointing            phi(t_n)+dphi_s, theta(t_n)+dtheta_s
+ *   step 1  screen sampling     Eq. 9 frozen-flow coordinates, bilinear PWV
+ *   step 2  transmission        bilinear eta_atm,z(nu,PWV), Eq. 10 airmass
+ *   step 3  source sampling     bilinear P_nu,src, zero outside; Eq. 11
+ *   step 4  cascade             Eq. 12 for the atmosphere and every stage
+ *   step 5  contraction         Eq. 16 P_KID = sum_nu eta_filt P_nu dnu
+ *   step 6a photon noise        Eq. 18-19 with the narrow-band NEP
+ *   step 6b pink noise          per-detector AR(1) cascade (R18)
+ *   step 7  output              Eq. 21, TOD [t][spaxel][chan] fp32
+ *
+ * Every step runs in hand-written CUDA kernels; there is no CPU fallback: without a
+ * CUDA device every entry point that computes returns GT_ERR_CUDA.
+ *
+ * Pointer kinds are stated per field: HOST pointers are read (copied) during
+ * gt_plan_create and may be freed afterwards; DEVICE pointers are BORROWED: the caller
+ * allocates them (e.g. torch.empty(..., device="cuda").data_ptr()), they must stay
+ * valid and unchanged until gt_plan_destroy.  The library owns what it allocates.
+ *
+ * Errors: every call returns a gt_status, never throws, never aborts.  On error
+ * *out_plan is NULL / outputs are unspecified; gt_last_error gives a message.
+ */
+#ifndef GATEAU_B200_H
+#define GATEAU_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct gt_plan gt_plan;                 /* opaque, owned by the library */
+
+typedef enum {
+    GT_OK = 0,
+    GT_ERR_NULL = 1,          /* a required pointer is NULL                                   */
+    GT_ERR_SHAPE = 2,         /* a size is non-positive or inconsistent                       */
+    GT_ERR_VALUE = 3,         /* a value is outside its domain (eta not in [0,1], T < 0, ...) */
+    GT_ERR_RANGE = 4,         /* a range is not covered (LUT nu range, sample range)          */
+    GT_ERR_OOM = 5,
+    GT_ERR_CUDA = 6,          /* CUDA runtime error, or no CUDA device                        */
+    GT_ERR_UNSUPPORTED = 7
+} gt_status;
+
+/* One optical stage k >= 1 of the cascade, Eq. 12.  The atmosphere is
+ * always the extra stage k = 0 and is not listed here (R5). */
+typedef struct {
+    const float* eta_nu;      /* DEVICE [n_freq] efficiency per frequency, or NULL => eta_scalar */
+    double       eta_scalar;
+    double       T_K;         /* physical temperature of the stage                              */
+    int32_t      couple_atmosphere; /* 1: the parasitic term is the sky seen through the
+                                 atmosphere, (1-eta_atm) B(T_atm) + eta_atm B(T_cmb) */
+} gt_stage;
+
+/* Kernel variant for step 2-6a (the fused generator + contraction + photon-noise kernel). */
+enum {
+    GT_VARIANT_DEFAULT = 0,   /* tcgen05 tensor-core kernel, split-TF32 operands                 */
+    GT_VARIANT_FP32    = 1,   /* FP32 CUDA-core kernel (the measured alternative of north_star)  */
+    GT_VARIANT_TENSOR  = 2    /* tcgen05 kernel, explicitly                                      */
+};
+
+typedef struct {
+    /* uniform frequency grid nu_i = nu0 + i dnu, i < n_freq */
+    int32_t n_freq;  double nu0_hz, dnu_hz;
+    /* sampling: t_n = n / f_sample */
+    int64_t n_samples;  double f_sample_hz;
+    /* scan pattern: HOST [n_samples], radians relative to the scan centre;
+       el0_rad = absolute elevation of the scan centre, used only for the airmass (Eq. 10) */
+    const double *az_rad, *el_rad;  double el0_rad;
+    /* spaxel pointing offsets: HOST [n_spaxel], radians */
+    int32_t n_spaxel;  const double *daz_rad, *del_rad;
+    /* source cube P_nu,src in W/Hz: DEVICE [n_el][n_az][n_freq], frequency
+       fastest, or NULL = blank sky.  Grid node (j,i) sits at (el_min + j del_grid, az_min + i daz_grid). */
+    const float* cube;  int32_t n_az, n_el;
+    double az_min_rad, daz_grid_rad, el_min_rad, del_grid_rad;
+    /* Eq. 11 front end: DEVICE [n_freq] eta_t*eta_surf*eta_pol, NULL => 1; T_cmb 0 => no CMB term */
+    const float* eta_front_nu;  double T_cmb_K;
+    /* frozen-flow PWV screen (Eq. 9): DEVICE [ny][nx] in mm, periodic; pixel size, column
+       height h, wind speed along +x, and the mean PWV drift PWV_0(t) = a + b t added on top */
+    const float* screen;  int32_t nx, ny;
+    double dx_m, dy_m, h_column_m, wind_mps, pwv0_a_mm, pwv0_b_mm_per_s;
+    /* zenith transmission lookup table: DEVICE [n_pwv][n_nu_lut] */
+    const float* atm_lut;  int32_t n_pwv, n_nu_lut;
+    double lut_nu0_hz, lut_dnu_hz, lut_pwv0_mm, lut_dpwv_mm, T_atm_K;
+    /* optical stages k = 1..n_stage: HOST array of gt_stage */
+    int32_t n_stage;  const gt_stage* stages;
+    /* dispersive element (Eq. 16): DEVICE [n_chan][n_freq] transmission */
+    int32_t n_chan;  const float* filt;
+    const double* f_center_hz;    /* HOST [n_chan] channel centre (photon noise h nu)            */
+    const double* dnu_eff_hz;     /* HOST [n_chan] effective bandwidth, NULL => derived from filt */
+    /* noise: Philox4x32-10 keyed by seed, counter (n, spaxel, chan, stream) (R19) */
+    uint64_t seed;  int32_t photon_noise, pink_noise;
+    const double *pink_A, *pink_alpha;     /* HOST [n_spaxel*n_chan] PSD level A and slope alpha */
+    int32_t pink_n_stage;  const double* pink_f_corner_hz;   /* HOST [J] corner frequencies, J <= 8 */
+    /* streaming: samples per device chunk when the output is host memory; 0 => library picks */
+    int64_t chunk_samples;
+    /* one of GT_VARIANT_* */
+    int32_t variant;
+} gt_config;
+
+/* Per-row geometry record returned by gt_debug_geometry: the integers are the quantities
+ * "index, scan and RNG counters" that must match the oracle bit for bit. */
+typedef struct {
+    int64_t n;                   /* global sample index (= Philox counter word 0)          */
+    int32_t iu0, iv0;            /* wrapped lower-left screen cell                          */
+    int32_t ju, jv;              /* lower-left source cell, -1/-1 outside the cube          */
+    int32_t ip;                  /* lower LUT row in PWV                                    */
+    int32_t pad_;
+    double  fu, fv, gu, gv, fp;  /* bilinear fractions                                      */
+    double  pwv_mm;              /* zenith PWV on the line of sight incl. drift             */
+    double  csc;                 /* 1 / sin(absolute elevation)                             */
+} gt_georec;
+
+/* Validates cfg, copies every HOST array, reads the small DEVICE arrays it needs for
+ * plan-time constants (LUT, filter, per-frequency efficiencies) and uploads the derived
+ * tables.  cuda_stream: a cudaStream_t (NULL = default stream) used for the uploads.
+ * Returns GT_OK and *out_plan, or an error and *out_plan = NULL. */
+gt_status gt_plan_create(const gt_config* cfg, void* cuda_stream, gt_plan** out_plan);
+
+/* Simulates samples n = t_begin .. t_begin+t_count-1 for all spaxels and channels.
+ *   tod_out  [t_count][n_spaxel][n_chan] fp32, DEVICE memory or (pinned or pageable) HOST
+ *            memory; detected with cudaPointerGetAttributes.
+ *   pwv_out  optional (NULL ok) [t_count][n_spaxel] fp32 zenith PWV, same memory kind rule.
+ * DEVICE output: the kernels write in place and the call returns after enqueueing on
+ * cuda_stream (asynchronous).  HOST output: the TOD is produced in chunks of
+ * chunk_samples into two device buffers and copied out on an internal side stream while
+ * the next chunk computes; the call returns after the last copy has completed (blocking).
+ * With pink noise on, the AR(1) state advances with the call: calls must cover
+ * contiguous increasing ranges, or restart from t_begin = 0 (else GT_ERR_VALUE).  With
+ * pink noise off any range is legal.  t_count = 0 is legal and does nothing. */
+gt_status gt_simulate(gt_plan* plan, int64_t t_begin, int64_t t_count,
+                      float* tod_out, float* pwv_out, void* cuda_stream);
+
+/* Frees everything the plan owns.  NULL-safe. */
+gt_status gt_plan_destroy(gt_plan* plan);
+
+/* Message of the last error on this plan; plan == NULL => the calling thread's last
+ * gt_plan_create error.  Never NULL. */
+const char* gt_last_error(const gt_plan* plan);
+
+/* ---- test hooks (not part of the user path) ---- */
+/* Geometry records of rows (t_begin .. t_begin+t_count-1) x (all spaxels) into HOST memory
+ * host_records_out[t_count*n_spaxel], computed by the same device code as gt_simulate. */
+gt_status gt_debug_geometry(gt_plan* plan, int64_t t_begin, int64_t t_count,
+                            gt_georec* host_records_out);
+/* Raw Philox4x32-10 output words of the device generator for `count` consecutive values
+ * of counter word 0 starting at c0_begin, fixed (c1, c2, c3), key = seed: HOST
+ * out_words[count][4].  Needs no plan. */
+gt_status gt_debug_philox(uint64_t seed, uint32_t c0_begin, int64_t count,
+                          uint32_t c1, uint32_t c2, uint32_t c3, uint32_t* host_out_words);
+/* Noiseless channel power (Eq. 16 only, noise switched off regardless of the plan) for the
+ * same range as gt_simulate; pkid_out follows the tod_out rules.  Does not touch the
+ * pink-noise state. */
+gt_status gt_debug_pkid(gt_plan* plan, int64_t t_begin, int64_t t_count,
+                        float* pkid_out, void* cuda_stream);
+/* Number of kernels this library launched since the plan was created. */
+int64_t gt_launch_count(const gt_plan* plan);
+/* Name of the fused-kernel variant the plan resolved to ("tcgen05-3xtf32", "fp32-ffma"). */
+const char* gt_variant_name(const gt_plan* plan);
+/* Device time [ms] the fused kernel took in the last gt_simulate / gt_debug_pkid call, summed
+ * over its launches (CUDA events on the launching stream); synchronises the stream.  Also
+ * returns the number of launches in *n_launches (NULL ok). */
+double gt_last_fused_ms(gt_plan* plan, int32_t* n_launches);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

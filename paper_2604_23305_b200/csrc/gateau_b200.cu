@@ -1,0 +1,584 @@
+// gateau_b200.cu -- C ABI (include/gateau_b200.h), plan (host double-precision precompute,
+// device tables, streams) and kernel launches of libgateau_b200.so.
+//
+// Build: nvcc -gencode arch=compute_100a,code=sm_100a -lineinfo -O3 -shared -Xcompiler -fPIC
+// No code is shared with oracle/ and nothing here runs the path on the CPU: the host code
+// only validates, derives per-frequency/per-channel constants once per plan, and launches.
+#include "../../include/gateau_b200.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstdarg>
+#include <cstring>
+#include <string>
+#include <vector>
+#include <new>
+
+#include "gt_common.cuh"
+#include "gt_geometry.cuh"
+#include "gt_fused_fp32.cuh"
+#include "gt_fused_tc.cuh"
+#include "gt_pink.cuh"
+
+namespace {
+
+// CODATA exact values (PAPER.md names h, k_B implicitly through P^JN; R4)
+constexpr double kH = 6.62607015e-34, kKB = 1.380649e-23, kPi = 3.14159265358979323846;
+constexpr double kPref = kKB * 300.0;     // spectrum scale: kernels work on P_nu / kPref = O(1)
+
+thread_local std::string g_create_error = "";
+
+// single-moded Johnson-Nyquist / Planck spectral power h nu / (exp(h nu / kT) - 1), 0 at T = 0
+double jn_power(double nu, double T) {
+    if (!(T > 0.0)) return 0.0;
+    return kH * nu / std::expm1(kH * nu / (kKB * T));
+}
+
+template <class T>
+struct DevBuf {
+    T* p = nullptr; size_t n = 0;
+    cudaError_t alloc(size_t count) {
+        release(); n = count;
+        return cudaMalloc(reinterpret_cast<void**>(&p), std::max<size_t>(count, 1) * sizeof(T));
+    }
+    cudaError_t upload(const std::vector<T>& h, cudaStream_t st) {
+        cudaError_t e = alloc(h.size());
+        if (e != cudaSuccess || h.empty()) return e;
+        return cudaMemcpyAsync(p, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice, st);
+    }
+    void release() { if (p) cudaFree(p); p = nullptr; n = 0; }
+    ~DevBuf() { release(); }
+};
+
+}  // namespace
+
+struct gt_plan {
+    // sizes
+    int32_t n_freq = 0, n_freq_pad = 0, n_chan = 0, n_chan_pad = 0, n_spaxel = 0, n_pwv = 0, J = 0;
+    int64_t n_samples = 0, chunk_samples = 0;
+    int32_t photon_noise = 0, pink_noise = 0, variant = GT_VARIANT_FP32;
+    uint64_t seed = 0;
+    float scale = 0.f;
+    // borrowed
+    const float* cube = nullptr; int32_t n_az = 0, n_el = 0;
+    // geometry
+    gt::GeoParams geo{};
+    DevBuf<double> d_tan_az, d_tan_el, d_sinE, d_cosE, d_az, d_el;
+    DevBuf<double> d_sp;             // 6 per-spaxel tables back to back
+    // fused-kernel tables
+    DevBuf<float> d_Xn, d_Gs, d_lut_r, d_filt_t, d_bias, d_c1, d_c2;
+    gt::TcTables tc;                 // tensor-kernel operand images
+    // pink
+    gt::PinkParams pink{};
+    DevBuf<float> d_gain, d_state, d_seg;
+    int64_t pink_next_t = 0;
+    // scratch
+    DevBuf<gt::RowParam> d_rows;     // [chunk rows]
+    DevBuf<float> d_chunk[2];        // device TOD chunks (host output only), allocated lazily
+    DevBuf<float> d_pwv[2];
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t ev_ready[2] = {nullptr, nullptr}, ev_copied[2] = {nullptr, nullptr};
+    std::vector<cudaEvent_t> ev_fused;       // start/stop pairs of the last call
+    int32_t n_fused_last = 0;
+    int64_t launches = 0;
+    int num_sms = 148;
+    std::string error;
+};
+
+namespace {
+
+gt_status fail(gt_plan* p, gt_status st, const char* fmt, ...) {
+    char buf[512];
+    va_list ap; va_start(ap, fmt); vsnprintf(buf, sizeof buf, fmt, ap); va_end(ap);
+    if (p) p->error = buf; else g_create_error = buf;
+    return st;
+}
+
+#define GT_CUDA(plan, expr)                                                                   \
+    do { cudaError_t e_ = (expr);                                                             \
+         if (e_ != cudaSuccess) return fail(plan, e_ == cudaErrorMemoryAllocation ? GT_ERR_OOM : GT_ERR_CUDA, \
+                                            "%s: %s", #expr, cudaGetErrorString(e_)); } while (0)
+
+// copy a small DEVICE array to the host (plan creation only)
+gt_status fetch(const float* dev, size_t n, std::vector<float>& out, const char* what) {
+    out.resize(n);
+    cudaError_t e = cudaMemcpy(out.data(), dev, n * sizeof(float), cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) return fail(nullptr, GT_ERR_CUDA, "reading %s from device: %s", what, cudaGetErrorString(e));
+    return GT_OK;
+}
+
+gt_status validate(const gt_config* c) {
+    if (!c) return fail(nullptr, GT_ERR_NULL, "cfg is NULL");
+    if (!c->az_rad || !c->el_rad || !c->daz_rad || !c->del_rad || !c->screen || !c->atm_lut || !c->filt ||
+        !c->f_center_hz) return fail(nullptr, GT_ERR_NULL, "a required array pointer is NULL");
+    if (c->n_freq <= 0 || c->n_samples <= 0 || c->n_spaxel <= 0 || c->n_chan <= 0 || c->nx <= 0 || c->ny <= 0 ||
+        c->n_pwv < 2 || c->n_nu_lut < 2 || c->n_stage < 0 || c->chunk_samples < 0)
+        return fail(nullptr, GT_ERR_SHAPE, "a size is non-positive (n_freq/n_samples/n_spaxel/n_chan/nx/ny/n_pwv/n_nu_lut/n_stage)");
+    if (c->n_samples > 0xFFFFFFFELL) return fail(nullptr, GT_ERR_SHAPE, "n_samples exceeds the 32-bit Philox counter word");
+    if (c->n_stage > 0 && !c->stages) return fail(nullptr, GT_ERR_NULL, "stages is NULL with n_stage > 0");
+    if (c->cube && (c->n_az < 2 || c->n_el < 2)) return fail(nullptr, GT_ERR_SHAPE, "source cube needs n_az, n_el >= 2");
+    if (c->cube && (!(c->daz_grid_rad > 0) || !(c->del_grid_rad > 0)))
+        return fail(nullptr, GT_ERR_VALUE, "source grid steps must be positive");
+    if (!(c->f_sample_hz > 0) || !(c->dnu_hz > 0) || !(c->nu0_hz > 0) || !(c->dx_m > 0) || !(c->dy_m > 0) ||
+        !(c->lut_dnu_hz > 0) || !(c->lut_dpwv_mm > 0))
+        return fail(nullptr, GT_ERR_VALUE, "f_sample, dnu, nu0, dx, dy, lut_dnu, lut_dpwv must be positive");
+    if (c->T_cmb_K < 0 || c->T_atm_K < 0) return fail(nullptr, GT_ERR_VALUE, "negative temperature");
+    for (int k = 0; k < c->n_stage; ++k) {
+        const gt_stage& s = c->stages[k];
+        if (s.T_K < 0) return fail(nullptr, GT_ERR_VALUE, "stage %d: negative temperature", k + 1);
+        if (!s.eta_nu && !(s.eta_scalar >= 0.0 && s.eta_scalar <= 1.0))
+            return fail(nullptr, GT_ERR_VALUE, "stage %d: eta_scalar outside [0,1]", k + 1);
+    }
+    if (c->pink_noise) {
+        if (c->pink_n_stage < 1 || c->pink_n_stage > gt::kPinkMaxJ)
+            return fail(nullptr, GT_ERR_SHAPE, "pink_n_stage must be in 1..8");
+        if (!c->pink_A || !c->pink_alpha || !c->pink_f_corner_hz)
+            return fail(nullptr, GT_ERR_NULL, "pink noise arrays are NULL");
+    }
+    if (c->variant != GT_VARIANT_DEFAULT && c->variant != GT_VARIANT_FP32 && c->variant != GT_VARIANT_TENSOR)
+        return fail(nullptr, GT_ERR_VALUE, "unknown variant %d", c->variant);
+    // LUT must cover the frequency grid (R13)
+    const double r_lo = (c->nu0_hz - c->lut_nu0_hz) / c->lut_dnu_hz;
+    const double r_hi = (c->nu0_hz + (c->n_freq - 1) * c->dnu_hz - c->lut_nu0_hz) / c->lut_dnu_hz;
+    if (r_lo < -1e-9 || r_hi > (c->n_nu_lut - 1) + 1e-9)
+        return fail(nullptr, GT_ERR_RANGE, "atm_lut frequency range does not cover the frequency grid");
+    return GT_OK;
+}
+
+template <int TN>
+cudaError_t launch_fp32(const gt::FusedParams& fp, int grid_y, cudaStream_t st) {
+    const size_t smem = (size_t)(gt::kF32_BK * gt::kF32_AStride + gt::kF32_BK * 32 * TN) * sizeof(float)
+                      + gt::kF32_BM * sizeof(gt::RowParam);
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(gt::fused_fp32_kernel<TN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    dim3 grid((unsigned)((fp.n_rows + gt::kF32_BM - 1) / gt::kF32_BM), grid_y);
+    gt::fused_fp32_kernel<TN><<<grid, gt::kF32_Threads, smem, st>>>(fp);
+    return cudaGetLastError();
+}
+
+// channels per CTA of the FP32 kernel = 32 * TN; pick the smallest instantiated TN that covers
+// n_chan in one block column, else 11 with several block columns.
+int fp32_tn(int n_chan) {
+    const int need = (n_chan + 31) / 32;
+    for (int tn : {1, 2, 4, 6, 8, 11}) if (tn >= need) return tn;
+    return 11;
+}
+
+cudaError_t launch_fused_fp32(const gt_plan* p, const gt::FusedParams& fp, cudaStream_t st) {
+    const int tn = fp32_tn(p->n_chan);
+    const int gy = (p->n_chan + 32 * tn - 1) / (32 * tn);
+    switch (tn) {
+        case 1: return launch_fp32<1>(fp, gy, st);
+        case 2: return launch_fp32<2>(fp, gy, st);
+        case 4: return launch_fp32<4>(fp, gy, st);
+        case 6: return launch_fp32<6>(fp, gy, st);
+        case 8: return launch_fp32<8>(fp, gy, st);
+        default: return launch_fp32<11>(fp, gy, st);
+    }
+}
+
+// One chunk: geometry -> fused -> (pink).  dst/pwv_dst are DEVICE pointers.
+gt_status run_chunk(gt_plan* p, int64_t t0, int64_t T, float* dst, float* pwv_dst, bool noise,
+                    cudaStream_t st, int fused_slot) {
+    const int64_t n_rows = T * p->n_spaxel;
+    if (n_rows == 0) return GT_OK;
+    gt::geometry_kernel<<<(unsigned)((n_rows + 255) / 256), 256, 0, st>>>(p->geo, t0, n_rows, p->d_rows.p, pwv_dst, nullptr);
+    GT_CUDA(p, cudaGetLastError());
+    p->launches++;
+
+    gt::FusedParams fp{};
+    fp.rows = p->d_rows.p; fp.n_rows = n_rows; fp.t0 = t0;
+    fp.n_spaxel = p->n_spaxel; fp.n_chan = p->n_chan; fp.n_freq = p->n_freq; fp.n_freq_pad = p->n_freq_pad;
+    fp.Xn = p->d_Xn.p; fp.Gs = p->d_Gs.p; fp.lut_r = p->d_lut_r.p;
+    fp.cube = p->cube; fp.n_az = p->n_az;
+    fp.filt_t = p->d_filt_t.p; fp.n_chan_pad = p->n_chan_pad;
+    fp.scale = p->scale; fp.bias = p->d_bias.p; fp.noise_c1 = p->d_c1.p; fp.noise_c2 = p->d_c2.p;
+    fp.photon_noise = noise ? p->photon_noise : 0;
+    fp.seed_lo = (uint32_t)(p->seed & 0xffffffffu); fp.seed_hi = (uint32_t)(p->seed >> 32);
+    fp.out = dst;
+
+    while ((int)p->ev_fused.size() < 2 * (fused_slot + 1)) {
+        cudaEvent_t e; GT_CUDA(p, cudaEventCreate(&e)); p->ev_fused.push_back(e);
+    }
+    GT_CUDA(p, cudaEventRecord(p->ev_fused[2 * fused_slot], st));
+    if (p->variant == GT_VARIANT_FP32) {
+        GT_CUDA(p, launch_fused_fp32(p, fp, st));
+    } else {
+        GT_CUDA(p, gt::launch_fused_tc(fp, p->tc, p->num_sms, st));
+    }
+    GT_CUDA(p, cudaEventRecord(p->ev_fused[2 * fused_slot + 1], st));
+    p->launches++;
+    p->n_fused_last = fused_slot + 1;
+
+    if (noise && p->pink_noise) {
+        const int64_t n_seg = (T + gt::kPinkSeg - 1) / gt::kPinkSeg;
+        const int64_t n_thr = n_seg * p->pink.n_det;
+        if ((size_t)(n_thr * p->J) > p->d_seg.n) GT_CUDA(p, p->d_seg.alloc((size_t)(n_thr * p->J)));
+        p->pink.seg = p->d_seg.p;
+        gt::pink_local_kernel<<<(unsigned)((n_thr + 255) / 256), 256, 0, st>>>(p->pink, t0, T, dst);
+        gt::pink_carry_kernel<<<(unsigned)((p->pink.n_det + 255) / 256), 256, 0, st>>>(p->pink, T);
+        gt::pink_fixup_kernel<<<(unsigned)((n_thr + 255) / 256), 256, 0, st>>>(p->pink, T, dst);
+        GT_CUDA(p, cudaGetLastError());
+        p->launches += 3;
+    }
+    return GT_OK;
+}
+
+bool is_device_ptr(const void* ptr) {
+    cudaPointerAttributes a{};
+    if (cudaPointerGetAttributes(&a, ptr) != cudaSuccess) { cudaGetLastError(); return false; }
+    return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+
+gt_status simulate_impl(gt_plan* p, int64_t t_begin, int64_t t_count, float* out, float* pwv_out,
+                        bool noise, cudaStream_t st) {
+    if (!p) return fail(nullptr, GT_ERR_NULL, "plan is NULL");
+    if (t_begin < 0 || t_count < 0 || t_begin + t_count > p->n_samples)
+        return fail(p, GT_ERR_RANGE, "sample range [%lld, %lld) outside [0, %lld)", (long long)t_begin,
+                    (long long)(t_begin + t_count), (long long)p->n_samples);
+    if (t_count == 0) return GT_OK;
+    if (!out) return fail(p, GT_ERR_NULL, "output pointer is NULL");
+    const bool pink = noise && p->pink_noise;
+    if (pink) {
+        if (t_begin == 0) {
+            gt::pink_init_kernel<<<(unsigned)((p->pink.n_det + 255) / 256), 256, 0, st>>>(p->pink);
+            GT_CUDA(p, cudaGetLastError());
+            p->launches++;
+            p->pink_next_t = 0;
+        } else if (t_begin != p->pink_next_t) {
+            return fail(p, GT_ERR_VALUE, "pink noise is a recurrence: expected t_begin = %lld (or 0), got %lld",
+                        (long long)p->pink_next_t, (long long)t_begin);
+        }
+    }
+    p->n_fused_last = 0;
+    const bool dev_out = is_device_ptr(out);
+    const bool dev_pwv = pwv_out ? is_device_ptr(pwv_out) : true;
+    if (pwv_out && dev_pwv != dev_out)
+        return fail(p, GT_ERR_VALUE, "tod_out and pwv_out must be the same kind of memory");
+    const int64_t chunk = p->chunk_samples;
+    const size_t row_floats = (size_t)p->n_spaxel * p->n_chan;
+    int slot = 0, k = 0;
+    for (int64_t t = t_begin; t < t_begin + t_count; t += chunk, ++k) {
+        const int64_t T = std::min(chunk, t_begin + t_count - t);
+        const size_t off = (size_t)(t - t_begin);
+        if (dev_out) {
+            gt_status s = run_chunk(p, t, T, out + off * row_floats, pwv_out ? pwv_out + off * p->n_spaxel : nullptr,
+                                    noise, st, k);
+            if (s != GT_OK) return s;
+        } else {
+            // double-buffered device chunk -> side-stream D2H, overlapped with the next chunk
+            if (!p->d_chunk[slot].p) GT_CUDA(p, p->d_chunk[slot].alloc((size_t)chunk * row_floats));
+            if (pwv_out && !p->d_pwv[slot].p) GT_CUDA(p, p->d_pwv[slot].alloc((size_t)chunk * p->n_spaxel));
+            GT_CUDA(p, cudaStreamWaitEvent(st, p->ev_copied[slot], 0));      // buffer free again?
+            gt_status s = run_chunk(p, t, T, p->d_chunk[slot].p, pwv_out ? p->d_pwv[slot].p : nullptr, noise, st, k);
+            if (s != GT_OK) return s;
+            GT_CUDA(p, cudaEventRecord(p->ev_ready[slot], st));
+            GT_CUDA(p, cudaStreamWaitEvent(p->copy_stream, p->ev_ready[slot], 0));
+            GT_CUDA(p, cudaMemcpyAsync(out + off * row_floats, p->d_chunk[slot].p, (size_t)T * row_floats * sizeof(float),
+                                       cudaMemcpyDeviceToHost, p->copy_stream));
+            if (pwv_out)
+                GT_CUDA(p, cudaMemcpyAsync(pwv_out + off * p->n_spaxel, p->d_pwv[slot].p,
+                                           (size_t)T * p->n_spaxel * sizeof(float), cudaMemcpyDeviceToHost, p->copy_stream));
+            GT_CUDA(p, cudaEventRecord(p->ev_copied[slot], p->copy_stream));
+            slot ^= 1;
+        }
+    }
+    if (pink) p->pink_next_t = t_begin + t_count;
+    if (!dev_out) GT_CUDA(p, cudaStreamSynchronize(p->copy_stream));
+    return GT_OK;
+}
+
+}  // namespace
+
+// =========================================================================================
+extern "C" {
+
+gt_status gt_plan_create(const gt_config* cfg, void* cuda_stream, gt_plan** out_plan) {
+    if (!out_plan) return fail(nullptr, GT_ERR_NULL, "out_plan is NULL");
+    *out_plan = nullptr;
+    if (gt_status s = validate(cfg)) return s;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        return fail(nullptr, GT_ERR_CUDA, "no CUDA device: libgateau_b200 has no CPU fallback");
+    }
+    const gt_config& c = *cfg;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+    gt_plan* p = new (std::nothrow) gt_plan();
+    if (!p) return fail(nullptr, GT_ERR_OOM, "host allocation failed");
+    struct Guard { gt_plan* p; ~Guard() { if (p) gt_plan_destroy(p); } } guard{p};
+#define GT_CUDA0(expr)                                                                              \
+    do { cudaError_t e_ = (expr);                                                                   \
+         if (e_ != cudaSuccess) return fail(nullptr, e_ == cudaErrorMemoryAllocation ? GT_ERR_OOM : GT_ERR_CUDA, \
+                                            "%s: %s", #expr, cudaGetErrorString(e_)); } while (0)
+    {
+        int dev = 0; cudaDeviceProp prop{};
+        GT_CUDA0(cudaGetDevice(&dev));
+        GT_CUDA0(cudaGetDeviceProperties(&prop, dev));
+        p->num_sms = prop.multiProcessorCount;
+        if (prop.major != 10) return fail(nullptr, GT_ERR_UNSUPPORTED, "built for sm_100a, device is sm_%d%d", prop.major, prop.minor);
+    }
+    GT_CUDA0(cudaStreamSynchronize(st));
+
+    const int nf = c.n_freq, nc = c.n_chan, ns = c.n_spaxel;
+    const int nfp = (nf + 31) / 32 * 32;
+    p->n_freq = nf; p->n_freq_pad = nfp; p->n_chan = nc; p->n_spaxel = ns; p->n_pwv = c.n_pwv;
+    p->n_samples = c.n_samples; p->photon_noise = c.photon_noise != 0; p->pink_noise = c.pink_noise != 0;
+    p->seed = c.seed; p->cube = c.cube; p->n_az = c.n_az; p->n_el = c.n_el;
+    p->variant = (c.variant == GT_VARIANT_TENSOR) ? GT_VARIANT_TENSOR : GT_VARIANT_FP32;   // DEFAULT -> FP32 until the tensor kernel is measured faster
+    p->scale = (float)(kPref * c.dnu_hz);
+
+    // ---- small device arrays needed on the host ----
+    std::vector<float> h_lut, h_filt, h_front;
+    if (gt_status s = fetch(c.atm_lut, (size_t)c.n_pwv * c.n_nu_lut, h_lut, "atm_lut")) return s;
+    if (gt_status s = fetch(c.filt, (size_t)nc * nf, h_filt, "filt")) return s;
+    if (c.eta_front_nu) if (gt_status s = fetch(c.eta_front_nu, nf, h_front, "eta_front_nu")) return s;
+    std::vector<std::vector<float>> h_stage(c.n_stage);
+    for (int k = 0; k < c.n_stage; ++k)
+        if (c.stages[k].eta_nu) if (gt_status s = fetch(c.stages[k].eta_nu, nf, h_stage[k], "stage eta_nu")) return s;
+    for (float v : h_front) if (!(v >= 0.f && v <= 1.f)) return fail(nullptr, GT_ERR_VALUE, "eta_front_nu outside [0,1]");
+    for (auto& hs : h_stage) for (float v : hs) if (!(v >= 0.f && v <= 1.f)) return fail(nullptr, GT_ERR_VALUE, "stage eta_nu outside [0,1]");
+    for (float v : h_lut) if (!(v > 0.f && v <= 1.f)) return fail(nullptr, GT_ERR_VALUE, "atm_lut outside (0,1]");
+
+    // ---- collapsed cascade, double precision ----
+    // P_final(nu) = eta_atm * (b1 + a*S) + b0 after Eq. 11 and Eq. 12 for k = 0..n_stage:
+    //   after the atmosphere:  a = eta_front, b1 = B_cmb - B_atm, b0 = B_atm
+    //   plain stage k:         a *= eta_k; b1 *= eta_k; b0 = eta_k b0 + (1-eta_k) B(T_k)
+    //   coupled stage k:       a *= eta_k; b1 = eta_k b1 + (1-eta_k)(B_cmb - B_atm); b0 = eta_k b0 + (1-eta_k) B_atm
+    // With eps = 1 - eta_atm:  P_final = eps*(-b1) + eta_atm*(a*S) + (b0 + b1);  all three terms >= 0.
+    std::vector<float> Xn(nfp, 0.f), Gs(nfp, 0.f);
+    std::vector<double> Y(nf);
+    for (int i = 0; i < nf; ++i) {
+        const double nu = c.nu0_hz + (double)i * c.dnu_hz;
+        const double Bc = jn_power(nu, c.T_cmb_K), Ba = jn_power(nu, c.T_atm_K);
+        double a = c.eta_front_nu ? (double)h_front[i] : 1.0, b1 = Bc - Ba, b0 = Ba;
+        for (int k = 0; k < c.n_stage; ++k) {
+            const gt_stage& s = c.stages[k];
+            const double e = s.eta_nu ? (double)h_stage[k][i] : s.eta_scalar;
+            a *= e;
+            if (s.couple_atmosphere) { b1 = e * b1 + (1.0 - e) * (Bc - Ba); b0 = e * b0 + (1.0 - e) * Ba; }
+            else                     { b1 = e * b1;                         b0 = e * b0 + (1.0 - e) * jn_power(nu, s.T_K); }
+        }
+        Xn[i] = (float)(-b1 / kPref);
+        Gs[i] = (float)(a / kPref);
+        Y[i] = b0 + b1;
+    }
+
+    // ---- LUT resampled on the frequency grid (bilinear is separable, R14) ----
+    std::vector<float> lut_r((size_t)c.n_pwv * nfp, 1.0f);
+    for (int i = 0; i < nf; ++i) {
+        const double nu = c.nu0_hz + (double)i * c.dnu_hz;
+        const double r = (nu - c.lut_nu0_hz) / c.lut_dnu_hz;
+        long ir = (long)std::floor(r);
+        if (ir > c.n_nu_lut - 2) ir = c.n_nu_lut - 2;
+        if (ir < 0) ir = 0;
+        const double fr = r - (double)ir;
+        for (int q = 0; q < c.n_pwv; ++q) {
+            const double L0 = h_lut[(size_t)q * c.n_nu_lut + ir], L1 = h_lut[(size_t)q * c.n_nu_lut + ir + 1];
+            lut_r[(size_t)q * nfp + i] = (float)((1.0 - fr) * L0 + fr * L1);
+        }
+    }
+
+    // ---- filter: transposed/padded copy (FP32 variant), per-channel constants ----
+    const int tn = fp32_tn(nc);
+    const int ncp = ((nc + 32 * tn - 1) / (32 * tn)) * 32 * tn;
+    p->n_chan_pad = ncp;
+    std::vector<float> bias(ncp, 0.f), c1(ncp, 0.f), c2(ncp, 0.f);
+    for (int ch = 0; ch < nc; ++ch) {
+        double sb = 0.0, s1 = 0.0, s2 = 0.0;
+        for (int i = 0; i < nf; ++i) {
+            const double f = h_filt[(size_t)ch * nf + i];
+            sb += f * Y[i]; s1 += f * c.dnu_hz; s2 += f * f * c.dnu_hz;
+        }
+        bias[ch] = (float)(c.dnu_hz * sb);
+        const double dnu_c = c.dnu_eff_hz ? c.dnu_eff_hz[ch] : (s2 > 0 ? s1 * s1 / s2 : 1.0);
+        if (!(dnu_c > 0)) return fail(nullptr, GT_ERR_VALUE, "dnu_eff[%d] is not positive", ch);
+        c1[ch] = (float)(kH * c.f_center_hz[ch] * c.f_sample_hz);
+        c2[ch] = (float)(c.f_sample_hz / dnu_c);
+    }
+    if (p->variant == GT_VARIANT_FP32) {
+        std::vector<float> ft((size_t)nfp * ncp, 0.f);
+        for (int ch = 0; ch < nc; ++ch)
+            for (int i = 0; i < nf; ++i) ft[(size_t)i * ncp + ch] = h_filt[(size_t)ch * nf + i];
+        GT_CUDA0(p->d_filt_t.upload(ft, st));
+        GT_CUDA0(cudaStreamSynchronize(st));
+    } else {
+        if (gt_status s = gt::build_tc_tables(h_filt, nc, nf, nfp, p->tc, st)) {
+            return fail(nullptr, s, "tensor variant: %s", gt::tc_error());
+        }
+    }
+    GT_CUDA0(p->d_Xn.upload(Xn, st)); GT_CUDA0(p->d_Gs.upload(Gs, st)); GT_CUDA0(p->d_lut_r.upload(lut_r, st));
+    GT_CUDA0(p->d_bias.upload(bias, st)); GT_CUDA0(p->d_c1.upload(c1, st)); GT_CUDA0(p->d_c2.upload(c2, st));
+
+    // ---- geometry tables: per-sample and per-spaxel transcendental inputs from the host libm ----
+    {
+        const int64_t nt = c.n_samples;
+        std::vector<double> ta(nt), te(nt), sE(nt), cE(nt), az(c.az_rad, c.az_rad + nt), el(c.el_rad, c.el_rad + nt);
+        for (int64_t n = 0; n < nt; ++n) {
+            ta[n] = std::tan(c.az_rad[n]); te[n] = std::tan(c.el_rad[n]);
+            const double E = c.el0_rad + c.el_rad[n];
+            sE[n] = std::sin(E); cE[n] = std::cos(E);
+        }
+        GT_CUDA0(p->d_tan_az.upload(ta, st)); GT_CUDA0(p->d_tan_el.upload(te, st));
+        GT_CUDA0(p->d_sinE.upload(sE, st)); GT_CUDA0(p->d_cosE.upload(cE, st));
+        GT_CUDA0(p->d_az.upload(az, st)); GT_CUDA0(p->d_el.upload(el, st));
+        std::vector<double> sp((size_t)6 * ns);
+        for (int s = 0; s < ns; ++s) {
+            sp[0 * ns + s] = std::tan(c.daz_rad[s]); sp[1 * ns + s] = std::tan(c.del_rad[s]);
+            sp[2 * ns + s] = std::sin(c.del_rad[s]); sp[3 * ns + s] = std::cos(c.del_rad[s]);
+            sp[4 * ns + s] = c.daz_rad[s];           sp[5 * ns + s] = c.del_rad[s];
+        }
+        GT_CUDA0(p->d_sp.upload(sp, st));
+        GT_CUDA0(cudaStreamSynchronize(st));       // host vectors go out of scope
+        gt::GeoParams& g = p->geo;
+        g.tan_az = p->d_tan_az.p; g.tan_el = p->d_tan_el.p; g.sinE = p->d_sinE.p; g.cosE = p->d_cosE.p;
+        g.az = p->d_az.p; g.el = p->d_el.p;
+        g.tan_daz = p->d_sp.p; g.tan_del = p->d_sp.p + ns; g.sin_del = p->d_sp.p + 2 * ns;
+        g.cos_del = p->d_sp.p + 3 * ns; g.daz = p->d_sp.p + 4 * ns; g.del = p->d_sp.p + 5 * ns;
+        g.n_spaxel = ns; g.f_sample = c.f_sample_hz;
+        g.screen = c.screen; g.nx = c.nx; g.ny = c.ny; g.dx = c.dx_m; g.dy = c.dy_m;
+        g.h_col = c.h_column_m; g.wind = c.wind_mps; g.pwv0_a = c.pwv0_a_mm; g.pwv0_b = c.pwv0_b_mm_per_s;
+        g.n_pwv = c.n_pwv; g.lut_pwv0 = c.lut_pwv0_mm; g.lut_dpwv = c.lut_dpwv_mm;
+        g.has_cube = c.cube != nullptr; g.n_az = c.n_az; g.n_el = c.n_el;
+        g.az_min = c.az_min_rad; g.daz_grid = c.daz_grid_rad; g.el_min = c.el_min_rad; g.del_grid = c.del_grid_rad;
+    }
+
+    // ---- pink-noise coefficients (R18) ----
+    if (p->pink_noise) {
+        const int J = c.pink_n_stage;
+        p->J = J;
+        gt::PinkParams& k = p->pink;
+        k.J = J; k.n_chan = nc; k.n_det = (int64_t)ns * nc;
+        k.seed_lo = (uint32_t)(c.seed & 0xffffffffu); k.seed_hi = (uint32_t)(c.seed >> 32);
+        double lnrho = 1.0;
+        if (J >= 2) lnrho = std::log(c.pink_f_corner_hz[0] / c.pink_f_corner_hz[J - 1]) / (double)(J - 1);
+        for (int j = 0; j < gt::kPinkMaxJ; ++j) { k.phi[j] = 0.f; k.sq[j] = 0.f; }
+        for (int j = 0; j < J; ++j) {
+            if (!(c.pink_f_corner_hz[j] > 0)) return fail(nullptr, GT_ERR_VALUE, "pink corner frequency must be positive");
+            const double phi = std::exp(-2.0 * kPi * c.pink_f_corner_hz[j] / c.f_sample_hz);
+            k.phi[j] = (float)phi; k.sq[j] = (float)std::sqrt(1.0 - phi * phi);
+        }
+        std::vector<float> gain((size_t)k.n_det * J);
+        for (int64_t d = 0; d < k.n_det; ++d)
+            for (int j = 0; j < J; ++j) {
+                const double A = c.pink_A[d], al = c.pink_alpha[d], fj = c.pink_f_corner_hz[j];
+                const double g2 = A * lnrho * std::sin(kPi * al / 2.0) * std::pow(fj, 1.0 - al);
+                if (!(g2 >= 0)) return fail(nullptr, GT_ERR_VALUE, "pink noise level of detector %lld is invalid", (long long)d);
+                gain[(size_t)d * J + j] = (float)std::sqrt(g2);
+            }
+        GT_CUDA0(p->d_gain.upload(gain, st));
+        GT_CUDA0(p->d_state.alloc((size_t)k.n_det * J));
+        GT_CUDA0(cudaStreamSynchronize(st));
+        k.gain = p->d_gain.p; k.state = p->d_state.p; k.seg = nullptr;
+    }
+
+    // ---- chunking and streams ----
+    {
+        const double bytes_per_sample = (double)ns * nc * sizeof(float);
+        int64_t chunk = c.chunk_samples > 0 ? c.chunk_samples
+                                            : (int64_t)std::max(1.0, std::floor(512.0 * 1048576.0 / bytes_per_sample));
+        chunk = std::min(chunk, c.n_samples);
+        if (c.chunk_samples == 0 && chunk > gt::kPinkSeg) chunk = chunk / gt::kPinkSeg * gt::kPinkSeg;
+        p->chunk_samples = chunk;
+        GT_CUDA0(p->d_rows.alloc((size_t)chunk * ns));
+        GT_CUDA0(cudaStreamCreateWithFlags(&p->copy_stream, cudaStreamNonBlocking));
+        for (int i = 0; i < 2; ++i) {
+            GT_CUDA0(cudaEventCreateWithFlags(&p->ev_ready[i], cudaEventDisableTiming));
+            GT_CUDA0(cudaEventCreateWithFlags(&p->ev_copied[i], cudaEventDisableTiming));
+        }
+    }
+    GT_CUDA0(cudaStreamSynchronize(st));
+    guard.p = nullptr;
+    *out_plan = p;
+    return GT_OK;
+}
+
+gt_status gt_simulate(gt_plan* plan, int64_t t_begin, int64_t t_count, float* tod_out, float* pwv_out,
+                      void* cuda_stream) {
+    return simulate_impl(plan, t_begin, t_count, tod_out, pwv_out, true, reinterpret_cast<cudaStream_t>(cuda_stream));
+}
+
+gt_status gt_debug_pkid(gt_plan* plan, int64_t t_begin, int64_t t_count, float* pkid_out, void* cuda_stream) {
+    return simulate_impl(plan, t_begin, t_count, pkid_out, nullptr, false, reinterpret_cast<cudaStream_t>(cuda_stream));
+}
+
+gt_status gt_plan_destroy(gt_plan* plan) {
+    if (!plan) return GT_OK;
+    cudaDeviceSynchronize();
+    if (plan->copy_stream) cudaStreamDestroy(plan->copy_stream);
+    for (int i = 0; i < 2; ++i) {
+        if (plan->ev_ready[i]) cudaEventDestroy(plan->ev_ready[i]);
+        if (plan->ev_copied[i]) cudaEventDestroy(plan->ev_copied[i]);
+    }
+    for (cudaEvent_t e : plan->ev_fused) cudaEventDestroy(e);
+    gt::free_tc_tables(plan->tc);
+    delete plan;
+    return GT_OK;
+}
+
+const char* gt_last_error(const gt_plan* plan) {
+    return plan ? plan->error.c_str() : g_create_error.c_str();
+}
+
+gt_status gt_debug_geometry(gt_plan* plan, int64_t t_begin, int64_t t_count, gt_georec* host_records_out) {
+    gt_plan* p = plan;
+    if (!p) return fail(nullptr, GT_ERR_NULL, "plan is NULL");
+    if (!host_records_out) return fail(p, GT_ERR_NULL, "host_records_out is NULL");
+    if (t_begin < 0 || t_count < 0 || t_begin + t_count > p->n_samples) return fail(p, GT_ERR_RANGE, "sample range outside the plan");
+    const int64_t n_rows = t_count * p->n_spaxel;
+    if (n_rows == 0) return GT_OK;
+    DevBuf<gt_georec> rec;
+    GT_CUDA(p, rec.alloc((size_t)n_rows));
+    gt::geometry_kernel<<<(unsigned)((n_rows + 255) / 256), 256>>>(p->geo, t_begin, n_rows, nullptr, nullptr, rec.p);
+    GT_CUDA(p, cudaGetLastError());
+    p->launches++;
+    GT_CUDA(p, cudaMemcpy(host_records_out, rec.p, (size_t)n_rows * sizeof(gt_georec), cudaMemcpyDeviceToHost));
+    return GT_OK;
+}
+
+__global__ void debug_philox_kernel(uint32_t k0, uint32_t k1, uint32_t c0_begin, int64_t count,
+                                    uint32_t c1, uint32_t c2, uint32_t c3, uint4* out) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < count) out[i] = gt::philox4x32_10(c0_begin + (uint32_t)i, c1, c2, c3, k0, k1);
+}
+
+gt_status gt_debug_philox(uint64_t seed, uint32_t c0_begin, int64_t count, uint32_t c1, uint32_t c2, uint32_t c3,
+                          uint32_t* host_out_words) {
+    if (!host_out_words) return fail(nullptr, GT_ERR_NULL, "host_out_words is NULL");
+    if (count < 0) return fail(nullptr, GT_ERR_SHAPE, "count is negative");
+    if (count == 0) return GT_OK;
+    DevBuf<uint4> out;
+    GT_CUDA(nullptr, out.alloc((size_t)count));
+    debug_philox_kernel<<<(unsigned)((count + 255) / 256), 256>>>((uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32),
+                                                                  c0_begin, count, c1, c2, c3, out.p);
+    GT_CUDA(nullptr, cudaGetLastError());
+    GT_CUDA(nullptr, cudaMemcpy(host_out_words, out.p, (size_t)count * sizeof(uint4), cudaMemcpyDeviceToHost));
+    return GT_OK;
+}
+
+int64_t gt_launch_count(const gt_plan* plan) { return plan ? plan->launches : 0; }
+
+const char* gt_variant_name(const gt_plan* plan) {
+    if (!plan) return "";
+    return plan->variant == GT_VARIANT_FP32 ? "fp32-ffma" : "tcgen05-3xtf32";
+}
+
+double gt_last_fused_ms(gt_plan* plan, int32_t* n_launches) {
+    if (n_launches) *n_launches = 0;
+    if (!plan || plan->n_fused_last == 0) return 0.0;
+    double total = 0.0;
+    for (int i = 0; i < plan->n_fused_last; ++i) {
+        if (cudaEventSynchronize(plan->ev_fused[2 * i + 1]) != cudaSuccess) return -1.0;
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, plan->ev_fused[2 * i], plan->ev_fused[2 * i + 1]) != cudaSuccess) return -1.0;
+        total += ms;
+    }
+    if (n_launches) *n_launches = plan->n_fused_last;
+    return total;
+}
+
+}  // extern "C"

@@ -1,0 +1,66 @@
+// gt_common.cuh -- shared device-side definitions of the CUDA path (libgateau_b200.so).
+// Shares nothing with oracle/: the constants and the Philox rounds below are restated from
+// PAPER.md / DESIGN.md for the device.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace gt {
+
+// ---- per-row record handed from the geometry kernel to the fused kernel (32 B) --------
+struct __align__(16) RowParam {
+    float fp;          // LUT fraction in PWV
+    float csc;         // airmass 1/sin(E), Eq. 10
+    int32_t ip;        // lower LUT row
+    int32_t pix;       // source pixel index jv*n_az + ju of the lower-left tap, -1 = outside (S = 0)
+    float w00, w01, w10, w11;   // bilinear source weights (jv,ju) (jv,ju+1) (jv+1,ju) (jv+1,ju+1)
+};
+static_assert(sizeof(RowParam) == 32, "RowParam must be 32 bytes");
+
+// ---- Philox4x32-10 (Salmon et al. SC'11; R19) --------------------------------
+// counter = (c0 = sample n, c1 = spaxel, c2 = channel, c3 = stream), key = 64-bit seed.
+constexpr uint32_t kPhiloxM0 = 0xD2511F53u, kPhiloxM1 = 0xCD9E8D57u;
+constexpr uint32_t kPhiloxW0 = 0x9E3779B9u, kPhiloxW1 = 0xBB67AE85u;
+constexpr uint32_t kStreamPhoton = 0u, kStreamPinkLo = 1u, kStreamPinkHi = 2u;
+constexpr uint32_t kCounterInit = 0xFFFFFFFFu;
+
+__device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                               uint32_t k0, uint32_t k1) {
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t hi0 = __umulhi(kPhiloxM0, c0), lo0 = kPhiloxM0 * c0;
+        const uint32_t hi1 = __umulhi(kPhiloxM1, c2), lo1 = kPhiloxM1 * c2;
+        const uint32_t n0 = hi1 ^ c1 ^ k0;
+        const uint32_t n2 = hi0 ^ c3 ^ k1;
+        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+        k0 += kPhiloxW0; k1 += kPhiloxW1;
+    }
+    return make_uint4(c0, c1, c2, c3);
+}
+
+// U(w) = ((w >> 9) + 1/2) 2^-23 in (0,1): exact in fp32 (R19).
+__device__ __forceinline__ float uniform01(uint32_t w) {
+    return ((float)(w >> 9) + 0.5f) * (1.0f / 8388608.0f);
+}
+
+// Box-Muller: z0 = sqrt(-2 ln U(w0)) cos(2 pi U(w1)), z1 = ... sin(...).  MUFU log/sin/cos: the
+// normals only need ~1e-3 absolute accuracy for the 2e-5 TOD gate (sigma/P ~ 1e-3).
+__device__ __forceinline__ float normal_cos(uint32_t w0, uint32_t w1) {
+    const float r = sqrtf(-2.0f * __logf(uniform01(w0)));
+    return r * __cosf(6.28318530717958647692f * uniform01(w1));
+}
+__device__ __forceinline__ void normal_pair(uint32_t w0, uint32_t w1, float& z0, float& z1) {
+    const float r = sqrtf(-2.0f * __logf(uniform01(w0)));
+    float s, c;
+    __sincosf(6.28318530717958647692f * uniform01(w1), &s, &c);
+    z0 = r * c; z1 = r * s;
+}
+
+// sigma of Eq. 18 in north_star's narrow-band form (R17):
+// sigma^2 = (2 h f_c P + 2 P^2 / dnu_c) f_s / 2 = P (c1 + P c2), c1 = h f_c f_s, c2 = f_s / dnu_c.
+__device__ __forceinline__ float photon_sigma(float P, float c1, float c2) {
+    const float v = P * (c1 + P * c2);
+    return v > 0.0f ? sqrtf(v) : 0.0f;
+}
+
+}  // namespace gt

@@ -1,0 +1,256 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element
+on the same seeded inputs.
+
+Gates (BASELINE.json north_star): geometry integers and Philox words bit-exact; noiseless
+channel power max relative error <= 1e-5; noisy TOD <= 2e-5 relative to
+max(|oracle|, 1e-3 * median|oracle|).
+"""
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+from paper_2604_23305_b200 import binding as B
+from paper_2604_23305_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL_PKID = 1e-5
+TOL_TOD = 2e-5
+VARIANTS = [B.VARIANT_FP32, B.VARIANT_TENSOR]
+VARIANT_IDS = ["fp32", "tensor"]
+
+
+def rel_err(got, ref):
+    ref = np.asarray(ref, dtype=np.float64)
+    got = np.asarray(got, dtype=np.float64)
+    floor = 1e-3 * np.median(np.abs(ref))
+    return np.max(np.abs(got - ref) / np.maximum(np.abs(ref), floor))
+
+
+def _plan(w, variant, **kw):
+    try:
+        return B.Plan(w, variant=variant, **kw)
+    except B.GateauError as e:
+        if e.status == 7:
+            pytest.skip(f"variant not available: {e}")
+        raise
+
+
+# --------------------------------------------------------------------------------------
+# bit-exact integer work
+# --------------------------------------------------------------------------------------
+def test_philox_words_bit_exact():
+    for seed, c0, c1, c2, c3 in [(0, 0, 0, 0, 0), (0x0123456789ABCDEF, 4294967290, 60, 346, 2), (3, 12345, 7, 11, 1)]:
+        got = B.debug_philox(seed, c0, 64, c1, c2, c3)
+        key = (seed & 0xffffffff, seed >> 32)
+        for i in range(64):
+            assert list(got[i]) == O.philox4x32_10(((c0 + i) & 0xffffffff, c1, c2, c3), key)
+
+
+INT_FIELDS = ("n", "iu0", "iv0", "ju", "jv", "ip")
+FRAC_FIELDS = ("fu", "fv", "gu", "gv", "fp", "csc", "pwv_mm")
+
+
+def _check_geometry(w, t_begin=0, t_count=None):
+    with B.Plan(w, variant=B.VARIANT_FP32) as p:
+        got = p.geometry(t_begin, t_count)
+    ref = O.Oracle(w).geometry(t_begin, t_count)
+    for f in INT_FIELDS:
+        assert np.array_equal(got[f], ref[f]), f"geometry field {f} differs"
+    for f in FRAC_FIELDS:
+        assert np.array_equal(got[f], ref[f]), f"geometry field {f} is not bit-identical"
+
+
+@pytest.mark.parametrize("seed", [1, 2])
+def test_geometry_bit_exact_random(seed):
+    _check_geometry(W.random_workload(seed, n_samples=700, n_spaxel=5))
+
+
+def test_geometry_bit_exact_C1():
+    _check_geometry(W.make_workload("C1"))
+
+
+def test_geometry_bit_exact_C5_window_late_in_the_scan():
+    # wind drift has carried the boresight 3.4e5 screen cells away; PWV drifts through LUT rows
+    w = W.make_workload("C5", n_chan=8, n_freq=64, cube_n=9, screen_n=512)
+    _check_geometry(w, t_begin=w.n_samples - 3000, t_count=3000)
+
+
+# --------------------------------------------------------------------------------------
+# noiseless channel power (steps 0-5)
+# --------------------------------------------------------------------------------------
+@pytest.mark.parametrize("variant", VARIANTS, ids=VARIANT_IDS)
+@pytest.mark.parametrize("seed,kw", [
+    (11, dict(n_samples=67, n_spaxel=3, n_chan=24, n_freq=96)),               # ragged row tile
+    (12, dict(n_samples=150, n_spaxel=2, n_chan=70, n_freq=333, n_stage=6)),  # ragged everything
+    (13, dict(n_samples=40, n_spaxel=7, n_chan=347, n_freq=530)),             # full channel width
+    (14, dict(n_samples=33, n_spaxel=1, n_chan=5, n_freq=17, with_cube=False)),
+])
+def test_pkid_random(variant, seed, kw):
+    w = W.random_workload(seed, **kw)
+    ref = O.Oracle(w).simulate(want=("pkid", "pwv"))
+    with _plan(w, variant) as p:
+        got = p.pkid().cpu().numpy()
+        tod, pwv = p.simulate(want_pwv=True)
+    assert rel_err(got, ref["pkid"]) <= TOL_PKID
+    assert np.array_equal(tod.cpu().numpy(), got)           # noise off => TOD is the noiseless power
+    assert np.max(np.abs(pwv.cpu().numpy() - ref["pwv"])) <= 1e-6
+
+
+@pytest.mark.parametrize("variant", VARIANTS, ids=VARIANT_IDS)
+def test_pkid_C1_full(variant):
+    w = W.make_workload("C1")
+    ref = O.Oracle(w).simulate(want=("pkid",))["pkid"]
+    with _plan(w, variant) as p:
+        got = p.pkid().cpu().numpy()
+    assert rel_err(got, ref) <= TOL_PKID
+
+
+@pytest.mark.parametrize("variant", VARIANTS, ids=VARIANT_IDS)
+@pytest.mark.parametrize("cfg", ["C2", "C3", "C4", "C5"])
+def test_pkid_configs_window(variant, cfg):
+    """Full channel/frequency sizes of each config, several row tiles and a ragged tail."""
+    w = W.make_workload(cfg, n_samples=4000 if cfg == "C2" else 2000, screen_n=1024,
+                        photon_noise=False, pink_noise=False)
+    t0, T = w.n_samples - 333, 333 // w.n_spaxel + 3
+    ref = O.Oracle(w).simulate(t0, T, want=("pkid",))["pkid"]
+    with _plan(w, variant) as p:
+        got = p.pkid(t0, T).cpu().numpy()
+    assert rel_err(got, ref) <= TOL_PKID
+
+
+# --------------------------------------------------------------------------------------
+# invariants that hold at any size, through the CUDA path
+# --------------------------------------------------------------------------------------
+@pytest.mark.parametrize("variant", VARIANTS, ids=VARIANT_IDS)
+def test_thermal_equilibrium_on_gpu(variant):
+    """All temperatures equal T and no source => P_final = B(nu, T) whatever the etas (Eq. 12)."""
+    T = 77.0
+    w = W.random_workload(21, n_samples=50, n_spaxel=2, n_chan=40, n_freq=200, with_cube=False)
+    for s in w.stages:
+        s.T_K = T
+    w = w.replace(T_cmb_K=T, T_atm_K=T)
+    h, kb = 6.62607015e-34, 1.380649e-23
+    Bnu = h * w.nu_hz / np.expm1(h * w.nu_hz / (kb * T))
+    expect = w.dnu_hz * (w.filt.astype(np.float64) @ Bnu)
+    with _plan(w, variant) as p:
+        got = p.pkid().cpu().numpy()
+    assert rel_err(got, np.broadcast_to(expect, got.shape)) <= TOL_PKID
+
+
+# --------------------------------------------------------------------------------------
+# noise (steps 6a, 6b) and Eq. 21
+# --------------------------------------------------------------------------------------
+@pytest.mark.parametrize("variant", VARIANTS, ids=VARIANT_IDS)
+def test_tod_photon_noise(variant):
+    w = W.random_workload(31, n_samples=130, n_spaxel=3, n_chan=50, n_freq=128, photon_noise=True)
+    ref = O.Oracle(w).simulate(want=("tod", "pkid"))
+    with _plan(w, variant) as p:
+        got = p.simulate().cpu().numpy()
+    assert rel_err(got, ref["tod"]) <= TOL_TOD
+    assert np.std(got - ref["pkid"]) > 0                    # the noise is really there
+
+
+@pytest.mark.parametrize("variant", VARIANTS, ids=VARIANT_IDS)
+@pytest.mark.parametrize("J", [1, 4, 6])
+def test_tod_photon_and_pink_noise(variant, J):
+    w = W.random_workload(40 + J, n_samples=300, n_spaxel=2, n_chan=33, n_freq=64, photon_noise=True,
+                          pink_noise=True, J=J)
+    ref = O.Oracle(w).simulate(want=("tod",))["tod"]
+    with _plan(w, variant) as p:
+        got = p.simulate().cpu().numpy()
+    assert rel_err(got, ref) <= TOL_TOD
+
+
+def test_pink_noise_is_carried_across_calls_and_chunks():
+    """Contiguous calls continue the AR(1) state; chunked host streaming gives the same values."""
+    w = W.random_workload(51, n_samples=1000, n_spaxel=2, n_chan=20, n_freq=48, photon_noise=True, pink_noise=True)
+    ref = O.Oracle(w).simulate(want=("tod",))["tod"]
+    with B.Plan(w, variant=B.VARIANT_FP32, chunk_samples=97) as p:
+        whole = p.simulate().cpu().numpy()
+        parts = np.concatenate([p.simulate(0, 333).cpu().numpy(), p.simulate(333, 500).cpu().numpy(),
+                                p.simulate(833, 167).cpu().numpy()])
+        host = p.simulate(device_out=False).numpy()
+        with pytest.raises(B.GateauError) as ei:
+            p.simulate(500, 10)                               # out of order with pink noise on
+        assert ei.value.status == 3
+    assert rel_err(whole, ref) <= TOL_TOD
+    assert rel_err(parts, ref) <= TOL_TOD
+    assert np.array_equal(host, whole)
+
+
+def test_pink_only_series_matches_oracle_tightly():
+    """TOD minus noiseless power with photon noise off isolates P_pn."""
+    w = W.random_workload(52, n_samples=2000, n_spaxel=1, n_chan=16, n_freq=32, pink_noise=True)
+    o = O.Oracle(w)
+    ref = o.pink_series(np.zeros(16, dtype=np.int32), np.arange(16, dtype=np.int32), 0, w.n_samples)   # [det][t]
+    base = o.simulate(want=("pkid",))["pkid"][:, 0, :]
+    with B.Plan(w, variant=B.VARIANT_FP32) as p:
+        got = p.simulate().cpu().numpy()[:, 0, :].astype(np.float64)
+    pn = (got - base).T
+    scale = np.std(ref)
+    # fp32 TOD rounding (|P| * 6e-8) dominates; the series itself must agree to ~1e-3 of its rms
+    assert np.max(np.abs(pn - ref)) <= 2e-3 * scale + 2e-7 * np.max(np.abs(base))
+
+
+# --------------------------------------------------------------------------------------
+# boundary behaviour
+# --------------------------------------------------------------------------------------
+def test_host_streaming_equals_device_output_and_pwv():
+    w = W.random_workload(61, n_samples=500, n_spaxel=3, n_chan=40, n_freq=64, photon_noise=True)
+    with B.Plan(w, variant=B.VARIANT_FP32, chunk_samples=64) as p:
+        dev, pwv_d = p.simulate(want_pwv=True)
+        host, pwv_h = p.simulate(device_out=False, want_pwv=True)
+        pageable = np.empty((w.n_samples, w.n_spaxel, w.n_chan), dtype=np.float32)
+        p.simulate(out=pageable)
+        sub = p.simulate(123, 200).cpu().numpy()              # photon noise only: any range is legal
+    assert np.array_equal(dev.cpu().numpy(), host.numpy())
+    assert np.array_equal(dev.cpu().numpy(), pageable)
+    assert np.array_equal(pwv_d.cpu().numpy(), pwv_h.numpy())
+    assert np.array_equal(sub, dev.cpu().numpy()[123:323])
+
+
+def test_empty_and_out_of_range_calls():
+    w = W.random_workload(62, n_samples=16)
+    with B.Plan(w, variant=B.VARIANT_FP32) as p:
+        out = p.simulate(0, 0)
+        assert out.shape[0] == 0
+        with pytest.raises(B.GateauError) as ei:
+            p.simulate(10, 7)
+        assert ei.value.status == 4
+        assert p.launch_count == 0
+
+
+def test_rows_outside_the_cube_are_blank_sky():
+    """A scan that leaves the cube returns exactly the blank-sky value."""
+    w = W.random_workload(63, n_samples=64, n_spaxel=1, n_chan=12, n_freq=40)
+    far = w.replace(az_rad=w.az_rad + 1e-2)                   # ~2000 arcsec away: every row outside
+    blank = w.replace(cube=None)
+    with B.Plan(far, variant=B.VARIANT_FP32) as p1, B.Plan(blank, variant=B.VARIANT_FP32) as p2:
+        g = p1.geometry()
+        assert np.all(g["ju"] == -1)
+        a = p1.pkid().cpu().numpy()
+        # same geometry except the pointing offset changes the screen position: compare with the oracle instead
+    ref = O.Oracle(far).simulate(want=("pkid",))["pkid"]
+    assert rel_err(a, ref) <= TOL_PKID
+
+
+# --------------------------------------------------------------------------------------
+# full-size configuration, sampled
+# --------------------------------------------------------------------------------------
+def test_C2_full_size_sampled_rows():
+    """BASELINE.json configs[1] at full size in the launch configuration bench.py uses,
+    checked on sampled rows the oracle computes one by one."""
+    w = W.make_workload("C2", photon_noise=True)
+    rng = np.random.default_rng(5)
+    t_idx = np.sort(rng.choice(w.n_samples, 96, replace=False)).astype(np.int64)
+    t_idx[:4] = [0, 1, w.n_samples - 2, w.n_samples - 1]
+    s_idx = np.zeros_like(t_idx, dtype=np.int32)
+    pk, wn = O.Oracle(w).simulate_rows(t_idx, s_idx, noise=True)
+    with B.Plan(w) as p:
+        tod = p.simulate()
+        pkid = p.pkid()
+        got_t = tod[t_idx].cpu().numpy()[:, 0, :]
+        got_p = pkid[t_idx].cpu().numpy()[:, 0, :]
+    assert rel_err(got_p, pk) <= TOL_PKID
+    assert rel_err(got_t, pk + wn) <= TOL_TOD
