@@ -112,7 +112,8 @@ def test_pkid_configs_window(variant, cfg):
     """Full channel/frequency sizes of each config, several row tiles and a ragged tail."""
     w = W.make_workload(cfg, n_samples=4000 if cfg == "C2" else 2000, screen_n=1024,
                         photon_noise=False, pink_noise=False)
-    t0, T = w.n_samples - 333, 333 // w.n_spaxel + 3
+    T = 333 // w.n_spaxel + 3
+    t0 = w.n_samples - T
     ref = O.Oracle(w).simulate(t0, T, want=("pkid",))["pkid"]
     with _plan(w, variant) as p:
         got = p.pkid(t0, T).cpu().numpy()
