@@ -10,6 +10,7 @@
 #include <cstdio>
 #include <cstdarg>
 #include <cstring>
+#include <cstdlib>
 #include <string>
 #include <vector>
 #include <new>
@@ -409,6 +410,11 @@ gt_status gt_plan_create(const gt_config* cfg, void* cuda_stream, gt_plan** out_
     } else {
         if (gt_status s = gt::build_tc_tables(h_filt, nc, nf, nfp, p->tc, st)) {
             return fail(nullptr, s, "tensor variant: %s", gt::tc_error());
+        }
+        if (gt_status s = gt::alloc_tc_scratch(p->tc, p->num_sms)) return fail(nullptr, s, "tensor variant: %s", gt::tc_error());
+        if (const char* e = std::getenv("GATEAU_TC_SEG")) {          // tuning/diagnostic knob: slabs per accumulation segment
+            const int v = std::atoi(e);
+            if (v > 0) p->tc.seg = v;
         }
     }
     GT_CUDA0(p->d_Xn.upload(Xn, st)); GT_CUDA0(p->d_Gs.upload(Gs, st)); GT_CUDA0(p->d_lut_r.upload(lut_r, st));

@@ -9,15 +9,23 @@
 //                           tf32 hi + lo -> shared memory in the UMMA K-major SWIZZLE_128B layout
 //   loader warp (1 lane)  : filter slab images (hi, lo; pre-split, pre-swizzled at plan time)
 //                           global -> shared by cp.async.bulk, mbarrier complete_tx
-//   MMA warp (1 lane)     : tcgen05.mma.kind::tf32, M = 128, N = NB (<= 256), K = 8:
+//   MMA warp (1 lane)     : tcgen05.mma.kind::tf32, M = 128, N <= 128 per column group, K = 8:
 //                           acc += A_hi.B_hi + A_lo.B_hi + A_hi.B_lo     ("3xTF32", fp32 accumulate
 //                           in tensor memory; the dropped A_lo.B_lo term is ~2^-22 relative)
-//   epilogue warps (4)    : tcgen05.ld the accumulators, P = acc*scale + bias[c] -> TOD, release
-//                           the accumulators, then add the photon noise (Eq. 18-19) in a
-//                           coalesced second pass that overlaps the next tile's main loop.
+//   epilogue warps (4)    : SEGMENTED ACCUMULATION.  The tensor core's fp32 accumulate truncates
+//                           (measured: -2.7e-5 relative after 500 chained MMAs of positive terms,
+//                           DESIGN.md "Accumulation in tensor memory"), so no accumulator lives
+//                           longer than `seg` slabs: the <= 384 padded channels of a tile are cut
+//                           into <= 3 column groups of <= 128 columns that rotate through FOUR
+//                           128-column tensor-memory buffers; at a (staggered) segment boundary a
+//                           group moves to the spare buffer and the epilogue warps add the
+//                           finished partial sums (tcgen05.ld) into a per-CTA, L2-resident fp32
+//                           scratch tile [column][row] with round-to-nearest FADDs.  After the
+//                           last segment they transpose the scratch tile into the TOD:
+//                           P = sum*scale + bias[c], photon noise (Eq. 18-19), coalesced stores.
 //
-// Pipelines: A ring (2 stages, generator -> MMA), B ring (NBS units, loader -> MMA),
-// accumulator full/empty (MMA <-> epilogue); all mbarrier based.
+// Pipelines: A ring (2 stages, generator -> MMA), B ring (loader -> MMA), accumulator buffers
+// flush_full / buf_free (MMA <-> epilogue); all mbarrier based.
 #pragma once
 #include <vector>
 #include <cstring>
@@ -36,17 +44,28 @@ constexpr int kTcAStages = 2;
 constexpr int kTcAPartBytes = kTcBM * kTcBK * 4;            // 16 KB (hi or lo)
 constexpr int kTcAStageBytes = 2 * kTcAPartBytes;           // 32 KB
 constexpr int kTcEpiWarps = 4, kTcGenWarps = 8;
-constexpr int kTcWarpLoader = kTcEpiWarps, kTcWarpMma = kTcEpiWarps + 1, kTcWarpGen0 = kTcEpiWarps + 2;
-constexpr int kTcThreads = 32 * (kTcEpiWarps + 2 + kTcGenWarps);     // 448
-constexpr int kTcMaxGroupChan = 384;       // channels per accumulator group (tensor memory: 512 columns)
+// warp roles, aligned to warpgroups of 4 warps so that setmaxnreg can move registers between them:
+//   WG0 = warps 0-3 flush (tensor-memory lane quarter = warp), WG1 = loader, MMA, 2 idle,
+//   WG2-3 = generators, WG4 = finishers.  The kernel starts with 96 registers per thread (640 threads);
+//   setmaxnreg can only redistribute that pool: 128 x (112 + 40 + 2*128 + 72) = 128 x 5*96.
+constexpr int kTcWarpLoader = 4, kTcWarpMma = 5, kTcWarpGen0 = 8;
+constexpr int kTcFinWarps = 4, kTcWarpFin0 = kTcWarpGen0 + kTcGenWarps;            // 16
+constexpr int kTcThreads = 32 * (kTcWarpFin0 + kTcFinWarps);                        // 640
+constexpr int kTcRegsFlush = 112, kTcRegsCtl = 40, kTcRegsGen = 128, kTcRegsFin = 72;
+static_assert(kTcRegsFlush + kTcRegsCtl + 2 * kTcRegsGen + kTcRegsFin <= 5 * 96, "setmaxnreg pool");
+constexpr int kTcMaxGroupChan = 384;       // channels per tile: 3 column groups of 128 (+ 1 spare buffer = 512 columns)
+constexpr int kTcBufCols = 128, kTcNumBuf = 4, kTcMaxCg = 3;
+constexpr int kTcSegDefault = 8;           // slabs (of 32 frequencies) per accumulation segment
 constexpr int kTcMaxBStages = 4;
 constexpr int kTcSmemLimit = 227 * 1024;
 
 struct TcTables {
     unsigned char* filt_img = nullptr;   // [group][kb][part hi/lo][NBtot rows][128 B swizzled]
-    int32_t n_groups = 0;                // accumulator groups of channels
-    int32_t nb_tot = 0;                  // padded channels per group (multiple of 16; of 32 when split in two)
-    int32_t n_blk = 0, nb = 0;           // MMAs along N per K step and their N
+    float* scratch = nullptr;            // [num CTAs][2][nb_tot][128] fp32 partial sums (L2 resident)
+    int32_t n_groups = 0;                // channel groups (tiles along the channel axis) of <= 384 channels
+    int32_t nb_tot = 0;                  // padded channels per group (multiple of 32)
+    int32_t n_cg = 0;                    // column groups per tile, widths 128,..,remainder
+    int32_t seg = kTcSegDefault;         // slabs per accumulation segment
     int32_t n_kb = 0;                    // n_freq_pad / 32
     int32_t unit_bytes = 0;              // nb_tot * 128
     int32_t b_stages = 0;
@@ -70,13 +89,12 @@ inline gt_status build_tc_tables(const std::vector<float>& filt, int n_chan, int
                                  TcTables& t, cudaStream_t st) {
     const int G = (n_chan + kTcMaxGroupChan - 1) / kTcMaxGroupChan;
     int per = (n_chan + G - 1) / G;
-    int nbt = (per + 15) / 16 * 16;
-    if (nbt > 256) nbt = (per + 31) / 32 * 32;
+    const int nbt = (per + 31) / 32 * 32;
     t.n_groups = G; t.nb_tot = nbt;
-    t.n_blk = nbt > 256 ? 2 : 1; t.nb = nbt / t.n_blk;
+    t.n_cg = (nbt + kTcBufCols - 1) / kTcBufCols;
     t.n_kb = n_freq_pad / kTcBK;
     t.unit_bytes = nbt * 128;
-    const int fixed = kTcAStages * kTcAStageBytes + 1024 /*alignment slack*/ + 256 /*barriers*/;
+    const int fixed = kTcAStages * kTcAStageBytes + 1024 /*alignment slack*/ + 256 /*barriers*/;   // barriers use 164 B
     t.b_stages = std::min(kTcMaxBStages, (kTcSmemLimit - fixed) / t.unit_bytes);
     if (t.b_stages < 2) { tc_error_ref() = "filter slab does not fit in shared memory"; return GT_ERR_UNSUPPORTED; }
     t.smem_bytes = fixed + t.b_stages * t.unit_bytes;
@@ -106,12 +124,26 @@ inline gt_status build_tc_tables(const std::vector<float>& filt, int n_chan, int
     }
     return GT_OK;
 }
-inline void free_tc_tables(TcTables& t) { if (t.filt_img) cudaFree(t.filt_img); t.filt_img = nullptr; }
+// per-CTA scratch tile of partial sums; grid = one CTA per SM
+inline gt_status alloc_tc_scratch(TcTables& t, int num_sms) {
+    if (t.scratch) return GT_OK;
+    const size_t bytes = (size_t)num_sms * 2 * t.nb_tot * kTcBM * sizeof(float);     // two tiles per CTA
+    if (cudaMalloc(reinterpret_cast<void**>(&t.scratch), bytes) != cudaSuccess) {
+        cudaGetLastError(); tc_error_ref() = "cudaMalloc of the partial-sum scratch failed"; return GT_ERR_OOM;
+    }
+    return GT_OK;
+}
+inline void free_tc_tables(TcTables& t) {
+    if (t.filt_img) cudaFree(t.filt_img);
+    if (t.scratch) cudaFree(t.scratch);
+    t.filt_img = nullptr; t.scratch = nullptr;
+}
 
 struct TcParams {
     FusedParams f;
     const unsigned char* filt_img;
-    int32_t n_groups, nb_tot, n_blk, nb, n_kb, unit_bytes, b_stages;
+    float* scratch;
+    int32_t n_groups, nb_tot, n_cg, seg, n_kb, unit_bytes, b_stages;
     int32_t n_row_tiles;
     int32_t cube_vec;           // 1: cube spectra can be read as aligned float4
 };
@@ -119,15 +151,44 @@ struct TcParams {
 // shared-memory map relative to the 1024-byte aligned base:
 //   [0, 64 KB)                      A ring: stage s at s*32 KB = {hi 16 KB, lo 16 KB}
 //   [64 KB, 64 KB + NBS*unit)       B ring
-//   then barriers: a_full[2] a_empty[2] b_full[4] b_empty[4] acc_full acc_empty, tensor-memory slot
+//   then barriers: a_full[2] a_empty[2] b_full[4] b_empty[4] flush_full[4] buf_free[4] tile_done[2]
+//   scratch_free[2], tensor-memory slot
 struct TcSmem {
-    uint32_t a, b, a_full, a_empty, b_full, b_empty, acc_full, acc_empty, slot;
+    uint32_t a, b, a_full, a_empty, b_full, b_empty, flush_full, buf_free, tile_done, scratch_free, slot;
     __device__ TcSmem(uint32_t base, int b_stages, int unit_bytes) {
         a = base; b = base + kTcAStages * kTcAStageBytes;
         const uint32_t bar = b + (uint32_t)b_stages * (uint32_t)unit_bytes;
         a_full = bar; a_empty = bar + 16; b_full = bar + 32; b_empty = bar + 64;
-        acc_full = bar + 96; acc_empty = bar + 104; slot = bar + 112;
+        flush_full = bar + 96; buf_free = bar + 128; tile_done = bar + 160; scratch_free = bar + 176; slot = bar + 192;
     }
+};
+
+// Column groups of a tile and the rotation of their accumulators through the tensor-memory
+// buffers.  The MMA thread and the epilogue warps each run one instance over the same
+// (tile, slab, group) sequence, so they agree on which buffer a group occupies without talking.
+struct TcRotation {
+    int n_cg, seg, n_kb;
+    int buf[kTcMaxCg];             // buffer each group accumulates into
+    int fifo[kTcNumBuf]; int head, count;   // free buffers, oldest first
+    __device__ TcRotation(int n_cg_, int seg_, int n_kb_) : n_cg(n_cg_), seg(seg_), n_kb(n_kb_), head(0), count(0) {
+        for (int g = 0; g < kTcMaxCg; ++g) buf[g] = g;
+        for (int b = n_cg_; b < kTcNumBuf; ++b) fifo[count++] = b;
+    }
+    // group g closes a segment after slab kb (staggered so that flushes do not coincide)
+    __device__ bool boundary(int kb, int g) const {
+        return kb == n_kb - 1 || ((kb + 1 + (g * seg) / n_cg) % seg) == 0;
+    }
+    // moves group g to the oldest free buffer; returns the buffer it leaves
+    __device__ int rotate(int g) {
+        const int old = buf[g];
+        const int nb = fifo[head];
+        fifo[head] = old;                   // count stays the same: pop head, push tail (ring of size count)
+        head = (head + 1) % count;
+        buf[g] = nb;
+        return old;
+    }
+    __device__ static int col0(int g) { return g * kTcBufCols; }
+    __device__ int width(int g, int nb_tot) const { return min(kTcBufCols, nb_tot - g * kTcBufCols); }
 };
 
 __device__ __forceinline__ float4 ldg4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
@@ -151,8 +212,14 @@ fused_tc_kernel(const TcParams p) {
             ptx::mbar_init(sm.b_full + 8 * s, 1);
             ptx::mbar_init(sm.b_empty + 8 * s, 1);
         }
-        ptx::mbar_init(sm.acc_full, 1);
-        ptx::mbar_init(sm.acc_empty, 32 * kTcEpiWarps);
+        for (int b = 0; b < kTcNumBuf; ++b) {
+            ptx::mbar_init(sm.flush_full + 8 * b, 1);
+            ptx::mbar_init(sm.buf_free + 8 * b, 32 * kTcEpiWarps);
+        }
+        for (int b = 0; b < 2; ++b) {
+            ptx::mbar_init(sm.tile_done + 8 * b, 32 * kTcEpiWarps);
+            ptx::mbar_init(sm.scratch_free + 8 * b, 32 * kTcFinWarps);
+        }
         ptx::fence_mbar_init();
     }
     if (warp == kTcWarpMma) {
@@ -166,8 +233,9 @@ fused_tc_kernel(const TcParams p) {
 
     const int64_t n_tiles = (int64_t)p.n_row_tiles * p.n_groups;
 
-    if (warp >= kTcWarpGen0) {
+    if (warp >= kTcWarpGen0 && warp < kTcWarpFin0) {
         // =========================== generator: steps 2-4 -> A ring ===========================
+        ptx::setmaxnreg_inc<kTcRegsGen>();
         const int gw = warp - kTcWarpGen0;
         const int rsub = gw * 4 + (lane >> 3), chunk = lane & 7;
         const uint32_t swz = (uint32_t)((chunk ^ (rsub & 7)) << 4);
@@ -247,7 +315,9 @@ fused_tc_kernel(const TcParams p) {
                 ptx::mbar_arrive(sm.a_full + 8 * stage);
             }
         }
-    } else if (warp == kTcWarpLoader) {
+    } else if (warp >= kTcWarpLoader && warp < kTcWarpGen0) {
+      ptx::setmaxnreg_dec<kTcRegsCtl>();
+      if (warp == kTcWarpLoader) {
         // =========================== loader: filter slab images -> B ring =====================
         if (lane == 0) {
             uint32_t ub = 0;
@@ -264,16 +334,28 @@ fused_tc_kernel(const TcParams p) {
             }
         }
         __syncwarp();
-    } else if (warp == kTcWarpMma) {
+      } else if (warp == kTcWarpMma) {
         // =========================== MMA issuer =================================================
         if (lane == 0) {
-            const uint32_t idesc = ptx::idesc_tf32(kTcBM, p.nb);
-            uint32_t it = 0, ub = 0, tcount = 0;
-            for (int64_t tl = blockIdx.x; tl < n_tiles; tl += gridDim.x, ++tcount) {
-                ptx::mbar_wait(sm.acc_empty, (tcount & 1u) ^ 1u);
-                ptx::tc_fence_after();
+            TcRotation rot(p.n_cg, p.seg, p.n_kb);
+            uint32_t idesc[kTcMaxCg], uses[kTcNumBuf] = {0u, 0u, 0u, 0u};
+            bool fresh[kTcMaxCg];              // next MMA into buf[g] overwrites (first of a segment)
+#pragma unroll
+            for (int g = 0; g < kTcMaxCg; ++g) {
+                idesc[g] = ptx::idesc_tf32(kTcBM, g < p.n_cg ? rot.width(g, p.nb_tot) : 16);
+                fresh[g] = true;
+            }
+            uint32_t it = 0, ub = 0;
+            for (int64_t tl = blockIdx.x; tl < n_tiles; tl += gridDim.x) {
                 for (int kb = 0; kb < p.n_kb; ++kb, ++it) {
                     const uint32_t stage = it & 1u, ph = (it >> 1) & 1u;
+                    // a group that has just moved to another buffer waits until the epilogue has drained it
+#pragma unroll
+                    for (int g = 0; g < kTcMaxCg; ++g)
+                        if (g < p.n_cg && fresh[g]) {
+                            const int b = rot.buf[g];
+                            if (uses[b] > 0) ptx::mbar_wait(sm.buf_free + 8 * b, (uses[b] - 1u) & 1u);
+                        }
                     ptx::mbar_wait(sm.a_full + 8 * stage, ph);
                     const uint32_t a_hi = sm.a + stage * kTcAStageBytes, a_lo = a_hi + kTcAPartBytes;
                     {   // filter hi part: acc += A_hi.B_hi + A_lo.B_hi
@@ -283,12 +365,14 @@ fused_tc_kernel(const TcParams p) {
                         const uint32_t b0 = sm.b + bs * (uint32_t)p.unit_bytes;
 #pragma unroll
                         for (int k = 0; k < kTcBK / kTcUK; ++k)
-                            for (int j = 0; j < p.n_blk; ++j) {
-                                const uint64_t bd = ptx::smem_desc_sw128(b0 + (uint32_t)(j * p.nb) * 128u + k * 32u);
-                                const uint32_t d = tmem_base + (uint32_t)(j * p.nb);
-                                ptx::mma_tf32_ss(d, ptx::smem_desc_sw128(a_hi + k * 32u), bd, idesc, (kb | k) != 0);
-                                ptx::mma_tf32_ss(d, ptx::smem_desc_sw128(a_lo + k * 32u), bd, idesc, 1u);
-                            }
+#pragma unroll
+                            for (int g = 0; g < kTcMaxCg; ++g)
+                                if (g < p.n_cg) {
+                                    const uint64_t bd = ptx::smem_desc_sw128(b0 + (uint32_t)(g * kTcBufCols) * 128u + k * 32u);
+                                    const uint32_t d = tmem_base + (uint32_t)(rot.buf[g] * kTcBufCols);
+                                    ptx::mma_tf32_ss(d, ptx::smem_desc_sw128(a_hi + k * 32u), bd, idesc[g], (k != 0 || !fresh[g]) ? 1u : 0u);
+                                    ptx::mma_tf32_ss(d, ptx::smem_desc_sw128(a_lo + k * 32u), bd, idesc[g], 1u);
+                                }
                         ptx::tc_commit(sm.b_empty + 8 * bs);
                         ++ub;
                     }
@@ -299,61 +383,135 @@ fused_tc_kernel(const TcParams p) {
                         const uint32_t b0 = sm.b + bs * (uint32_t)p.unit_bytes;
 #pragma unroll
                         for (int k = 0; k < kTcBK / kTcUK; ++k)
-                            for (int j = 0; j < p.n_blk; ++j) {
-                                const uint64_t bd = ptx::smem_desc_sw128(b0 + (uint32_t)(j * p.nb) * 128u + k * 32u);
-                                ptx::mma_tf32_ss(tmem_base + (uint32_t)(j * p.nb), ptx::smem_desc_sw128(a_hi + k * 32u),
-                                                 bd, idesc, 1u);
-                            }
+#pragma unroll
+                            for (int g = 0; g < kTcMaxCg; ++g)
+                                if (g < p.n_cg) {
+                                    const uint64_t bd = ptx::smem_desc_sw128(b0 + (uint32_t)(g * kTcBufCols) * 128u + k * 32u);
+                                    ptx::mma_tf32_ss(tmem_base + (uint32_t)(rot.buf[g] * kTcBufCols),
+                                                     ptx::smem_desc_sw128(a_hi + k * 32u), bd, idesc[g], 1u);
+                                }
                         ptx::tc_commit(sm.b_empty + 8 * bs);
                         ++ub;
                     }
                     ptx::tc_commit(sm.a_empty + 8 * stage);
+                    // segment boundaries: hand the finished partial sums to the epilogue, move on to a free buffer
+#pragma unroll
+                    for (int g = 0; g < kTcMaxCg; ++g) {
+                        if (g >= p.n_cg) continue;
+                        fresh[g] = false;
+                        if (rot.boundary(kb, g)) {
+                            const int old = rot.rotate(g);
+                            ptx::tc_commit(sm.flush_full + 8 * old);
+                            ++uses[old];
+                            fresh[g] = true;
+                        }
+                    }
                 }
-                ptx::tc_commit(sm.acc_full);
             }
         }
         __syncwarp();
-    } else {
-        // =========================== epilogue: drain, then photon noise ========================
-        const int q = warp;                                    // tensor-memory lane quarter
-        uint32_t tcount = 0;
-        for (int64_t tl = blockIdx.x; tl < n_tiles; tl += gridDim.x, ++tcount) {
+      }
+    } else if (warp >= kTcWarpFin0) {
+        // ============ finisher: scratch tile -> P = sum*scale + bias, photon noise -> TOD ========
+        ptx::setmaxnreg_dec<kTcRegsFin>();
+        const int q = warp - kTcWarpFin0;
+        uint32_t ti = 0;
+        for (int64_t tl = blockIdx.x; tl < n_tiles; tl += gridDim.x, ++ti) {
             const int64_t row0 = (tl / p.n_groups) * kTcBM;
             const int cg0 = (int)(tl % p.n_groups) * p.nb_tot;
             const int n_valid = min(p.nb_tot, f.n_chan - cg0);            // real channels of this group
-            ptx::mbar_wait(sm.acc_full, tcount & 1u);
-            ptx::tc_fence_after();
-            const int64_t R = row0 + 32 * q + lane;
-            float* orow = f.out + (size_t)R * f.n_chan + cg0;
-            for (int col0 = 0; col0 < n_valid; col0 += 32) {
-                uint32_t v[32];
-                ptx::tmem_ld_32x32(tmem_base + ((uint32_t)(32 * q) << 16) + (uint32_t)col0, v);
-                ptx::tmem_ld_wait();
-                if (R < f.n_rows) {
+            const uint32_t sb = ti & 1u;
+            const float* sc = p.scratch + ((size_t)blockIdx.x * 2 + sb) * p.nb_tot * kTcBM;
+            ptx::mbar_wait(sm.tile_done + 8 * sb, (ti >> 1) & 1u);
+            constexpr int kMaxPerLane = kTcMaxGroupChan / 32;             // 12
+            for (int r = q; r < kTcBM; r += kTcFinWarps) {
+                const int64_t Rr = row0 + r;
+                if (Rr >= f.n_rows) break;
+                const uint32_t n = (uint32_t)(f.t0 + Rr / f.n_spaxel), s = (uint32_t)(Rr % f.n_spaxel);
+                float* o = f.out + (size_t)Rr * f.n_chan + cg0;
+                float x[kMaxPerLane];
 #pragma unroll
-                    for (int i = 0; i < 32; ++i)
-                        if (col0 + i < n_valid)
-                            orow[col0 + i] = fmaf(__uint_as_float(v[i]), f.scale, __ldg(f.bias + cg0 + col0 + i));
+                for (int j = 0; j < kMaxPerLane; ++j) {
+                    const int c = lane + 32 * j;
+                    x[j] = c < n_valid ? __ldcg(sc + (size_t)c * kTcBM + r) : 0.f;
                 }
-            }
-            ptx::tc_fence_before();
-            ptx::mbar_arrive(sm.acc_empty);
-            if (f.photon_noise) {
-                asm volatile("bar.sync 1, %0;" :: "n"(32 * kTcEpiWarps) : "memory");
-                for (int r = q; r < kTcBM; r += kTcEpiWarps) {
-                    const int64_t Rr = row0 + r;
-                    if (Rr >= f.n_rows) break;
-                    const uint32_t n = (uint32_t)(f.t0 + Rr / f.n_spaxel), s = (uint32_t)(Rr % f.n_spaxel);
-                    float* o = f.out + (size_t)Rr * f.n_chan + cg0;
-                    for (int c = lane; c < n_valid; c += 32) {
-                        float P = __ldcg(o + c);
-                        const uint4 w = philox4x32_10(n, s, (uint32_t)(cg0 + c), kStreamPhoton, f.seed_lo, f.seed_hi);
-                        P = fmaf(photon_sigma(P, __ldg(f.noise_c1 + cg0 + c), __ldg(f.noise_c2 + cg0 + c)),
-                                 normal_cos(w.x, w.y), P);
+#pragma unroll
+                for (int j = 0; j < kMaxPerLane; ++j) {
+                    const int c = lane + 32 * j;
+                    if (c < n_valid) {
+                        float P = fmaf(x[j], f.scale, __ldg(f.bias + cg0 + c));
+                        if (f.photon_noise) {
+                            const uint4 w = philox4x32_10(n, s, (uint32_t)(cg0 + c), kStreamPhoton, f.seed_lo, f.seed_hi);
+                            P = fmaf(photon_sigma(P, __ldg(f.noise_c1 + cg0 + c), __ldg(f.noise_c2 + cg0 + c)),
+                                     normal_cos(w.x, w.y), P);
+                        }
                         o[c] = P;
                     }
                 }
             }
+            ptx::mbar_arrive(sm.scratch_free + 8 * sb);
+        }
+    } else {
+        // ============ epilogue: segment flushes of the accumulators into the scratch tile =======
+        ptx::setmaxnreg_inc<kTcRegsFlush>();
+        const int q = warp;                                    // tensor-memory lane quarter
+        const int trow = 32 * q + lane;                        // tile row = tensor-memory lane
+        TcRotation rot(p.n_cg, p.seg, p.n_kb);
+        uint32_t fulls[kTcNumBuf] = {0u, 0u, 0u, 0u};
+        uint32_t ti = 0;
+        for (int64_t tl = blockIdx.x; tl < n_tiles; tl += gridDim.x, ++ti) {
+            const uint32_t sb = ti & 1u;
+            float* const sc = p.scratch + ((size_t)blockIdx.x * 2 + sb) * p.nb_tot * kTcBM;
+            if (ti >= 2) ptx::mbar_wait(sm.scratch_free + 8 * sb, ((ti >> 1) - 1u) & 1u);   // finisher done with tile ti-2
+            bool first[kTcMaxCg] = {true, true, true};
+            for (int kb = 0; kb < p.n_kb; ++kb)
+#pragma unroll
+                for (int g = 0; g < kTcMaxCg; ++g) {
+                    if (g >= p.n_cg || !rot.boundary(kb, g)) continue;
+                    const int b = rot.rotate(g);
+                    const int wg = rot.width(g, p.nb_tot);
+                    float* scg = sc + (size_t)(g * kTcBufCols) * kTcBM + trow;
+                    const uint32_t taddr = tmem_base + ((uint32_t)(32 * q) << 16) + (uint32_t)(b * kTcBufCols);
+                    const bool add = !first[g];
+                    uint32_t v[32];
+                    float pa[32], pb[32];
+                    // the running sums of the first 32 columns are fetched while the MMAs still run
+                    if (add) {
+#pragma unroll
+                        for (int i = 0; i < 32; ++i) pa[i] = __ldcg(scg + (size_t)i * kTcBM);
+                    }
+                    ptx::mbar_wait(sm.flush_full + 8 * b, fulls[b] & 1u);
+                    ++fulls[b];
+                    ptx::tc_fence_after();
+                    for (int c0 = 0; c0 < wg; c0 += 64) {
+                        const bool two = c0 + 32 < wg;
+                        ptx::tmem_ld_32x32(taddr + (uint32_t)c0, v);
+                        if (add && two) {
+#pragma unroll
+                            for (int i = 0; i < 32; ++i) pb[i] = __ldcg(scg + (size_t)(c0 + 32 + i) * kTcBM);
+                        }
+                        ptx::tmem_ld_wait();
+#pragma unroll
+                        for (int i = 0; i < 32; ++i)
+                            __stcg(scg + (size_t)(c0 + i) * kTcBM, add ? pa[i] + __uint_as_float(v[i]) : __uint_as_float(v[i]));
+                        if (two) {
+                            ptx::tmem_ld_32x32(taddr + (uint32_t)(c0 + 32), v);
+                            if (add && c0 + 64 < wg) {
+#pragma unroll
+                                for (int i = 0; i < 32; ++i) pa[i] = __ldcg(scg + (size_t)(c0 + 64 + i) * kTcBM);
+                            }
+                            ptx::tmem_ld_wait();
+#pragma unroll
+                            for (int i = 0; i < 32; ++i)
+                                __stcg(scg + (size_t)(c0 + 32 + i) * kTcBM, add ? pb[i] + __uint_as_float(v[i]) : __uint_as_float(v[i]));
+                        }
+                    }
+                    ptx::tc_fence_before();
+                    ptx::mbar_arrive(sm.buf_free + 8 * b);
+                    first[g] = false;
+                }
+            // every partial sum of the tile is in the scratch tile: hand it to the finisher warps
+            ptx::mbar_arrive(sm.tile_done + 8 * sb);
         }
     }
 
@@ -368,7 +526,8 @@ fused_tc_kernel(const TcParams p) {
 inline cudaError_t launch_fused_tc(const FusedParams& fp, const TcTables& t, int num_sms, cudaStream_t st) {
     TcParams p{};
     p.f = fp; p.filt_img = t.filt_img;
-    p.n_groups = t.n_groups; p.nb_tot = t.nb_tot; p.n_blk = t.n_blk; p.nb = t.nb; p.n_kb = t.n_kb;
+    p.scratch = t.scratch;
+    p.n_groups = t.n_groups; p.nb_tot = t.nb_tot; p.n_cg = t.n_cg; p.seg = t.seg > 0 ? t.seg : kTcSegDefault; p.n_kb = t.n_kb;
     p.unit_bytes = t.unit_bytes; p.b_stages = t.b_stages;
     p.n_row_tiles = (int32_t)((fp.n_rows + kTcBM - 1) / kTcBM);
     p.cube_vec = (fp.cube == nullptr) || ((fp.n_freq % 4 == 0) && ((reinterpret_cast<uintptr_t>(fp.cube) & 15u) == 0));
