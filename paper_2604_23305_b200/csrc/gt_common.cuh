@@ -38,6 +38,29 @@ __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_
     return make_uint4(c0, c1, c2, c3);
 }
 
+// W independent Philox4x32-10 blocks at once: the ten rounds of one block are a strictly serial
+// chain (~10 cycles per round), so a lone warp only fills its issue slots if it interleaves
+// several blocks.  Same arithmetic as philox4x32_10; counters differ in word 2 (the channel).
+template <int W>
+__device__ __forceinline__ void philox4x32_10_multi(uint32_t c0, uint32_t c1, const uint32_t (&c2)[W], uint32_t c3,
+                                                    uint32_t k0, uint32_t k1, uint32_t (&o0)[W], uint32_t (&o1)[W]) {
+    uint32_t a[W], b[W], c[W], d[W];
+#pragma unroll
+    for (int i = 0; i < W; ++i) { a[i] = c0; b[i] = c1; c[i] = c2[i]; d[i] = c3; }
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+#pragma unroll
+        for (int i = 0; i < W; ++i) {
+            const uint32_t hi0 = __umulhi(kPhiloxM0, a[i]), lo0 = kPhiloxM0 * a[i];
+            const uint32_t hi1 = __umulhi(kPhiloxM1, c[i]), lo1 = kPhiloxM1 * c[i];
+            a[i] = hi1 ^ b[i] ^ k0; b[i] = lo1; c[i] = hi0 ^ d[i] ^ k1; d[i] = lo0;
+        }
+        k0 += kPhiloxW0; k1 += kPhiloxW1;
+    }
+#pragma unroll
+    for (int i = 0; i < W; ++i) { o0[i] = a[i]; o1[i] = b[i]; }      // words 0 and 1 (the photon-noise normal uses only these)
+}
+
 // U(w) = ((w >> 9) + 1/2) 2^-23 in (0,1): exact in fp32 (R19).
 __device__ __forceinline__ float uniform01(uint32_t w) {
     return ((float)(w >> 9) + 0.5f) * (1.0f / 8388608.0f);
@@ -45,12 +68,16 @@ __device__ __forceinline__ float uniform01(uint32_t w) {
 
 // Box-Muller: z0 = sqrt(-2 ln U(w0)) cos(2 pi U(w1)), z1 = ... sin(...).  MUFU log/sin/cos: the
 // normals only need ~1e-3 absolute accuracy for the 2e-5 TOD gate (sigma/P ~ 1e-3).
+// MUFU.SQRT (2^-22 relative): sqrtf's IEEE path costs a dozen instructions and a slow-path call
+__device__ __forceinline__ float sqrt_fast(float x) {
+    float r; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r;
+}
 __device__ __forceinline__ float normal_cos(uint32_t w0, uint32_t w1) {
-    const float r = sqrtf(-2.0f * __logf(uniform01(w0)));
+    const float r = sqrt_fast(-2.0f * __logf(uniform01(w0)));
     return r * __cosf(6.28318530717958647692f * uniform01(w1));
 }
 __device__ __forceinline__ void normal_pair(uint32_t w0, uint32_t w1, float& z0, float& z1) {
-    const float r = sqrtf(-2.0f * __logf(uniform01(w0)));
+    const float r = sqrt_fast(-2.0f * __logf(uniform01(w0)));
     float s, c;
     __sincosf(6.28318530717958647692f * uniform01(w1), &s, &c);
     z0 = r * c; z1 = r * s;
@@ -60,7 +87,7 @@ __device__ __forceinline__ void normal_pair(uint32_t w0, uint32_t w1, float& z0,
 // sigma^2 = (2 h f_c P + 2 P^2 / dnu_c) f_s / 2 = P (c1 + P c2), c1 = h f_c f_s, c2 = f_s / dnu_c.
 __device__ __forceinline__ float photon_sigma(float P, float c1, float c2) {
     const float v = P * (c1 + P * c2);
-    return v > 0.0f ? sqrtf(v) : 0.0f;
+    return v > 0.0f ? sqrt_fast(v) : 0.0f;
 }
 
 }  // namespace gt

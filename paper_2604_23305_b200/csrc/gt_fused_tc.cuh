@@ -30,6 +30,8 @@
 #include <vector>
 #include <cstring>
 #include <algorithm>
+#include <cstdlib>
+#include <cstdio>
 #include "gt_common.cuh"
 #include "gt_fused_fp32.cuh"
 #include "gt_tc_ptx.cuh"
@@ -43,16 +45,23 @@ constexpr int kTcUK = 8;                   // K of one tcgen05.mma.kind::tf32
 constexpr int kTcAStages = 2;
 constexpr int kTcAPartBytes = kTcBM * kTcBK * 4;            // 16 KB (hi or lo)
 constexpr int kTcAStageBytes = 2 * kTcAPartBytes;           // 32 KB
-constexpr int kTcEpiWarps = 4, kTcGenWarps = 8;
+constexpr int kTcEpiWarps = 4, kTcGenWarps = 16;
 // warp roles, aligned to warpgroups of 4 warps so that setmaxnreg can move registers between them:
-//   WG0 = warps 0-3 flush (tensor-memory lane quarter = warp), WG1 = loader, MMA, 2 idle,
-//   WG2-3 = generators, WG4 = finishers.  The kernel starts with 96 registers per thread (640 threads);
-//   setmaxnreg can only redistribute that pool: 128 x (112 + 40 + 2*128 + 72) = 128 x 5*96.
-constexpr int kTcWarpLoader = 4, kTcWarpMma = 5, kTcWarpGen0 = 8;
-constexpr int kTcFinWarps = 4, kTcWarpFin0 = kTcWarpGen0 + kTcGenWarps;            // 16
-constexpr int kTcThreads = 32 * (kTcWarpFin0 + kTcFinWarps);                        // 640
-constexpr int kTcRegsFlush = 112, kTcRegsCtl = 40, kTcRegsGen = 128, kTcRegsFin = 72;
-static_assert(kTcRegsFlush + kTcRegsCtl + 2 * kTcRegsGen + kTcRegsFin <= 5 * 96, "setmaxnreg pool");
+//   WG0 = warps 0-3 flush (tensor-memory lane quarter = warp), WG1-4 = generators, WG5 = finishers,
+//   WG6 = 2 idle, loader, MMA.  Generators (4 warps per scheduler: the per-element dependency chain lg2 -> ex2 -> split
+//   only fills the issue slots with thread-level parallelism), WG6 = finishers.  The kernel starts
+//   with 72 registers per thread (896 threads); setmaxnreg can only redistribute that pool:
+//   128 x (56 + 40 + 4*80 + 88) = 128 x 7*72.
+// The warp scheduler favours the highest warp id among eligible warps: the two single-thread control
+// roles sit in the LAST warpgroup so that the MMA issue stream is never starved by generator warps.
+constexpr int kTcWarpGen0 = 4;
+constexpr int kTcRowsPerThread = kTcBM / (4 * kTcGenWarps), kTcRowStride = 4 * kTcGenWarps;   // 2 rows, 64 apart
+constexpr int kTcFinWarps = 4, kTcWarpFin0 = kTcWarpGen0 + kTcGenWarps;            // 20
+constexpr int kTcWarpCtl0 = kTcWarpFin0 + kTcFinWarps;                              // 24
+constexpr int kTcWarpLoader = kTcWarpCtl0 + 2, kTcWarpMma = kTcWarpCtl0 + 3;        // 26, 27
+constexpr int kTcThreads = 32 * (kTcWarpCtl0 + 4);                                  // 896
+constexpr int kTcRegsFlush = 56, kTcRegsCtl = 40, kTcRegsGen = 80, kTcRegsFin = 88;
+static_assert(kTcRegsFlush + kTcRegsCtl + 4 * kTcRegsGen + kTcRegsFin <= 7 * 72, "setmaxnreg pool");
 constexpr int kTcMaxGroupChan = 384;       // channels per tile: 3 column groups of 128 (+ 1 spare buffer = 512 columns)
 constexpr int kTcBufCols = 128, kTcNumBuf = 4, kTcMaxCg = 3;
 constexpr int kTcSegDefault = 8;           // slabs (of 32 frequencies) per accumulation segment
@@ -94,7 +103,7 @@ inline gt_status build_tc_tables(const std::vector<float>& filt, int n_chan, int
     t.n_cg = (nbt + kTcBufCols - 1) / kTcBufCols;
     t.n_kb = n_freq_pad / kTcBK;
     t.unit_bytes = nbt * 128;
-    const int fixed = kTcAStages * kTcAStageBytes + 1024 /*alignment slack*/ + 256 /*barriers*/;   // barriers use 164 B
+    const int fixed = kTcAStages * kTcAStageBytes + 1024 /*alignment slack*/ + 256 /*barriers*/ + kTcBM * 32 /*row constants*/;   // barriers use 164 B
     t.b_stages = std::min(kTcMaxBStages, (kTcSmemLimit - fixed) / t.unit_bytes);
     if (t.b_stages < 2) { tc_error_ref() = "filter slab does not fit in shared memory"; return GT_ERR_UNSUPPORTED; }
     t.smem_bytes = fixed + t.b_stages * t.unit_bytes;
@@ -146,6 +155,7 @@ struct TcParams {
     int32_t n_groups, nb_tot, n_cg, seg, n_kb, unit_bytes, b_stages;
     int32_t n_row_tiles;
     int32_t cube_vec;           // 1: cube spectra can be read as aligned float4
+    int32_t debug;              // timing diagnostics only (GATEAU_TC_DEBUG): 1 = generator skips its arithmetic, 2 = no MMAs issued, 4 = no filter copies, 8 = no finisher work
 };
 
 // shared-memory map relative to the 1024-byte aligned base:
@@ -154,42 +164,59 @@ struct TcParams {
 //   then barriers: a_full[2] a_empty[2] b_full[4] b_empty[4] flush_full[4] buf_free[4] tile_done[2]
 //   scratch_free[2], tensor-memory slot
 struct TcSmem {
-    uint32_t a, b, a_full, a_empty, b_full, b_empty, flush_full, buf_free, tile_done, scratch_free, slot;
+    uint32_t a, b, a_full, a_empty, b_full, b_empty, flush_full, buf_free, tile_done, scratch_free, slot, rowp;
     __device__ TcSmem(uint32_t base, int b_stages, int unit_bytes) {
         a = base; b = base + kTcAStages * kTcAStageBytes;
         const uint32_t bar = b + (uint32_t)b_stages * (uint32_t)unit_bytes;
         a_full = bar; a_empty = bar + 16; b_full = bar + 32; b_empty = bar + 64;
         flush_full = bar + 96; buf_free = bar + 128; tile_done = bar + 160; scratch_free = bar + 176; slot = bar + 192;
+        rowp = bar + 256;
     }
 };
 
 // Column groups of a tile and the rotation of their accumulators through the tensor-memory
 // buffers.  The MMA thread and the epilogue warps each run one instance over the same
 // (tile, slab, group) sequence, so they agree on which buffer a group occupies without talking.
+// All state is packed into registers (2 bits per buffer id): the MMA thread's issue loop must
+// stay far below the 2112 cycles the tensor pipe needs per slab.
 struct TcRotation {
     int n_cg, seg, n_kb;
-    int buf[kTcMaxCg];             // buffer each group accumulates into
-    int fifo[kTcNumBuf]; int head, count;   // free buffers, oldest first
-    __device__ TcRotation(int n_cg_, int seg_, int n_kb_) : n_cg(n_cg_), seg(seg_), n_kb(n_kb_), head(0), count(0) {
-        for (int g = 0; g < kTcMaxCg; ++g) buf[g] = g;
-        for (int b = n_cg_; b < kTcNumBuf; ++b) fifo[count++] = b;
+    uint32_t bufs;                 // buffer of group g in bits [2g, 2g+2)
+    uint32_t fifo;                 // free buffers, oldest in bits [0, 2)
+    int shift;                     // 2 * (number of free buffers - 1)
+    int cnt[kTcMaxCg];             // slabs since the group's last segment boundary (staggered start)
+    __device__ TcRotation(int n_cg_, int seg_, int n_kb_) : n_cg(n_cg_), seg(seg_), n_kb(n_kb_) {
+        bufs = 0u | (1u << 2) | (2u << 4);
+        fifo = 0u; int c = 0;
+        for (int b = n_cg_; b < kTcNumBuf; ++b, ++c) fifo |= (uint32_t)b << (2 * c);
+        shift = 2 * (c - 1);
+#pragma unroll
+        for (int g = 0; g < kTcMaxCg; ++g) cnt[g] = (g * seg_) / n_cg_;
     }
-    // group g closes a segment after slab kb (staggered so that flushes do not coincide)
-    __device__ bool boundary(int kb, int g) const {
-        return kb == n_kb - 1 || ((kb + 1 + (g * seg) / n_cg) % seg) == 0;
+    __device__ __forceinline__ int buf(int g) const { return (int)((bufs >> (2 * g)) & 3u); }
+    // called once per (slab, group) in slab order: does group g close a segment after slab kb?
+    __device__ __forceinline__ bool boundary(int kb, int g) {
+        if (kb == n_kb - 1) { cnt[g] = (g * seg) / n_cg; return true; }
+        if (++cnt[g] == seg) { cnt[g] = 0; return true; }
+        return false;
     }
     // moves group g to the oldest free buffer; returns the buffer it leaves
-    __device__ int rotate(int g) {
-        const int old = buf[g];
-        const int nb = fifo[head];
-        fifo[head] = old;                   // count stays the same: pop head, push tail (ring of size count)
-        head = (head + 1) % count;
-        buf[g] = nb;
-        return old;
+    __device__ __forceinline__ int rotate(int g) {
+        const uint32_t old = (bufs >> (2 * g)) & 3u, nb = fifo & 3u;
+        fifo = (fifo >> 2) | (old << shift);
+        bufs = (bufs & ~(3u << (2 * g))) | (nb << (2 * g));
+        return (int)old;
     }
-    __device__ static int col0(int g) { return g * kTcBufCols; }
-    __device__ int width(int g, int nb_tot) const { return min(kTcBufCols, nb_tot - g * kTcBufCols); }
+    __device__ __forceinline__ int width(int g, int nb_tot) const { return min(kTcBufCols, nb_tot - g * kTcBufCols); }
 };
+
+// steps 2-4 for one (row, nu) element as in element_value (gt_fused_fp32.cuh), with the two MUFU
+// operations issued as single instructions: eta_z is in (0,1] and csc >= 1, so log2 is <= 0 and finite
+// and 2^(csc log2 eta_z) underflows to 0 exactly where eta_atm is below 1e-38.
+__device__ __forceinline__ float element_value_fast(float eta_z, float csc, float Xn, float GS) {
+    const float eta = ptx::ex2_ftz(csc * ptx::lg2_ftz(eta_z));
+    return fmaf(1.0f - eta, Xn, eta * GS);
+}
 
 __device__ __forceinline__ float4 ldg4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
 
@@ -205,7 +232,7 @@ fused_tc_kernel(const TcParams p) {
 
     if (tid == 0) {
         for (int s = 0; s < kTcAStages; ++s) {
-            ptx::mbar_init(sm.a_full + 8 * s, 32 * kTcGenWarps);
+            ptx::mbar_init(sm.a_full + 8 * s, kTcGenWarps);
             ptx::mbar_init(sm.a_empty + 8 * s, 1);
         }
         for (int s = 0; s < kTcMaxBStages; ++s) {
@@ -214,11 +241,11 @@ fused_tc_kernel(const TcParams p) {
         }
         for (int b = 0; b < kTcNumBuf; ++b) {
             ptx::mbar_init(sm.flush_full + 8 * b, 1);
-            ptx::mbar_init(sm.buf_free + 8 * b, 32 * kTcEpiWarps);
+            ptx::mbar_init(sm.buf_free + 8 * b, kTcEpiWarps);
         }
         for (int b = 0; b < 2; ++b) {
-            ptx::mbar_init(sm.tile_done + 8 * b, 32 * kTcEpiWarps);
-            ptx::mbar_init(sm.scratch_free + 8 * b, 32 * kTcFinWarps);
+            ptx::mbar_init(sm.tile_done + 8 * b, kTcEpiWarps);
+            ptx::mbar_init(sm.scratch_free + 8 * b, kTcFinWarps);
         }
         ptx::fence_mbar_init();
     }
@@ -241,14 +268,107 @@ fused_tc_kernel(const TcParams p) {
         const uint32_t swz = (uint32_t)((chunk ^ (rsub & 7)) << 4);
         const size_t nf = (size_t)f.n_freq, nfp = (size_t)f.n_freq_pad;
         uint32_t it = 0;
+        if constexpr (VEC) {
+            // One step = one row of this thread (4 frequencies of it): 2 LUT rows + 4 cube taps as
+            // 16-byte loads, steps 2-4, tf32 split, two 16-byte shared stores.  The loads of the
+            // next step are issued before the current one is computed; the other three warps of the
+            // scheduler cover the rest of the latency.  The per-row constants live in shared
+            // memory (each warp only reads rows it wrote itself).
+            struct Tap { float4 L0, L1, c00, c01, c10, c11; };
+            RowParam* rowp = reinterpret_cast<RowParam*>(smem_raw + (sm.rowp - raw));
+            const float4 zero4 = make_float4(0.f, 0.f, 0.f, 0.f);
+            for (int64_t tl = blockIdx.x; tl < n_tiles; tl += gridDim.x) {
+                const int64_t row0 = (tl / p.n_groups) * kTcBM;
+                __syncwarp();
+                if (chunk < kTcRowsPerThread) {
+                    const int rr = rsub + kTcRowStride * chunk;
+                    const int64_t R = row0 + rr;
+                    RowParam rp;
+                    if (R < f.n_rows) {
+                        const int4* src = reinterpret_cast<const int4*>(f.rows + R);
+                        const int4 a = __ldg(src), b = __ldg(src + 1);
+                        rp.fp = __int_as_float(a.x); rp.csc = __int_as_float(a.y); rp.ip = a.z; rp.pix = a.w;
+                        rp.w00 = __int_as_float(b.x); rp.w01 = __int_as_float(b.y);
+                        rp.w10 = __int_as_float(b.z); rp.w11 = __int_as_float(b.w);
+                    } else {
+                        rp.fp = 0.f; rp.csc = 1.f; rp.ip = 0; rp.pix = -1; rp.w00 = rp.w01 = rp.w10 = rp.w11 = 0.f;
+                    }
+                    if (f.cube == nullptr) rp.pix = -1;
+                    rowp[rr] = rp;
+                }
+                __syncwarp();
+                auto issue = [&](int kb, int j, Tap& t) {
+                    const int4 a = *reinterpret_cast<const int4*>(rowp + rsub + kTcRowStride * j);   // fp, csc, ip, pix
+                    const int nu0 = kb * kTcBK + chunk * 4;
+                    const float* lp = f.lut_r + (size_t)a.z * nfp + nu0;
+                    t.c00 = zero4; t.c01 = zero4; t.c10 = zero4; t.c11 = zero4;
+                    if (p.debug & 16) { t.L0 = make_float4(0.5f, 0.5f, 0.5f, 0.5f); t.L1 = t.L0; return; }
+                    t.L0 = ldg4(lp); t.L1 = ldg4(lp + nfp);
+                    if (a.w >= 0 && nu0 < f.n_freq) {
+                        const float* c = f.cube + (size_t)a.w * nf + nu0;
+                        t.c00 = ldg4(c); t.c01 = ldg4(c + nf);
+                        c += (size_t)f.n_az * nf;
+                        t.c10 = ldg4(c); t.c11 = ldg4(c + nf);
+                    }
+                };
+                auto compute = [&](int j, const Tap& cur, const float4& X, const float4& G, uint32_t stage) {
+                    const RowParam* rp = rowp + rsub + kTcRowStride * j;
+                    const float2 fc = *reinterpret_cast<const float2*>(rp);                    // fp, csc
+                    const float4 w = *reinterpret_cast<const float4*>(&rp->w00);
+                    float4 S, v, hi, lo;
+                    if (p.debug & 32) {
+                        unsigned char* a_hi = smem_raw + (sm.a - raw) + stage * kTcAStageBytes;
+                        const uint32_t off = (uint32_t)(rsub + kTcRowStride * j) * 128u + swz;
+                        *reinterpret_cast<float4*>(a_hi + off) = cur.L0;
+                        *reinterpret_cast<float4*>(a_hi + kTcAPartBytes + off) = cur.c00;
+                        return;
+                    }
+                    S.x = w.x * cur.c00.x + w.y * cur.c01.x + w.z * cur.c10.x + w.w * cur.c11.x;
+                    S.y = w.x * cur.c00.y + w.y * cur.c01.y + w.z * cur.c10.y + w.w * cur.c11.y;
+                    S.z = w.x * cur.c00.z + w.y * cur.c01.z + w.z * cur.c10.z + w.w * cur.c11.z;
+                    S.w = w.x * cur.c00.w + w.y * cur.c01.w + w.z * cur.c10.w + w.w * cur.c11.w;
+                    v.x = element_value_fast(fmaf(fc.x, cur.L1.x - cur.L0.x, cur.L0.x), fc.y, X.x, G.x * S.x);
+                    v.y = element_value_fast(fmaf(fc.x, cur.L1.y - cur.L0.y, cur.L0.y), fc.y, X.y, G.y * S.y);
+                    v.z = element_value_fast(fmaf(fc.x, cur.L1.z - cur.L0.z, cur.L0.z), fc.y, X.z, G.z * S.z);
+                    v.w = element_value_fast(fmaf(fc.x, cur.L1.w - cur.L0.w, cur.L0.w), fc.y, X.w, G.w * S.w);
+                    hi.x = ptx::tf32_trunc(v.x); hi.y = ptx::tf32_trunc(v.y); hi.z = ptx::tf32_trunc(v.z); hi.w = ptx::tf32_trunc(v.w);
+                    lo.x = v.x - hi.x; lo.y = v.y - hi.y; lo.z = v.z - hi.z; lo.w = v.w - hi.w;
+                    unsigned char* a_hi = smem_raw + (sm.a - raw) + stage * kTcAStageBytes;
+                    const uint32_t off = (uint32_t)(rsub + kTcRowStride * j) * 128u + swz;
+                    *reinterpret_cast<float4*>(a_hi + off) = hi;
+                    *reinterpret_cast<float4*>(a_hi + kTcAPartBytes + off) = lo;
+                };
+                Tap t0, t1;
+                issue(0, 0, t0);
+                for (int kb = 0; kb < p.n_kb; ++kb, ++it) {
+                    const uint32_t stage = it & 1u, ph = (it >> 1) & 1u;
+                    if (p.debug & 1) {
+                        ptx::mbar_wait(sm.a_empty + 8 * stage, ph ^ 1u);
+                        __syncwarp();
+                        if (lane == 0) ptx::mbar_arrive(sm.a_full + 8 * stage);
+                        continue;
+                    }
+                    const float4 X = ldg4(f.Xn + kb * kTcBK + chunk * 4), G = ldg4(f.Gs + kb * kTcBK + chunk * 4);
+                    issue(kb, 1, t1);
+                    ptx::mbar_wait(sm.a_empty + 8 * stage, ph ^ 1u);
+                    compute(0, t0, X, G, stage);
+                    if (kb + 1 < p.n_kb) issue(kb + 1, 0, t0);
+                    compute(1, t1, X, G, stage);
+                    // one arrival per warp: 512 per-thread arrivals on one mbarrier serialise (~5 cycles each)
+                    ptx::fence_proxy_async_smem();
+                    __syncwarp();
+                    if (lane == 0) ptx::mbar_arrive(sm.a_full + 8 * stage);
+                }
+            }
+        } else
         for (int64_t tl = blockIdx.x; tl < n_tiles; tl += gridDim.x) {
             const int64_t row0 = (tl / p.n_groups) * kTcBM;
-            float fp[4], csc[4], w00[4], w01[4], w10[4], w11[4];
-            const float* lutp[4];
-            const float* cubep[4];
+            float fp[kTcRowsPerThread], csc[kTcRowsPerThread], w00[kTcRowsPerThread], w01[kTcRowsPerThread], w10[kTcRowsPerThread], w11[kTcRowsPerThread];
+            const float* lutp[kTcRowsPerThread];
+            const float* cubep[kTcRowsPerThread];
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                const int64_t R = row0 + rsub + 32 * j;
+            for (int j = 0; j < kTcRowsPerThread; ++j) {
+                const int64_t R = row0 + rsub + kTcRowStride * j;
                 RowParam rp;
                 if (R < f.n_rows) {
                     const int4* src = reinterpret_cast<const int4*>(f.rows + R);
@@ -265,11 +385,17 @@ fused_tc_kernel(const TcParams p) {
             }
             for (int kb = 0; kb < p.n_kb; ++kb, ++it) {
                 const uint32_t stage = it & 1u, ph = (it >> 1) & 1u;
+                if (p.debug & 1) {
+                    ptx::mbar_wait(sm.a_empty + 8 * stage, ph ^ 1u);
+                    __syncwarp();
+                    if (lane == 0) ptx::mbar_arrive(sm.a_full + 8 * stage);
+                    continue;
+                }
                 const int nu0 = kb * kTcBK + chunk * 4;
                 const float4 X = ldg4(f.Xn + nu0), G = ldg4(f.Gs + nu0);
-                float4 L0[4], L1[4], S[4];
+                float4 L0[kTcRowsPerThread], L1[kTcRowsPerThread], S[kTcRowsPerThread];
 #pragma unroll
-                for (int j = 0; j < 4; ++j) {
+                for (int j = 0; j < kTcRowsPerThread; ++j) {
                     L0[j] = ldg4(lutp[j] + kb * kTcBK);
                     L1[j] = ldg4(lutp[j] + nfp + kb * kTcBK);
                     S[j] = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -298,24 +424,26 @@ fused_tc_kernel(const TcParams p) {
                 ptx::mbar_wait(sm.a_empty + 8 * stage, ph ^ 1u);
                 unsigned char* a_hi = smem_raw + (sm.a - raw) + stage * kTcAStageBytes;
 #pragma unroll
-                for (int j = 0; j < 4; ++j) {
+                for (int j = 0; j < kTcRowsPerThread; ++j) {
                     float4 v, hi, lo;
-                    v.x = element_value(fmaf(fp[j], L1[j].x - L0[j].x, L0[j].x), csc[j], X.x, G.x * S[j].x);
-                    v.y = element_value(fmaf(fp[j], L1[j].y - L0[j].y, L0[j].y), csc[j], X.y, G.y * S[j].y);
-                    v.z = element_value(fmaf(fp[j], L1[j].z - L0[j].z, L0[j].z), csc[j], X.z, G.z * S[j].z);
-                    v.w = element_value(fmaf(fp[j], L1[j].w - L0[j].w, L0[j].w), csc[j], X.w, G.w * S[j].w);
-                    hi.x = ptx::to_tf32(v.x); hi.y = ptx::to_tf32(v.y); hi.z = ptx::to_tf32(v.z); hi.w = ptx::to_tf32(v.w);
-                    lo.x = ptx::to_tf32(v.x - hi.x); lo.y = ptx::to_tf32(v.y - hi.y);
-                    lo.z = ptx::to_tf32(v.z - hi.z); lo.w = ptx::to_tf32(v.w - hi.w);
-                    const uint32_t off = (uint32_t)(rsub + 32 * j) * 128u + swz;
+                    v.x = element_value_fast(fmaf(fp[j], L1[j].x - L0[j].x, L0[j].x), csc[j], X.x, G.x * S[j].x);
+                    v.y = element_value_fast(fmaf(fp[j], L1[j].y - L0[j].y, L0[j].y), csc[j], X.y, G.y * S[j].y);
+                    v.z = element_value_fast(fmaf(fp[j], L1[j].z - L0[j].z, L0[j].z), csc[j], X.z, G.z * S[j].z);
+                    v.w = element_value_fast(fmaf(fp[j], L1[j].w - L0[j].w, L0[j].w), csc[j], X.w, G.w * S[j].w);
+                    // tf32 split: hi = top 19 bits of v (the tensor core reads no more), lo = v - hi exactly;
+                    // the hardware's own truncation of lo to tf32 leaves an error of 2^-21 |v| at most
+                    hi.x = ptx::tf32_trunc(v.x); hi.y = ptx::tf32_trunc(v.y); hi.z = ptx::tf32_trunc(v.z); hi.w = ptx::tf32_trunc(v.w);
+                    lo.x = v.x - hi.x; lo.y = v.y - hi.y; lo.z = v.z - hi.z; lo.w = v.w - hi.w;
+                    const uint32_t off = (uint32_t)(rsub + kTcRowStride * j) * 128u + swz;
                     *reinterpret_cast<float4*>(a_hi + off) = hi;
                     *reinterpret_cast<float4*>(a_hi + kTcAPartBytes + off) = lo;
                 }
                 ptx::fence_proxy_async_smem();
-                ptx::mbar_arrive(sm.a_full + 8 * stage);
+                __syncwarp();
+                if (lane == 0) ptx::mbar_arrive(sm.a_full + 8 * stage);
             }
         }
-    } else if (warp >= kTcWarpLoader && warp < kTcWarpGen0) {
+    } else if (warp >= kTcWarpCtl0) {
       ptx::setmaxnreg_dec<kTcRegsCtl>();
       if (warp == kTcWarpLoader) {
         // =========================== loader: filter slab images -> B ring =====================
@@ -327,6 +455,7 @@ fused_tc_kernel(const TcParams p) {
                 for (int u = 0; u < 2 * p.n_kb; ++u, ++ub) {
                     const uint32_t bs = ub % (uint32_t)p.b_stages, bph = (ub / (uint32_t)p.b_stages) & 1u;
                     ptx::mbar_wait(sm.b_empty + 8 * bs, bph ^ 1u);
+                    if (p.debug & 4) { ptx::mbar_arrive(sm.b_full + 8 * bs); continue; }
                     ptx::mbar_arrive_expect_tx(sm.b_full + 8 * bs, (uint32_t)p.unit_bytes);
                     ptx::bulk_g2s(sm.b + bs * (uint32_t)p.unit_bytes, src + (size_t)u * p.unit_bytes,
                                   (uint32_t)p.unit_bytes, sm.b_full + 8 * bs);
@@ -336,74 +465,84 @@ fused_tc_kernel(const TcParams p) {
         __syncwarp();
       } else if (warp == kTcWarpMma) {
         // =========================== MMA issuer =================================================
+        if (lane == 0 && (p.debug & 64) && blockIdx.x == 0) {
+            // latency probe: tcgen05.commit -> mbarrier flip, 64 round trips
+            const uint32_t dbar = sm.slot + 16;
+            ptx::mbar_init(dbar, 1); ptx::fence_mbar_init();
+            long long t0 = clock64();
+            for (uint32_t i = 0; i < 64; ++i) { ptx::tc_commit(dbar); ptx::mbar_wait(dbar, i & 1u); }
+            long long t1 = clock64();
+            printf("tcgen05.commit -> wait round trip: %lld cycles\n", (t1 - t0) / 64);
+        }
         if (lane == 0) {
             TcRotation rot(p.n_cg, p.seg, p.n_kb);
-            uint32_t idesc[kTcMaxCg], uses[kTcNumBuf] = {0u, 0u, 0u, 0u};
-            bool fresh[kTcMaxCg];              // next MMA into buf[g] overwrites (first of a segment)
+            uint32_t idesc[kTcMaxCg];
+            uint32_t fresh = 7u;               // bit g: next MMA into buf(g) overwrites (first of a segment)
+            uint32_t used = 0u, par = 0u;      // bit b: buffer b was flushed before / parity of its flush count
 #pragma unroll
-            for (int g = 0; g < kTcMaxCg; ++g) {
-                idesc[g] = ptx::idesc_tf32(kTcBM, g < p.n_cg ? rot.width(g, p.nb_tot) : 16);
-                fresh[g] = true;
-            }
-            uint32_t it = 0, ub = 0;
+            for (int g = 0; g < kTcMaxCg; ++g) idesc[g] = ptx::idesc_tf32(kTcBM, g < p.n_cg ? rot.width(g, p.nb_tot) : 16);
+            const bool issue = !(p.debug & 2);
+            uint32_t it = 0, bs = 0, bph = 0;
             for (int64_t tl = blockIdx.x; tl < n_tiles; tl += gridDim.x) {
                 for (int kb = 0; kb < p.n_kb; ++kb, ++it) {
                     const uint32_t stage = it & 1u, ph = (it >> 1) & 1u;
+                    uint32_t d[kTcMaxCg];
                     // a group that has just moved to another buffer waits until the epilogue has drained it
 #pragma unroll
-                    for (int g = 0; g < kTcMaxCg; ++g)
-                        if (g < p.n_cg && fresh[g]) {
-                            const int b = rot.buf[g];
-                            if (uses[b] > 0) ptx::mbar_wait(sm.buf_free + 8 * b, (uses[b] - 1u) & 1u);
-                        }
+                    for (int g = 0; g < kTcMaxCg; ++g) {
+                        const uint32_t b = (uint32_t)rot.buf(g);
+                        d[g] = tmem_base + b * (uint32_t)kTcBufCols;
+                        if (g < p.n_cg && (fresh >> g & 1u) && (used >> b & 1u))
+                            ptx::mbar_wait(sm.buf_free + 8 * b, par >> b & 1u);
+                    }
                     ptx::mbar_wait(sm.a_full + 8 * stage, ph);
-                    const uint32_t a_hi = sm.a + stage * kTcAStageBytes, a_lo = a_hi + kTcAPartBytes;
+                    const uint64_t ad_hi = ptx::smem_desc_sw128(sm.a + stage * kTcAStageBytes);
+                    const uint64_t ad_lo = ad_hi + (uint64_t)(kTcAPartBytes >> 4);
                     {   // filter hi part: acc += A_hi.B_hi + A_lo.B_hi
-                        const uint32_t bs = ub % (uint32_t)p.b_stages, bph = (ub / (uint32_t)p.b_stages) & 1u;
                         ptx::mbar_wait(sm.b_full + 8 * bs, bph);
                         ptx::tc_fence_after();
-                        const uint32_t b0 = sm.b + bs * (uint32_t)p.unit_bytes;
+                        const uint64_t bd0 = ptx::smem_desc_sw128(sm.b + bs * (uint32_t)p.unit_bytes);
+                        if (issue) {
 #pragma unroll
-                        for (int k = 0; k < kTcBK / kTcUK; ++k)
+                            for (int k = 0; k < kTcBK / kTcUK; ++k)
 #pragma unroll
-                            for (int g = 0; g < kTcMaxCg; ++g)
-                                if (g < p.n_cg) {
-                                    const uint64_t bd = ptx::smem_desc_sw128(b0 + (uint32_t)(g * kTcBufCols) * 128u + k * 32u);
-                                    const uint32_t d = tmem_base + (uint32_t)(rot.buf[g] * kTcBufCols);
-                                    ptx::mma_tf32_ss(d, ptx::smem_desc_sw128(a_hi + k * 32u), bd, idesc[g], (k != 0 || !fresh[g]) ? 1u : 0u);
-                                    ptx::mma_tf32_ss(d, ptx::smem_desc_sw128(a_lo + k * 32u), bd, idesc[g], 1u);
-                                }
+                                for (int g = 0; g < kTcMaxCg; ++g)
+                                    if (g < p.n_cg) {
+                                        const uint64_t bd = bd0 + (uint64_t)(g * (kTcBufCols * 128 >> 4) + k * 2);
+                                        ptx::mma_tf32_ss(d[g], ad_hi + (uint64_t)(k * 2), bd, idesc[g], (k != 0 || !(fresh >> g & 1u)) ? 1u : 0u);
+                                        ptx::mma_tf32_ss(d[g], ad_lo + (uint64_t)(k * 2), bd, idesc[g], 1u);
+                                    }
+                        }
                         ptx::tc_commit(sm.b_empty + 8 * bs);
-                        ++ub;
+                        if (++bs == (uint32_t)p.b_stages) { bs = 0; bph ^= 1u; }
                     }
                     {   // filter lo part: acc += A_hi.B_lo
-                        const uint32_t bs = ub % (uint32_t)p.b_stages, bph = (ub / (uint32_t)p.b_stages) & 1u;
                         ptx::mbar_wait(sm.b_full + 8 * bs, bph);
                         ptx::tc_fence_after();
-                        const uint32_t b0 = sm.b + bs * (uint32_t)p.unit_bytes;
+                        const uint64_t bd0 = ptx::smem_desc_sw128(sm.b + bs * (uint32_t)p.unit_bytes);
+                        if (issue) {
 #pragma unroll
-                        for (int k = 0; k < kTcBK / kTcUK; ++k)
+                            for (int k = 0; k < kTcBK / kTcUK; ++k)
 #pragma unroll
-                            for (int g = 0; g < kTcMaxCg; ++g)
-                                if (g < p.n_cg) {
-                                    const uint64_t bd = ptx::smem_desc_sw128(b0 + (uint32_t)(g * kTcBufCols) * 128u + k * 32u);
-                                    ptx::mma_tf32_ss(tmem_base + (uint32_t)(rot.buf[g] * kTcBufCols),
-                                                     ptx::smem_desc_sw128(a_hi + k * 32u), bd, idesc[g], 1u);
-                                }
+                                for (int g = 0; g < kTcMaxCg; ++g)
+                                    if (g < p.n_cg)
+                                        ptx::mma_tf32_ss(d[g], ad_hi + (uint64_t)(k * 2),
+                                                         bd0 + (uint64_t)(g * (kTcBufCols * 128 >> 4) + k * 2), idesc[g], 1u);
+                        }
                         ptx::tc_commit(sm.b_empty + 8 * bs);
-                        ++ub;
+                        if (++bs == (uint32_t)p.b_stages) { bs = 0; bph ^= 1u; }
                     }
                     ptx::tc_commit(sm.a_empty + 8 * stage);
                     // segment boundaries: hand the finished partial sums to the epilogue, move on to a free buffer
+                    fresh = 0u;
 #pragma unroll
                     for (int g = 0; g < kTcMaxCg; ++g) {
-                        if (g >= p.n_cg) continue;
-                        fresh[g] = false;
-                        if (rot.boundary(kb, g)) {
-                            const int old = rot.rotate(g);
+                        if (g < p.n_cg && rot.boundary(kb, g)) {
+                            const uint32_t old = (uint32_t)rot.rotate(g);
                             ptx::tc_commit(sm.flush_full + 8 * old);
-                            ++uses[old];
-                            fresh[g] = true;
+                            par ^= (used >> old & 1u) << old;      // parity of (flush count - 1) once used
+                            used |= 1u << old;
+                            fresh |= 1u << g;
                         }
                     }
                 }
@@ -411,9 +550,9 @@ fused_tc_kernel(const TcParams p) {
         }
         __syncwarp();
       }
-    } else if (warp >= kTcWarpFin0) {
+    } else if (warp >= kTcWarpFin0 && warp < kTcWarpCtl0) {
         // ============ finisher: scratch tile -> P = sum*scale + bias, photon noise -> TOD ========
-        ptx::setmaxnreg_dec<kTcRegsFin>();
+        ptx::setmaxnreg_inc<kTcRegsFin>();
         const int q = warp - kTcWarpFin0;
         uint32_t ti = 0;
         for (int64_t tl = blockIdx.x; tl < n_tiles; tl += gridDim.x, ++ti) {
@@ -426,7 +565,7 @@ fused_tc_kernel(const TcParams p) {
             constexpr int kMaxPerLane = kTcMaxGroupChan / 32;             // 12
             for (int r = q; r < kTcBM; r += kTcFinWarps) {
                 const int64_t Rr = row0 + r;
-                if (Rr >= f.n_rows) break;
+                if (Rr >= f.n_rows || (p.debug & 8)) break;
                 const uint32_t n = (uint32_t)(f.t0 + Rr / f.n_spaxel), s = (uint32_t)(Rr % f.n_spaxel);
                 float* o = f.out + (size_t)Rr * f.n_chan + cg0;
                 float x[kMaxPerLane];
@@ -435,29 +574,42 @@ fused_tc_kernel(const TcParams p) {
                     const int c = lane + 32 * j;
                     x[j] = c < n_valid ? __ldcg(sc + (size_t)c * kTcBM + r) : 0.f;
                 }
+                constexpr int W = 4;                                      // channels in flight per lane
 #pragma unroll
-                for (int j = 0; j < kMaxPerLane; ++j) {
-                    const int c = lane + 32 * j;
-                    if (c < n_valid) {
-                        float P = fmaf(x[j], f.scale, __ldg(f.bias + cg0 + c));
-                        if (f.photon_noise) {
-                            const uint4 w = philox4x32_10(n, s, (uint32_t)(cg0 + c), kStreamPhoton, f.seed_lo, f.seed_hi);
-                            P = fmaf(photon_sigma(P, __ldg(f.noise_c1 + cg0 + c), __ldg(f.noise_c2 + cg0 + c)),
-                                     normal_cos(w.x, w.y), P);
-                        }
-                        o[c] = P;
+                for (int j0 = 0; j0 < kMaxPerLane; j0 += W) {
+                    if (lane + 32 * j0 >= n_valid) break;
+                    float P[W], n1[W], n2[W];
+                    uint32_t cc[W], w0[W], w1[W];
+#pragma unroll
+                    for (int i = 0; i < W; ++i) {
+                        const int c = min(lane + 32 * (j0 + i), n_valid - 1);
+                        cc[i] = (uint32_t)(cg0 + c);
+                        P[i] = fmaf(x[j0 + i], f.scale, __ldg(f.bias + cc[i]));
+                        n1[i] = __ldg(f.noise_c1 + cc[i]); n2[i] = __ldg(f.noise_c2 + cc[i]);
+                    }
+                    if (f.photon_noise) {
+                        philox4x32_10_multi<W>(n, s, cc, kStreamPhoton, f.seed_lo, f.seed_hi, w0, w1);
+#pragma unroll
+                        for (int i = 0; i < W; ++i)
+                            P[i] = fmaf(photon_sigma(P[i], n1[i], n2[i]), normal_cos(w0[i], w1[i]), P[i]);
+                    }
+#pragma unroll
+                    for (int i = 0; i < W; ++i) {
+                        const int c = lane + 32 * (j0 + i);
+                        if (c < n_valid) o[c] = P[i];
                     }
                 }
             }
-            ptx::mbar_arrive(sm.scratch_free + 8 * sb);
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(sm.scratch_free + 8 * sb);
         }
     } else {
         // ============ epilogue: segment flushes of the accumulators into the scratch tile =======
-        ptx::setmaxnreg_inc<kTcRegsFlush>();
+        ptx::setmaxnreg_dec<kTcRegsFlush>();
         const int q = warp;                                    // tensor-memory lane quarter
         const int trow = 32 * q + lane;                        // tile row = tensor-memory lane
         TcRotation rot(p.n_cg, p.seg, p.n_kb);
-        uint32_t fulls[kTcNumBuf] = {0u, 0u, 0u, 0u};
+        uint32_t fulls = 0u;                                   // bit b: parity of buffer b's flush count
         uint32_t ti = 0;
         for (int64_t tl = blockIdx.x; tl < n_tiles; tl += gridDim.x, ++ti) {
             const uint32_t sb = ti & 1u;
@@ -473,45 +625,35 @@ fused_tc_kernel(const TcParams p) {
                     float* scg = sc + (size_t)(g * kTcBufCols) * kTcBM + trow;
                     const uint32_t taddr = tmem_base + ((uint32_t)(32 * q) << 16) + (uint32_t)(b * kTcBufCols);
                     const bool add = !first[g];
-                    uint32_t v[32];
-                    float pa[32], pb[32];
-                    // the running sums of the first 32 columns are fetched while the MMAs still run
+                    uint32_t v[16];
+                    float pa[16];
+                    // the running sums of the first 16 columns are fetched while the MMAs still run
                     if (add) {
 #pragma unroll
-                        for (int i = 0; i < 32; ++i) pa[i] = __ldcg(scg + (size_t)i * kTcBM);
+                        for (int i = 0; i < 16; ++i) pa[i] = __ldcg(scg + (size_t)i * kTcBM);
                     }
-                    ptx::mbar_wait(sm.flush_full + 8 * b, fulls[b] & 1u);
-                    ++fulls[b];
+                    ptx::mbar_wait(sm.flush_full + 8 * b, fulls >> b & 1u);
+                    fulls ^= 1u << b;
                     ptx::tc_fence_after();
-                    for (int c0 = 0; c0 < wg; c0 += 64) {
-                        const bool two = c0 + 32 < wg;
-                        ptx::tmem_ld_32x32(taddr + (uint32_t)c0, v);
-                        if (add && two) {
-#pragma unroll
-                            for (int i = 0; i < 32; ++i) pb[i] = __ldcg(scg + (size_t)(c0 + 32 + i) * kTcBM);
-                        }
+                    for (int c0 = 0; c0 < wg; c0 += 16) {
+                        ptx::tmem_ld_32x16(taddr + (uint32_t)c0, v);
                         ptx::tmem_ld_wait();
 #pragma unroll
-                        for (int i = 0; i < 32; ++i)
-                            __stcg(scg + (size_t)(c0 + i) * kTcBM, add ? pa[i] + __uint_as_float(v[i]) : __uint_as_float(v[i]));
-                        if (two) {
-                            ptx::tmem_ld_32x32(taddr + (uint32_t)(c0 + 32), v);
-                            if (add && c0 + 64 < wg) {
-#pragma unroll
-                                for (int i = 0; i < 32; ++i) pa[i] = __ldcg(scg + (size_t)(c0 + 64 + i) * kTcBM);
-                            }
-                            ptx::tmem_ld_wait();
-#pragma unroll
-                            for (int i = 0; i < 32; ++i)
-                                __stcg(scg + (size_t)(c0 + 32 + i) * kTcBM, add ? pb[i] + __uint_as_float(v[i]) : __uint_as_float(v[i]));
+                        for (int i = 0; i < 16; ++i) {
+                            const float sum = add ? pa[i] + __uint_as_float(v[i]) : __uint_as_float(v[i]);
+                            __stcg(scg + (size_t)(c0 + i) * kTcBM, sum);
+                            if (add && c0 + 16 < wg) pa[i] = __ldcg(scg + (size_t)(c0 + 16 + i) * kTcBM);
                         }
                     }
                     ptx::tc_fence_before();
-                    ptx::mbar_arrive(sm.buf_free + 8 * b);
+                    __syncwarp();
+                    if (lane == 0) ptx::mbar_arrive(sm.buf_free + 8 * b);
                     first[g] = false;
                 }
             // every partial sum of the tile is in the scratch tile: hand it to the finisher warps
-            ptx::mbar_arrive(sm.tile_done + 8 * sb);
+            __threadfence_block();
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(sm.tile_done + 8 * sb);
         }
     }
 
@@ -530,6 +672,7 @@ inline cudaError_t launch_fused_tc(const FusedParams& fp, const TcTables& t, int
     p.n_groups = t.n_groups; p.nb_tot = t.nb_tot; p.n_cg = t.n_cg; p.seg = t.seg > 0 ? t.seg : kTcSegDefault; p.n_kb = t.n_kb;
     p.unit_bytes = t.unit_bytes; p.b_stages = t.b_stages;
     p.n_row_tiles = (int32_t)((fp.n_rows + kTcBM - 1) / kTcBM);
+    if (const char* e = std::getenv("GATEAU_TC_DEBUG")) p.debug = std::atoi(e);
     p.cube_vec = (fp.cube == nullptr) || ((fp.n_freq % 4 == 0) && ((reinterpret_cast<uintptr_t>(fp.cube) & 15u) == 0));
     const int64_t n_tiles = (int64_t)p.n_row_tiles * p.n_groups;
     const unsigned grid = (unsigned)std::min<int64_t>(n_tiles, num_sms);
