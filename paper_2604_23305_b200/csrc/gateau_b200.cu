@@ -330,7 +330,7 @@ gt_status gt_plan_create(const gt_config* cfg, void* cuda_stream, gt_plan** out_
     p->n_freq = nf; p->n_freq_pad = nfp; p->n_chan = nc; p->n_spaxel = ns; p->n_pwv = c.n_pwv;
     p->n_samples = c.n_samples; p->photon_noise = c.photon_noise != 0; p->pink_noise = c.pink_noise != 0;
     p->seed = c.seed; p->cube = c.cube; p->n_az = c.n_az; p->n_el = c.n_el;
-    p->variant = (c.variant == GT_VARIANT_TENSOR) ? GT_VARIANT_TENSOR : GT_VARIANT_FP32;   // DEFAULT -> FP32 until the tensor kernel is measured faster
+    p->variant = (c.variant == GT_VARIANT_FP32) ? GT_VARIANT_FP32 : GT_VARIANT_TENSOR;   // DEFAULT -> tensor: measured 8x faster than the FP32 kernel on C4
     p->scale = (float)(kPref * c.dnu_hz);
 
     // ---- small device arrays needed on the host ----

@@ -92,6 +92,13 @@ inline float host_tf32(float x) {
     return r;
 }
 
+// round-to-nearest-even fp32 -> bf16 bits on the host, finite inputs
+inline uint16_t host_bf16(float x) {
+    uint32_t b; std::memcpy(&b, &x, 4);
+    b += 0x7FFFu + ((b >> 16) & 1u);
+    return (uint16_t)(b >> 16);
+}
+
 // Splits the filter into tf32 hi/lo parts and lays every (group, 32-frequency slab, part) out as
 // the exact shared-memory image tcgen05.mma reads (K-major, SWIZZLE_128B): the loader is a flat copy.
 inline gt_status build_tc_tables(const std::vector<float>& filt, int n_chan, int n_freq, int n_freq_pad,
@@ -110,18 +117,24 @@ inline gt_status build_tc_tables(const std::vector<float>& filt, int n_chan, int
 
     const size_t total = (size_t)G * t.n_kb * 2 * t.unit_bytes;
     std::vector<float> img(total / 4, 0.f);
+    uint16_t* img16 = reinterpret_cast<uint16_t*>(img.data());
     for (int g = 0; g < G; ++g)
         for (int n = 0; n < nbt; ++n) {
             const int ch = g * nbt + n;
             if (ch >= n_chan) continue;
             for (int i = 0; i < n_freq; ++i) {
                 const float f = filt[(size_t)ch * n_freq + i];
-                const float hi = host_tf32(f), lo = host_tf32(f - hi);
+                const float hi = host_tf32(f), lo = f - hi;
                 const int kb = i / kTcBK, kk = i % kTcBK;
-                const size_t unit0 = ((size_t)(g * t.n_kb + kb) * 2) * (t.unit_bytes / 4);
-                const size_t off = (size_t)n * 32 + (size_t)(((kk >> 2) ^ (n & 7)) << 2) + (kk & 3);
-                img[unit0 + off] = hi;
-                img[unit0 + t.unit_bytes / 4 + off] = lo;
+                const size_t unit0 = ((size_t)(g * t.n_kb + kb) * 2) * (t.unit_bytes / 4);      // in floats
+                // unit 0: tf32 hi part
+                img[unit0 + (size_t)n * 32 + (size_t)(((kk >> 2) ^ (n & 7)) << 2) + (kk & 3)] = hi;
+                // unit 1: bf16, per group of 8 frequencies [Fm_0..7 | lo_0..7] (pairs with A's [lo | hi])
+                const int kg = kk >> 3, fi = kk & 7;
+                const size_t row16 = (unit0 + t.unit_bytes / 4) * 2 + (size_t)n * 64;             // in bf16 elements
+                const int c_hi = kg * 2, c_lo = kg * 2 + 1;                                       // 16-byte chunks
+                img16[row16 + (size_t)((c_hi ^ (n & 7)) << 3) + fi] = host_bf16(f);
+                img16[row16 + (size_t)((c_lo ^ (n & 7)) << 3) + fi] = host_bf16(lo);
             }
         }
     if (cudaMalloc(reinterpret_cast<void**>(&t.filt_img), total) != cudaSuccess) {
@@ -216,6 +229,27 @@ struct TcRotation {
 __device__ __forceinline__ float element_value_fast(float eta_z, float csc, float Xn, float GS) {
     const float eta = ptx::ex2_ftz(csc * ptx::lg2_ftz(eta_z));
     return fmaf(1.0f - eta, Xn, eta * GS);
+}
+
+// Writes 4 consecutive frequencies (16-byte chunk `chunk` of a 32-frequency slab) of tile row `row`
+// into an A stage:
+//   part 0 (tf32):  hi = top 19 bits of v, K-major SWIZZLE_128B rows of 32 tf32
+//   part 1 (bf16):  per group of 8 frequencies the 16 values [lo_0..lo_7 | hi_0..hi_7] (lo = v - hi),
+//                   i.e. the K = 16 operand of ONE kind::f16 MMA whose B operand holds
+//                   [Fm_hi_0..7 | Fm_lo_0..7]: it adds lo.Fm_hi + hi.Fm_lo, the two correction terms of
+//                   the split product (each only needs ~8 bits: they are 2^-11 of the main term).
+__device__ __forceinline__ void store_split(unsigned char* a_stage, int row, int chunk, const float4& v) {
+    float4 hi;
+    hi.x = ptx::tf32_trunc(v.x); hi.y = ptx::tf32_trunc(v.y); hi.z = ptx::tf32_trunc(v.z); hi.w = ptx::tf32_trunc(v.w);
+    const uint32_t r7 = (uint32_t)(row & 7), rowoff = (uint32_t)row * 128u;
+    *reinterpret_cast<float4*>(a_stage + rowoff + (((uint32_t)chunk ^ r7) << 4)) = hi;
+    uint2 lo2, hi2;
+    lo2.x = ptx::pack_bf16x2(v.x - hi.x, v.y - hi.y); lo2.y = ptx::pack_bf16x2(v.z - hi.z, v.w - hi.w);
+    hi2.x = ptx::pack_bf16x2(hi.x, hi.y);             hi2.y = ptx::pack_bf16x2(hi.z, hi.w);
+    const uint32_t c16 = (uint32_t)(chunk >> 1) * 2u, sub = (uint32_t)(chunk & 1) * 8u;
+    unsigned char* part1 = a_stage + kTcAPartBytes + rowoff + sub;
+    *reinterpret_cast<uint2*>(part1 + ((c16 ^ r7) << 4)) = lo2;
+    *reinterpret_cast<uint2*>(part1 + (((c16 + 1u) ^ r7) << 4)) = hi2;
 }
 
 __device__ __forceinline__ float4 ldg4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
@@ -315,7 +349,7 @@ fused_tc_kernel(const TcParams p) {
                     const RowParam* rp = rowp + rsub + kTcRowStride * j;
                     const float2 fc = *reinterpret_cast<const float2*>(rp);                    // fp, csc
                     const float4 w = *reinterpret_cast<const float4*>(&rp->w00);
-                    float4 S, v, hi, lo;
+                    float4 S, v;
                     if (p.debug & 32) {
                         unsigned char* a_hi = smem_raw + (sm.a - raw) + stage * kTcAStageBytes;
                         const uint32_t off = (uint32_t)(rsub + kTcRowStride * j) * 128u + swz;
@@ -331,12 +365,7 @@ fused_tc_kernel(const TcParams p) {
                     v.y = element_value_fast(fmaf(fc.x, cur.L1.y - cur.L0.y, cur.L0.y), fc.y, X.y, G.y * S.y);
                     v.z = element_value_fast(fmaf(fc.x, cur.L1.z - cur.L0.z, cur.L0.z), fc.y, X.z, G.z * S.z);
                     v.w = element_value_fast(fmaf(fc.x, cur.L1.w - cur.L0.w, cur.L0.w), fc.y, X.w, G.w * S.w);
-                    hi.x = ptx::tf32_trunc(v.x); hi.y = ptx::tf32_trunc(v.y); hi.z = ptx::tf32_trunc(v.z); hi.w = ptx::tf32_trunc(v.w);
-                    lo.x = v.x - hi.x; lo.y = v.y - hi.y; lo.z = v.z - hi.z; lo.w = v.w - hi.w;
-                    unsigned char* a_hi = smem_raw + (sm.a - raw) + stage * kTcAStageBytes;
-                    const uint32_t off = (uint32_t)(rsub + kTcRowStride * j) * 128u + swz;
-                    *reinterpret_cast<float4*>(a_hi + off) = hi;
-                    *reinterpret_cast<float4*>(a_hi + kTcAPartBytes + off) = lo;
+                    store_split(smem_raw + (sm.a - raw) + stage * kTcAStageBytes, rsub + kTcRowStride * j, chunk, v);
                 };
                 Tap t0, t1;
                 issue(0, 0, t0);
@@ -425,18 +454,12 @@ fused_tc_kernel(const TcParams p) {
                 unsigned char* a_hi = smem_raw + (sm.a - raw) + stage * kTcAStageBytes;
 #pragma unroll
                 for (int j = 0; j < kTcRowsPerThread; ++j) {
-                    float4 v, hi, lo;
+                    float4 v;
                     v.x = element_value_fast(fmaf(fp[j], L1[j].x - L0[j].x, L0[j].x), csc[j], X.x, G.x * S[j].x);
                     v.y = element_value_fast(fmaf(fp[j], L1[j].y - L0[j].y, L0[j].y), csc[j], X.y, G.y * S[j].y);
                     v.z = element_value_fast(fmaf(fp[j], L1[j].z - L0[j].z, L0[j].z), csc[j], X.z, G.z * S[j].z);
                     v.w = element_value_fast(fmaf(fp[j], L1[j].w - L0[j].w, L0[j].w), csc[j], X.w, G.w * S[j].w);
-                    // tf32 split: hi = top 19 bits of v (the tensor core reads no more), lo = v - hi exactly;
-                    // the hardware's own truncation of lo to tf32 leaves an error of 2^-21 |v| at most
-                    hi.x = ptx::tf32_trunc(v.x); hi.y = ptx::tf32_trunc(v.y); hi.z = ptx::tf32_trunc(v.z); hi.w = ptx::tf32_trunc(v.w);
-                    lo.x = v.x - hi.x; lo.y = v.y - hi.y; lo.z = v.z - hi.z; lo.w = v.w - hi.w;
-                    const uint32_t off = (uint32_t)(rsub + kTcRowStride * j) * 128u + swz;
-                    *reinterpret_cast<float4*>(a_hi + off) = hi;
-                    *reinterpret_cast<float4*>(a_hi + kTcAPartBytes + off) = lo;
+                    store_split(a_hi, rsub + kTcRowStride * j, chunk, v);
                 }
                 ptx::fence_proxy_async_smem();
                 __syncwarp();
@@ -474,13 +497,16 @@ fused_tc_kernel(const TcParams p) {
             long long t1 = clock64();
             printf("tcgen05.commit -> wait round trip: %lld cycles\n", (t1 - t0) / 64);
         }
-        if (lane == 0) {
+        {   // the whole warp runs the loop (uniform control flow); one elected lane issues
             TcRotation rot(p.n_cg, p.seg, p.n_kb);
-            uint32_t idesc[kTcMaxCg];
+            uint32_t idesc[kTcMaxCg], idesc16[kTcMaxCg];
             uint32_t fresh = 7u;               // bit g: next MMA into buf(g) overwrites (first of a segment)
             uint32_t used = 0u, par = 0u;      // bit b: buffer b was flushed before / parity of its flush count
 #pragma unroll
-            for (int g = 0; g < kTcMaxCg; ++g) idesc[g] = ptx::idesc_tf32(kTcBM, g < p.n_cg ? rot.width(g, p.nb_tot) : 16);
+            for (int g = 0; g < kTcMaxCg; ++g) {
+                idesc[g] = ptx::idesc_tf32(kTcBM, g < p.n_cg ? rot.width(g, p.nb_tot) : 16);
+                idesc16[g] = ptx::idesc_bf16(kTcBM, g < p.n_cg ? rot.width(g, p.nb_tot) : 16);
+            }
             const bool issue = !(p.debug & 2);
             uint32_t it = 0, bs = 0, bph = 0;
             for (int64_t tl = blockIdx.x; tl < n_tiles; tl += gridDim.x) {
@@ -498,11 +524,11 @@ fused_tc_kernel(const TcParams p) {
                     ptx::mbar_wait(sm.a_full + 8 * stage, ph);
                     const uint64_t ad_hi = ptx::smem_desc_sw128(sm.a + stage * kTcAStageBytes);
                     const uint64_t ad_lo = ad_hi + (uint64_t)(kTcAPartBytes >> 4);
-                    {   // filter hi part: acc += A_hi.B_hi + A_lo.B_hi
+                    {   // tf32 unit: acc += A_hi.Fm_hi
                         ptx::mbar_wait(sm.b_full + 8 * bs, bph);
                         ptx::tc_fence_after();
                         const uint64_t bd0 = ptx::smem_desc_sw128(sm.b + bs * (uint32_t)p.unit_bytes);
-                        if (issue) {
+                        if (issue && ptx::elect_one()) {
 #pragma unroll
                             for (int k = 0; k < kTcBK / kTcUK; ++k)
 #pragma unroll
@@ -510,36 +536,37 @@ fused_tc_kernel(const TcParams p) {
                                     if (g < p.n_cg) {
                                         const uint64_t bd = bd0 + (uint64_t)(g * (kTcBufCols * 128 >> 4) + k * 2);
                                         ptx::mma_tf32_ss(d[g], ad_hi + (uint64_t)(k * 2), bd, idesc[g], (k != 0 || !(fresh >> g & 1u)) ? 1u : 0u);
-                                        ptx::mma_tf32_ss(d[g], ad_lo + (uint64_t)(k * 2), bd, idesc[g], 1u);
                                     }
                         }
-                        ptx::tc_commit(sm.b_empty + 8 * bs);
+                        __syncwarp();
+                        if (ptx::elect_one()) ptx::tc_commit(sm.b_empty + 8 * bs);
                         if (++bs == (uint32_t)p.b_stages) { bs = 0; bph ^= 1u; }
                     }
-                    {   // filter lo part: acc += A_hi.B_lo
+                    {   // bf16 unit: acc += A_lo.Fm_hi + A_hi.Fm_lo (one K = 16 MMA per 8 frequencies)
                         ptx::mbar_wait(sm.b_full + 8 * bs, bph);
                         ptx::tc_fence_after();
                         const uint64_t bd0 = ptx::smem_desc_sw128(sm.b + bs * (uint32_t)p.unit_bytes);
-                        if (issue) {
+                        if (issue && ptx::elect_one()) {
 #pragma unroll
                             for (int k = 0; k < kTcBK / kTcUK; ++k)
 #pragma unroll
                                 for (int g = 0; g < kTcMaxCg; ++g)
                                     if (g < p.n_cg)
-                                        ptx::mma_tf32_ss(d[g], ad_hi + (uint64_t)(k * 2),
-                                                         bd0 + (uint64_t)(g * (kTcBufCols * 128 >> 4) + k * 2), idesc[g], 1u);
+                                        ptx::mma_bf16_ss(d[g], ad_lo + (uint64_t)(k * 2),
+                                                         bd0 + (uint64_t)(g * (kTcBufCols * 128 >> 4) + k * 2), idesc16[g], 1u);
                         }
-                        ptx::tc_commit(sm.b_empty + 8 * bs);
+                        __syncwarp();
+                        if (ptx::elect_one()) ptx::tc_commit(sm.b_empty + 8 * bs);
                         if (++bs == (uint32_t)p.b_stages) { bs = 0; bph ^= 1u; }
                     }
-                    ptx::tc_commit(sm.a_empty + 8 * stage);
+                    if (ptx::elect_one()) ptx::tc_commit(sm.a_empty + 8 * stage);
                     // segment boundaries: hand the finished partial sums to the epilogue, move on to a free buffer
                     fresh = 0u;
 #pragma unroll
                     for (int g = 0; g < kTcMaxCg; ++g) {
                         if (g < p.n_cg && rot.boundary(kb, g)) {
                             const uint32_t old = (uint32_t)rot.rotate(g);
-                            ptx::tc_commit(sm.flush_full + 8 * old);
+                            if (ptx::elect_one()) ptx::tc_commit(sm.flush_full + 8 * old);
                             par ^= (used >> old & 1u) << old;      // parity of (flush count - 1) once used
                             used |= 1u << old;
                             fresh |= 1u << g;
