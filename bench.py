@@ -176,6 +176,7 @@ def run_ours(args):
     import torch.distributed as dist
     from paper_2604_23305_b200 import binding as B
     from paper_2604_23305_b200 import workloads as W
+    from paper_2604_23305_b200 import shard
 
     rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
@@ -191,7 +192,7 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     w = W.make_workload(args.workload, n_samples=args.samples)
-    w = w.replace(seed=w.seed + 1000 * rank)                      # independent observation per rank
+    w = w.replace(seed=shard.replica_seed(w.seed, rank))          # independent observation per rank
     variant = {"default": B.VARIANT_DEFAULT, "fp32": B.VARIANT_FP32, "tensor": B.VARIANT_TENSOR}[args.variant]
     plan = B.Plan(w, variant=variant, device=f"cuda:{local}")
     units = w.detector_samples()
@@ -216,11 +217,8 @@ def run_ours(args):
     total_ms = float(sum(step_ms))
     launches = plan.launch_count - launches0
     clocks = sampler.stop()
-    t = torch.tensor([total_ms], dtype=torch.float64, device=f"cuda:{local}")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms = float(t.item())
-    value = world * units * args.steps / (total_ms * 1e-3)
+    total_ms = shard.max_over_ranks(total_ms, dist if world > 1 else None, device=f"cuda:{local}")
+    value = shard.aggregate_throughput(units, world, args.steps, total_ms)
 
     # ---- roofline of the dominant kernel (the fused kernel) ----
     pk, pk_src = peaks()
