@@ -31,7 +31,6 @@
 #include <cstring>
 #include <algorithm>
 #include <cstdlib>
-#include <cstdio>
 #include "gt_common.cuh"
 #include "gt_fused_fp32.cuh"
 #include "gt_tc_ptx.cuh"
@@ -488,25 +487,14 @@ fused_tc_kernel(const TcParams p) {
         __syncwarp();
       } else if (warp == kTcWarpMma) {
         // =========================== MMA issuer =================================================
-        if (lane == 0 && (p.debug & 64) && blockIdx.x == 0) {
-            // latency probe: tcgen05.commit -> mbarrier flip, 64 round trips
-            const uint32_t dbar = sm.slot + 16;
-            ptx::mbar_init(dbar, 1); ptx::fence_mbar_init();
-            long long t0 = clock64();
-            for (uint32_t i = 0; i < 64; ++i) { ptx::tc_commit(dbar); ptx::mbar_wait(dbar, i & 1u); }
-            long long t1 = clock64();
-            printf("tcgen05.commit -> wait round trip: %lld cycles\n", (t1 - t0) / 64);
-        }
         {   // the whole warp runs the loop (uniform control flow); one elected lane issues
             TcRotation rot(p.n_cg, p.seg, p.n_kb);
-            uint32_t idesc[kTcMaxCg], idesc16[kTcMaxCg];
+            uint32_t idesc[kTcMaxCg];
+            constexpr uint32_t kToBf16 = (3u << 7) | (3u << 10);      // tf32 (2) -> bf16 (1) in both operand-format fields
             uint32_t fresh = 7u;               // bit g: next MMA into buf(g) overwrites (first of a segment)
             uint32_t used = 0u, par = 0u;      // bit b: buffer b was flushed before / parity of its flush count
 #pragma unroll
-            for (int g = 0; g < kTcMaxCg; ++g) {
-                idesc[g] = ptx::idesc_tf32(kTcBM, g < p.n_cg ? rot.width(g, p.nb_tot) : 16);
-                idesc16[g] = ptx::idesc_bf16(kTcBM, g < p.n_cg ? rot.width(g, p.nb_tot) : 16);
-            }
+            for (int g = 0; g < kTcMaxCg; ++g) idesc[g] = ptx::idesc_tf32(kTcBM, g < p.n_cg ? rot.width(g, p.nb_tot) : 16);
             const bool issue = !(p.debug & 2);
             uint32_t it = 0, bs = 0, bph = 0;
             for (int64_t tl = blockIdx.x; tl < n_tiles; tl += gridDim.x) {
@@ -553,7 +541,7 @@ fused_tc_kernel(const TcParams p) {
                                 for (int g = 0; g < kTcMaxCg; ++g)
                                     if (g < p.n_cg)
                                         ptx::mma_bf16_ss(d[g], ad_lo + (uint64_t)(k * 2),
-                                                         bd0 + (uint64_t)(g * (kTcBufCols * 128 >> 4) + k * 2), idesc16[g], 1u);
+                                                         bd0 + (uint64_t)(g * (kTcBufCols * 128 >> 4) + k * 2), idesc[g] ^ kToBf16, 1u);
                         }
                         __syncwarp();
                         if (ptx::elect_one()) ptx::tc_commit(sm.b_empty + 8 * bs);
