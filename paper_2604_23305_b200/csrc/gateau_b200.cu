@@ -118,6 +118,8 @@ gt_status validate(const gt_config* c) {
     if (c->n_samples > 0xFFFFFFFELL) return fail(nullptr, GT_ERR_SHAPE, "n_samples exceeds the 32-bit Philox counter word");
     if (c->n_stage > 0 && !c->stages) return fail(nullptr, GT_ERR_NULL, "stages is NULL with n_stage > 0");
     if (c->cube && (c->n_az < 2 || c->n_el < 2)) return fail(nullptr, GT_ERR_SHAPE, "source cube needs n_az, n_el >= 2");
+    if (c->cube && (double)c->n_az * (double)c->n_el * (double)c->n_freq >= 4294967296.0)
+        return fail(nullptr, GT_ERR_SHAPE, "source cube of 2^32 elements or more is not supported (32-bit tap offsets)");
     if (c->cube && (!(c->daz_grid_rad > 0) || !(c->del_grid_rad > 0)))
         return fail(nullptr, GT_ERR_VALUE, "source grid steps must be positive");
     if (!(c->f_sample_hz > 0) || !(c->dnu_hz > 0) || !(c->nu0_hz > 0) || !(c->dx_m > 0) || !(c->dy_m > 0) ||

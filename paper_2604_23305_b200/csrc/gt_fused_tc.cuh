@@ -309,7 +309,6 @@ fused_tc_kernel(const TcParams p) {
             // memory (each warp only reads rows it wrote itself).
             struct Tap { float4 L0, L1, c00, c01, c10, c11; };
             RowParam* rowp = reinterpret_cast<RowParam*>(smem_raw + (sm.rowp - raw));
-            const float4 zero4 = make_float4(0.f, 0.f, 0.f, 0.f);
             for (int64_t tl = blockIdx.x; tl < n_tiles; tl += gridDim.x) {
                 const int64_t row0 = (tl / p.n_groups) * kTcBM;
                 __syncwarp();
@@ -326,23 +325,32 @@ fused_tc_kernel(const TcParams p) {
                     } else {
                         rp.fp = 0.f; rp.csc = 1.f; rp.ip = 0; rp.pix = -1; rp.w00 = rp.w01 = rp.w10 = rp.w11 = 0.f;
                     }
-                    if (f.cube == nullptr) rp.pix = -1;
+                    if (f.cube == nullptr || rp.pix < 0) { rp.pix = 0; rp.w00 = rp.w01 = rp.w10 = rp.w11 = 0.f; }
                     rowp[rr] = rp;
                 }
                 __syncwarp();
-                auto issue = [&](int kb, int j, Tap& t) {
+                // 32-bit element offsets of this thread's two rows (plan creation rejects tables of 2^32 elements
+                // or more): one IMAD.WIDE per load instead of 64-bit pointer chains.  Rows outside the cube
+                // carry zero weights and read pixel 0; padded frequencies read the last real chunk (their
+                // filter entries are zero), so every load is unconditional and in bounds.
+                uint32_t lut_off[kTcRowsPerThread], cube_off[kTcRowsPerThread];
+#pragma unroll
+                for (int j = 0; j < kTcRowsPerThread; ++j) {
                     const int4 a = *reinterpret_cast<const int4*>(rowp + rsub + kTcRowStride * j);   // fp, csc, ip, pix
-                    const int nu0 = kb * kTcBK + chunk * 4;
-                    const float* lp = f.lut_r + (size_t)a.z * nfp + nu0;
-                    t.c00 = zero4; t.c01 = zero4; t.c10 = zero4; t.c11 = zero4;
-                    if (p.debug & 16) { t.L0 = make_float4(0.5f, 0.5f, 0.5f, 0.5f); t.L1 = t.L0; return; }
-                    t.L0 = ldg4(lp); t.L1 = ldg4(lp + nfp);
-                    if (a.w >= 0 && nu0 < f.n_freq) {
-                        const float* c = f.cube + (size_t)a.w * nf + nu0;
-                        t.c00 = ldg4(c); t.c01 = ldg4(c + nf);
-                        c += (size_t)f.n_az * nf;
-                        t.c10 = ldg4(c); t.c11 = ldg4(c + nf);
-                    }
+                    lut_off[j] = (uint32_t)a.z * (uint32_t)nfp + (uint32_t)chunk * 4u;
+                    cube_off[j] = (uint32_t)a.w * (uint32_t)nf;
+                }
+                const float* const cube_base = f.cube != nullptr ? f.cube : f.lut_r;
+                const uint32_t tap01 = f.cube != nullptr ? (uint32_t)nf : 0u;
+                const uint32_t tap10 = f.cube != nullptr ? (uint32_t)f.n_az * (uint32_t)nf : 0u;
+                const uint32_t nu_last = (uint32_t)(max(f.n_freq, 4) - 4) & ~3u;     // 16-byte aligned (n_freq % 4 == 0 with a cube)
+                auto issue = [&](int kb, int j, Tap& t) {
+                    const uint32_t lo = lut_off[j] + (uint32_t)kb * kTcBK;
+                    t.L0 = ldg4(f.lut_r + lo); t.L1 = ldg4(f.lut_r + (lo + (uint32_t)nfp));
+                    if (p.debug & 16) return;
+                    const uint32_t co = cube_off[j] + min((uint32_t)kb * kTcBK + (uint32_t)chunk * 4u, nu_last);
+                    t.c00 = ldg4(cube_base + co);           t.c01 = ldg4(cube_base + (co + tap01));
+                    t.c10 = ldg4(cube_base + (co + tap10)); t.c11 = ldg4(cube_base + (co + tap10 + tap01));
                 };
                 auto compute = [&](int j, const Tap& cur, const float4& X, const float4& G, uint32_t stage) {
                     const RowParam* rp = rowp + rsub + kTcRowStride * j;
