@@ -64,6 +64,7 @@ static_assert(kTcRegsFlush + kTcRegsCtl + 4 * kTcRegsGen + kTcRegsFin <= 7 * 72,
 constexpr int kTcMaxGroupChan = 384;       // channels per tile: 3 column groups of 128 (+ 1 spare buffer = 512 columns)
 constexpr int kTcBufCols = 128, kTcNumBuf = 4, kTcMaxCg = 3;
 constexpr int kTcSegDefault = 8;           // slabs (of 32 frequencies) per accumulation segment
+constexpr float kTcTruncPerMma = 5.0e-8f;  // measured mean relative truncation loss per chained MMA (half the worst case)
 constexpr int kTcMaxBStages = 4;
 constexpr int kTcSmemLimit = 227 * 1024;
 
@@ -196,21 +197,24 @@ struct TcRotation {
     uint32_t bufs;                 // buffer of group g in bits [2g, 2g+2)
     uint32_t fifo;                 // free buffers, oldest in bits [0, 2)
     int shift;                     // 2 * (number of free buffers - 1)
-    int cnt[kTcMaxCg];             // slabs since the group's last segment boundary (staggered start)
+    int cnt[kTcMaxCg];             // position of the group in its (staggered) segment grid
+    int len[kTcMaxCg];             // slabs accumulated since the group's last boundary
     __device__ TcRotation(int n_cg_, int seg_, int n_kb_) : n_cg(n_cg_), seg(seg_), n_kb(n_kb_) {
         bufs = 0u | (1u << 2) | (2u << 4);
         fifo = 0u; int c = 0;
         for (int b = n_cg_; b < kTcNumBuf; ++b, ++c) fifo |= (uint32_t)b << (2 * c);
         shift = 2 * (c - 1);
 #pragma unroll
-        for (int g = 0; g < kTcMaxCg; ++g) cnt[g] = (g * seg_) / n_cg_;
+        for (int g = 0; g < kTcMaxCg; ++g) { cnt[g] = (g * seg_) / n_cg_; len[g] = 0; }
     }
     __device__ __forceinline__ int buf(int g) const { return (int)((bufs >> (2 * g)) & 3u); }
     // called once per (slab, group) in slab order: does group g close a segment after slab kb?
-    __device__ __forceinline__ bool boundary(int kb, int g) {
-        if (kb == n_kb - 1) { cnt[g] = (g * seg) / n_cg; return true; }
-        if (++cnt[g] == seg) { cnt[g] = 0; return true; }
-        return false;
+    // Returns the number of slabs of the segment that closes (0: no boundary).
+    __device__ __forceinline__ int boundary(int kb, int g) {
+        const int n = ++len[g];
+        if (kb == n_kb - 1) { cnt[g] = (g * seg) / n_cg; len[g] = 0; return n; }
+        if (++cnt[g] == seg) { cnt[g] = 0; len[g] = 0; return n; }
+        return 0;
     }
     // moves group g to the oldest free buffer; returns the buffer it leaves
     __device__ __forceinline__ int rotate(int g) {
@@ -642,7 +646,12 @@ fused_tc_kernel(const TcParams p) {
             for (int kb = 0; kb < p.n_kb; ++kb)
 #pragma unroll
                 for (int g = 0; g < kTcMaxCg; ++g) {
-                    if (g >= p.n_cg || !rot.boundary(kb, g)) continue;
+                    const int n_slabs = g < p.n_cg ? rot.boundary(kb, g) : 0;
+                    if (n_slabs == 0) continue;
+                    // Truncation compensation: the tensor core drops up to ~1e-7 of the
+                    // running sum per chained MMA, always toward zero, so a segment of n MMAs comes out low
+                    // by between 0 and ~1e-7 n; adding half of that centres the one-sided error interval.
+                    const float comp = 1.0f + kTcTruncPerMma * (float)(n_slabs * 2 * (kTcBK / kTcUK));
                     const int b = rot.rotate(g);
                     const int wg = rot.width(g, p.nb_tot);
                     float* scg = sc + (size_t)(g * kTcBufCols) * kTcBM + trow;
@@ -663,7 +672,7 @@ fused_tc_kernel(const TcParams p) {
                         ptx::tmem_ld_wait();
 #pragma unroll
                         for (int i = 0; i < 16; ++i) {
-                            const float sum = add ? pa[i] + __uint_as_float(v[i]) : __uint_as_float(v[i]);
+                            const float sum = add ? fmaf(__uint_as_float(v[i]), comp, pa[i]) : __uint_as_float(v[i]) * comp;
                             __stcg(scg + (size_t)(c0 + i) * kTcBM, sum);
                             if (add && c0 + 16 < wg) pa[i] = __ldcg(scg + (size_t)(c0 + 16 + i) * kTcBM);
                         }
