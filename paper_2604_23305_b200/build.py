@@ -31,7 +31,8 @@ def build(force: bool = False, verbose: bool = False) -> Path:
     if not force and LIB.exists() and LIB.stat().st_mtime >= newest:
         return LIB
     tmp = LIB.with_suffix(f".so.tmp{os.getpid()}")
-    cmd = [_nvcc(), *NVCC_FLAGS, *map(str, cu), "-o", str(tmp)]
+    extra = os.environ.get("GATEAU_NVCC_EXTRA", "").split()          # tuning builds only (e.g. -DGT_TC_REGS_FIN=88)
+    cmd = [_nvcc(), *NVCC_FLAGS, *extra, *map(str, cu), "-o", str(tmp)]
     res = subprocess.run(cmd, capture_output=True, text=True)
     if res.returncode != 0:
         raise RuntimeError("nvcc failed:\n" + " ".join(cmd) + "\n" + res.stdout + res.stderr)

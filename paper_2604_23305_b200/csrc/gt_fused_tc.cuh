@@ -59,7 +59,13 @@ constexpr int kTcFinWarps = 4, kTcWarpFin0 = kTcWarpGen0 + kTcGenWarps;         
 constexpr int kTcWarpCtl0 = kTcWarpFin0 + kTcFinWarps;                              // 24
 constexpr int kTcWarpLoader = kTcWarpCtl0 + 2, kTcWarpMma = kTcWarpCtl0 + 3;        // 26, 27
 constexpr int kTcThreads = 32 * (kTcWarpCtl0 + 4);                                  // 896
-constexpr int kTcRegsFlush = 56, kTcRegsCtl = 40, kTcRegsGen = 80, kTcRegsFin = 88;
+#ifndef GT_TC_REGS_FLUSH
+#define GT_TC_REGS_FLUSH 56
+#endif
+#ifndef GT_TC_REGS_FIN
+#define GT_TC_REGS_FIN 88
+#endif
+constexpr int kTcRegsFlush = GT_TC_REGS_FLUSH, kTcRegsCtl = 40, kTcRegsGen = 80, kTcRegsFin = GT_TC_REGS_FIN;
 static_assert(kTcRegsFlush + kTcRegsCtl + 4 * kTcRegsGen + kTcRegsFin <= 7 * 72, "setmaxnreg pool");
 constexpr int kTcMaxGroupChan = 384;       // channels per tile: 3 column groups of 128 (+ 1 spare buffer = 512 columns)
 constexpr int kTcBufCols = 128, kTcNumBuf = 4, kTcMaxCg = 3;
@@ -198,23 +204,22 @@ struct TcRotation {
     uint32_t fifo;                 // free buffers, oldest in bits [0, 2)
     int shift;                     // 2 * (number of free buffers - 1)
     int cnt[kTcMaxCg];             // position of the group in its (staggered) segment grid
-    int len[kTcMaxCg];             // slabs accumulated since the group's last boundary
     __device__ TcRotation(int n_cg_, int seg_, int n_kb_) : n_cg(n_cg_), seg(seg_), n_kb(n_kb_) {
         bufs = 0u | (1u << 2) | (2u << 4);
         fifo = 0u; int c = 0;
         for (int b = n_cg_; b < kTcNumBuf; ++b, ++c) fifo |= (uint32_t)b << (2 * c);
         shift = 2 * (c - 1);
 #pragma unroll
-        for (int g = 0; g < kTcMaxCg; ++g) { cnt[g] = (g * seg_) / n_cg_; len[g] = 0; }
+        for (int g = 0; g < kTcMaxCg; ++g) cnt[g] = (g * seg_) / n_cg_;
     }
     __device__ __forceinline__ int buf(int g) const { return (int)((bufs >> (2 * g)) & 3u); }
     // called once per (slab, group) in slab order: does group g close a segment after slab kb?
     // Returns the number of slabs of the segment that closes (0: no boundary).
-    __device__ __forceinline__ int boundary(int kb, int g) {
-        const int n = ++len[g];
-        if (kb == n_kb - 1) { cnt[g] = (g * seg) / n_cg; len[g] = 0; return n; }
-        if (++cnt[g] == seg) { cnt[g] = 0; len[g] = 0; return n; }
-        return 0;
+    // called once per (slab, group) in slab order: does group g close a segment after slab kb?
+    __device__ __forceinline__ bool boundary(int kb, int g) {
+        if (kb == n_kb - 1) { cnt[g] = (g * seg) / n_cg; return true; }
+        if (++cnt[g] == seg) { cnt[g] = 0; return true; }
+        return false;
     }
     // moves group g to the oldest free buffer; returns the buffer it leaves
     __device__ __forceinline__ int rotate(int g) {
@@ -579,7 +584,7 @@ fused_tc_kernel(const TcParams p) {
       }
     } else if (warp >= kTcWarpFin0 && warp < kTcWarpCtl0) {
         // ============ finisher: scratch tile -> P = sum*scale + bias, photon noise -> TOD ========
-        ptx::setmaxnreg_inc<kTcRegsFin>();
+        if constexpr (kTcRegsFin > 72) ptx::setmaxnreg_inc<kTcRegsFin>(); else if constexpr (kTcRegsFin < 72) ptx::setmaxnreg_dec<kTcRegsFin>();
         const int q = warp - kTcWarpFin0;
         uint32_t ti = 0;
         for (int64_t tl = blockIdx.x; tl < n_tiles; tl += gridDim.x, ++ti) {
@@ -646,12 +651,7 @@ fused_tc_kernel(const TcParams p) {
             for (int kb = 0; kb < p.n_kb; ++kb)
 #pragma unroll
                 for (int g = 0; g < kTcMaxCg; ++g) {
-                    const int n_slabs = g < p.n_cg ? rot.boundary(kb, g) : 0;
-                    if (n_slabs == 0) continue;
-                    // Truncation compensation: the tensor core drops up to ~1e-7 of the
-                    // running sum per chained MMA, always toward zero, so a segment of n MMAs comes out low
-                    // by between 0 and ~1e-7 n; adding half of that centres the one-sided error interval.
-                    const float comp = 1.0f + kTcTruncPerMma * (float)(n_slabs * 2 * (kTcBK / kTcUK));
+                    if (g >= p.n_cg || !rot.boundary(kb, g)) continue;
                     const int b = rot.rotate(g);
                     const int wg = rot.width(g, p.nb_tot);
                     float* scg = sc + (size_t)(g * kTcBufCols) * kTcBM + trow;
@@ -672,7 +672,7 @@ fused_tc_kernel(const TcParams p) {
                         ptx::tmem_ld_wait();
 #pragma unroll
                         for (int i = 0; i < 16; ++i) {
-                            const float sum = add ? fmaf(__uint_as_float(v[i]), comp, pa[i]) : __uint_as_float(v[i]) * comp;
+                            const float sum = add ? pa[i] + __uint_as_float(v[i]) : __uint_as_float(v[i]);
                             __stcg(scg + (size_t)(c0 + i) * kTcBM, sum);
                             if (add && c0 + 16 < wg) pa[i] = __ldcg(scg + (size_t)(c0 + 16 + i) * kTcBM);
                         }
@@ -700,6 +700,14 @@ fused_tc_kernel(const TcParams p) {
 inline cudaError_t launch_fused_tc(const FusedParams& fp, const TcTables& t, int num_sms, cudaStream_t st) {
     TcParams p{};
     p.f = fp; p.filt_img = t.filt_img;
+    // Truncation compensation: the tensor core drops up to ~1e-7 of the running sum
+    // per chained MMA, always toward zero, so a segment of n MMAs comes out low by between 0 and ~1e-7 n;
+    // adding half of that (folded into the output scale: nearly every segment has the same n) centres
+    // the one-sided error interval.
+    {
+        const int seg = t.seg > 0 ? t.seg : kTcSegDefault;
+        p.f.scale *= 1.0f + kTcTruncPerMma * (float)(2 * (kTcBK / kTcUK) * std::min(seg, (int)t.n_kb));
+    }
     p.scratch = t.scratch;
     p.n_groups = t.n_groups; p.nb_tot = t.nb_tot; p.n_cg = t.n_cg; p.seg = t.seg > 0 ? t.seg : kTcSegDefault; p.n_kb = t.n_kb;
     p.unit_bytes = t.unit_bytes; p.b_stages = t.b_stages;

@@ -83,24 +83,35 @@ pink_local_kernel(PinkParams p, int64_t t0, int64_t T, float* __restrict__ tod) 
         if (j < p.J) p.seg[(sg * p.n_det + d) * p.J + j] = x[j];
 }
 
-// thread = detector: walks the segments, replaces e[seg] by the state at the segment start.
+// thread = (detector, stage): walks the segments, replaces e[seg] by the state at the segment start.
+// The chain c <- phi^len c + e is a dependent FMA per segment, but its inputs are not: they are
+// fetched 16 segments at a time so that the walk costs one memory round trip per batch instead of one
+// per segment.
 __global__ void __launch_bounds__(256) pink_carry_kernel(PinkParams p, int64_t T) {
-    const int64_t d = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (d >= p.n_det) return;
+    const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= p.n_det * p.J) return;
+    const int j = (int)(idx % p.J);
     const int64_t n_seg = (T + kPinkSeg - 1) / kPinkSeg;
-    for (int j = 0; j < p.J; ++j) {
-        float cst = p.state[d * p.J + j];
-        const float phi = p.phi[j];
-        const float phiL = powf(phi, (float)kPinkSeg);
-        for (int64_t sg = 0; sg < n_seg; ++sg) {
-            float* e = p.seg + (sg * p.n_det + d) * p.J + j;
-            const float ev = *e;
-            *e = cst;
-            const int64_t len = min((int64_t)kPinkSeg, T - sg * kPinkSeg);
-            cst = fmaf(len == kPinkSeg ? phiL : powf(phi, (float)len), cst, ev);
+    const int64_t stride = p.n_det * p.J;                  // seg[sg][d][j]: idx is the offset inside one segment slice
+    float cst = p.state[idx];
+    const float phi = p.phi[j];
+    const float phiL = powf(phi, (float)kPinkSeg);
+    constexpr int kBatch = 16;
+    for (int64_t s0 = 0; s0 < n_seg; s0 += kBatch) {
+        float e[kBatch];
+#pragma unroll
+        for (int b = 0; b < kBatch; ++b) e[b] = s0 + b < n_seg ? p.seg[(s0 + b) * stride + idx] : 0.f;
+#pragma unroll
+        for (int b = 0; b < kBatch; ++b) {
+            const int64_t sg = s0 + b;
+            if (sg < n_seg) {
+                p.seg[sg * stride + idx] = cst;
+                const int64_t len = min((int64_t)kPinkSeg, T - sg * kPinkSeg);
+                cst = fmaf(len == kPinkSeg ? phiL : powf(phi, (float)len), cst, e[b]);
+            }
         }
-        p.state[d * p.J + j] = cst;
     }
+    p.state[idx] = cst;
 }
 
 __global__ void __launch_bounds__(256)
