@@ -68,6 +68,7 @@ struct gt_plan {
     DevBuf<double> d_sp;             // 6 per-spaxel tables back to back
     // fused-kernel tables
     DevBuf<float> d_Xn, d_Gs, d_lut_r, d_filt_t, d_bias, d_c1, d_c2;
+    DevBuf<float4> d_chan4;
     gt::TcTables tc;                 // tensor-kernel operand images
     // pink
     gt::PinkParams pink{};
@@ -199,7 +200,7 @@ gt_status run_chunk(gt_plan* p, int64_t t0, int64_t T, float* dst, float* pwv_ds
     fp.Xn = p->d_Xn.p; fp.Gs = p->d_Gs.p; fp.lut_r = p->d_lut_r.p;
     fp.cube = p->cube; fp.n_az = p->n_az;
     fp.filt_t = p->d_filt_t.p; fp.n_chan_pad = p->n_chan_pad;
-    fp.scale = p->scale; fp.bias = p->d_bias.p; fp.noise_c1 = p->d_c1.p; fp.noise_c2 = p->d_c2.p;
+    fp.scale = p->scale; fp.bias = p->d_bias.p; fp.noise_c1 = p->d_c1.p; fp.noise_c2 = p->d_c2.p; fp.chan4 = p->d_chan4.p;
     fp.photon_noise = noise ? p->photon_noise : 0;
     fp.seed_lo = (uint32_t)(p->seed & 0xffffffffu); fp.seed_hi = (uint32_t)(p->seed >> 32);
     fp.out = dst;
@@ -421,6 +422,12 @@ gt_status gt_plan_create(const gt_config* cfg, void* cuda_stream, gt_plan** out_
     }
     GT_CUDA0(p->d_Xn.upload(Xn, st)); GT_CUDA0(p->d_Gs.upload(Gs, st)); GT_CUDA0(p->d_lut_r.upload(lut_r, st));
     GT_CUDA0(p->d_bias.upload(bias, st)); GT_CUDA0(p->d_c1.upload(c1, st)); GT_CUDA0(p->d_c2.upload(c2, st));
+    {
+        std::vector<float4> c4(ncp);
+        for (int ch = 0; ch < ncp; ++ch) c4[ch] = make_float4(bias[ch], c1[ch], c2[ch], 0.f);
+        GT_CUDA0(p->d_chan4.upload(c4, st));
+        GT_CUDA0(cudaStreamSynchronize(st));
+    }
 
     // ---- geometry tables: per-sample and per-spaxel transcendental inputs from the host libm ----
     {

@@ -35,6 +35,7 @@ struct FusedParams {
     float scale;              // P_ref * dnu
     const float *bias;        // [n_chan_pad] dnu * sum_nu Fm * Y   (W)
     const float *noise_c1, *noise_c2;   // [n_chan_pad] h f_c f_s, f_s / dnu_c
+    const float4* chan4;                // [n_chan_pad] {bias, noise_c1, noise_c2, 0}: one 16-byte load per output
     int32_t photon_noise; uint32_t seed_lo, seed_hi;
     float* out;               // [n_rows][n_chan]
 };

@@ -41,7 +41,10 @@ namespace gt {
 constexpr int kTcBM = 128;                 // rows per tile (UMMA M)
 constexpr int kTcBK = 32;                  // frequencies per A stage / B unit: one 128-byte swizzle row
 constexpr int kTcUK = 8;                   // K of one tcgen05.mma.kind::tf32
-constexpr int kTcAStages = 2;
+#ifndef GT_TC_A_STAGES
+#define GT_TC_A_STAGES 3
+#endif
+constexpr int kTcAStages = GT_TC_A_STAGES;   // <= 4
 constexpr int kTcAPartBytes = kTcBM * kTcBK * 4;            // 16 KB (hi or lo)
 constexpr int kTcAStageBytes = 2 * kTcAPartBytes;           // 32 KB
 constexpr int kTcEpiWarps = 4, kTcGenWarps = 16;
@@ -187,8 +190,8 @@ struct TcSmem {
     __device__ TcSmem(uint32_t base, int b_stages, int unit_bytes) {
         a = base; b = base + kTcAStages * kTcAStageBytes;
         const uint32_t bar = b + (uint32_t)b_stages * (uint32_t)unit_bytes;
-        a_full = bar; a_empty = bar + 16; b_full = bar + 32; b_empty = bar + 64;
-        flush_full = bar + 96; buf_free = bar + 128; tile_done = bar + 160; scratch_free = bar + 176; slot = bar + 192;
+        a_full = bar; a_empty = bar + 32; b_full = bar + 64; b_empty = bar + 96;
+        flush_full = bar + 128; buf_free = bar + 160; tile_done = bar + 192; scratch_free = bar + 208; slot = bar + 224;
         rowp = bar + 256;
     }
 };
@@ -309,7 +312,7 @@ fused_tc_kernel(const TcParams p) {
         const int rsub = gw * 4 + (lane >> 3), chunk = lane & 7;
         const uint32_t swz = (uint32_t)((chunk ^ (rsub & 7)) << 4);
         const size_t nf = (size_t)f.n_freq, nfp = (size_t)f.n_freq_pad;
-        uint32_t it = 0;
+        uint32_t a_st = 0, a_ph = 0;           // A-ring stage and its phase parity
         if constexpr (VEC) {
             // One step = one row of this thread (4 frequencies of it): 2 LUT rows + 4 cube taps as
             // 16-byte loads, steps 2-4, tf32 split, two 16-byte shared stores.  The loads of the
@@ -385,8 +388,8 @@ fused_tc_kernel(const TcParams p) {
                 };
                 Tap t0, t1;
                 issue(0, 0, t0);
-                for (int kb = 0; kb < p.n_kb; ++kb, ++it) {
-                    const uint32_t stage = it & 1u, ph = (it >> 1) & 1u;
+                for (int kb = 0; kb < p.n_kb; ++kb, a_ph ^= (++a_st == kTcAStages), a_st = a_st == kTcAStages ? 0u : a_st) {
+                    const uint32_t stage = a_st, ph = a_ph;
                     if (p.debug & 1) {
                         ptx::mbar_wait(sm.a_empty + 8 * stage, ph ^ 1u);
                         __syncwarp();
@@ -428,8 +431,8 @@ fused_tc_kernel(const TcParams p) {
                 lutp[j] = f.lut_r + (size_t)rp.ip * nfp + chunk * 4;
                 cubep[j] = (rp.pix >= 0 && f.cube) ? f.cube + (size_t)rp.pix * nf + chunk * 4 : nullptr;
             }
-            for (int kb = 0; kb < p.n_kb; ++kb, ++it) {
-                const uint32_t stage = it & 1u, ph = (it >> 1) & 1u;
+            for (int kb = 0; kb < p.n_kb; ++kb, a_ph ^= (++a_st == kTcAStages), a_st = a_st == kTcAStages ? 0u : a_st) {
+                const uint32_t stage = a_st, ph = a_ph;
                 if (p.debug & 1) {
                     ptx::mbar_wait(sm.a_empty + 8 * stage, ph ^ 1u);
                     __syncwarp();
@@ -513,10 +516,10 @@ fused_tc_kernel(const TcParams p) {
 #pragma unroll
             for (int g = 0; g < kTcMaxCg; ++g) idesc[g] = ptx::idesc_tf32(kTcBM, g < p.n_cg ? rot.width(g, p.nb_tot) : 16);
             const bool issue = !(p.debug & 2);
-            uint32_t it = 0, bs = 0, bph = 0;
+            uint32_t a_st = 0, a_ph = 0, bs = 0, bph = 0;
             for (int64_t tl = blockIdx.x; tl < n_tiles; tl += gridDim.x) {
-                for (int kb = 0; kb < p.n_kb; ++kb, ++it) {
-                    const uint32_t stage = it & 1u, ph = (it >> 1) & 1u;
+                for (int kb = 0; kb < p.n_kb; ++kb, a_ph ^= (++a_st == kTcAStages), a_st = a_st == kTcAStages ? 0u : a_st) {
+                    const uint32_t stage = a_st, ph = a_ph;
                     uint32_t d[kTcMaxCg];
                     // a group that has just moved to another buffer waits until the epilogue has drained it
 #pragma unroll
@@ -595,16 +598,28 @@ fused_tc_kernel(const TcParams p) {
             const float* sc = p.scratch + ((size_t)blockIdx.x * 2 + sb) * p.nb_tot * kTcBM;
             ptx::mbar_wait(sm.tile_done + 8 * sb, (ti >> 1) & 1u);
             constexpr int kMaxPerLane = kTcMaxGroupChan / 32;             // 12
+            // (sample, spaxel) of this warp's first row; later rows advance by kTcFinWarps without dividing
+            int64_t n64 = (row0 + q) / f.n_spaxel;
+            int sp = (int)((row0 + q) - n64 * f.n_spaxel);
+            float x[kMaxPerLane], xn[kMaxPerLane];
+#pragma unroll
+            for (int j = 0; j < kMaxPerLane; ++j) {
+                const int c = lane + 32 * j;
+                xn[j] = c < n_valid ? __ldcg(sc + (size_t)c * kTcBM + q) : 0.f;
+            }
             for (int r = q; r < kTcBM; r += kTcFinWarps) {
                 const int64_t Rr = row0 + r;
                 if (Rr >= f.n_rows || (p.debug & 8)) break;
-                const uint32_t n = (uint32_t)(f.t0 + Rr / f.n_spaxel), s = (uint32_t)(Rr % f.n_spaxel);
+                const uint32_t n = (uint32_t)(f.t0 + n64), s = (uint32_t)sp;
+                sp += kTcFinWarps;
+                while (sp >= f.n_spaxel) { sp -= f.n_spaxel; ++n64; }
                 float* o = f.out + (size_t)Rr * f.n_chan + cg0;
-                float x[kMaxPerLane];
+                // this row's partial sums were fetched during the previous row; fetch the next row's now
 #pragma unroll
                 for (int j = 0; j < kMaxPerLane; ++j) {
+                    x[j] = xn[j];
                     const int c = lane + 32 * j;
-                    x[j] = c < n_valid ? __ldcg(sc + (size_t)c * kTcBM + r) : 0.f;
+                    xn[j] = (c < n_valid && r + kTcFinWarps < kTcBM) ? __ldcg(sc + (size_t)c * kTcBM + r + kTcFinWarps) : 0.f;
                 }
                 constexpr int W = 4;                                      // channels in flight per lane
 #pragma unroll
@@ -616,8 +631,9 @@ fused_tc_kernel(const TcParams p) {
                     for (int i = 0; i < W; ++i) {
                         const int c = min(lane + 32 * (j0 + i), n_valid - 1);
                         cc[i] = (uint32_t)(cg0 + c);
-                        P[i] = fmaf(x[j0 + i], f.scale, __ldg(f.bias + cc[i]));
-                        n1[i] = __ldg(f.noise_c1 + cc[i]); n2[i] = __ldg(f.noise_c2 + cc[i]);
+                        const float4 k4 = __ldg(f.chan4 + cc[i]);          // bias, h f_c f_s, f_s / dnu_c
+                        P[i] = fmaf(x[j0 + i], f.scale, k4.x);
+                        n1[i] = k4.y; n2[i] = k4.z;
                     }
                     if (f.photon_noise) {
                         philox4x32_10_multi<W>(n, s, cc, kStreamPhoton, f.seed_lo, f.seed_hi, w0, w1);
