@@ -391,14 +391,14 @@ fused_tc_kernel(const TcParams p) {
                 for (int kb = 0; kb < p.n_kb; ++kb, a_ph ^= (++a_st == kTcAStages), a_st = a_st == kTcAStages ? 0u : a_st) {
                     const uint32_t stage = a_st, ph = a_ph;
                     if (p.debug & 1) {
-                        ptx::mbar_wait(sm.a_empty + 8 * stage, ph ^ 1u);
+                        ptx::mbar_wait_relaxed(sm.a_empty + 8 * stage, ph ^ 1u);
                         __syncwarp();
                         if (lane == 0) ptx::mbar_arrive(sm.a_full + 8 * stage);
                         continue;
                     }
                     const float4 X = ldg4(f.Xn + kb * kTcBK + chunk * 4), G = ldg4(f.Gs + kb * kTcBK + chunk * 4);
                     issue(kb, 1, t1);
-                    ptx::mbar_wait(sm.a_empty + 8 * stage, ph ^ 1u);
+                    ptx::mbar_wait_relaxed(sm.a_empty + 8 * stage, ph ^ 1u);
                     compute(0, t0, X, G, stage);
                     if (kb + 1 < p.n_kb) issue(kb + 1, 0, t0);
                     compute(1, t1, X, G, stage);
@@ -434,7 +434,7 @@ fused_tc_kernel(const TcParams p) {
             for (int kb = 0; kb < p.n_kb; ++kb, a_ph ^= (++a_st == kTcAStages), a_st = a_st == kTcAStages ? 0u : a_st) {
                 const uint32_t stage = a_st, ph = a_ph;
                 if (p.debug & 1) {
-                    ptx::mbar_wait(sm.a_empty + 8 * stage, ph ^ 1u);
+                    ptx::mbar_wait_relaxed(sm.a_empty + 8 * stage, ph ^ 1u);
                     __syncwarp();
                     if (lane == 0) ptx::mbar_arrive(sm.a_full + 8 * stage);
                     continue;
@@ -469,7 +469,7 @@ fused_tc_kernel(const TcParams p) {
                         }
                     }
                 }
-                ptx::mbar_wait(sm.a_empty + 8 * stage, ph ^ 1u);
+                ptx::mbar_wait_relaxed(sm.a_empty + 8 * stage, ph ^ 1u);
                 unsigned char* a_hi = smem_raw + (sm.a - raw) + stage * kTcAStageBytes;
 #pragma unroll
                 for (int j = 0; j < kTcRowsPerThread; ++j) {
@@ -596,7 +596,7 @@ fused_tc_kernel(const TcParams p) {
             const int n_valid = min(p.nb_tot, f.n_chan - cg0);            // real channels of this group
             const uint32_t sb = ti & 1u;
             const float* sc = p.scratch + ((size_t)blockIdx.x * 2 + sb) * p.nb_tot * kTcBM;
-            ptx::mbar_wait(sm.tile_done + 8 * sb, (ti >> 1) & 1u);
+            ptx::mbar_wait_relaxed(sm.tile_done + 8 * sb, (ti >> 1) & 1u);
             constexpr int kMaxPerLane = kTcMaxGroupChan / 32;             // 12
             // (sample, spaxel) of this warp's first row; later rows advance by kTcFinWarps without dividing
             int64_t n64 = (row0 + q) / f.n_spaxel;
@@ -662,7 +662,7 @@ fused_tc_kernel(const TcParams p) {
         for (int64_t tl = blockIdx.x; tl < n_tiles; tl += gridDim.x, ++ti) {
             const uint32_t sb = ti & 1u;
             float* const sc = p.scratch + ((size_t)blockIdx.x * 2 + sb) * p.nb_tot * kTcBM;
-            if (ti >= 2) ptx::mbar_wait(sm.scratch_free + 8 * sb, ((ti >> 1) - 1u) & 1u);   // finisher done with tile ti-2
+            if (ti >= 2) ptx::mbar_wait_relaxed(sm.scratch_free + 8 * sb, ((ti >> 1) - 1u) & 1u);   // finisher done with tile ti-2
             bool first[kTcMaxCg] = {true, true, true};
             for (int kb = 0; kb < p.n_kb; ++kb)
 #pragma unroll
@@ -680,7 +680,7 @@ fused_tc_kernel(const TcParams p) {
 #pragma unroll
                         for (int i = 0; i < 16; ++i) pa[i] = __ldcg(scg + (size_t)i * kTcBM);
                     }
-                    ptx::mbar_wait(sm.flush_full + 8 * b, fulls >> b & 1u);
+                    ptx::mbar_wait_relaxed(sm.flush_full + 8 * b, fulls >> b & 1u);
                     fulls ^= 1u << b;
                     ptx::tc_fence_after();
                     for (int c0 = 0; c0 < wg; c0 += 16) {

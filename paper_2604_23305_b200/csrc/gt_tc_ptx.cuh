@@ -46,6 +46,12 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     while (!mbar_try_wait(bar, parity)) { }
 }
 
+// wait of a role that is not latency critical: back off between polls so that the spinning warp does not
+// take issue slots from the generator warps of its scheduler
+__device__ __forceinline__ void mbar_wait_relaxed(uint32_t bar, uint32_t parity) {
+    while (!mbar_try_wait(bar, parity)) { __nanosleep(64); }
+}
+
 // ---- proxy fence: generic-proxy st.shared -> visible to the async proxy (tcgen05.mma reads) ----
 __device__ __forceinline__ void fence_proxy_async_smem() {
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");

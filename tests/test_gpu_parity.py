@@ -98,6 +98,18 @@ def test_pkid_random(variant, seed, kw):
 
 
 @pytest.mark.parametrize("variant", VARIANTS, ids=VARIANT_IDS)
+@pytest.mark.parametrize("n_chan,n_freq", [(32, 256), (130, 300), (256, 520), (400, 288), (800, 100)])
+def test_pkid_channel_group_layouts(variant, n_chan, n_freq):
+    """Tensor kernel: 1, 2 and 3 column groups per tile, and more than 384 channels (several channel groups
+    per row tile); n_freq spans several accumulation segments with a ragged last slab."""
+    w = W.random_workload(70 + n_chan, n_samples=90, n_spaxel=3, n_chan=n_chan, n_freq=n_freq)
+    ref = O.Oracle(w).simulate(want=("pkid",))["pkid"]
+    with _plan(w, variant) as p:
+        got = p.pkid().cpu().numpy()
+    assert rel_err(got, ref) <= TOL_PKID
+
+
+@pytest.mark.parametrize("variant", VARIANTS, ids=VARIANT_IDS)
 def test_pkid_C1_full(variant):
     w = W.make_workload("C1")
     ref = O.Oracle(w).simulate(want=("pkid",))["pkid"]
@@ -153,7 +165,7 @@ def test_tod_photon_noise(variant):
 
 
 @pytest.mark.parametrize("variant", VARIANTS, ids=VARIANT_IDS)
-@pytest.mark.parametrize("J", [1, 4, 6])
+@pytest.mark.parametrize("J", [1, 4, 6, 8])
 def test_tod_photon_and_pink_noise(variant, J):
     w = W.random_workload(40 + J, n_samples=300, n_spaxel=2, n_chan=33, n_freq=64, photon_noise=True,
                           pink_noise=True, J=J)
