@@ -171,6 +171,21 @@ def peaks():
         "fallback (B200_PROFILING.md)"
 
 
+def ncu_traffic(kernel, rows_per_launch):
+    """DRAM bytes per launch of the dominant kernel from the committed ncu capture (profiles/*_traffic.csv),
+    scaled by rows when bench's launch size differs from the captured one; None if there is no capture."""
+    import csv
+    best = None
+    for f in sorted((ROOT / "profiles").glob("*_traffic.csv")):
+        for r in csv.DictReader(open(f)):
+            if r["kernel"] == kernel:
+                best = r
+    if best is None:
+        return None, None
+    per_row = (float(best["dram_bytes_read"]) + float(best["dram_bytes_write"])) / float(best["launch_rows"])
+    return per_row * rows_per_launch, best["source"]
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -239,6 +254,7 @@ def run_ours(args):
         roof = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                 "traffic": None, "kernel": "fused_fp32_kernel",
                 "peak_source": f"FP32 FMA = 148 SM x 128 lanes x 2 x {mhz:.0f} MHz (median SM clock under load)"}
+    roof["traffic"], roof["traffic_source"] = ncu_traffic(roof["kernel"], (w.n_samples * w.n_spaxel) / max(fused_n / args.steps, 1))
     roof["fused_ms_per_step"] = fused_ms / args.steps
     roof["fused_share_of_step"] = fused_ms / total_ms if world == 1 else None
 

@@ -644,7 +644,7 @@ fused_tc_kernel(const TcParams p) {
 #pragma unroll
                     for (int i = 0; i < W; ++i) {
                         const int c = lane + 32 * (j0 + i);
-                        if (c < n_valid) o[c] = P[i];
+                        if (c < n_valid) __stcs(o + c, P[i]);      // streaming store: the TOD must not evict the scratch tiles from L2
                     }
                 }
             }
