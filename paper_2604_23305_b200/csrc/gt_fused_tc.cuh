@@ -79,7 +79,7 @@ constexpr int kTcSmemLimit = 227 * 1024;
 
 struct TcTables {
     unsigned char* filt_img = nullptr;   // [group][kb][part hi/lo][NBtot rows][128 B swizzled]
-    float* scratch = nullptr;            // [num CTAs][2][nb_tot][128] fp32 partial sums (L2 resident)
+    float* scratch = nullptr;            // [num CTAs][2][nb_tot / 4][128][4] fp32 partial sums (L2 resident)
     int32_t n_groups = 0;                // channel groups (tiles along the channel axis) of <= 384 channels
     int32_t nb_tot = 0;                  // padded channels per group (multiple of 32)
     int32_t n_cg = 0;                    // column groups per tile, widths 128,..,remainder
@@ -261,6 +261,11 @@ __device__ __forceinline__ void store_split(unsigned char* a_stage, int row, int
     unsigned char* part1 = a_stage + kTcAPartBytes + rowoff + sub;
     *reinterpret_cast<uint2*>(part1 + ((c16 ^ r7) << 4)) = lo2;
     *reinterpret_cast<uint2*>(part1 + (((c16 + 1u) ^ r7) << 4)) = hi2;
+}
+
+// element (column, row) of a scratch tile laid out [column / 4][row][column % 4]
+__device__ __forceinline__ size_t tc_scratch_index(int col, int row) {
+    return ((size_t)(col >> 2) * kTcBM + (size_t)row) * 4 + (size_t)(col & 3);
 }
 
 __device__ __forceinline__ float4 ldg4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
@@ -605,7 +610,7 @@ fused_tc_kernel(const TcParams p) {
 #pragma unroll
             for (int j = 0; j < kMaxPerLane; ++j) {
                 const int c = lane + 32 * j;
-                xn[j] = c < n_valid ? __ldcg(sc + (size_t)c * kTcBM + q) : 0.f;
+                xn[j] = c < n_valid ? __ldcg(sc + tc_scratch_index(c, q)) : 0.f;
             }
             for (int r = q; r < kTcBM; r += kTcFinWarps) {
                 const int64_t Rr = row0 + r;
@@ -619,7 +624,7 @@ fused_tc_kernel(const TcParams p) {
                 for (int j = 0; j < kMaxPerLane; ++j) {
                     x[j] = xn[j];
                     const int c = lane + 32 * j;
-                    xn[j] = (c < n_valid && r + kTcFinWarps < kTcBM) ? __ldcg(sc + (size_t)c * kTcBM + r + kTcFinWarps) : 0.f;
+                    xn[j] = (c < n_valid && r + kTcFinWarps < kTcBM) ? __ldcg(sc + tc_scratch_index(c, r + kTcFinWarps)) : 0.f;
                 }
                 constexpr int W = 4;                                      // channels in flight per lane
 #pragma unroll
@@ -670,15 +675,17 @@ fused_tc_kernel(const TcParams p) {
                     if (g >= p.n_cg || !rot.boundary(kb, g)) continue;
                     const int b = rot.rotate(g);
                     const int wg = rot.width(g, p.nb_tot);
-                    float* scg = sc + (size_t)(g * kTcBufCols) * kTcBM + trow;
+                    // scratch tile layout [column / 4][row][column % 4]: a thread (= row) moves 4 columns as one
+                    // 16-byte access, a warp 512 contiguous bytes
+                    float4* scg = reinterpret_cast<float4*>(sc) + (size_t)(g * (kTcBufCols / 4)) * kTcBM + trow;
                     const uint32_t taddr = tmem_base + ((uint32_t)(32 * q) << 16) + (uint32_t)(b * kTcBufCols);
                     const bool add = !first[g];
                     uint32_t v[16];
-                    float pa[16];
+                    float4 pa[4];
                     // the running sums of the first 16 columns are fetched while the MMAs still run
                     if (add) {
 #pragma unroll
-                        for (int i = 0; i < 16; ++i) pa[i] = __ldcg(scg + (size_t)i * kTcBM);
+                        for (int i = 0; i < 4; ++i) pa[i] = __ldcg(scg + (size_t)i * kTcBM);
                     }
                     ptx::mbar_wait_relaxed(sm.flush_full + 8 * b, fulls >> b & 1u);
                     fulls ^= 1u << b;
@@ -687,10 +694,12 @@ fused_tc_kernel(const TcParams p) {
                         ptx::tmem_ld_32x16(taddr + (uint32_t)c0, v);
                         ptx::tmem_ld_wait();
 #pragma unroll
-                        for (int i = 0; i < 16; ++i) {
-                            const float sum = add ? pa[i] + __uint_as_float(v[i]) : __uint_as_float(v[i]);
-                            __stcg(scg + (size_t)(c0 + i) * kTcBM, sum);
-                            if (add && c0 + 16 < wg) pa[i] = __ldcg(scg + (size_t)(c0 + 16 + i) * kTcBM);
+                        for (int i = 0; i < 4; ++i) {
+                            float4 sum = make_float4(__uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1]),
+                                                     __uint_as_float(v[4 * i + 2]), __uint_as_float(v[4 * i + 3]));
+                            if (add) { sum.x += pa[i].x; sum.y += pa[i].y; sum.z += pa[i].z; sum.w += pa[i].w; }
+                            __stcg(scg + (size_t)(c0 / 4 + i) * kTcBM, sum);
+                            if (add && c0 + 16 < wg) pa[i] = __ldcg(scg + (size_t)(c0 / 4 + 4 + i) * kTcBM);
                         }
                     }
                     ptx::tc_fence_before();
