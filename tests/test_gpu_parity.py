@@ -270,3 +270,38 @@ def test_C2_full_size_sampled_rows():
         got_p = pkid[t_idx].cpu().numpy()[:, 0, :]
     assert rel_err(got_p, pk) <= TOL_PKID
     assert rel_err(got_t, pk + wn) <= TOL_TOD
+
+
+def test_C4_bench_configuration_full_size_sampled():
+    """BASELINE.json configs[3] (the bench.py workload) at full size and in bench.py's launch configuration
+    (default variant, device output, 26 chunks of 6340 samples): noiseless power on sampled rows, and the noisy TOD
+    (photon + pink) on sampled rows x sampled channels whose pink series the oracle runs from sample 0."""
+    w = W.make_workload("C4")
+    assert w.photon_noise and w.pink_noise and w.n_samples == 160000 and w.n_spaxel == 61 and w.n_chan == 347
+    rng = np.random.default_rng(11)
+    n_rows = 64
+    t_idx = np.sort(rng.choice(w.n_samples, n_rows, replace=False)).astype(np.int64)
+    t_idx[:3] = [0, 1, 6339]                               # first samples and the last sample of the first chunk
+    t_idx[-3:] = [6340, w.n_samples - 2, w.n_samples - 1]  # first sample of the second chunk, last samples
+    t_idx = np.sort(t_idx)
+    s_idx = rng.integers(0, w.n_spaxel, n_rows).astype(np.int32)
+    chans = np.array([0, 1, 63, 127, 128, 255, 256, 346], dtype=np.int32)      # both sides of every column-group seam
+    o = O.Oracle(w)
+    pk, wn = o.simulate_rows(t_idx, s_idx, noise=True)                          # [row][chan]
+    ss = np.repeat(s_idx, chans.size).astype(np.int32)
+    cc = np.tile(chans, n_rows).astype(np.int32)
+    pink = o.pink_series(ss, cc, 0, w.n_samples).reshape(n_rows, chans.size, w.n_samples)
+    pn = pink[np.arange(n_rows)[:, None], np.arange(chans.size)[None, :], t_idx[:, None]]
+    with B.Plan(w) as p:
+        assert p.variant_name.startswith("tcgen05")
+        tod = p.simulate()
+        got_t = tod[t_idx, s_idx.astype(np.int64)].cpu().numpy()
+        del tod
+        pkid = p.pkid()
+        got_p = pkid[t_idx, s_idx.astype(np.int64)].cpu().numpy()
+        del pkid
+    assert rel_err(got_p, pk) <= TOL_PKID
+    expect = (pk + wn)[:, chans] + pn
+    assert rel_err(got_t[:, chans], expect) <= TOL_TOD
+    # the remaining channels carry the same photon noise plus their own pink noise (a few 1e-4 of P)
+    assert rel_err(got_t, pk + wn) <= 1e-2
