@@ -45,6 +45,12 @@ constexpr int kTcUK = 8;                   // K of one tcgen05.mma.kind::tf32
 #define GT_TC_A_STAGES 3
 #endif
 constexpr int kTcAStages = GT_TC_A_STAGES;   // <= 4
+#ifndef GT_TC_PAIR
+#define GT_TC_PAIR 1
+#endif
+// CTA pair (cta_group::2): two CTAs on one TPC compute two row tiles with M = 256 MMAs; each holds half of every
+// filter unit in shared memory, so the filter is fetched from L2, written to and read from shared memory once per pair.
+constexpr bool kTcPair = GT_TC_PAIR != 0;
 constexpr int kTcAPartBytes = kTcBM * kTcBK * 4;            // 16 KB (hi or lo)
 constexpr int kTcAStageBytes = 2 * kTcAPartBytes;           // 32 KB
 constexpr int kTcEpiWarps = 4, kTcGenWarps = 16;
@@ -74,7 +80,10 @@ constexpr int kTcMaxGroupChan = 384;       // channels per tile: 3 column groups
 constexpr int kTcBufCols = 128, kTcNumBuf = 4, kTcMaxCg = 3;
 constexpr int kTcSegDefault = 8;           // slabs (of 32 frequencies) per accumulation segment
 constexpr float kTcTruncPerMma = 5.0e-8f;  // measured mean relative truncation loss per chained MMA (half the worst case)
-constexpr int kTcMaxBStages = 4;
+#ifndef GT_TC_MAX_B_STAGES
+#define GT_TC_MAX_B_STAGES 4
+#endif
+constexpr int kTcMaxBStages = GT_TC_MAX_B_STAGES;   // <= 4 (barrier slots)
 constexpr int kTcSmemLimit = 227 * 1024;
 
 struct TcTables {
@@ -118,32 +127,41 @@ inline gt_status build_tc_tables(const std::vector<float>& filt, int n_chan, int
     t.n_groups = G; t.nb_tot = nbt;
     t.n_cg = (nbt + kTcBufCols - 1) / kTcBufCols;
     t.n_kb = n_freq_pad / kTcBK;
-    t.unit_bytes = nbt * 128;
-    const int fixed = kTcAStages * kTcAStageBytes + 1024 /*alignment slack*/ + 256 /*barriers*/ + kTcBM * 32 /*row constants*/;   // barriers use 164 B
+    // one unit = the rows one CTA holds of one (slab, part): all nb_tot rows, or (CTA pair) the half of every
+    // column group this CTA supplies to the M = 256 MMAs (rank r: columns [r w/2, (r+1) w/2) of a group of width w)
+    constexpr int kRanks = kTcPair ? 2 : 1;
+    t.unit_bytes = nbt * 128 / kRanks;
+    const int fixed = kTcAStages * kTcAStageBytes + 1024 /*alignment slack*/ + 320 /*barriers*/ + kTcBM * 32 /*row constants*/;
     t.b_stages = std::min(kTcMaxBStages, (kTcSmemLimit - fixed) / t.unit_bytes);
     if (t.b_stages < 2) { tc_error_ref() = "filter slab does not fit in shared memory"; return GT_ERR_UNSUPPORTED; }
     t.smem_bytes = fixed + t.b_stages * t.unit_bytes;
 
-    const size_t total = (size_t)G * t.n_kb * 2 * t.unit_bytes;
+    const size_t total = (size_t)G * t.n_kb * 2 * kRanks * t.unit_bytes;
     std::vector<float> img(total / 4, 0.f);
     uint16_t* img16 = reinterpret_cast<uint16_t*>(img.data());
     for (int g = 0; g < G; ++g)
         for (int n = 0; n < nbt; ++n) {
             const int ch = g * nbt + n;
             if (ch >= n_chan) continue;
+            // which CTA holds row n, and where inside its unit
+            const int cg = n / kTcBufCols, col0 = cg * kTcBufCols, w = std::min(kTcBufCols, nbt - col0);
+            const int rk = kTcPair ? (n - col0) / (w / 2) : 0;
+            const int nl = kTcPair ? col0 / 2 + (n - col0) - rk * (w / 2) : n;        // local row
             for (int i = 0; i < n_freq; ++i) {
                 const float f = filt[(size_t)ch * n_freq + i];
                 const float hi = host_tf32(f), lo = f - hi;
                 const int kb = i / kTcBK, kk = i % kTcBK;
-                const size_t unit0 = ((size_t)(g * t.n_kb + kb) * 2) * (t.unit_bytes / 4);      // in floats
+                // float index of (group tile, slab, unit 0, rank): units are laid out [g][kb][unit][rank]
+                const size_t unit0 = ((size_t)((g * t.n_kb + kb) * 2 + 0) * kRanks + rk) * (t.unit_bytes / 4);
+                const size_t unit1 = ((size_t)((g * t.n_kb + kb) * 2 + 1) * kRanks + rk) * (t.unit_bytes / 4);
                 // unit 0: tf32 hi part
-                img[unit0 + (size_t)n * 32 + (size_t)(((kk >> 2) ^ (n & 7)) << 2) + (kk & 3)] = hi;
+                img[unit0 + (size_t)nl * 32 + (size_t)(((kk >> 2) ^ (nl & 7)) << 2) + (kk & 3)] = hi;
                 // unit 1: bf16, per group of 8 frequencies [Fm_0..7 | lo_0..7] (pairs with A's [lo | hi])
                 const int kg = kk >> 3, fi = kk & 7;
-                const size_t row16 = (unit0 + t.unit_bytes / 4) * 2 + (size_t)n * 64;             // in bf16 elements
+                const size_t row16 = unit1 * 2 + (size_t)nl * 64;                                 // in bf16 elements
                 const int c_hi = kg * 2, c_lo = kg * 2 + 1;                                       // 16-byte chunks
-                img16[row16 + (size_t)((c_hi ^ (n & 7)) << 3) + fi] = host_bf16(f);
-                img16[row16 + (size_t)((c_lo ^ (n & 7)) << 3) + fi] = host_bf16(lo);
+                img16[row16 + (size_t)((c_hi ^ (nl & 7)) << 3) + fi] = host_bf16(f);
+                img16[row16 + (size_t)((c_lo ^ (nl & 7)) << 3) + fi] = host_bf16(lo);
             }
         }
     if (cudaMalloc(reinterpret_cast<void**>(&t.filt_img), total) != cudaSuccess) {
@@ -186,13 +204,13 @@ struct TcParams {
 //   then barriers: a_full[2] a_empty[2] b_full[4] b_empty[4] flush_full[4] buf_free[4] tile_done[2]
 //   scratch_free[2], tensor-memory slot
 struct TcSmem {
-    uint32_t a, b, a_full, a_empty, b_full, b_empty, flush_full, buf_free, tile_done, scratch_free, slot, rowp;
+    uint32_t a, b, a_full, a_empty, b_full, b_empty, flush_full, buf_free, tile_done, scratch_free, b_peer, slot, rowp;
     __device__ TcSmem(uint32_t base, int b_stages, int unit_bytes) {
         a = base; b = base + kTcAStages * kTcAStageBytes;
         const uint32_t bar = b + (uint32_t)b_stages * (uint32_t)unit_bytes;
         a_full = bar; a_empty = bar + 32; b_full = bar + 64; b_empty = bar + 96;
-        flush_full = bar + 128; buf_free = bar + 160; tile_done = bar + 192; scratch_free = bar + 208; slot = bar + 224;
-        rowp = bar + 256;
+        flush_full = bar + 128; buf_free = bar + 160; tile_done = bar + 192; scratch_free = bar + 208; b_peer = bar + 224; slot = bar + 256;
+        rowp = bar + 320;
     }
 };
 
@@ -282,16 +300,17 @@ fused_tc_kernel(const TcParams p) {
 
     if (tid == 0) {
         for (int s = 0; s < kTcAStages; ++s) {
-            ptx::mbar_init(sm.a_full + 8 * s, kTcGenWarps);
+            ptx::mbar_init(sm.a_full + 8 * s, (kTcPair ? 2 : 1) * kTcGenWarps);      // pair: the leader also counts the peer's generators
             ptx::mbar_init(sm.a_empty + 8 * s, 1);
         }
         for (int s = 0; s < kTcMaxBStages; ++s) {
             ptx::mbar_init(sm.b_full + 8 * s, 1);
             ptx::mbar_init(sm.b_empty + 8 * s, 1);
+            ptx::mbar_init(sm.b_peer + 8 * s, 1);
         }
         for (int b = 0; b < kTcNumBuf; ++b) {
             ptx::mbar_init(sm.flush_full + 8 * b, 1);
-            ptx::mbar_init(sm.buf_free + 8 * b, kTcEpiWarps);
+            ptx::mbar_init(sm.buf_free + 8 * b, (kTcPair ? 2 : 1) * kTcEpiWarps);
         }
         for (int b = 0; b < 2; ++b) {
             ptx::mbar_init(sm.tile_done + 8 * b, kTcEpiWarps);
@@ -300,15 +319,44 @@ fused_tc_kernel(const TcParams p) {
         ptx::fence_mbar_init();
     }
     if (warp == kTcWarpMma) {
-        ptx::tmem_alloc(sm.slot, 512);
-        ptx::tmem_relinquish();
+        if constexpr (kTcPair) { ptx::tmem_alloc2(sm.slot, 512); ptx::tmem_relinquish2(); }
+        else { ptx::tmem_alloc(sm.slot, 512); ptx::tmem_relinquish(); }
     }
     ptx::tc_fence_before();
-    __syncthreads();
+    if constexpr (kTcPair) ptx::cluster_sync_all(); else __syncthreads();
     ptx::tc_fence_after();
     const uint32_t tmem_base = *reinterpret_cast<const volatile uint32_t*>(smem_raw + (sm.slot - raw));
 
-    const int64_t n_tiles = (int64_t)p.n_row_tiles * p.n_groups;
+    // Work distribution.  Single CTA: tile = (row tile, channel group), strided over the grid.  CTA pair: the
+    // pair takes two consecutive row tiles of one channel group (rank r the r-th of them); both CTAs run the
+    // same number of iterations, a row tile past the end is computed on default rows and never stored.
+    const uint32_t rank = kTcPair ? ptx::cluster_ctarank() : 0u;
+    const int64_t worker = kTcPair ? (int64_t)ptx::cluster_id_x() : (int64_t)blockIdx.x;
+    const int64_t n_workers = kTcPair ? (int64_t)ptx::cluster_nctaid_x() : (int64_t)gridDim.x;
+    const int64_t n_tiles = kTcPair ? (int64_t)((p.n_row_tiles + 1) / 2) * p.n_groups : (int64_t)p.n_row_tiles * p.n_groups;
+    // arrive on a barrier the leader CTA waits on / wait for a signal that may come from the peer CTA
+    auto arrive_leader = [&](uint32_t bar) {
+        if (kTcPair && rank != 0) ptx::mbar_arrive_cluster(ptx::mapa(bar, 0)); else ptx::mbar_arrive(bar);
+    };
+    auto wait_pair = [&](uint32_t bar, uint32_t parity) {
+        ptx::mbar_wait_relaxed(bar, parity);      // CTA-scope acquire: a cluster-scope one would invalidate L1 on every wait
+    };
+    auto wait_lead = [&](uint32_t bar, uint32_t parity) {          // leader's waits on barriers the peer also arrives on
+        ptx::mbar_wait(bar, parity);
+    };
+    auto commit_pair = [&](uint32_t bar) {                          // completion of the MMAs issued so far, signalled to both CTAs
+        if constexpr (kTcPair) ptx::tc_commit2(bar, (uint16_t)3); else ptx::tc_commit(bar);
+    };
+    auto mma_tf32 = [&](uint32_t d, uint64_t a, uint64_t b, uint32_t id, uint32_t acc) {
+        if constexpr (kTcPair) ptx::mma2_tf32_ss(d, a, b, id, acc); else ptx::mma_tf32_ss(d, a, b, id, acc);
+    };
+    auto mma_bf16 = [&](uint32_t d, uint64_t a, uint64_t b, uint32_t id, uint32_t acc) {
+        if constexpr (kTcPair) ptx::mma2_bf16_ss(d, a, b, id, acc); else ptx::mma_bf16_ss(d, a, b, id, acc);
+    };
+    auto tile_row0 = [&](int64_t tl) -> int64_t {
+        const int64_t rt = tl / p.n_groups;
+        return (kTcPair ? 2 * rt + rank : rt) * kTcBM;
+    };
 
     if (warp >= kTcWarpGen0 && warp < kTcWarpFin0) {
         // =========================== generator: steps 2-4 -> A ring ===========================
@@ -326,8 +374,8 @@ fused_tc_kernel(const TcParams p) {
             // memory (each warp only reads rows it wrote itself).
             struct Tap { float4 L0, L1, c00, c01, c10, c11; };
             RowParam* rowp = reinterpret_cast<RowParam*>(smem_raw + (sm.rowp - raw));
-            for (int64_t tl = blockIdx.x; tl < n_tiles; tl += gridDim.x) {
-                const int64_t row0 = (tl / p.n_groups) * kTcBM;
+            for (int64_t tl = worker; tl < n_tiles; tl += n_workers) {
+                const int64_t row0 = tile_row0(tl);
                 __syncwarp();
                 if (chunk < kTcRowsPerThread) {
                     const int rr = rsub + kTcRowStride * chunk;
@@ -396,26 +444,26 @@ fused_tc_kernel(const TcParams p) {
                 for (int kb = 0; kb < p.n_kb; ++kb, a_ph ^= (++a_st == kTcAStages), a_st = a_st == kTcAStages ? 0u : a_st) {
                     const uint32_t stage = a_st, ph = a_ph;
                     if (p.debug & 1) {
-                        ptx::mbar_wait_relaxed(sm.a_empty + 8 * stage, ph ^ 1u);
+                        wait_pair(sm.a_empty + 8 * stage, ph ^ 1u);
                         __syncwarp();
-                        if (lane == 0) ptx::mbar_arrive(sm.a_full + 8 * stage);
+                        if (lane == 0) arrive_leader(sm.a_full + 8 * stage);
                         continue;
                     }
                     const float4 X = ldg4(f.Xn + kb * kTcBK + chunk * 4), G = ldg4(f.Gs + kb * kTcBK + chunk * 4);
                     issue(kb, 1, t1);
-                    ptx::mbar_wait_relaxed(sm.a_empty + 8 * stage, ph ^ 1u);
+                    wait_pair(sm.a_empty + 8 * stage, ph ^ 1u);
                     compute(0, t0, X, G, stage);
                     if (kb + 1 < p.n_kb) issue(kb + 1, 0, t0);
                     compute(1, t1, X, G, stage);
                     // one arrival per warp: 512 per-thread arrivals on one mbarrier serialise (~5 cycles each)
                     ptx::fence_proxy_async_smem();
                     __syncwarp();
-                    if (lane == 0) ptx::mbar_arrive(sm.a_full + 8 * stage);
+                    if (lane == 0) arrive_leader(sm.a_full + 8 * stage);
                 }
             }
         } else
-        for (int64_t tl = blockIdx.x; tl < n_tiles; tl += gridDim.x) {
-            const int64_t row0 = (tl / p.n_groups) * kTcBM;
+        for (int64_t tl = worker; tl < n_tiles; tl += n_workers) {
+            const int64_t row0 = tile_row0(tl);
             float fp[kTcRowsPerThread], csc[kTcRowsPerThread], w00[kTcRowsPerThread], w01[kTcRowsPerThread], w10[kTcRowsPerThread], w11[kTcRowsPerThread];
             const float* lutp[kTcRowsPerThread];
             const float* cubep[kTcRowsPerThread];
@@ -439,9 +487,9 @@ fused_tc_kernel(const TcParams p) {
             for (int kb = 0; kb < p.n_kb; ++kb, a_ph ^= (++a_st == kTcAStages), a_st = a_st == kTcAStages ? 0u : a_st) {
                 const uint32_t stage = a_st, ph = a_ph;
                 if (p.debug & 1) {
-                    ptx::mbar_wait_relaxed(sm.a_empty + 8 * stage, ph ^ 1u);
+                    wait_pair(sm.a_empty + 8 * stage, ph ^ 1u);
                     __syncwarp();
-                    if (lane == 0) ptx::mbar_arrive(sm.a_full + 8 * stage);
+                    if (lane == 0) arrive_leader(sm.a_full + 8 * stage);
                     continue;
                 }
                 const int nu0 = kb * kTcBK + chunk * 4;
@@ -474,7 +522,7 @@ fused_tc_kernel(const TcParams p) {
                         }
                     }
                 }
-                ptx::mbar_wait_relaxed(sm.a_empty + 8 * stage, ph ^ 1u);
+                wait_pair(sm.a_empty + 8 * stage, ph ^ 1u);
                 unsigned char* a_hi = smem_raw + (sm.a - raw) + stage * kTcAStageBytes;
 #pragma unroll
                 for (int j = 0; j < kTcRowsPerThread; ++j) {
@@ -487,31 +535,47 @@ fused_tc_kernel(const TcParams p) {
                 }
                 ptx::fence_proxy_async_smem();
                 __syncwarp();
-                if (lane == 0) ptx::mbar_arrive(sm.a_full + 8 * stage);
+                if (lane == 0) arrive_leader(sm.a_full + 8 * stage);
             }
         }
     } else if (warp >= kTcWarpCtl0) {
       ptx::setmaxnreg_dec<kTcRegsCtl>();
       if (warp == kTcWarpLoader) {
         // =========================== loader: filter slab images -> B ring =====================
+        // (pair: each CTA copies its half of every unit, the rows of the N/2 columns it supplies to the MMA)
         if (lane == 0) {
-            uint32_t ub = 0;
-            for (int64_t tl = blockIdx.x; tl < n_tiles; tl += gridDim.x) {
+            uint32_t bs = 0, bph = 0;
+            for (int64_t tl = worker; tl < n_tiles; tl += n_workers) {
                 const int g = (int)(tl % p.n_groups);
-                const unsigned char* src = p.filt_img + (size_t)g * p.n_kb * 2 * (size_t)p.unit_bytes;
-                for (int u = 0; u < 2 * p.n_kb; ++u, ++ub) {
-                    const uint32_t bs = ub % (uint32_t)p.b_stages, bph = (ub / (uint32_t)p.b_stages) & 1u;
-                    ptx::mbar_wait(sm.b_empty + 8 * bs, bph ^ 1u);
-                    if (p.debug & 4) { ptx::mbar_arrive(sm.b_full + 8 * bs); continue; }
-                    ptx::mbar_arrive_expect_tx(sm.b_full + 8 * bs, (uint32_t)p.unit_bytes);
-                    ptx::bulk_g2s(sm.b + bs * (uint32_t)p.unit_bytes, src + (size_t)u * p.unit_bytes,
-                                  (uint32_t)p.unit_bytes, sm.b_full + 8 * bs);
+                const size_t stride = (size_t)p.unit_bytes * (kTcPair ? 2 : 1);
+                const unsigned char* src = p.filt_img + (size_t)g * p.n_kb * 2 * stride + (size_t)rank * p.unit_bytes;
+                for (int u = 0; u < 2 * p.n_kb; ++u) {
+                    wait_pair(sm.b_empty + 8 * bs, bph ^ 1u);
+                    if (p.debug & 4) ptx::mbar_arrive(sm.b_full + 8 * bs);
+                    else {
+                        ptx::mbar_arrive_expect_tx(sm.b_full + 8 * bs, (uint32_t)p.unit_bytes);
+                        ptx::bulk_g2s(sm.b + bs * (uint32_t)p.unit_bytes, src + (size_t)u * stride,
+                                      (uint32_t)p.unit_bytes, sm.b_full + 8 * bs);
+                    }
+                    if (++bs == (uint32_t)p.b_stages) { bs = 0; bph ^= 1u; }
                 }
             }
         }
         __syncwarp();
-      } else if (warp == kTcWarpMma) {
-        // =========================== MMA issuer =================================================
+      } else if (kTcPair && warp == kTcWarpCtl0 && rank != 0) {
+        // =========================== forwarder (peer CTA): tells the leader that our half unit has landed ====
+        if (lane == 0) {
+            uint32_t bs = 0, bph = 0;
+            for (int64_t tl = worker; tl < n_tiles; tl += n_workers)
+                for (int u = 0; u < 2 * p.n_kb; ++u) {
+                    ptx::mbar_wait(sm.b_full + 8 * bs, bph);
+                    ptx::mbar_arrive_cluster(ptx::mapa(sm.b_peer + 8 * bs, 0));
+                    if (++bs == (uint32_t)p.b_stages) { bs = 0; bph ^= 1u; }
+                }
+        }
+        __syncwarp();
+      } else if (warp == kTcWarpMma && rank == 0) {
+        // =========================== MMA issuer (pair: the leader CTA issues for both) ===============
         {   // the whole warp runs the loop (uniform control flow); one elected lane issues
             TcRotation rot(p.n_cg, p.seg, p.n_kb);
             uint32_t idesc[kTcMaxCg];
@@ -519,10 +583,11 @@ fused_tc_kernel(const TcParams p) {
             uint32_t fresh = 7u;               // bit g: next MMA into buf(g) overwrites (first of a segment)
             uint32_t used = 0u, par = 0u;      // bit b: buffer b was flushed before / parity of its flush count
 #pragma unroll
-            for (int g = 0; g < kTcMaxCg; ++g) idesc[g] = ptx::idesc_tf32(kTcBM, g < p.n_cg ? rot.width(g, p.nb_tot) : 16);
+            for (int g = 0; g < kTcMaxCg; ++g) idesc[g] = ptx::idesc_tf32(kTcPair ? 2 * kTcBM : kTcBM, g < p.n_cg ? rot.width(g, p.nb_tot) : 16);
             const bool issue = !(p.debug & 2);
+            constexpr int kGroupDesc = (kTcBufCols * 128 >> 4) / (kTcPair ? 2 : 1);   // descriptor step between column groups (pair: half the rows)
             uint32_t a_st = 0, a_ph = 0, bs = 0, bph = 0;
-            for (int64_t tl = blockIdx.x; tl < n_tiles; tl += gridDim.x) {
+            for (int64_t tl = worker; tl < n_tiles; tl += n_workers) {
                 for (int kb = 0; kb < p.n_kb; ++kb, a_ph ^= (++a_st == kTcAStages), a_st = a_st == kTcAStages ? 0u : a_st) {
                     const uint32_t stage = a_st, ph = a_ph;
                     uint32_t d[kTcMaxCg];
@@ -532,13 +597,14 @@ fused_tc_kernel(const TcParams p) {
                         const uint32_t b = (uint32_t)rot.buf(g);
                         d[g] = tmem_base + b * (uint32_t)kTcBufCols;
                         if (g < p.n_cg && (fresh >> g & 1u) && (used >> b & 1u))
-                            ptx::mbar_wait(sm.buf_free + 8 * b, par >> b & 1u);
+                            wait_lead(sm.buf_free + 8 * b, par >> b & 1u);
                     }
-                    ptx::mbar_wait(sm.a_full + 8 * stage, ph);
+                    wait_lead(sm.a_full + 8 * stage, ph);
                     const uint64_t ad_hi = ptx::smem_desc_sw128(sm.a + stage * kTcAStageBytes);
                     const uint64_t ad_lo = ad_hi + (uint64_t)(kTcAPartBytes >> 4);
                     {   // tf32 unit: acc += A_hi.Fm_hi
                         ptx::mbar_wait(sm.b_full + 8 * bs, bph);
+                        if constexpr (kTcPair) ptx::mbar_wait(sm.b_peer + 8 * bs, bph);
                         ptx::tc_fence_after();
                         const uint64_t bd0 = ptx::smem_desc_sw128(sm.b + bs * (uint32_t)p.unit_bytes);
                         if (issue && ptx::elect_one()) {
@@ -547,16 +613,17 @@ fused_tc_kernel(const TcParams p) {
 #pragma unroll
                                 for (int g = 0; g < kTcMaxCg; ++g)
                                     if (g < p.n_cg) {
-                                        const uint64_t bd = bd0 + (uint64_t)(g * (kTcBufCols * 128 >> 4) + k * 2);
-                                        ptx::mma_tf32_ss(d[g], ad_hi + (uint64_t)(k * 2), bd, idesc[g], (k != 0 || !(fresh >> g & 1u)) ? 1u : 0u);
+                                        const uint64_t bd = bd0 + (uint64_t)(g * kGroupDesc + k * 2);
+                                        mma_tf32(d[g], ad_hi + (uint64_t)(k * 2), bd, idesc[g], (k != 0 || !(fresh >> g & 1u)) ? 1u : 0u);
                                     }
                         }
                         __syncwarp();
-                        if (ptx::elect_one()) ptx::tc_commit(sm.b_empty + 8 * bs);
+                        if (ptx::elect_one()) commit_pair(sm.b_empty + 8 * bs);
                         if (++bs == (uint32_t)p.b_stages) { bs = 0; bph ^= 1u; }
                     }
                     {   // bf16 unit: acc += A_lo.Fm_hi + A_hi.Fm_lo (one K = 16 MMA per 8 frequencies)
                         ptx::mbar_wait(sm.b_full + 8 * bs, bph);
+                        if constexpr (kTcPair) ptx::mbar_wait(sm.b_peer + 8 * bs, bph);
                         ptx::tc_fence_after();
                         const uint64_t bd0 = ptx::smem_desc_sw128(sm.b + bs * (uint32_t)p.unit_bytes);
                         if (issue && ptx::elect_one()) {
@@ -565,21 +632,21 @@ fused_tc_kernel(const TcParams p) {
 #pragma unroll
                                 for (int g = 0; g < kTcMaxCg; ++g)
                                     if (g < p.n_cg)
-                                        ptx::mma_bf16_ss(d[g], ad_lo + (uint64_t)(k * 2),
-                                                         bd0 + (uint64_t)(g * (kTcBufCols * 128 >> 4) + k * 2), idesc[g] ^ kToBf16, 1u);
+                                        mma_bf16(d[g], ad_lo + (uint64_t)(k * 2),
+                                                         bd0 + (uint64_t)(g * kGroupDesc + k * 2), idesc[g] ^ kToBf16, 1u);
                         }
                         __syncwarp();
-                        if (ptx::elect_one()) ptx::tc_commit(sm.b_empty + 8 * bs);
+                        if (ptx::elect_one()) commit_pair(sm.b_empty + 8 * bs);
                         if (++bs == (uint32_t)p.b_stages) { bs = 0; bph ^= 1u; }
                     }
-                    if (ptx::elect_one()) ptx::tc_commit(sm.a_empty + 8 * stage);
+                    if (ptx::elect_one()) commit_pair(sm.a_empty + 8 * stage);
                     // segment boundaries: hand the finished partial sums to the epilogue, move on to a free buffer
                     fresh = 0u;
 #pragma unroll
                     for (int g = 0; g < kTcMaxCg; ++g) {
                         if (g < p.n_cg && rot.boundary(kb, g)) {
                             const uint32_t old = (uint32_t)rot.rotate(g);
-                            if (ptx::elect_one()) ptx::tc_commit(sm.flush_full + 8 * old);
+                            if (ptx::elect_one()) commit_pair(sm.flush_full + 8 * old);
                             par ^= (used >> old & 1u) << old;      // parity of (flush count - 1) once used
                             used |= 1u << old;
                             fresh |= 1u << g;
@@ -595,8 +662,8 @@ fused_tc_kernel(const TcParams p) {
         if constexpr (kTcRegsFin > 72) ptx::setmaxnreg_inc<kTcRegsFin>(); else if constexpr (kTcRegsFin < 72) ptx::setmaxnreg_dec<kTcRegsFin>();
         const int q = warp - kTcWarpFin0;
         uint32_t ti = 0;
-        for (int64_t tl = blockIdx.x; tl < n_tiles; tl += gridDim.x, ++ti) {
-            const int64_t row0 = (tl / p.n_groups) * kTcBM;
+        for (int64_t tl = worker; tl < n_tiles; tl += n_workers, ++ti) {
+            const int64_t row0 = tile_row0(tl);
             const int cg0 = (int)(tl % p.n_groups) * p.nb_tot;
             const int n_valid = min(p.nb_tot, f.n_chan - cg0);            // real channels of this group
             const uint32_t sb = ti & 1u;
@@ -664,7 +731,7 @@ fused_tc_kernel(const TcParams p) {
         TcRotation rot(p.n_cg, p.seg, p.n_kb);
         uint32_t fulls = 0u;                                   // bit b: parity of buffer b's flush count
         uint32_t ti = 0;
-        for (int64_t tl = blockIdx.x; tl < n_tiles; tl += gridDim.x, ++ti) {
+        for (int64_t tl = worker; tl < n_tiles; tl += n_workers, ++ti) {
             const uint32_t sb = ti & 1u;
             float* const sc = p.scratch + ((size_t)blockIdx.x * 2 + sb) * p.nb_tot * kTcBM;
             if (ti >= 2) ptx::mbar_wait_relaxed(sm.scratch_free + 8 * sb, ((ti >> 1) - 1u) & 1u);   // finisher done with tile ti-2
@@ -687,7 +754,7 @@ fused_tc_kernel(const TcParams p) {
 #pragma unroll
                         for (int i = 0; i < 4; ++i) pa[i] = __ldcg(scg + (size_t)i * kTcBM);
                     }
-                    ptx::mbar_wait_relaxed(sm.flush_full + 8 * b, fulls >> b & 1u);
+                    wait_pair(sm.flush_full + 8 * b, fulls >> b & 1u);
                     fulls ^= 1u << b;
                     ptx::tc_fence_after();
                     for (int c0 = 0; c0 < wg; c0 += 16) {
@@ -704,7 +771,7 @@ fused_tc_kernel(const TcParams p) {
                     }
                     ptx::tc_fence_before();
                     __syncwarp();
-                    if (lane == 0) ptx::mbar_arrive(sm.buf_free + 8 * b);
+                    if (lane == 0) arrive_leader(sm.buf_free + 8 * b);
                     first[g] = false;
                 }
             // every partial sum of the tile is in the scratch tile: hand it to the finisher warps
@@ -715,10 +782,10 @@ fused_tc_kernel(const TcParams p) {
     }
 
     ptx::tc_fence_before();
-    __syncthreads();
+    if constexpr (kTcPair) ptx::cluster_sync_all(); else __syncthreads();     // pair: the peer's shared and tensor memory stay alive until both are done
     if (warp == kTcWarpMma) {
         ptx::tc_fence_after();
-        ptx::tmem_dealloc(tmem_base, 512);
+        if constexpr (kTcPair) ptx::tmem_dealloc2(tmem_base, 512); else ptx::tmem_dealloc(tmem_base, 512);
     }
 }
 
@@ -739,25 +806,26 @@ inline cudaError_t launch_fused_tc(const FusedParams& fp, const TcTables& t, int
     p.n_row_tiles = (int32_t)((fp.n_rows + kTcBM - 1) / kTcBM);
     if (const char* e = std::getenv("GATEAU_TC_DEBUG")) p.debug = std::atoi(e);
     p.cube_vec = (fp.cube == nullptr) || ((fp.n_freq % 4 == 0) && ((reinterpret_cast<uintptr_t>(fp.cube) & 15u) == 0));
-    const int64_t n_tiles = (int64_t)p.n_row_tiles * p.n_groups;
-    const unsigned grid = (unsigned)std::min<int64_t>(n_tiles, num_sms);
+    const int64_t n_tiles = kTcPair ? (int64_t)((p.n_row_tiles + 1) / 2) * p.n_groups : (int64_t)p.n_row_tiles * p.n_groups;
+    const int64_t workers = kTcPair ? num_sms / 2 : num_sms;
+    const unsigned grid = (unsigned)(std::min<int64_t>(n_tiles, workers) * (kTcPair ? 2 : 1));
     static int smem_set[2] = {0, 0};
+    auto kern = p.cube_vec ? fused_tc_kernel<true> : fused_tc_kernel<false>;
+    int& set = smem_set[p.cube_vec ? 1 : 0];
     cudaError_t e;
-    if (p.cube_vec) {
-        if (smem_set[1] < t.smem_bytes) {
-            e = cudaFuncSetAttribute(fused_tc_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, t.smem_bytes);
-            if (e != cudaSuccess) return e;
-            smem_set[1] = t.smem_bytes;
-        }
-        fused_tc_kernel<true><<<grid, kTcThreads, t.smem_bytes, st>>>(p);
-    } else {
-        if (smem_set[0] < t.smem_bytes) {
-            e = cudaFuncSetAttribute(fused_tc_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, t.smem_bytes);
-            if (e != cudaSuccess) return e;
-            smem_set[0] = t.smem_bytes;
-        }
-        fused_tc_kernel<false><<<grid, kTcThreads, t.smem_bytes, st>>>(p);
+    if (set < t.smem_bytes) {
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, t.smem_bytes);
+        if (e != cudaSuccess) return e;
+        set = t.smem_bytes;
     }
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(kTcThreads); cfg.dynamicSmemBytes = (size_t)t.smem_bytes; cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = kTcPair ? 2 : 1; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    e = cudaLaunchKernelEx(&cfg, kern, p);
+    if (e != cudaSuccess) return e;
     return cudaGetLastError();
 }
 
