@@ -255,9 +255,9 @@ struct TcRotation {
 // steps 2-4 for one (row, nu) element as in element_value (gt_fused_fp32.cuh), with the two MUFU
 // operations issued as single instructions: eta_z is in (0,1] and csc >= 1, so log2 is <= 0 and finite
 // and 2^(csc log2 eta_z) underflows to 0 exactly where eta_atm is below 1e-38.
-__device__ __forceinline__ float element_value_fast(float eta_z, float csc, float Xn, float GS) {
+__device__ __forceinline__ float element_value_fast(float eta_z, float csc, float Xn, float G, float S) {
     const float eta = ptx::ex2_ftz(csc * ptx::lg2_ftz(eta_z));
-    return fmaf(1.0f - eta, Xn, eta * GS);
+    return fmaf(eta, fmaf(G, S, -Xn), Xn);           // (1 - eta) Xn + eta G S in two FMAs
 }
 
 // Writes 4 consecutive frequencies (16-byte chunk `chunk` of a 32-frequency slab) of tile row `row`
@@ -433,10 +433,10 @@ fused_tc_kernel(const TcParams p) {
                     S.y = w.x * cur.c00.y + w.y * cur.c01.y + w.z * cur.c10.y + w.w * cur.c11.y;
                     S.z = w.x * cur.c00.z + w.y * cur.c01.z + w.z * cur.c10.z + w.w * cur.c11.z;
                     S.w = w.x * cur.c00.w + w.y * cur.c01.w + w.z * cur.c10.w + w.w * cur.c11.w;
-                    v.x = element_value_fast(fmaf(fc.x, cur.L1.x - cur.L0.x, cur.L0.x), fc.y, X.x, G.x * S.x);
-                    v.y = element_value_fast(fmaf(fc.x, cur.L1.y - cur.L0.y, cur.L0.y), fc.y, X.y, G.y * S.y);
-                    v.z = element_value_fast(fmaf(fc.x, cur.L1.z - cur.L0.z, cur.L0.z), fc.y, X.z, G.z * S.z);
-                    v.w = element_value_fast(fmaf(fc.x, cur.L1.w - cur.L0.w, cur.L0.w), fc.y, X.w, G.w * S.w);
+                    v.x = element_value_fast(fmaf(fc.x, cur.L1.x - cur.L0.x, cur.L0.x), fc.y, X.x, G.x, S.x);
+                    v.y = element_value_fast(fmaf(fc.x, cur.L1.y - cur.L0.y, cur.L0.y), fc.y, X.y, G.y, S.y);
+                    v.z = element_value_fast(fmaf(fc.x, cur.L1.z - cur.L0.z, cur.L0.z), fc.y, X.z, G.z, S.z);
+                    v.w = element_value_fast(fmaf(fc.x, cur.L1.w - cur.L0.w, cur.L0.w), fc.y, X.w, G.w, S.w);
                     store_split(smem_raw + (sm.a - raw) + stage * kTcAStageBytes, rsub + kTcRowStride * j, chunk, v);
                 };
                 Tap t0, t1;
@@ -527,10 +527,10 @@ fused_tc_kernel(const TcParams p) {
 #pragma unroll
                 for (int j = 0; j < kTcRowsPerThread; ++j) {
                     float4 v;
-                    v.x = element_value_fast(fmaf(fp[j], L1[j].x - L0[j].x, L0[j].x), csc[j], X.x, G.x * S[j].x);
-                    v.y = element_value_fast(fmaf(fp[j], L1[j].y - L0[j].y, L0[j].y), csc[j], X.y, G.y * S[j].y);
-                    v.z = element_value_fast(fmaf(fp[j], L1[j].z - L0[j].z, L0[j].z), csc[j], X.z, G.z * S[j].z);
-                    v.w = element_value_fast(fmaf(fp[j], L1[j].w - L0[j].w, L0[j].w), csc[j], X.w, G.w * S[j].w);
+                    v.x = element_value_fast(fmaf(fp[j], L1[j].x - L0[j].x, L0[j].x), csc[j], X.x, G.x, S[j].x);
+                    v.y = element_value_fast(fmaf(fp[j], L1[j].y - L0[j].y, L0[j].y), csc[j], X.y, G.y, S[j].y);
+                    v.z = element_value_fast(fmaf(fp[j], L1[j].z - L0[j].z, L0[j].z), csc[j], X.z, G.z, S[j].z);
+                    v.w = element_value_fast(fmaf(fp[j], L1[j].w - L0[j].w, L0[j].w), csc[j], X.w, G.w, S[j].w);
                     store_split(a_hi, rsub + kTcRowStride * j, chunk, v);
                 }
                 ptx::fence_proxy_async_smem();
