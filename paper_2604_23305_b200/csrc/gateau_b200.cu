@@ -223,9 +223,11 @@ gt_status run_chunk(gt_plan* p, int64_t t0, int64_t T, float* dst, float* pwv_ds
         const int64_t n_thr = n_seg * p->pink.n_det;
         if ((size_t)(n_thr * p->J) > p->d_seg.n) GT_CUDA(p, p->d_seg.alloc((size_t)(n_thr * p->J)));
         p->pink.seg = p->d_seg.p;
-        gt::pink_local_kernel<<<(unsigned)((n_thr + 255) / 256), 256, 0, st>>>(p->pink, t0, T, dst);
+        if (p->J <= 4) gt::pink_local_kernel<4><<<(unsigned)((n_thr + 255) / 256), 256, 0, st>>>(p->pink, t0, T, dst);
+        else           gt::pink_local_kernel<8><<<(unsigned)((n_thr + 255) / 256), 256, 0, st>>>(p->pink, t0, T, dst);
         gt::pink_carry_kernel<<<(unsigned)((p->pink.n_det * p->J + 255) / 256), 256, 0, st>>>(p->pink, T);
-        gt::pink_fixup_kernel<<<(unsigned)((n_thr + 255) / 256), 256, 0, st>>>(p->pink, T, dst);
+        if (p->J <= 4) gt::pink_fixup_kernel<4><<<(unsigned)((n_thr + 255) / 256), 256, 0, st>>>(p->pink, T, dst);
+        else           gt::pink_fixup_kernel<8><<<(unsigned)((n_thr + 255) / 256), 256, 0, st>>>(p->pink, T, dst);
         GT_CUDA(p, cudaGetLastError());
         p->launches += 3;
     }

@@ -18,6 +18,7 @@
 namespace gt {
 
 constexpr int kPinkSeg = 64;
+constexpr int kPinkBatch = 8;      // TOD values fetched ahead per thread
 constexpr int kPinkMaxJ = 8;
 
 struct PinkParams {
@@ -56,6 +57,7 @@ __global__ void __launch_bounds__(256) pink_init_kernel(PinkParams p) {
 }
 
 // thread = (segment, detector); detectors fastest so that TOD accesses coalesce.
+template <int JM>      // JM = 4 or 8: number of AR(1) stages the unrolled loops cover (J <= JM)
 __global__ void __launch_bounds__(256)
 pink_local_kernel(PinkParams p, int64_t t0, int64_t T, float* __restrict__ tod) {
     const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -65,21 +67,32 @@ pink_local_kernel(PinkParams p, int64_t t0, int64_t T, float* __restrict__ tod) 
     const uint32_t s = (uint32_t)(d / p.n_chan), c = (uint32_t)(d % p.n_chan);
     float g[kPinkMaxJ], x[kPinkMaxJ];
 #pragma unroll
-    for (int j = 0; j < kPinkMaxJ; ++j) { g[j] = j < p.J ? p.gain[d * p.J + j] : 0.f; x[j] = 0.f; }
+    for (int j = 0; j < JM; ++j) { g[j] = j < p.J ? p.gain[d * p.J + j] : 0.f; x[j] = 0.f; }
     const int64_t m0 = sg * kPinkSeg, m1 = min(m0 + (int64_t)kPinkSeg, T);
-    for (int64_t m = m0; m < m1; ++m) {
-        float z[kPinkMaxJ];
-        pink_normals(p, (uint32_t)(t0 + m), s, c, z);
-        float pn = 0.f;
+    // batches of kPinkBatch samples: the TOD values are fetched first (independent loads in flight while the
+    // Philox / Box-Muller arithmetic runs), the recurrence itself stays strictly sequential in m
+    for (int64_t mb = m0; mb < m1; mb += kPinkBatch) {
+        float cur[kPinkBatch];
 #pragma unroll
-        for (int j = 0; j < kPinkMaxJ; ++j) {
-            x[j] = fmaf(p.phi[j], x[j], p.sq[j] * z[j]);
-            pn = fmaf(g[j], x[j], pn);
+        for (int b = 0; b < kPinkBatch; ++b) cur[b] = mb + b < m1 ? __ldcs(tod + (mb + b) * p.n_det + d) : 0.f;
+#pragma unroll
+        for (int b = 0; b < kPinkBatch; ++b) {
+            const int64_t m = mb + b;
+            if (m < m1) {
+                float z[kPinkMaxJ];
+                pink_normals(p, (uint32_t)(t0 + m), s, c, z);
+                float pn = 0.f;
+#pragma unroll
+                for (int j = 0; j < JM; ++j) {
+                    x[j] = fmaf(p.phi[j], x[j], p.sq[j] * z[j]);
+                    pn = fmaf(g[j], x[j], pn);
+                }
+                tod[m * p.n_det + d] = cur[b] + pn;
+            }
         }
-        tod[m * p.n_det + d] += pn;
     }
 #pragma unroll
-    for (int j = 0; j < kPinkMaxJ; ++j)
+    for (int j = 0; j < JM; ++j)
         if (j < p.J) p.seg[(sg * p.n_det + d) * p.J + j] = x[j];
 }
 
@@ -114,6 +127,7 @@ __global__ void __launch_bounds__(256) pink_carry_kernel(PinkParams p, int64_t T
     p.state[idx] = cst;
 }
 
+template <int JM>
 __global__ void __launch_bounds__(256)
 pink_fixup_kernel(PinkParams p, int64_t T, float* __restrict__ tod) {
     const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -122,14 +136,23 @@ pink_fixup_kernel(PinkParams p, int64_t T, float* __restrict__ tod) {
     const int64_t sg = idx / p.n_det, d = idx % p.n_det;
     float a[kPinkMaxJ];       // g_j * phi_j^(m+1) * c_j
 #pragma unroll
-    for (int j = 0; j < kPinkMaxJ; ++j)
+    for (int j = 0; j < JM; ++j)
         a[j] = j < p.J ? p.gain[d * p.J + j] * p.seg[(sg * p.n_det + d) * p.J + j] : 0.f;
     const int64_t m0 = sg * kPinkSeg, m1 = min(m0 + (int64_t)kPinkSeg, T);
-    for (int64_t m = m0; m < m1; ++m) {
-        float add = 0.f;
+    for (int64_t mb = m0; mb < m1; mb += kPinkBatch) {
+        float cur[kPinkBatch];
 #pragma unroll
-        for (int j = 0; j < kPinkMaxJ; ++j) { a[j] *= p.phi[j]; add += a[j]; }
-        tod[m * p.n_det + d] += add;
+        for (int b = 0; b < kPinkBatch; ++b) cur[b] = mb + b < m1 ? __ldcs(tod + (mb + b) * p.n_det + d) : 0.f;
+#pragma unroll
+        for (int b = 0; b < kPinkBatch; ++b) {
+            const int64_t m = mb + b;
+            if (m < m1) {
+                float add = 0.f;
+#pragma unroll
+                for (int j = 0; j < JM; ++j) { a[j] *= p.phi[j]; add += a[j]; }
+                tod[m * p.n_det + d] = cur[b] + add;
+            }
+        }
     }
 }
 
