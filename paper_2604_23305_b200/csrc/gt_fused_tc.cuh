@@ -51,6 +51,13 @@ constexpr int kTcAStages = GT_TC_A_STAGES;   // <= 4
 // CTA pair (cta_group::2): two CTAs on one TPC compute two row tiles with M = 256 MMAs; each holds half of every
 // filter unit in shared memory, so the filter is fetched from L2, written to and read from shared memory once per pair.
 constexpr bool kTcPair = GT_TC_PAIR != 0;
+// Timing diagnostics (parts of the kernel switched off through GATEAU_TC_DEBUG) exist only in tuning builds
+// (-DGT_TC_DIAG): the product kernel carries no such branches.
+#ifdef GT_TC_DIAG
+#define GT_DIAG(p, bit) (((p).debug & (bit)) != 0)
+#else
+#define GT_DIAG(p, bit) false
+#endif
 constexpr int kTcAPartBytes = kTcBM * kTcBK * 4;            // 16 KB (hi or lo)
 constexpr int kTcAStageBytes = 2 * kTcAPartBytes;           // 32 KB
 constexpr int kTcEpiWarps = 4, kTcGenWarps = 16;
@@ -412,7 +419,7 @@ fused_tc_kernel(const TcParams p) {
                 auto issue = [&](int kb, int j, Tap& t) {
                     const uint32_t lo = lut_off[j] + (uint32_t)kb * kTcBK;
                     t.L0 = ldg4(f.lut_r + lo); t.L1 = ldg4(f.lut_r + (lo + (uint32_t)nfp));
-                    if (p.debug & 16) return;
+                    if (GT_DIAG(p, 16)) return;
                     const uint32_t co = cube_off[j] + min((uint32_t)kb * kTcBK + (uint32_t)chunk * 4u, nu_last);
                     t.c00 = ldg4(cube_base + co);           t.c01 = ldg4(cube_base + (co + tap01));
                     t.c10 = ldg4(cube_base + (co + tap10)); t.c11 = ldg4(cube_base + (co + tap10 + tap01));
@@ -422,7 +429,7 @@ fused_tc_kernel(const TcParams p) {
                     const float2 fc = *reinterpret_cast<const float2*>(rp);                    // fp, csc
                     const float4 w = *reinterpret_cast<const float4*>(&rp->w00);
                     float4 S, v;
-                    if (p.debug & 32) {
+                    if (GT_DIAG(p, 32)) {
                         unsigned char* a_hi = smem_raw + (sm.a - raw) + stage * kTcAStageBytes;
                         const uint32_t off = (uint32_t)(rsub + kTcRowStride * j) * 128u + swz;
                         *reinterpret_cast<float4*>(a_hi + off) = cur.L0;
@@ -443,7 +450,7 @@ fused_tc_kernel(const TcParams p) {
                 issue(0, 0, t0);
                 for (int kb = 0; kb < p.n_kb; ++kb, a_ph ^= (++a_st == kTcAStages), a_st = a_st == kTcAStages ? 0u : a_st) {
                     const uint32_t stage = a_st, ph = a_ph;
-                    if (p.debug & 1) {
+                    if (GT_DIAG(p, 1)) {
                         wait_pair(sm.a_empty + 8 * stage, ph ^ 1u);
                         __syncwarp();
                         if (lane == 0) arrive_leader(sm.a_full + 8 * stage);
@@ -486,7 +493,7 @@ fused_tc_kernel(const TcParams p) {
             }
             for (int kb = 0; kb < p.n_kb; ++kb, a_ph ^= (++a_st == kTcAStages), a_st = a_st == kTcAStages ? 0u : a_st) {
                 const uint32_t stage = a_st, ph = a_ph;
-                if (p.debug & 1) {
+                if (GT_DIAG(p, 1)) {
                     wait_pair(sm.a_empty + 8 * stage, ph ^ 1u);
                     __syncwarp();
                     if (lane == 0) arrive_leader(sm.a_full + 8 * stage);
@@ -551,7 +558,7 @@ fused_tc_kernel(const TcParams p) {
                 const unsigned char* src = p.filt_img + (size_t)g * p.n_kb * 2 * stride + (size_t)rank * p.unit_bytes;
                 for (int u = 0; u < 2 * p.n_kb; ++u) {
                     wait_pair(sm.b_empty + 8 * bs, bph ^ 1u);
-                    if (p.debug & 4) ptx::mbar_arrive(sm.b_full + 8 * bs);
+                    if (GT_DIAG(p, 4)) ptx::mbar_arrive(sm.b_full + 8 * bs);
                     else {
                         ptx::mbar_arrive_expect_tx(sm.b_full + 8 * bs, (uint32_t)p.unit_bytes);
                         ptx::bulk_g2s(sm.b + bs * (uint32_t)p.unit_bytes, src + (size_t)u * stride,
@@ -584,7 +591,7 @@ fused_tc_kernel(const TcParams p) {
             uint32_t used = 0u, par = 0u;      // bit b: buffer b was flushed before / parity of its flush count
 #pragma unroll
             for (int g = 0; g < kTcMaxCg; ++g) idesc[g] = ptx::idesc_tf32(kTcPair ? 2 * kTcBM : kTcBM, g < p.n_cg ? rot.width(g, p.nb_tot) : 16);
-            const bool issue = !(p.debug & 2);
+            const bool issue = !GT_DIAG(p, 2);
             constexpr int kGroupDesc = (kTcBufCols * 128 >> 4) / (kTcPair ? 2 : 1);   // descriptor step between column groups (pair: half the rows)
             uint32_t a_st = 0, a_ph = 0, bs = 0, bph = 0;
             for (int64_t tl = worker; tl < n_tiles; tl += n_workers) {
@@ -681,7 +688,7 @@ fused_tc_kernel(const TcParams p) {
             }
             for (int r = q; r < kTcBM; r += kTcFinWarps) {
                 const int64_t Rr = row0 + r;
-                if (Rr >= f.n_rows || (p.debug & 8)) break;
+                if (Rr >= f.n_rows || GT_DIAG(p, 8)) break;
                 const uint32_t n = (uint32_t)(f.t0 + n64), s = (uint32_t)sp;
                 sp += kTcFinWarps;
                 while (sp >= f.n_spaxel) { sp -= f.n_spaxel; ++n64; }
