@@ -67,4 +67,4 @@ def test_filterbank_peak_and_front_end_constants():
     w = W.make_workload("C2", n_samples=16)
     check("t_cmb_K", w.T_cmb_K)
     ef = W.eta_front_aste(np.array([1e9]))[0]                                                      # Ruze term -> 1 at low nu
-    assert np.isclose(ef / 0.85, GOLD["eta_pol"][0], rtol=1e-6)
+    assert np.isclose(ef / 0.85, GOLD["eta_pol"][0], rtol=1e-5)          # the Ruze factor at 1 GHz is 1 - 3e-6
