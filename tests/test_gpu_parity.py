@@ -305,3 +305,58 @@ def test_C4_bench_configuration_full_size_sampled():
     assert rel_err(got_t[:, chans], expect) <= TOL_TOD
     # the remaining channels carry the same photon noise plus their own pink noise (a few 1e-4 of P)
     assert rel_err(got_t, pk + wn) <= 1e-2
+
+
+def test_C5_long_survey_streamed_in_60s_chunks():
+    """BASELINE.json configs[4] at full size the way the config describes it: the TOD of the 1 h, 37-spaxel
+    survey is produced in 60 s chunks (9600 samples) into ONE reused pinned host buffer by consecutive
+    gt_simulate calls (the pink-noise state carries over); rows sampled on both sides of chunk seams are compared
+    with the oracle, pink noise included."""
+    import torch
+    w = W.make_workload("C5")
+    assert w.n_samples == 576000 and w.n_spaxel == 37 and w.photon_noise and w.pink_noise
+    chunk = 9600
+    n_chunks = w.n_samples // chunk
+    rng = np.random.default_rng(23)
+    seams = rng.choice(np.arange(1, n_chunks), 10, replace=False) * chunk
+    t_idx = np.unique(np.concatenate([[0, 1], seams - 1, seams, seams + 1, rng.choice(w.n_samples, 20, replace=False),
+                                      [w.n_samples - 1]])).astype(np.int64)
+    s_idx = rng.integers(0, w.n_spaxel, t_idx.size).astype(np.int32)
+    chans = np.array([0, 127, 128, 255, 256, 346], dtype=np.int32)
+    o = O.Oracle(w)
+    pk, wn = o.simulate_rows(t_idx, s_idx, noise=True)
+    ss = np.repeat(s_idx, chans.size).astype(np.int32)
+    cc = np.tile(chans, t_idx.size).astype(np.int32)
+    pink = o.pink_series(ss, cc, 0, w.n_samples).reshape(t_idx.size, chans.size, w.n_samples)
+    pn = pink[np.arange(t_idx.size)[:, None], np.arange(chans.size)[None, :], t_idx[:, None]]
+    got = np.empty((t_idx.size, w.n_chan), dtype=np.float32)
+    buf = torch.empty((chunk, w.n_spaxel, w.n_chan), dtype=torch.float32, pin_memory=True)
+    with B.Plan(w, chunk_samples=chunk) as p:
+        for k in range(n_chunks):
+            p.simulate(k * chunk, chunk, out=buf)                      # blocking: returns after the D2H copies
+            sel = np.nonzero((t_idx >= k * chunk) & (t_idx < (k + 1) * chunk))[0]
+            for i in sel:
+                got[i] = buf[t_idx[i] - k * chunk, s_idx[i]].numpy()
+    expect = (pk + wn)[:, chans] + pn
+    assert rel_err(got[:, chans], expect) <= TOL_TOD
+    assert rel_err(got, pk + wn) <= 1e-2
+
+
+def test_C3_full_size_sampled_rows():
+    """BASELINE.json configs[2] (7-spaxel IFU, 1 h daisy scan, photon noise) at full size on sampled rows."""
+    w = W.make_workload("C3")
+    assert w.n_samples == 576000 and w.n_spaxel == 7 and w.photon_noise and not w.pink_noise
+    rng = np.random.default_rng(7)
+    t_idx = np.sort(rng.choice(w.n_samples, 96, replace=False)).astype(np.int64)
+    t_idx[:2] = [0, 1]; t_idx[-1] = w.n_samples - 1
+    s_idx = rng.integers(0, w.n_spaxel, t_idx.size).astype(np.int32)
+    pk, wn = O.Oracle(w).simulate_rows(t_idx, s_idx, noise=True)
+    with B.Plan(w) as p:
+        tod = p.simulate()
+        got_t = tod[t_idx, s_idx.astype(np.int64)].cpu().numpy()
+        del tod
+        pkid = p.pkid()
+        got_p = pkid[t_idx, s_idx.astype(np.int64)].cpu().numpy()
+        del pkid
+    assert rel_err(got_p, pk) <= TOL_PKID
+    assert rel_err(got_t, pk + wn) <= TOL_TOD
