@@ -73,6 +73,7 @@ struct gt_plan {
     // pink
     gt::PinkParams pink{};
     DevBuf<float> d_gain, d_state, d_seg;
+    DevBuf<uint32_t> d_pink_sync;   // ticket counter + per-(segment, detector block) flags of the chained pink kernel
     int64_t pink_next_t = 0;
     // scratch
     DevBuf<gt::RowParam> d_rows;     // [chunk rows]
@@ -223,13 +224,22 @@ gt_status run_chunk(gt_plan* p, int64_t t0, int64_t T, float* dst, float* pwv_ds
         const int64_t n_thr = n_seg * p->pink.n_det;
         if ((size_t)(n_thr * p->J) > p->d_seg.n) GT_CUDA(p, p->d_seg.alloc((size_t)(n_thr * p->J)));
         p->pink.seg = p->d_seg.p;
-        if (p->J <= 4) gt::pink_local_kernel<4><<<(unsigned)((n_thr + 255) / 256), 256, 0, st>>>(p->pink, t0, T, dst);
-        else           gt::pink_local_kernel<8><<<(unsigned)((n_thr + 255) / 256), 256, 0, st>>>(p->pink, t0, T, dst);
-        gt::pink_carry_kernel<<<(unsigned)((p->pink.n_det * p->J + 255) / 256), 256, 0, st>>>(p->pink, T);
-        if (p->J <= 4) gt::pink_fixup_kernel<4><<<(unsigned)((n_thr + 255) / 256), 256, 0, st>>>(p->pink, T, dst);
-        else           gt::pink_fixup_kernel<8><<<(unsigned)((n_thr + 255) / 256), 256, 0, st>>>(p->pink, T, dst);
+        const int64_t n_dblk = (p->pink.n_det + 255) / 256;
+        const size_t n_flags = (size_t)(n_seg * n_dblk) + 1;                 // + the ticket counter
+        if (n_flags > p->d_pink_sync.n) GT_CUDA(p, p->d_pink_sync.alloc(n_flags));
+        GT_CUDA(p, cudaMemsetAsync(p->d_pink_sync.p, 0, n_flags * sizeof(uint32_t), st));
+        p->pink.flags = p->d_pink_sync.p + 1; p->pink.ticket = p->d_pink_sync.p;
+        const size_t smem = (size_t)gt::kPinkSeg * 256 * sizeof(float);
+        static bool attr_set = false;
+        if (!attr_set) {
+            GT_CUDA(p, cudaFuncSetAttribute(gt::pink_chain_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            GT_CUDA(p, cudaFuncSetAttribute(gt::pink_chain_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            attr_set = true;
+        }
+        if (p->J <= 4) gt::pink_chain_kernel<4><<<(unsigned)(n_seg * n_dblk), 256, smem, st>>>(p->pink, t0, T, dst);
+        else           gt::pink_chain_kernel<8><<<(unsigned)(n_seg * n_dblk), 256, smem, st>>>(p->pink, t0, T, dst);
         GT_CUDA(p, cudaGetLastError());
-        p->launches += 3;
+        p->launches += 1;
     }
     return GT_OK;
 }

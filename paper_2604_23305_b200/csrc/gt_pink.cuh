@@ -4,14 +4,10 @@
 //   eps_j[n] = normal j of Philox(seed; n, spaxel, chan, stream 1 (j<4) / 2 (j>=4)),
 //   x_j[-1]  = normal j of Philox(seed; 0xFFFFFFFF, spaxel, chan, stream 1/2).
 //
-// The recurrence is sequential in n but LINEAR, so a chunk of T samples is cut into segments
-// of kPinkSeg samples that run in parallel (detectors x segments threads):
-//   pink_local : x from a ZERO state inside each segment, adds sum_j g_j x_j to the TOD,
-//                stores the segment's end state e_j                       (HBM: TOD read+write)
-//   pink_carry : per detector, sequential over segments: true state at each segment start
-//                c[seg+1] = phi^len c[seg] + e[seg]; final state -> plan   (tiny)
-//   pink_fixup : adds sum_j g_j phi_j^(m+1) c_j[seg] at offset m of each segment (TOD read+write)
-// HBM-bound: 16 B per detector-sample of traffic on top of the fused kernel's 4 B.
+// The recurrence is sequential in n but LINEAR, so a chunk of T samples is cut into segments of
+// kPinkSeg samples that run in parallel (segments x detectors threads) and are chained through their end
+// states in a single kernel (pink_chain_kernel): 8 B per detector-sample of HBM traffic on top of the
+// fused kernel's 4 B, one Philox call per detector-sample.
 #pragma once
 #include "gt_common.cuh"
 
@@ -27,7 +23,9 @@ struct PinkParams {
     float phi[kPinkMaxJ], sq[kPinkMaxJ];     // phi_j, sqrt(1 - phi_j^2)
     const float* gain;             // [n_det][J]
     float* state;                  // [n_det][J] x_j at the sample before the chunk
-    float* seg;                    // [n_seg][n_det][J] scratch: e (after local), c (after carry)
+    float* seg;                    // [n_seg][n_det][J] scratch: inclusive end state of every segment
+    uint32_t* flags;               // [n_seg][n_det / 256] end state published; zeroed before every launch
+    uint32_t* ticket;              // block ticket counter; zeroed before every launch
     uint32_t seed_lo, seed_hi;
 };
 
@@ -56,101 +54,103 @@ __global__ void __launch_bounds__(256) pink_init_kernel(PinkParams p) {
         if (j < p.J) p.state[d * p.J + j] = z[j];
 }
 
-// thread = (segment, detector); detectors fastest so that TOD accesses coalesce.
+// ONE pass over the TOD.  Block = 256 detectors x one segment of kPinkSeg samples; blocks take their
+// (segment, detector block) from a ticket counter, so a block's predecessor (same detectors, previous
+// segment) always started earlier.  Per thread:
+//   1. the segment's series from a ZERO state (Philox + Box-Muller + J FMAs per sample), kept in shared
+//      memory, and its end state e_j;
+//   2. the true state at the segment start c_j: the plan state for segment 0, else the predecessor's
+//      inclusive end state, published through global memory and a flag (acquire / release);
+//   3. own inclusive end state phi_j^len c_j + e_j published at once (the chain advances before the TOD
+//      is touched), the last segment's goes back into the plan state;
+//   4. TOD += series + sum_j g_j phi_j^(m+1) c_j, one read-modify-write.
+// The recurrence is linear, so 1 + 4 equals running it from the true state.
 template <int JM>      // JM = 4 or 8: number of AR(1) stages the unrolled loops cover (J <= JM)
 __global__ void __launch_bounds__(256)
-pink_local_kernel(PinkParams p, int64_t t0, int64_t T, float* __restrict__ tod) {
-    const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    const int64_t n_seg = (T + kPinkSeg - 1) / kPinkSeg;
-    if (idx >= n_seg * p.n_det) return;
-    const int64_t sg = idx / p.n_det, d = idx % p.n_det;
-    const uint32_t s = (uint32_t)(d / p.n_chan), c = (uint32_t)(d % p.n_chan);
-    float g[kPinkMaxJ], x[kPinkMaxJ];
+pink_chain_kernel(PinkParams p, int64_t t0, int64_t T, float* __restrict__ tod) {
+    extern __shared__ float s_pn[];                     // [kPinkSeg][256]
+    __shared__ uint32_t s_ticket;
+    const int tid = threadIdx.x;
+    const uint32_t n_dblk = (uint32_t)((p.n_det + 255) / 256);
+    if (tid == 0) s_ticket = atomicAdd(p.ticket, 1u);
+    __syncthreads();
+    const int64_t sg = s_ticket / n_dblk;
+    const uint32_t db = s_ticket % n_dblk;
+    const int64_t d = (int64_t)db * 256 + tid;
+    const bool valid = d < p.n_det;
+    const int64_t m0 = sg * kPinkSeg;
+    const int len = (int)min((int64_t)kPinkSeg, T - m0);
+    float g[JM], x[JM];
 #pragma unroll
-    for (int j = 0; j < JM; ++j) { g[j] = j < p.J ? p.gain[d * p.J + j] : 0.f; x[j] = 0.f; }
-    const int64_t m0 = sg * kPinkSeg, m1 = min(m0 + (int64_t)kPinkSeg, T);
-    // batches of kPinkBatch samples: the TOD values are fetched first (independent loads in flight while the
-    // Philox / Box-Muller arithmetic runs), the recurrence itself stays strictly sequential in m
-    for (int64_t mb = m0; mb < m1; mb += kPinkBatch) {
-        float cur[kPinkBatch];
+    for (int j = 0; j < JM; ++j) { g[j] = (valid && j < p.J) ? p.gain[d * p.J + j] : 0.f; x[j] = 0.f; }
+    if (valid) {
+        const uint32_t s = (uint32_t)(d / p.n_chan), c = (uint32_t)(d % p.n_chan);
+        for (int m = 0; m < len; ++m) {
+            float z[kPinkMaxJ];
+            pink_normals(p, (uint32_t)(t0 + m0 + m), s, c, z);
+            float pn = 0.f;
 #pragma unroll
-        for (int b = 0; b < kPinkBatch; ++b) cur[b] = mb + b < m1 ? __ldcs(tod + (mb + b) * p.n_det + d) : 0.f;
+            for (int j = 0; j < JM; ++j) {
+                x[j] = fmaf(p.phi[j], x[j], p.sq[j] * z[j]);
+                pn = fmaf(g[j], x[j], pn);
+            }
+            s_pn[m * 256 + tid] = pn;
+        }
+    }
+    // state at the segment start
+    if (sg > 0) {
+        if (tid == 0) {
+            const uint32_t* flag = p.flags + (size_t)(sg - 1) * n_dblk + db;
+            uint32_t v;
+            do {
+                asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(flag) : "memory");
+                if (v == 0u) __nanosleep(100);
+            } while (v == 0u);
+        }
+        __syncthreads();
+    }
+    float cin[JM];
 #pragma unroll
-        for (int b = 0; b < kPinkBatch; ++b) {
-            const int64_t m = mb + b;
-            if (m < m1) {
-                float z[kPinkMaxJ];
-                pink_normals(p, (uint32_t)(t0 + m), s, c, z);
-                float pn = 0.f;
+    for (int j = 0; j < JM; ++j) {
+        cin[j] = 0.f;
+        if (valid && j < p.J)
+            cin[j] = sg > 0 ? __ldcg(p.seg + ((sg - 1) * p.n_det + d) * p.J + j) : p.state[d * p.J + j];
+    }
+    // publish the inclusive end state, then release the successor
+    if (valid) {
 #pragma unroll
-                for (int j = 0; j < JM; ++j) {
-                    x[j] = fmaf(p.phi[j], x[j], p.sq[j] * z[j]);
-                    pn = fmaf(g[j], x[j], pn);
+        for (int j = 0; j < JM; ++j)
+            if (j < p.J) {
+                const float cout = fmaf(powf(p.phi[j], (float)len), cin[j], x[j]);
+                __stcg(p.seg + (sg * p.n_det + d) * p.J + j, cout);
+                if (m0 + len >= T) p.state[d * p.J + j] = cout;
+            }
+    }
+    __threadfence();
+    __syncthreads();
+    if (tid == 0) {
+        uint32_t* flag = p.flags + (size_t)sg * n_dblk + db;
+        asm volatile("st.release.gpu.global.u32 [%0], %1;" :: "l"(flag), "r"(1u) : "memory");
+    }
+    // one read-modify-write of the TOD
+    if (valid) {
+        float a[JM];
+#pragma unroll
+        for (int j = 0; j < JM; ++j) a[j] = g[j] * cin[j];
+        float* col = tod + m0 * p.n_det + d;
+        for (int mb = 0; mb < len; mb += kPinkBatch) {
+            float cur[kPinkBatch];
+#pragma unroll
+            for (int b = 0; b < kPinkBatch; ++b) cur[b] = mb + b < len ? __ldcs(col + (int64_t)(mb + b) * p.n_det) : 0.f;
+#pragma unroll
+            for (int b = 0; b < kPinkBatch; ++b) {
+                const int m = mb + b;
+                if (m < len) {
+                    float add = 0.f;
+#pragma unroll
+                    for (int j = 0; j < JM; ++j) { a[j] *= p.phi[j]; add += a[j]; }
+                    col[(int64_t)m * p.n_det] = cur[b] + (s_pn[m * 256 + tid] + add);
                 }
-                tod[m * p.n_det + d] = cur[b] + pn;
-            }
-        }
-    }
-#pragma unroll
-    for (int j = 0; j < JM; ++j)
-        if (j < p.J) p.seg[(sg * p.n_det + d) * p.J + j] = x[j];
-}
-
-// thread = (detector, stage): walks the segments, replaces e[seg] by the state at the segment start.
-// The chain c <- phi^len c + e is a dependent FMA per segment, but its inputs are not: they are
-// fetched 16 segments at a time so that the walk costs one memory round trip per batch instead of one
-// per segment.
-__global__ void __launch_bounds__(256) pink_carry_kernel(PinkParams p, int64_t T) {
-    const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (idx >= p.n_det * p.J) return;
-    const int j = (int)(idx % p.J);
-    const int64_t n_seg = (T + kPinkSeg - 1) / kPinkSeg;
-    const int64_t stride = p.n_det * p.J;                  // seg[sg][d][j]: idx is the offset inside one segment slice
-    float cst = p.state[idx];
-    const float phi = p.phi[j];
-    const float phiL = powf(phi, (float)kPinkSeg);
-    constexpr int kBatch = 16;
-    for (int64_t s0 = 0; s0 < n_seg; s0 += kBatch) {
-        float e[kBatch];
-#pragma unroll
-        for (int b = 0; b < kBatch; ++b) e[b] = s0 + b < n_seg ? p.seg[(s0 + b) * stride + idx] : 0.f;
-#pragma unroll
-        for (int b = 0; b < kBatch; ++b) {
-            const int64_t sg = s0 + b;
-            if (sg < n_seg) {
-                p.seg[sg * stride + idx] = cst;
-                const int64_t len = min((int64_t)kPinkSeg, T - sg * kPinkSeg);
-                cst = fmaf(len == kPinkSeg ? phiL : powf(phi, (float)len), cst, e[b]);
-            }
-        }
-    }
-    p.state[idx] = cst;
-}
-
-template <int JM>
-__global__ void __launch_bounds__(256)
-pink_fixup_kernel(PinkParams p, int64_t T, float* __restrict__ tod) {
-    const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    const int64_t n_seg = (T + kPinkSeg - 1) / kPinkSeg;
-    if (idx >= n_seg * p.n_det) return;
-    const int64_t sg = idx / p.n_det, d = idx % p.n_det;
-    float a[kPinkMaxJ];       // g_j * phi_j^(m+1) * c_j
-#pragma unroll
-    for (int j = 0; j < JM; ++j)
-        a[j] = j < p.J ? p.gain[d * p.J + j] * p.seg[(sg * p.n_det + d) * p.J + j] : 0.f;
-    const int64_t m0 = sg * kPinkSeg, m1 = min(m0 + (int64_t)kPinkSeg, T);
-    for (int64_t mb = m0; mb < m1; mb += kPinkBatch) {
-        float cur[kPinkBatch];
-#pragma unroll
-        for (int b = 0; b < kPinkBatch; ++b) cur[b] = mb + b < m1 ? __ldcs(tod + (mb + b) * p.n_det + d) : 0.f;
-#pragma unroll
-        for (int b = 0; b < kPinkBatch; ++b) {
-            const int64_t m = mb + b;
-            if (m < m1) {
-                float add = 0.f;
-#pragma unroll
-                for (int j = 0; j < JM; ++j) { a[j] *= p.phi[j]; add += a[j]; }
-                tod[m * p.n_det + d] = cur[b] + add;
             }
         }
     }
