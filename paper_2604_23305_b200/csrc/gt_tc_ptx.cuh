@@ -49,7 +49,10 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
 // wait of a role that is not latency critical: back off between polls so that the spinning warp does not
 // take issue slots from the generator warps of its scheduler
 __device__ __forceinline__ void mbar_wait_relaxed(uint32_t bar, uint32_t parity) {
-    while (!mbar_try_wait(bar, parity)) { __nanosleep(64); }
+#ifndef GT_TC_RELAX_NS
+#define GT_TC_RELAX_NS 64
+#endif
+    while (!mbar_try_wait(bar, parity)) { __nanosleep(GT_TC_RELAX_NS); }
 }
 
 // ---- thread-block cluster (CTA pair) ----------------------------------------------------------
