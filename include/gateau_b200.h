@@ -60,7 +60,7 @@ typedef struct {
 
 /* Kernel variant for step 2-6a (the fused generator + contraction + photon-noise kernel). */
 enum {
-    GT_VARIANT_DEFAULT = 0,   /* tcgen05 tensor-core kernel, split-TF32 operands                 */
+    GT_VARIANT_DEFAULT = 0,   /* tcgen05 tensor-core kernel, three-term split of the fp32 operands */
     GT_VARIANT_FP32    = 1,   /* FP32 CUDA-core kernel (the measured alternative of north_star)  */
     GT_VARIANT_TENSOR  = 2    /* tcgen05 kernel, explicitly                                      */
 };
@@ -161,7 +161,7 @@ gt_status gt_debug_pkid(gt_plan* plan, int64_t t_begin, int64_t t_count,
                         float* pkid_out, void* cuda_stream);
 /* Number of kernels this library launched since the plan was created. */
 int64_t gt_launch_count(const gt_plan* plan);
-/* Name of the fused-kernel variant the plan resolved to ("tcgen05-3xtf32", "fp32-ffma"). */
+/* Name of the fused-kernel variant the plan resolved to ("tcgen05-3xf16-split", "fp32-ffma"). */
 const char* gt_variant_name(const gt_plan* plan);
 /* Device time [ms] the fused kernel took in the last gt_simulate / gt_debug_pkid call, summed
  * over its launches (CUDA events on the launching stream); synchronises the stream.  Also

@@ -341,7 +341,7 @@ gt_status gt_plan_create(const gt_config* cfg, void* cuda_stream, gt_plan** out_
     GT_CUDA0(cudaStreamSynchronize(st));
 
     const int nf = c.n_freq, nc = c.n_chan, ns = c.n_spaxel;
-    const int nfp = (nf + 31) / 32 * 32;
+    const int nfp = (nf + 63) / 64 * 64;      // the tensor kernel works in slabs of 64 frequencies
     p->n_freq = nf; p->n_freq_pad = nfp; p->n_chan = nc; p->n_spaxel = ns; p->n_pwv = c.n_pwv;
     p->n_samples = c.n_samples; p->photon_noise = c.photon_noise != 0; p->pink_noise = c.pink_noise != 0;
     p->seed = c.seed; p->cube = c.cube; p->n_az = c.n_az; p->n_el = c.n_el;
@@ -599,7 +599,7 @@ int64_t gt_launch_count(const gt_plan* plan) { return plan ? plan->launches : 0;
 
 const char* gt_variant_name(const gt_plan* plan) {
     if (!plan) return "";
-    return plan->variant == GT_VARIANT_FP32 ? "fp32-ffma" : "tcgen05-3xtf32";
+    return plan->variant == GT_VARIANT_FP32 ? "fp32-ffma" : "tcgen05-3xf16-split";
 }
 
 double gt_last_fused_ms(gt_plan* plan, int32_t* n_launches) {

@@ -5,14 +5,15 @@
 // (steps 2-4, collapsed cascade of DESIGN.md) and never exists in HBM.  Per persistent CTA
 // (one per SM) and per tile of 128 rows:
 //
-//   generator warps (8)   : 32-frequency slab of the spectrum for 128 rows -> split into
-//                           tf32 hi + lo -> shared memory in the UMMA K-major SWIZZLE_128B layout
-//   loader warp (1 lane)  : filter slab images (hi, lo; pre-split, pre-swizzled at plan time)
-//                           global -> shared by cp.async.bulk, mbarrier complete_tx
-//   MMA warp (1 lane)     : tcgen05.mma.kind::tf32, M = 128, N <= 128 per column group, K = 8:
-//                           acc += A_hi.B_hi + A_lo.B_hi + A_hi.B_lo     ("3xTF32", fp32 accumulate
-//                           in tensor memory; the dropped A_lo.B_lo term is ~2^-22 relative)
-//   epilogue warps (4)    : SEGMENTED ACCUMULATION.  The tensor core's fp32 accumulate truncates
+//   generator warps (16)  : 64-frequency slab of the spectrum for 128 rows -> fp16 pair (hi, lo) of the
+//                           scaled value (22 mantissa bits) -> shared memory, UMMA K-major SWIZZLE_128B
+//   loader warp (1 lane)  : filter slab images (hi, lo; pre-split, pre-swizzled at plan time; CTA pair:
+//                           this CTA's half) global -> shared by cp.async.bulk, mbarrier complete_tx
+//   MMA warp (1 lane)     : tcgen05.mma.cta_group::2.kind::f16, M = 256 per CTA pair, N <= 128 per column
+//                           group, K = 16:  acc += A_hi.B_hi + A_lo.B_hi + A_hi.B_lo  (the three-term split
+//                           of north_star with fp16 pieces: every product of two 11-bit pieces is exact in
+//                           the fp32 accumulate, the dropped A_lo.B_lo term is 2^-22 relative)
+//   flush warps (4)       : SEGMENTED ACCUMULATION.  The tensor core's fp32 accumulate truncates
 //                           (measured: -2.7e-5 relative after 500 chained MMAs of positive terms,
 //                           DESIGN.md "Accumulation in tensor memory"), so no accumulator lives
 //                           longer than `seg` slabs: the <= 384 padded channels of a tile are cut
@@ -21,16 +22,18 @@
 //                           group moves to the spare buffer and the epilogue warps add the
 //                           finished partial sums (tcgen05.ld) into a per-CTA, L2-resident fp32
 //                           scratch tile [column][row] with round-to-nearest FADDs.  After the
-//                           last segment they transpose the scratch tile into the TOD:
+//                           last segment the finisher warps (4) transpose the scratch tile into the TOD:
 //                           P = sum*scale + bias[c], photon noise (Eq. 18-19), coalesced stores.
 //
-// Pipelines: A ring (2 stages, generator -> MMA), B ring (loader -> MMA), accumulator buffers
-// flush_full / buf_free (MMA <-> epilogue); all mbarrier based.
+// Pipelines: A ring (3 stages, generators of both CTAs -> leader's MMA thread), B ring (loader -> MMA, the
+// peer's halves relayed by a forwarder), accumulator buffers flush_full / buf_free (MMA <-> flush), scratch
+// tiles tile_done / scratch_free (flush <-> finisher); all mbarrier based, CTA-scope waits.
 #pragma once
 #include <vector>
 #include <cstring>
 #include <algorithm>
 #include <cstdlib>
+#include <cuda_fp16.h>
 #include "gt_common.cuh"
 #include "gt_fused_fp32.cuh"
 #include "gt_tc_ptx.cuh"
@@ -39,8 +42,12 @@
 namespace gt {
 
 constexpr int kTcBM = 128;                 // rows per tile (UMMA M)
-constexpr int kTcBK = 32;                  // frequencies per A stage / B unit: one 128-byte swizzle row
-constexpr int kTcUK = 8;                   // K of one tcgen05.mma.kind::tf32
+constexpr int kTcBK = 64;                  // frequencies per A stage / B unit: one 128-byte swizzle row of 64 fp16
+constexpr int kTcHB = 32;                  // frequencies per generator step group (8 lanes x 4): half a slab
+constexpr int kTcKSteps = 4;               // K = 16 MMAs per 128-byte operand row
+// operand scaling into the fp16 range (exact powers of two, undone in the output scale): spectrum values are
+// O(1) (P_nu / (k_B 300 K)), filter transmissions are <= 1
+constexpr float kTcScaleA = 256.0f, kTcScaleB = 16384.0f;
 #ifndef GT_TC_A_STAGES
 #define GT_TC_A_STAGES 3
 #endif
@@ -58,7 +65,7 @@ constexpr bool kTcPair = GT_TC_PAIR != 0;
 #else
 #define GT_DIAG(p, bit) false
 #endif
-constexpr int kTcAPartBytes = kTcBM * kTcBK * 4;            // 16 KB (hi or lo)
+constexpr int kTcAPartBytes = kTcBM * 128;                  // 16 KB (hi or lo part: 128 rows of 64 fp16)
 constexpr int kTcAStageBytes = 2 * kTcAPartBytes;           // 32 KB
 constexpr int kTcEpiWarps = 4, kTcGenWarps = 16;
 // warp roles, aligned to warpgroups of 4 warps so that setmaxnreg can move registers between them:
@@ -85,8 +92,8 @@ constexpr int kTcRegsFlush = GT_TC_REGS_FLUSH, kTcRegsCtl = 40, kTcRegsGen = 80,
 static_assert(kTcRegsFlush + kTcRegsCtl + 4 * kTcRegsGen + kTcRegsFin <= 7 * 72, "setmaxnreg pool");
 constexpr int kTcMaxGroupChan = 384;       // channels per tile: 3 column groups of 128 (+ 1 spare buffer = 512 columns)
 constexpr int kTcBufCols = 128, kTcNumBuf = 4, kTcMaxCg = 3;
-constexpr int kTcSegDefault = 8;           // slabs (of 32 frequencies) per accumulation segment
-constexpr float kTcTruncPerMma = 5.0e-8f;  // measured mean relative truncation loss per chained MMA (half the worst case)
+constexpr int kTcSegDefault = 8;           // slabs (of 64 frequencies) per accumulation segment
+constexpr float kTcTruncPerMma = 4.0e-8f;  // measured mean relative truncation loss per chained kind::f16 MMA (about half the worst case)
 #ifndef GT_TC_MAX_B_STAGES
 #define GT_TC_MAX_B_STAGES 4
 #endif
@@ -100,7 +107,7 @@ struct TcTables {
     int32_t nb_tot = 0;                  // padded channels per group (multiple of 32)
     int32_t n_cg = 0;                    // column groups per tile, widths 128,..,remainder
     int32_t seg = kTcSegDefault;         // slabs per accumulation segment
-    int32_t n_kb = 0;                    // n_freq_pad / 32
+    int32_t n_kb = 0;                    // n_freq_pad / 64
     int32_t unit_bytes = 0;              // nb_tot * 128
     int32_t b_stages = 0;
     int32_t smem_bytes = 0;
@@ -109,22 +116,7 @@ struct TcTables {
 inline const char*& tc_error_ref() { static const char* e = ""; return e; }
 inline const char* tc_error() { return tc_error_ref(); }
 
-// round-to-nearest (ties away) fp32 -> tf32 on the host, finite inputs
-inline float host_tf32(float x) {
-    uint32_t b; std::memcpy(&b, &x, 4);
-    b = (b + 0x1000u) & 0xFFFFE000u;
-    float r; std::memcpy(&r, &b, 4);
-    return r;
-}
-
-// round-to-nearest-even fp32 -> bf16 bits on the host, finite inputs
-inline uint16_t host_bf16(float x) {
-    uint32_t b; std::memcpy(&b, &x, 4);
-    b += 0x7FFFu + ((b >> 16) & 1u);
-    return (uint16_t)(b >> 16);
-}
-
-// Splits the filter into tf32 hi/lo parts and lays every (group, 32-frequency slab, part) out as
+// Splits the (scaled) filter into fp16 hi/lo parts and lays every (group, 64-frequency slab, part) out as
 // the exact shared-memory image tcgen05.mma reads (K-major, SWIZZLE_128B): the loader is a flat copy.
 inline gt_status build_tc_tables(const std::vector<float>& filt, int n_chan, int n_freq, int n_freq_pad,
                                  TcTables& t, cudaStream_t st) {
@@ -155,20 +147,17 @@ inline gt_status build_tc_tables(const std::vector<float>& filt, int n_chan, int
             const int rk = kTcPair ? (n - col0) / (w / 2) : 0;
             const int nl = kTcPair ? col0 / 2 + (n - col0) - rk * (w / 2) : n;        // local row
             for (int i = 0; i < n_freq; ++i) {
-                const float f = filt[(size_t)ch * n_freq + i];
-                const float hi = host_tf32(f), lo = f - hi;
+                const float f = filt[(size_t)ch * n_freq + i] * kTcScaleB;
+                const __half fh = __float2half_rn(f);
+                const __half fl = __float2half_rn(f - __half2float(fh));
                 const int kb = i / kTcBK, kk = i % kTcBK;
-                // float index of (group tile, slab, unit 0, rank): units are laid out [g][kb][unit][rank]
-                const size_t unit0 = ((size_t)((g * t.n_kb + kb) * 2 + 0) * kRanks + rk) * (t.unit_bytes / 4);
-                const size_t unit1 = ((size_t)((g * t.n_kb + kb) * 2 + 1) * kRanks + rk) * (t.unit_bytes / 4);
-                // unit 0: tf32 hi part
-                img[unit0 + (size_t)nl * 32 + (size_t)(((kk >> 2) ^ (nl & 7)) << 2) + (kk & 3)] = hi;
-                // unit 1: bf16, per group of 8 frequencies [Fm_0..7 | lo_0..7] (pairs with A's [lo | hi])
-                const int kg = kk >> 3, fi = kk & 7;
-                const size_t row16 = unit1 * 2 + (size_t)nl * 64;                                 // in bf16 elements
-                const int c_hi = kg * 2, c_lo = kg * 2 + 1;                                       // 16-byte chunks
-                img16[row16 + (size_t)((c_hi ^ (nl & 7)) << 3) + fi] = host_bf16(f);
-                img16[row16 + (size_t)((c_lo ^ (nl & 7)) << 3) + fi] = host_bf16(lo);
+                // element index of (group tile, slab, unit, rank): units are laid out [g][kb][unit][rank]
+                const size_t unit0 = ((size_t)((g * t.n_kb + kb) * 2 + 0) * kRanks + rk) * (t.unit_bytes / 2);
+                const size_t unit1 = ((size_t)((g * t.n_kb + kb) * 2 + 1) * kRanks + rk) * (t.unit_bytes / 2);
+                // K-major SWIZZLE_128B row of 64 fp16: 16-byte chunk (kk / 8) XOR (row % 8)
+                const size_t off = (size_t)nl * 64 + (size_t)(((kk >> 3) ^ (nl & 7)) << 3) + (kk & 7);
+                img16[unit0 + off] = __half_as_ushort(fh);         // unit 0: Fm_hi
+                img16[unit1 + off] = __half_as_ushort(fl);         // unit 1: Fm_lo
             }
         }
     if (cudaMalloc(reinterpret_cast<void**>(&t.filt_img), total) != cudaSuccess) {
@@ -267,25 +256,26 @@ __device__ __forceinline__ float element_value_fast(float eta_z, float csc, floa
     return fmaf(eta, fmaf(G, S, -Xn), Xn);           // (1 - eta) Xn + eta G S in two FMAs
 }
 
-// Writes 4 consecutive frequencies (16-byte chunk `chunk` of a 32-frequency slab) of tile row `row`
-// into an A stage:
-//   part 0 (tf32):  hi = top 19 bits of v, K-major SWIZZLE_128B rows of 32 tf32
-//   part 1 (bf16):  per group of 8 frequencies the 16 values [lo_0..lo_7 | hi_0..hi_7] (lo = v - hi),
-//                   i.e. the K = 16 operand of ONE kind::f16 MMA whose B operand holds
-//                   [Fm_hi_0..7 | Fm_lo_0..7]: it adds lo.Fm_hi + hi.Fm_lo, the two correction terms of
-//                   the split product (each only needs ~8 bits: they are 2^-11 of the main term).
-__device__ __forceinline__ void store_split(unsigned char* a_stage, int row, int chunk, const float4& v) {
-    float4 hi;
-    hi.x = ptx::tf32_trunc(v.x); hi.y = ptx::tf32_trunc(v.y); hi.z = ptx::tf32_trunc(v.z); hi.w = ptx::tf32_trunc(v.w);
-    const uint32_t r7 = (uint32_t)(row & 7), rowoff = (uint32_t)row * 128u;
-    *reinterpret_cast<float4*>(a_stage + rowoff + (((uint32_t)chunk ^ r7) << 4)) = hi;
-    uint2 lo2, hi2;
-    lo2.x = ptx::pack_bf16x2(v.x - hi.x, v.y - hi.y); lo2.y = ptx::pack_bf16x2(v.z - hi.z, v.w - hi.w);
-    hi2.x = ptx::pack_bf16x2(hi.x, hi.y);             hi2.y = ptx::pack_bf16x2(hi.z, hi.w);
-    const uint32_t c16 = (uint32_t)(chunk >> 1) * 2u, sub = (uint32_t)(chunk & 1) * 8u;
-    unsigned char* part1 = a_stage + kTcAPartBytes + rowoff + sub;
-    *reinterpret_cast<uint2*>(part1 + ((c16 ^ r7) << 4)) = lo2;
-    *reinterpret_cast<uint2*>(part1 + (((c16 + 1u) ^ r7) << 4)) = hi2;
+// Writes 4 consecutive frequencies (lane-chunk `chunk` of half `h` of a 64-frequency slab) of tile row `row`
+// into an A stage as the fp16 pair (hi, lo) of the scaled value: hi = fp16(s v), lo = fp16(s v - hi), 22
+// mantissa bits together.  Part 0 holds hi, part 1 lo, each as K-major SWIZZLE_128B rows of 64 fp16.  The filter
+// is split the same way at plan time and the contraction is issued as hi.Fm_hi + lo.Fm_hi + hi.Fm_lo with
+// kind::f16 MMAs (K = 16, fp32 accumulate): north_star's three-term split with the accuracy of 3xTF32 (each
+// product of two 11-bit pieces is exact in fp32, the dropped lo.Fm_lo is 2^-22) at 3/8 of its tensor time and
+// half of its operand bytes.
+__device__ __forceinline__ void store_split(unsigned char* a_stage, int row, int chunk, int h, const float4& v) {
+    const float2 s01 = make_float2(v.x * kTcScaleA, v.y * kTcScaleA), s23 = make_float2(v.z * kTcScaleA, v.w * kTcScaleA);
+    const __half2 h01 = __float22half2_rn(s01), h23 = __float22half2_rn(s23);
+    const float2 b01 = __half22float2(h01), b23 = __half22float2(h23);
+    const __half2 l01 = __float22half2_rn(make_float2(s01.x - b01.x, s01.y - b01.y));
+    const __half2 l23 = __float22half2_rn(make_float2(s23.x - b23.x, s23.y - b23.y));
+    uint2 hi2, lo2;
+    hi2.x = *reinterpret_cast<const uint32_t*>(&h01); hi2.y = *reinterpret_cast<const uint32_t*>(&h23);
+    lo2.x = *reinterpret_cast<const uint32_t*>(&l01); lo2.y = *reinterpret_cast<const uint32_t*>(&l23);
+    const uint32_t c16 = (uint32_t)(h * 4 + (chunk >> 1)), sub = (uint32_t)(chunk & 1) * 8u;
+    unsigned char* dst = a_stage + (uint32_t)row * 128u + ((c16 ^ (uint32_t)(row & 7)) << 4) + sub;
+    *reinterpret_cast<uint2*>(dst) = hi2;
+    *reinterpret_cast<uint2*>(dst + kTcAPartBytes) = lo2;
 }
 
 // element (column, row) of a scratch tile laid out [column / 4][row][column % 4]
@@ -354,10 +344,7 @@ fused_tc_kernel(const TcParams p) {
     auto commit_pair = [&](uint32_t bar) {                          // completion of the MMAs issued so far, signalled to both CTAs
         if constexpr (kTcPair) ptx::tc_commit2(bar, (uint16_t)3); else ptx::tc_commit(bar);
     };
-    auto mma_tf32 = [&](uint32_t d, uint64_t a, uint64_t b, uint32_t id, uint32_t acc) {
-        if constexpr (kTcPair) ptx::mma2_tf32_ss(d, a, b, id, acc); else ptx::mma_tf32_ss(d, a, b, id, acc);
-    };
-    auto mma_bf16 = [&](uint32_t d, uint64_t a, uint64_t b, uint32_t id, uint32_t acc) {
+    auto mma_f16 = [&](uint32_t d, uint64_t a, uint64_t b, uint32_t id, uint32_t acc) {       // kind::f16, K = 16
         if constexpr (kTcPair) ptx::mma2_bf16_ss(d, a, b, id, acc); else ptx::mma_bf16_ss(d, a, b, id, acc);
     };
     auto tile_row0 = [&](int64_t tl) -> int64_t {
@@ -416,26 +403,19 @@ fused_tc_kernel(const TcParams p) {
                 const uint32_t tap01 = f.cube != nullptr ? (uint32_t)nf : 0u;
                 const uint32_t tap10 = f.cube != nullptr ? (uint32_t)f.n_az * (uint32_t)nf : 0u;
                 const uint32_t nu_last = (uint32_t)(max(f.n_freq, 4) - 4) & ~3u;     // 16-byte aligned (n_freq % 4 == 0 with a cube)
-                auto issue = [&](int kb, int j, Tap& t) {
-                    const uint32_t lo = lut_off[j] + (uint32_t)kb * kTcBK;
+                auto issue = [&](int hb, int j, Tap& t) {                 // hb = half-slab (32 frequencies)
+                    const uint32_t lo = lut_off[j] + (uint32_t)hb * kTcHB;
                     t.L0 = ldg4(f.lut_r + lo); t.L1 = ldg4(f.lut_r + (lo + (uint32_t)nfp));
                     if (GT_DIAG(p, 16)) return;
-                    const uint32_t co = cube_off[j] + min((uint32_t)kb * kTcBK + (uint32_t)chunk * 4u, nu_last);
+                    const uint32_t co = cube_off[j] + min((uint32_t)hb * kTcHB + (uint32_t)chunk * 4u, nu_last);
                     t.c00 = ldg4(cube_base + co);           t.c01 = ldg4(cube_base + (co + tap01));
                     t.c10 = ldg4(cube_base + (co + tap10)); t.c11 = ldg4(cube_base + (co + tap10 + tap01));
                 };
-                auto compute = [&](int j, const Tap& cur, const float4& X, const float4& G, uint32_t stage) {
+                auto compute = [&](int j, int h, const Tap& cur, const float4& X, const float4& G, uint32_t stage) {
                     const RowParam* rp = rowp + rsub + kTcRowStride * j;
                     const float2 fc = *reinterpret_cast<const float2*>(rp);                    // fp, csc
                     const float4 w = *reinterpret_cast<const float4*>(&rp->w00);
                     float4 S, v;
-                    if (GT_DIAG(p, 32)) {
-                        unsigned char* a_hi = smem_raw + (sm.a - raw) + stage * kTcAStageBytes;
-                        const uint32_t off = (uint32_t)(rsub + kTcRowStride * j) * 128u + swz;
-                        *reinterpret_cast<float4*>(a_hi + off) = cur.L0;
-                        *reinterpret_cast<float4*>(a_hi + kTcAPartBytes + off) = cur.c00;
-                        return;
-                    }
                     S.x = w.x * cur.c00.x + w.y * cur.c01.x + w.z * cur.c10.x + w.w * cur.c11.x;
                     S.y = w.x * cur.c00.y + w.y * cur.c01.y + w.z * cur.c10.y + w.w * cur.c11.y;
                     S.z = w.x * cur.c00.z + w.y * cur.c01.z + w.z * cur.c10.z + w.w * cur.c11.z;
@@ -444,10 +424,11 @@ fused_tc_kernel(const TcParams p) {
                     v.y = element_value_fast(fmaf(fc.x, cur.L1.y - cur.L0.y, cur.L0.y), fc.y, X.y, G.y, S.y);
                     v.z = element_value_fast(fmaf(fc.x, cur.L1.z - cur.L0.z, cur.L0.z), fc.y, X.z, G.z, S.z);
                     v.w = element_value_fast(fmaf(fc.x, cur.L1.w - cur.L0.w, cur.L0.w), fc.y, X.w, G.w, S.w);
-                    store_split(smem_raw + (sm.a - raw) + stage * kTcAStageBytes, rsub + kTcRowStride * j, chunk, v);
+                    store_split(smem_raw + (sm.a - raw) + stage * kTcAStageBytes, rsub + kTcRowStride * j, chunk, h, v);
                 };
                 Tap t0, t1;
                 issue(0, 0, t0);
+                const int n_hb = 2 * p.n_kb;
                 for (int kb = 0; kb < p.n_kb; ++kb, a_ph ^= (++a_st == kTcAStages), a_st = a_st == kTcAStages ? 0u : a_st) {
                     const uint32_t stage = a_st, ph = a_ph;
                     if (GT_DIAG(p, 1)) {
@@ -456,12 +437,16 @@ fused_tc_kernel(const TcParams p) {
                         if (lane == 0) arrive_leader(sm.a_full + 8 * stage);
                         continue;
                     }
-                    const float4 X = ldg4(f.Xn + kb * kTcBK + chunk * 4), G = ldg4(f.Gs + kb * kTcBK + chunk * 4);
-                    issue(kb, 1, t1);
-                    wait_pair(sm.a_empty + 8 * stage, ph ^ 1u);
-                    compute(0, t0, X, G, stage);
-                    if (kb + 1 < p.n_kb) issue(kb + 1, 0, t0);
-                    compute(1, t1, X, G, stage);
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        const int hb = 2 * kb + h;
+                        const float4 X = ldg4(f.Xn + hb * kTcHB + chunk * 4), G = ldg4(f.Gs + hb * kTcHB + chunk * 4);
+                        issue(hb, 1, t1);
+                        if (h == 0) wait_pair(sm.a_empty + 8 * stage, ph ^ 1u);
+                        compute(0, h, t0, X, G, stage);
+                        if (hb + 1 < n_hb) issue(hb + 1, 0, t0);
+                        compute(1, h, t1, X, G, stage);
+                    }
                     // one arrival per warp: 512 per-thread arrivals on one mbarrier serialise (~5 cycles each)
                     ptx::fence_proxy_async_smem();
                     __syncwarp();
@@ -499,16 +484,18 @@ fused_tc_kernel(const TcParams p) {
                     if (lane == 0) arrive_leader(sm.a_full + 8 * stage);
                     continue;
                 }
-                const int nu0 = kb * kTcBK + chunk * 4;
+                for (int h = 0; h < 2; ++h) {
+                const int hb = 2 * kb + h;
+                const int nu0 = hb * kTcHB + chunk * 4;
                 const float4 X = ldg4(f.Xn + nu0), G = ldg4(f.Gs + nu0);
                 float4 L0[kTcRowsPerThread], L1[kTcRowsPerThread], S[kTcRowsPerThread];
 #pragma unroll
                 for (int j = 0; j < kTcRowsPerThread; ++j) {
-                    L0[j] = ldg4(lutp[j] + kb * kTcBK);
-                    L1[j] = ldg4(lutp[j] + nfp + kb * kTcBK);
+                    L0[j] = ldg4(lutp[j] + hb * kTcHB);
+                    L1[j] = ldg4(lutp[j] + nfp + hb * kTcHB);
                     S[j] = make_float4(0.f, 0.f, 0.f, 0.f);
                     if (cubep[j] != nullptr && nu0 < f.n_freq) {
-                        const float* c00 = cubep[j] + kb * kTcBK;
+                        const float* c00 = cubep[j] + hb * kTcHB;
                         const float* c01 = c00 + nf;
                         const float* c10 = c00 + (size_t)f.n_az * nf;
                         const float* c11 = c10 + nf;
@@ -529,7 +516,7 @@ fused_tc_kernel(const TcParams p) {
                         }
                     }
                 }
-                wait_pair(sm.a_empty + 8 * stage, ph ^ 1u);
+                if (h == 0) wait_pair(sm.a_empty + 8 * stage, ph ^ 1u);
                 unsigned char* a_hi = smem_raw + (sm.a - raw) + stage * kTcAStageBytes;
 #pragma unroll
                 for (int j = 0; j < kTcRowsPerThread; ++j) {
@@ -538,7 +525,8 @@ fused_tc_kernel(const TcParams p) {
                     v.y = element_value_fast(fmaf(fp[j], L1[j].y - L0[j].y, L0[j].y), csc[j], X.y, G.y, S[j].y);
                     v.z = element_value_fast(fmaf(fp[j], L1[j].z - L0[j].z, L0[j].z), csc[j], X.z, G.z, S[j].z);
                     v.w = element_value_fast(fmaf(fp[j], L1[j].w - L0[j].w, L0[j].w), csc[j], X.w, G.w, S[j].w);
-                    store_split(a_hi, rsub + kTcRowStride * j, chunk, v);
+                    store_split(a_hi, rsub + kTcRowStride * j, chunk, h, v);
+                }
                 }
                 ptx::fence_proxy_async_smem();
                 __syncwarp();
@@ -586,11 +574,10 @@ fused_tc_kernel(const TcParams p) {
         {   // the whole warp runs the loop (uniform control flow); one elected lane issues
             TcRotation rot(p.n_cg, p.seg, p.n_kb);
             uint32_t idesc[kTcMaxCg];
-            constexpr uint32_t kToBf16 = (3u << 7) | (3u << 10);      // tf32 (2) -> bf16 (1) in both operand-format fields
             uint32_t fresh = 7u;               // bit g: next MMA into buf(g) overwrites (first of a segment)
             uint32_t used = 0u, par = 0u;      // bit b: buffer b was flushed before / parity of its flush count
 #pragma unroll
-            for (int g = 0; g < kTcMaxCg; ++g) idesc[g] = ptx::idesc_tf32(kTcPair ? 2 * kTcBM : kTcBM, g < p.n_cg ? rot.width(g, p.nb_tot) : 16);
+            for (int g = 0; g < kTcMaxCg; ++g) idesc[g] = ptx::idesc_f16(kTcPair ? 2 * kTcBM : kTcBM, g < p.n_cg ? rot.width(g, p.nb_tot) : 16);
             const bool issue = !GT_DIAG(p, 2);
             constexpr int kGroupDesc = (kTcBufCols * 128 >> 4) / (kTcPair ? 2 : 1);   // descriptor step between column groups (pair: half the rows)
             uint32_t a_st = 0, a_ph = 0, bs = 0, bph = 0;
@@ -609,38 +596,39 @@ fused_tc_kernel(const TcParams p) {
                     wait_lead(sm.a_full + 8 * stage, ph);
                     const uint64_t ad_hi = ptx::smem_desc_sw128(sm.a + stage * kTcAStageBytes);
                     const uint64_t ad_lo = ad_hi + (uint64_t)(kTcAPartBytes >> 4);
-                    {   // tf32 unit: acc += A_hi.Fm_hi
+                    {   // unit 0: acc += A_hi.Fm_hi + A_lo.Fm_hi
                         ptx::mbar_wait(sm.b_full + 8 * bs, bph);
                         if constexpr (kTcPair) ptx::mbar_wait(sm.b_peer + 8 * bs, bph);
                         ptx::tc_fence_after();
                         const uint64_t bd0 = ptx::smem_desc_sw128(sm.b + bs * (uint32_t)p.unit_bytes);
                         if (issue && ptx::elect_one()) {
 #pragma unroll
-                            for (int k = 0; k < kTcBK / kTcUK; ++k)
+                            for (int k = 0; k < kTcKSteps; ++k)
 #pragma unroll
                                 for (int g = 0; g < kTcMaxCg; ++g)
                                     if (g < p.n_cg) {
                                         const uint64_t bd = bd0 + (uint64_t)(g * kGroupDesc + k * 2);
-                                        mma_tf32(d[g], ad_hi + (uint64_t)(k * 2), bd, idesc[g], (k != 0 || !(fresh >> g & 1u)) ? 1u : 0u);
+                                        mma_f16(d[g], ad_hi + (uint64_t)(k * 2), bd, idesc[g], (k != 0 || !(fresh >> g & 1u)) ? 1u : 0u);
+                                        mma_f16(d[g], ad_lo + (uint64_t)(k * 2), bd, idesc[g], 1u);
                                     }
                         }
                         __syncwarp();
                         if (ptx::elect_one()) commit_pair(sm.b_empty + 8 * bs);
                         if (++bs == (uint32_t)p.b_stages) { bs = 0; bph ^= 1u; }
                     }
-                    {   // bf16 unit: acc += A_lo.Fm_hi + A_hi.Fm_lo (one K = 16 MMA per 8 frequencies)
+                    {   // unit 1: acc += A_hi.Fm_lo
                         ptx::mbar_wait(sm.b_full + 8 * bs, bph);
                         if constexpr (kTcPair) ptx::mbar_wait(sm.b_peer + 8 * bs, bph);
                         ptx::tc_fence_after();
                         const uint64_t bd0 = ptx::smem_desc_sw128(sm.b + bs * (uint32_t)p.unit_bytes);
                         if (issue && ptx::elect_one()) {
 #pragma unroll
-                            for (int k = 0; k < kTcBK / kTcUK; ++k)
+                            for (int k = 0; k < kTcKSteps; ++k)
 #pragma unroll
                                 for (int g = 0; g < kTcMaxCg; ++g)
                                     if (g < p.n_cg)
-                                        mma_bf16(d[g], ad_lo + (uint64_t)(k * 2),
-                                                         bd0 + (uint64_t)(g * kGroupDesc + k * 2), idesc[g] ^ kToBf16, 1u);
+                                        mma_f16(d[g], ad_hi + (uint64_t)(k * 2),
+                                                        bd0 + (uint64_t)(g * kGroupDesc + k * 2), idesc[g], 1u);
                         }
                         __syncwarp();
                         if (ptx::elect_one()) commit_pair(sm.b_empty + 8 * bs);
@@ -805,7 +793,7 @@ inline cudaError_t launch_fused_tc(const FusedParams& fp, const TcTables& t, int
     // the one-sided error interval.
     {
         const int seg = t.seg > 0 ? t.seg : kTcSegDefault;
-        p.f.scale *= 1.0f + kTcTruncPerMma * (float)(2 * (kTcBK / kTcUK) * std::min(seg, (int)t.n_kb));
+        p.f.scale *= (1.0f + kTcTruncPerMma * (float)(3 * kTcKSteps * std::min(seg, (int)t.n_kb))) / (kTcScaleA * kTcScaleB);
     }
     p.scratch = t.scratch;
     p.n_groups = t.n_groups; p.nb_tot = t.nb_tot; p.n_cg = t.n_cg; p.seg = t.seg > 0 ? t.seg : kTcSegDefault; p.n_kb = t.n_kb;

@@ -215,6 +215,11 @@ __host__ __device__ constexpr uint32_t idesc_bf16(int M, int N) {
     return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
 }
 
+// Instruction descriptor for .kind::f16 with FP16 inputs (format code 0): D = F32, K-major.
+__host__ __device__ constexpr uint32_t idesc_f16(int M, int N) {
+    return (1u << 4) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
+}
+
 // round-to-nearest fp32 -> tf32 (low 13 mantissa bits cleared)
 __device__ __forceinline__ float to_tf32(float x) {
     uint32_t r;
