@@ -356,8 +356,11 @@ fused_tc_kernel(const TcParams p) {
         // =========================== generator: steps 2-4 -> A ring ===========================
         ptx::setmaxnreg_inc<kTcRegsGen>();
         const int gw = warp - kTcWarpGen0;
-        const int rsub = gw * 4 + (lane >> 3), chunk = lane & 7;
-        const uint32_t swz = (uint32_t)((chunk ^ (rsub & 7)) << 4);
+        // rows of this thread: rsub and rsub + 64.  A warp's four rows are {0,1,4,5} or {2,3,6,7} of an 8-row
+        // swizzle group: the 64-byte pieces it stores per row then spread over all 32 banks (two rows whose 16-byte
+        // chunks land in banks 0-15, two in banks 16-31) instead of 4-way conflicting in one half.
+        const int q4 = lane >> 3;
+        const int rsub = (gw >> 1) * 8 + (gw & 1) * 2 + (q4 & 1) + (q4 >> 1) * 4, chunk = lane & 7;
         const size_t nf = (size_t)f.n_freq, nfp = (size_t)f.n_freq_pad;
         uint32_t a_st = 0, a_ph = 0;           // A-ring stage and its phase parity
         if constexpr (VEC) {
