@@ -25,7 +25,8 @@ namespace {
 
 // CODATA exact values (PAPER.md names h, k_B implicitly through P^JN; R4)
 constexpr double kH = 6.62607015e-34, kKB = 1.380649e-23, kPi = 3.14159265358979323846;
-constexpr double kPref = kKB * 300.0;     // spectrum scale: kernels work on P_nu / kPref = O(1)
+constexpr double kPref = kKB * 300.0 / gt::kTcScaleA;   // spectrum scale: kernels work on P_nu / kPref = O(256), the range the
+                                                        // tensor kernel's fp16 operand split wants (exact power of two on top of k_B 300 K)
 
 thread_local std::string g_create_error = "";
 

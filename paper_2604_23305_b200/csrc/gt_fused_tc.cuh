@@ -264,7 +264,7 @@ __device__ __forceinline__ float element_value_fast(float eta_z, float csc, floa
 // product of two 11-bit pieces is exact in fp32, the dropped lo.Fm_lo is 2^-22) at 3/8 of its tensor time and
 // half of its operand bytes.
 __device__ __forceinline__ void store_split(unsigned char* a_stage, int row, int chunk, int h, const float4& v) {
-    const float2 s01 = make_float2(v.x * kTcScaleA, v.y * kTcScaleA), s23 = make_float2(v.z * kTcScaleA, v.w * kTcScaleA);
+    const float2 s01 = make_float2(v.x, v.y), s23 = make_float2(v.z, v.w);      // v is already scaled: the plan folds kTcScaleA into Xn and Gs
     const __half2 h01 = __float22half2_rn(s01), h23 = __float22half2_rn(s23);
     const float2 b01 = __half22float2(h01), b23 = __half22float2(h23);
     const __half2 l01 = __float22half2_rn(make_float2(s01.x - b01.x, s01.y - b01.y));
@@ -796,7 +796,7 @@ inline cudaError_t launch_fused_tc(const FusedParams& fp, const TcTables& t, int
     // the one-sided error interval.
     {
         const int seg = t.seg > 0 ? t.seg : kTcSegDefault;
-        p.f.scale *= (1.0f + kTcTruncPerMma * (float)(3 * kTcKSteps * std::min(seg, (int)t.n_kb))) / (kTcScaleA * kTcScaleB);
+        p.f.scale *= (1.0f + kTcTruncPerMma * (float)(3 * kTcKSteps * std::min(seg, (int)t.n_kb))) / kTcScaleB;      // kTcScaleA is part of FusedParams::scale (plan)
     }
     p.scratch = t.scratch;
     p.n_groups = t.n_groups; p.nb_tot = t.nb_tot; p.n_cg = t.n_cg; p.seg = t.seg > 0 ? t.seg : kTcSegDefault; p.n_kb = t.n_kb;
