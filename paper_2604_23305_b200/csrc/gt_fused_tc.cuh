@@ -347,11 +347,19 @@ fused_tc_kernel(const TcParams p) {
     auto mma_f16 = [&](uint32_t d, uint64_t a, uint64_t b, uint32_t id, uint32_t acc) {       // kind::f16, K = 16
         if constexpr (kTcPair) ptx::mma2_bf16_ss(d, a, b, id, acc); else ptx::mma_bf16_ss(d, a, b, id, acc);
     };
-    auto tile_row0 = [&](int64_t tl) -> int64_t {
+    // Row tiles are TIME-MAJOR: row tile rt = (block of 128 consecutive samples tb, spaxel s), tile row r = sample
+    // tb*128 + r of the launch.  Consecutive samples of one spaxel point ~1 source pixel apart, so their 2 x 2 tap
+    // footprints share cube lines (L1 hits) and, almost always, the two LUT rows.
+    const int64_t n_t = f.n_rows / f.n_spaxel;                      // samples in this launch
+    auto tile_rt = [&](int64_t tl) -> int64_t {
         const int64_t rt = tl / p.n_groups;
-        return (kTcPair ? 2 * rt + rank : rt) * kTcBM;
+        return kTcPair ? 2 * rt + rank : rt;
     };
-
+    // global row (t * n_spaxel + s) of tile row r, or -1 past the end of the launch
+    auto tile_row = [&](int64_t rt, int r) -> int64_t {
+        const int64_t tb = rt / f.n_spaxel, s = rt - tb * f.n_spaxel, t = tb * kTcBM + r;
+        return t < n_t ? t * f.n_spaxel + s : -1;
+    };
     if (warp >= kTcWarpGen0 && warp < kTcWarpFin0) {
         // =========================== generator: steps 2-4 -> A ring ===========================
         ptx::setmaxnreg_inc<kTcRegsGen>();
@@ -372,13 +380,13 @@ fused_tc_kernel(const TcParams p) {
             struct Tap { float4 L0, L1, c00, c01, c10, c11; };
             RowParam* rowp = reinterpret_cast<RowParam*>(smem_raw + (sm.rowp - raw));
             for (int64_t tl = worker; tl < n_tiles; tl += n_workers) {
-                const int64_t row0 = tile_row0(tl);
+                const int64_t rt = tile_rt(tl);
                 __syncwarp();
                 if (chunk < kTcRowsPerThread) {
                     const int rr = rsub + kTcRowStride * chunk;
-                    const int64_t R = row0 + rr;
+                    const int64_t R = tile_row(rt, rr);
                     RowParam rp;
-                    if (R < f.n_rows) {
+                    if (R >= 0) {
                         const int4* src = reinterpret_cast<const int4*>(f.rows + R);
                         const int4 a = __ldg(src), b = __ldg(src + 1);
                         rp.fp = __int_as_float(a.x); rp.csc = __int_as_float(a.y); rp.ip = a.z; rp.pix = a.w;
@@ -458,15 +466,15 @@ fused_tc_kernel(const TcParams p) {
             }
         } else
         for (int64_t tl = worker; tl < n_tiles; tl += n_workers) {
-            const int64_t row0 = tile_row0(tl);
+            const int64_t rt = tile_rt(tl);
             float fp[kTcRowsPerThread], csc[kTcRowsPerThread], w00[kTcRowsPerThread], w01[kTcRowsPerThread], w10[kTcRowsPerThread], w11[kTcRowsPerThread];
             const float* lutp[kTcRowsPerThread];
             const float* cubep[kTcRowsPerThread];
 #pragma unroll
             for (int j = 0; j < kTcRowsPerThread; ++j) {
-                const int64_t R = row0 + rsub + kTcRowStride * j;
+                const int64_t R = tile_row(rt, rsub + kTcRowStride * j);
                 RowParam rp;
-                if (R < f.n_rows) {
+                if (R >= 0) {
                     const int4* src = reinterpret_cast<const int4*>(f.rows + R);
                     const int4 a = __ldg(src), b = __ldg(src + 1);
                     rp.fp = __int_as_float(a.x); rp.csc = __int_as_float(a.y); rp.ip = a.z; rp.pix = a.w;
@@ -661,16 +669,15 @@ fused_tc_kernel(const TcParams p) {
         const int q = warp - kTcWarpFin0;
         uint32_t ti = 0;
         for (int64_t tl = worker; tl < n_tiles; tl += n_workers, ++ti) {
-            const int64_t row0 = tile_row0(tl);
+            const int64_t rt = tile_rt(tl);
+            const int64_t tb = rt / f.n_spaxel;
+            const uint32_t s = (uint32_t)(rt - tb * f.n_spaxel);
             const int cg0 = (int)(tl % p.n_groups) * p.nb_tot;
             const int n_valid = min(p.nb_tot, f.n_chan - cg0);            // real channels of this group
             const uint32_t sb = ti & 1u;
             const float* sc = p.scratch + ((size_t)blockIdx.x * 2 + sb) * p.nb_tot * kTcBM;
             ptx::mbar_wait_relaxed(sm.tile_done + 8 * sb, (ti >> 1) & 1u);
             constexpr int kMaxPerLane = kTcMaxGroupChan / 32;             // 12
-            // (sample, spaxel) of this warp's first row; later rows advance by kTcFinWarps without dividing
-            int64_t n64 = (row0 + q) / f.n_spaxel;
-            int sp = (int)((row0 + q) - n64 * f.n_spaxel);
             float x[kMaxPerLane], xn[kMaxPerLane];
 #pragma unroll
             for (int j = 0; j < kMaxPerLane; ++j) {
@@ -678,12 +685,10 @@ fused_tc_kernel(const TcParams p) {
                 xn[j] = c < n_valid ? __ldcg(sc + tc_scratch_index(c, q)) : 0.f;
             }
             for (int r = q; r < kTcBM; r += kTcFinWarps) {
-                const int64_t Rr = row0 + r;
-                if (Rr >= f.n_rows || GT_DIAG(p, 8)) break;
-                const uint32_t n = (uint32_t)(f.t0 + n64), s = (uint32_t)sp;
-                sp += kTcFinWarps;
-                while (sp >= f.n_spaxel) { sp -= f.n_spaxel; ++n64; }
-                float* o = f.out + (size_t)Rr * f.n_chan + cg0;
+                const int64_t t = tb * kTcBM + r;                         // sample of this row within the launch
+                if (t >= n_t || GT_DIAG(p, 8)) break;
+                const uint32_t n = (uint32_t)(f.t0 + t);
+                float* o = f.out + (size_t)(t * f.n_spaxel + s) * f.n_chan + cg0;
                 // this row's partial sums were fetched during the previous row; fetch the next row's now
 #pragma unroll
                 for (int j = 0; j < kMaxPerLane; ++j) {
@@ -801,7 +806,7 @@ inline cudaError_t launch_fused_tc(const FusedParams& fp, const TcTables& t, int
     p.scratch = t.scratch;
     p.n_groups = t.n_groups; p.nb_tot = t.nb_tot; p.n_cg = t.n_cg; p.seg = t.seg > 0 ? t.seg : kTcSegDefault; p.n_kb = t.n_kb;
     p.unit_bytes = t.unit_bytes; p.b_stages = t.b_stages;
-    p.n_row_tiles = (int32_t)((fp.n_rows + kTcBM - 1) / kTcBM);
+    p.n_row_tiles = (int32_t)(((fp.n_rows / fp.n_spaxel + kTcBM - 1) / kTcBM) * fp.n_spaxel);      // time-major: blocks of 128 samples x spaxels
     if (const char* e = std::getenv("GATEAU_TC_DEBUG")) p.debug = std::atoi(e);
     p.cube_vec = (fp.cube == nullptr) || ((fp.n_freq % 4 == 0) && ((reinterpret_cast<uintptr_t>(fp.cube) & 15u) == 0));
     const int64_t n_tiles = kTcPair ? (int64_t)((p.n_row_tiles + 1) / 2) * p.n_groups : (int64_t)p.n_row_tiles * p.n_groups;
