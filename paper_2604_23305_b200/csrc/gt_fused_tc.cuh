@@ -396,7 +396,7 @@ fused_tc_kernel(const TcParams p) {
                         rp.fp = 0.f; rp.csc = 1.f; rp.ip = 0; rp.pix = -1; rp.w00 = rp.w01 = rp.w10 = rp.w11 = 0.f;
                     }
                     if (f.cube == nullptr || rp.pix < 0) { rp.pix = 0; rp.w00 = rp.w01 = rp.w10 = rp.w11 = 0.f; }
-                    rowp[rr] = rp;
+                    rowp[gw * 8 + chunk * 4 + q4] = rp;     // slot of row (q4, j = chunk): the warp's rows of one j are contiguous (conflict-free reads)
                 }
                 __syncwarp();
                 // 32-bit element offsets of this thread's two rows (plan creation rejects tables of 2^32 elements
@@ -406,7 +406,7 @@ fused_tc_kernel(const TcParams p) {
                 uint32_t lut_off[kTcRowsPerThread], cube_off[kTcRowsPerThread];
 #pragma unroll
                 for (int j = 0; j < kTcRowsPerThread; ++j) {
-                    const int4 a = *reinterpret_cast<const int4*>(rowp + rsub + kTcRowStride * j);   // fp, csc, ip, pix
+                    const int4 a = *reinterpret_cast<const int4*>(rowp + gw * 8 + j * 4 + q4);   // fp, csc, ip, pix
                     lut_off[j] = (uint32_t)a.z * (uint32_t)nfp + (uint32_t)chunk * 4u;
                     cube_off[j] = (uint32_t)a.w * (uint32_t)nf;
                 }
@@ -423,7 +423,7 @@ fused_tc_kernel(const TcParams p) {
                     t.c10 = ldg4(cube_base + (co + tap10)); t.c11 = ldg4(cube_base + (co + tap10 + tap01));
                 };
                 auto compute = [&](int j, int h, const Tap& cur, const float4& X, const float4& G, uint32_t stage) {
-                    const RowParam* rp = rowp + rsub + kTcRowStride * j;
+                    const RowParam* rp = rowp + gw * 8 + j * 4 + q4;
                     const float2 fc = *reinterpret_cast<const float2*>(rp);                    // fp, csc
                     const float4 w = *reinterpret_cast<const float4*>(&rp->w00);
                     float4 S, v;
