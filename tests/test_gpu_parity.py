@@ -360,3 +360,20 @@ def test_C3_full_size_sampled_rows():
         del pkid
     assert rel_err(got_p, pk) <= TOL_PKID
     assert rel_err(got_t, pk + wn) <= TOL_TOD
+
+
+@pytest.mark.parametrize("variant", VARIANTS, ids=VARIANT_IDS)
+@pytest.mark.parametrize("kw", [
+    dict(n_samples=1, n_spaxel=1, n_chan=1, n_freq=1),          # the smallest legal problem
+    dict(n_samples=2, n_spaxel=1, n_chan=3, n_freq=5, with_cube=False),
+    dict(n_samples=129, n_spaxel=1, n_chan=33, n_freq=65),      # one sample past a 128-sample row tile, one past a slab
+    dict(n_samples=3, n_spaxel=130, n_chan=2, n_freq=64),       # more spaxels than rows in a tile
+], ids=["1x1x1x1", "blank-2x1x3x5", "129x1x33x65", "3x130x2x64"])
+def test_degenerate_sizes(variant, kw):
+    w = W.random_workload(90, photon_noise=True, **kw)
+    ref = O.Oracle(w).simulate(want=("tod", "pkid"))
+    with _plan(w, variant) as p:
+        got_p = p.pkid().cpu().numpy()
+        got_t = p.simulate().cpu().numpy()
+    assert rel_err(got_p, ref["pkid"]) <= TOL_PKID
+    assert rel_err(got_t, ref["tod"]) <= TOL_TOD
