@@ -155,12 +155,9 @@ template <int TN>
 cudaError_t launch_fp32(const gt::FusedParams& fp, int grid_y, cudaStream_t st) {
     const size_t smem = (size_t)(gt::kF32_BK * gt::kF32_AStride + gt::kF32_BK * 32 * TN) * sizeof(float)
                       + gt::kF32_BM * sizeof(gt::RowParam);
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(gt::fused_fp32_kernel<TN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        attr_set = true;
-    }
+    // set on every launch: the attribute is per device and a microsecond is nothing next to the kernel
+    cudaError_t e = cudaFuncSetAttribute(gt::fused_fp32_kernel<TN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
     dim3 grid((unsigned)((fp.n_rows + gt::kF32_BM - 1) / gt::kF32_BM), grid_y);
     gt::fused_fp32_kernel<TN><<<grid, gt::kF32_Threads, smem, st>>>(fp);
     return cudaGetLastError();
@@ -231,12 +228,8 @@ gt_status run_chunk(gt_plan* p, int64_t t0, int64_t T, float* dst, float* pwv_ds
         GT_CUDA(p, cudaMemsetAsync(p->d_pink_sync.p, 0, n_flags * sizeof(uint32_t), st));
         p->pink.flags = p->d_pink_sync.p + 1; p->pink.ticket = p->d_pink_sync.p;
         const size_t smem = (size_t)gt::kPinkSeg * 256 * sizeof(float);
-        static bool attr_set = false;
-        if (!attr_set) {
-            GT_CUDA(p, cudaFuncSetAttribute(gt::pink_chain_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-            GT_CUDA(p, cudaFuncSetAttribute(gt::pink_chain_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-            attr_set = true;
-        }
+        GT_CUDA(p, cudaFuncSetAttribute(gt::pink_chain_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        GT_CUDA(p, cudaFuncSetAttribute(gt::pink_chain_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         if (p->J <= 4) gt::pink_chain_kernel<4><<<(unsigned)(n_seg * n_dblk), 256, smem, st>>>(p->pink, t0, T, dst);
         else           gt::pink_chain_kernel<8><<<(unsigned)(n_seg * n_dblk), 256, smem, st>>>(p->pink, t0, T, dst);
         GT_CUDA(p, cudaGetLastError());

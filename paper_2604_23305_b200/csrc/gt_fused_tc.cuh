@@ -812,15 +812,10 @@ inline cudaError_t launch_fused_tc(const FusedParams& fp, const TcTables& t, int
     const int64_t n_tiles = kTcPair ? (int64_t)((p.n_row_tiles + 1) / 2) * p.n_groups : (int64_t)p.n_row_tiles * p.n_groups;
     const int64_t workers = kTcPair ? num_sms / 2 : num_sms;
     const unsigned grid = (unsigned)(std::min<int64_t>(n_tiles, workers) * (kTcPair ? 2 : 1));
-    static int smem_set[2] = {0, 0};
     auto kern = p.cube_vec ? fused_tc_kernel<true> : fused_tc_kernel<false>;
-    int& set = smem_set[p.cube_vec ? 1 : 0];
-    cudaError_t e;
-    if (set < t.smem_bytes) {
-        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, t.smem_bytes);
-        if (e != cudaSuccess) return e;
-        set = t.smem_bytes;
-    }
+    // set on every launch: the attribute is per device
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, t.smem_bytes);
+    if (e != cudaSuccess) return e;
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3(grid); cfg.blockDim = dim3(kTcThreads); cfg.dynamicSmemBytes = (size_t)t.smem_bytes; cfg.stream = st;
     cudaLaunchAttribute attr[1];
