@@ -147,6 +147,25 @@ def lorentzian_filterbank(nu_hz: np.ndarray, f_c_hz: np.ndarray, R: float,
     return (eta_peak / (1.0 + 4.0 * R * R * x * x)).astype(np.float32)
 
 
+def filterbank_upstream_absorption(nu_hz: np.ndarray, f_c_hz: np.ndarray, R: float,
+                                   eta_peak: Union[float, np.ndarray] = 0.16) -> np.ndarray:
+    """Eq. 7: channels on a common transmission line, highest frequency first; a channel sees
+    the signal from which the channels upstream (f_bar > f) have already absorbed their share:
+        eta_filt(f, nu) = (eta_peak(f) - sum_{f_bar > f} eta_filt(f_bar, nu)) / (1 + 4 R^2 (nu/f - 1)^2)
+    (the '1 +' restored as in Eq. 6, reading R1).  Evaluated literally, in descending order of f; rows are
+    returned in the order of `f_c_hz`.  The hot path only sees the resulting matrix."""
+    f_c_hz = np.asarray(f_c_hz, dtype=np.float64)
+    peak = np.broadcast_to(np.asarray(eta_peak, dtype=np.float64), f_c_hz.shape)
+    order = np.argsort(-f_c_hz, kind="stable")
+    out = np.zeros((f_c_hz.size, nu_hz.size), dtype=np.float64)
+    absorbed = np.zeros(nu_hz.size, dtype=np.float64)              # sum over the channels upstream
+    for k in order:
+        x = nu_hz / f_c_hz[k] - 1.0
+        out[k] = (peak[k] - absorbed) / (1.0 + 4.0 * R * R * x * x)
+        absorbed = absorbed + out[k]
+    return out.astype(np.float32)
+
+
 def hex_spaxels(R_hex: int, pitch_rad: float) -> Tuple[np.ndarray, np.ndarray]:
     """Packed hexagon of circumradius R_hex spaxels: 1 + 3R(R+1)
     offsets, axial coordinates (j outer, i inner), one lattice axis along azimuth."""

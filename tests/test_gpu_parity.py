@@ -377,3 +377,16 @@ def test_degenerate_sizes(variant, kw):
         got_t = p.simulate().cpu().numpy()
     assert rel_err(got_p, ref["pkid"]) <= TOL_PKID
     assert rel_err(got_t, ref["tod"]) <= TOL_TOD
+
+
+@pytest.mark.parametrize("variant", VARIANTS, ids=VARIANT_IDS)
+def test_pkid_with_the_filterbank_model_of_eq7(variant):
+    """The paper's filterbank model (Eq. 7, upstream absorption) as the dispersive element: the hot path only
+    sees the matrix."""
+    w = W.random_workload(77, n_samples=140, n_spaxel=2, n_chan=96, n_freq=700)
+    filt = W.filterbank_upstream_absorption(w.nu_hz, w.f_center_hz, 300.0, 0.16)
+    w = w.replace(filt=filt, dnu_eff_hz=None)
+    ref = O.Oracle(w).simulate(want=("pkid",))["pkid"]
+    with _plan(w, variant) as p:
+        got = p.pkid().cpu().numpy()
+    assert rel_err(got, ref) <= TOL_PKID

@@ -68,3 +68,28 @@ def test_filterbank_peak_and_front_end_constants():
     check("t_cmb_K", w.T_cmb_K)
     ef = W.eta_front_aste(np.array([1e9]))[0]                                                      # Ruze term -> 1 at low nu
     assert np.isclose(ef / 0.85, GOLD["eta_pol"][0], rtol=1e-5)          # the Ruze factor at 1 GHz is 1 - 3e-6
+
+
+def test_filterbank_with_upstream_absorption_eq7():
+    """Eq. 7 against its closed form: with a common peak height the recursion telescopes to
+    eta_k = eta_peak L_k prod_{f_j > f_k} (1 - L_j), L = 1 / (1 + 4 R^2 (nu/f - 1)^2)."""
+    nu = np.linspace(200e9, 460e9, 1500)
+    fc = W.channel_centres_log(40)
+    R, pk = 300.0, 0.16
+    got = W.filterbank_upstream_absorption(nu, fc, R, pk).astype(np.float64)
+    L = 1.0 / (1.0 + 4.0 * R * R * (nu[None, :] / fc[:, None] - 1.0) ** 2)
+    want = np.empty_like(L)
+    for k in range(fc.size):
+        up = fc > fc[k]
+        want[k] = pk * L[k] * np.prod(1.0 - L[up], axis=0)
+    assert np.allclose(got, want, rtol=2e-6, atol=1e-12)
+    # the highest-frequency channel is fed first: it is the isolated Lorentzian of Eq. 6
+    top = np.argmax(fc)
+    assert np.allclose(got[top], W.lorentzian_filterbank(nu, fc[top:top + 1], R, pk)[0], rtol=1e-6)
+    # no frequency is absorbed more than once: the total never exceeds the peak height, and every downstream
+    # channel is below its isolated Lorentzian
+    assert np.all(got.sum(axis=0) <= pk * (1 + 1e-6))
+    assert np.all(got <= W.lorentzian_filterbank(nu, fc, R, pk).astype(np.float64) * (1 + 1e-6) + 1e-12)
+    # row order follows f_c_hz whatever its order
+    perm = np.random.default_rng(0).permutation(fc.size)
+    assert np.array_equal(W.filterbank_upstream_absorption(nu, fc[perm], R, pk), W.filterbank_upstream_absorption(nu, fc, R, pk)[perm])
