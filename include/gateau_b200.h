@@ -102,6 +102,11 @@ typedef struct {
     int64_t chunk_samples;
     /* one of GT_VARIANT_* */
     int32_t variant;
+    /* pink-noise method: 0 = per-detector AR(1) cascade (north_star; pink_n_stage, pink_f_corner_hz used),
+       1 = Timmer & Koenig: the whole series of every detector is drawn in the Fourier domain
+       with PSD A f^-alpha and transformed back at plan creation (R21; needs
+       n_spaxel*n_chan*n_samples*4 B of device memory; any sample range may then be simulated in any order) */
+    int32_t pink_method;
 } gt_config;
 
 /* Per-row geometry record returned by gt_debug_geometry: the integers are the quantities

@@ -217,6 +217,30 @@ class Oracle:
                                         C.c_void_p(out.ctypes.data)), "pink_series")
         return out
 
+    def pink_tk_series(self, s_idx, c_idx):
+        """Pink noise by the method the paper itself uses (Timmer & Koenig 1995; R21):
+        for detector (s, c) with one-sided PSD P(f) = A f^-alpha and N = n_samples, f_k = k f_s / N,
+            X_0 = 0,  X_k = sqrt(P(f_k) f_s N / 4) (z0 + i z1)  (0 < k < N/2),  X_{N/2} = sqrt(P f_s N) z0  (N even),
+        (z0, z1) = normals 0, 1 of Philox(seed; c0 = k, c1 = s, c2 = c, c3 = 3), and the series is the inverse real
+        FFT x_n = irfft(X) (numpy convention, 1/N).  Returns [len(s_idx)][n_samples] in double."""
+        w = self.w
+        N = int(w.n_samples)
+        K = N // 2
+        out = np.zeros((len(s_idx), N))
+        fk = np.arange(K + 1, dtype=np.float64) * (w.f_sample_hz / N)
+        for i, (s, c) in enumerate(zip(s_idx, c_idx)):
+            d = int(s) * w.n_chan + int(c)
+            z = normals_bulk(w.seed, 0, K + 1, int(s), int(c), 3)
+            X = np.zeros(K + 1, dtype=np.complex128)
+            if K >= 1:
+                P = np.zeros(K + 1)
+                P[1:] = float(w.pink_A[d]) * fk[1:] ** (-float(w.pink_alpha[d]))
+                X[1:] = np.sqrt(P[1:] * w.f_sample_hz * N / 4.0) * (z[1:, 0] + 1j * z[1:, 1])
+                if N % 2 == 0:
+                    X[K] = np.sqrt(P[K] * w.f_sample_hz * N) * z[K, 0]
+            out[i] = np.fft.irfft(X, n=N) if N > 1 else 0.0
+        return out
+
     def dnu_eff(self):
         out = np.zeros(self.w.n_chan)
         self.L.go_dnu_eff(C.byref(self.cfg), C.c_void_p(out.ctypes.data))

@@ -52,6 +52,7 @@ class GtConfig(C.Structure):
         ("pink_n_stage", C.c_int32), ("pink_f_corner_hz", C.c_void_p),
         ("chunk_samples", C.c_int64),
         ("variant", C.c_int32),
+        ("pink_method", C.c_int32),
     ]
 
 
@@ -155,6 +156,7 @@ def fill_config(w, dev: dict, keep: dict, variant: int = VARIANT_DEFAULT, chunk_
         c.pink_n_stage = 0
     c.chunk_samples = int(w.chunk_samples if chunk_samples is None else chunk_samples)
     c.variant = int(variant)
+    c.pink_method = int(getattr(w, "pink_method", 0))
     return c
 
 

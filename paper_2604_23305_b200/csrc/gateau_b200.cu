@@ -20,6 +20,8 @@
 #include "gt_fused_fp32.cuh"
 #include "gt_fused_tc.cuh"
 #include "gt_pink.cuh"
+#include "gt_pink_tk.cuh"
+#include <cufft.h>
 
 namespace {
 
@@ -74,7 +76,10 @@ struct gt_plan {
     // pink
     gt::PinkParams pink{};
     DevBuf<float> d_gain, d_state, d_seg;
-    DevBuf<uint32_t> d_pink_sync;   // ticket counter + per-(segment, detector block) flags of the chained pink kernel
+    DevBuf<uint32_t> d_pink_sync;
+    int32_t pink_method = 0;         // 0 AR(1) cascade, 1 Timmer & Koenig
+    gt::TkParams tk{};
+    DevBuf<float> d_tk_amp, d_tk_halpha, d_tk_series;   // ticket counter + per-(segment, detector block) flags of the chained pink kernel
     int64_t pink_next_t = 0;
     // scratch
     DevBuf<gt::RowParam> d_rows;     // [chunk rows]
@@ -135,12 +140,15 @@ gt_status validate(const gt_config* c) {
         if (!s.eta_nu && !(s.eta_scalar >= 0.0 && s.eta_scalar <= 1.0))
             return fail(nullptr, GT_ERR_VALUE, "stage %d: eta_scalar outside [0,1]", k + 1);
     }
-    if (c->pink_noise) {
+    if (c->pink_method != 0 && c->pink_method != 1) return fail(nullptr, GT_ERR_VALUE, "unknown pink_method %d", c->pink_method);
+    if (c->pink_noise && c->pink_method == 0) {
         if (c->pink_n_stage < 1 || c->pink_n_stage > gt::kPinkMaxJ)
             return fail(nullptr, GT_ERR_SHAPE, "pink_n_stage must be in 1..8");
         if (!c->pink_A || !c->pink_alpha || !c->pink_f_corner_hz)
             return fail(nullptr, GT_ERR_NULL, "pink noise arrays are NULL");
     }
+    if (c->pink_noise && c->pink_method == 1 && (!c->pink_A || !c->pink_alpha))
+        return fail(nullptr, GT_ERR_NULL, "pink noise arrays are NULL");
     if (c->variant != GT_VARIANT_DEFAULT && c->variant != GT_VARIANT_FP32 && c->variant != GT_VARIANT_TENSOR)
         return fail(nullptr, GT_ERR_VALUE, "unknown variant %d", c->variant);
     // LUT must cover the frequency grid (R13)
@@ -217,7 +225,12 @@ gt_status run_chunk(gt_plan* p, int64_t t0, int64_t T, float* dst, float* pwv_ds
     p->launches++;
     p->n_fused_last = fused_slot + 1;
 
-    if (noise && p->pink_noise) {
+    if (noise && p->pink_noise && p->pink_method == 1) {
+        dim3 grid((unsigned)((T + 31) / 32), (unsigned)((p->tk.n_det + 31) / 32));
+        gt::tk_add_kernel<<<grid, 256, 0, st>>>(p->tk, t0, T, dst);
+        GT_CUDA(p, cudaGetLastError());
+        p->launches += 1;
+    } else if (noise && p->pink_noise) {
         const int64_t n_seg = (T + gt::kPinkSeg - 1) / gt::kPinkSeg;
         const int64_t n_thr = n_seg * p->pink.n_det;
         if ((size_t)(n_thr * p->J) > p->d_seg.n) GT_CUDA(p, p->d_seg.alloc((size_t)(n_thr * p->J)));
@@ -252,7 +265,7 @@ gt_status simulate_impl(gt_plan* p, int64_t t_begin, int64_t t_count, float* out
                     (long long)(t_begin + t_count), (long long)p->n_samples);
     if (t_count == 0) return GT_OK;
     if (!out) return fail(p, GT_ERR_NULL, "output pointer is NULL");
-    const bool pink = noise && p->pink_noise;
+    const bool pink = noise && p->pink_noise && p->pink_method == 0;      // the AR(1) cascade carries state between calls
     if (pink) {
         if (t_begin == 0) {
             gt::pink_init_kernel<<<(unsigned)((p->pink.n_det + 255) / 256), 256, 0, st>>>(p->pink);
@@ -468,8 +481,45 @@ gt_status gt_plan_create(const gt_config* cfg, void* cuda_stream, gt_plan** out_
         g.az_min = c.az_min_rad; g.daz_grid = c.daz_grid_rad; g.el_min = c.el_min_rad; g.del_grid = c.del_grid_rad;
     }
 
-    // ---- pink-noise coefficients (R18) ----
-    if (p->pink_noise) {
+    p->pink_method = c.pink_method;
+    // ---- Timmer & Koenig pink noise (R21): the series of every detector, once ----
+    if (p->pink_noise && p->pink_method == 1) {
+        const int64_t N = c.n_samples, K = N / 2, n_det = (int64_t)ns * nc, ld = 2 * (K + 1);
+        std::vector<float> amp((size_t)n_det), halpha((size_t)n_det);
+        for (int64_t d = 0; d < n_det; ++d) {
+            if (!(c.pink_A[d] >= 0) || !(c.pink_alpha[d] >= 0))
+                return fail(nullptr, GT_ERR_VALUE, "pink noise level of detector %lld is invalid", (long long)d);
+            amp[d] = (float)std::sqrt(c.pink_A[d] * c.f_sample_hz / (4.0 * (double)N));
+            halpha[d] = (float)(0.5 * c.pink_alpha[d]);
+        }
+        GT_CUDA0(p->d_tk_amp.upload(amp, st)); GT_CUDA0(p->d_tk_halpha.upload(halpha, st));
+        GT_CUDA0(p->d_tk_series.alloc((size_t)(n_det * ld)));
+        gt::TkParams& k = p->tk;
+        k.n_det = n_det; k.n_samples = N; k.n_chan = nc; k.f_sample = c.f_sample_hz;
+        k.amp = p->d_tk_amp.p; k.half_alpha = p->d_tk_halpha.p; k.series = p->d_tk_series.p; k.ld = ld;
+        k.seed_lo = (uint32_t)(c.seed & 0xffffffffu); k.seed_hi = (uint32_t)(c.seed >> 32);
+        const int64_t n_thr = n_det * (K + 1);
+        gt::tk_spectrum_kernel<<<(unsigned)((n_thr + 255) / 256), 256, 0, st>>>(k);
+        GT_CUDA0(cudaGetLastError());
+        p->launches++;
+        if (N >= 2) {
+            cufftHandle h;
+            int n[1] = {(int)N}, inembed[1] = {(int)(K + 1)}, onembed[1] = {(int)ld};
+            if (N > 0x7fffffffLL) return fail(nullptr, GT_ERR_SHAPE, "n_samples too large for the FFT");
+            if (cufftPlanMany(&h, 1, n, inembed, 1, (int)(K + 1), onembed, 1, (int)ld, CUFFT_C2R, (int)n_det) != CUFFT_SUCCESS)
+                return fail(nullptr, GT_ERR_OOM, "cufftPlanMany failed (length %lld, batch %lld)", (long long)N, (long long)n_det);
+            cufftResult r = cufftSetStream(h, st);
+            if (r == CUFFT_SUCCESS)
+                r = cufftExecC2R(h, reinterpret_cast<cufftComplex*>(p->d_tk_series.p), p->d_tk_series.p);   // in place
+            cudaError_t e = cudaStreamSynchronize(st);
+            cufftDestroy(h);
+            if (r != CUFFT_SUCCESS || e != cudaSuccess) return fail(nullptr, GT_ERR_CUDA, "inverse FFT of the pink-noise spectra failed");
+        }
+        GT_CUDA0(cudaStreamSynchronize(st));       // amp / halpha host vectors go out of scope
+    }
+
+    // ---- pink-noise coefficients of the AR(1) cascade (R18) ----
+    if (p->pink_noise && p->pink_method == 0) {
         const int J = c.pink_n_stage;
         p->J = J;
         gt::PinkParams& k = p->pink;

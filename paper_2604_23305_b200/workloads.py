@@ -91,6 +91,7 @@ class Workload:
     seed: int = 0
     photon_noise: bool = False
     pink_noise: bool = False
+    pink_method: int = 0                   # 0: AR(1) cascade (north_star), 1: Timmer & Koenig FFT
     pink_A: Optional[np.ndarray] = None
     pink_alpha: Optional[np.ndarray] = None
     pink_f_corner_hz: Optional[np.ndarray] = None

@@ -390,3 +390,30 @@ def test_pkid_with_the_filterbank_model_of_eq7(variant):
     with _plan(w, variant) as p:
         got = p.pkid().cpu().numpy()
     assert rel_err(got, ref) <= TOL_PKID
+
+
+@pytest.mark.parametrize("variant", VARIANTS, ids=VARIANT_IDS)
+@pytest.mark.parametrize("n_samples", [600, 601, 1])
+def test_tod_with_timmer_koenig_pink_noise(variant, n_samples):
+    """The paper's own pink-noise method (R21): series drawn in the Fourier domain with
+    PSD A f^-alpha, inverse real FFT (cuFFT) at plan creation; any sample range can then be simulated."""
+    w = W.random_workload(81, n_samples=n_samples, n_spaxel=2, n_chan=20, n_freq=48, photon_noise=True, pink_noise=True)
+    w = w.replace(pink_method=1, pink_A=w.pink_A * 3e3)                  # pink rms ~ 1e-3 of P: visible at the 2e-5 gate
+    o = O.Oracle(w.replace(pink_noise=False))
+    base = o.simulate(want=("tod",))["tod"]                              # (P + wn), Eq. 21 order
+    s_idx = np.repeat(np.arange(w.n_spaxel), w.n_chan).astype(np.int32)
+    c_idx = np.tile(np.arange(w.n_chan), w.n_spaxel).astype(np.int32)
+    tk = O.Oracle(w).pink_tk_series(s_idx, c_idx).T.reshape(n_samples, w.n_spaxel, w.n_chan)
+    ref = base + tk
+    with _plan(w, variant) as p:
+        got = p.simulate().cpu().numpy()
+        if n_samples > 100:
+            part = p.simulate(313, 200).cpu().numpy()                    # no recurrence: any range, any order
+            assert np.array_equal(part, got[313:513])
+    assert rel_err(got, ref) <= TOL_TOD
+    if n_samples > 100:
+        # the pink series itself, isolated with the GPU's own photon-noise TOD
+        with _plan(w.replace(pink_noise=False), variant) as p0:
+            nop = p0.simulate().cpu().numpy().astype(np.float64)
+        pn = got.astype(np.float64) - nop
+        assert np.max(np.abs(pn - tk)) <= 2e-4 * np.std(tk) + 1.3e-7 * np.max(np.abs(nop))

@@ -183,3 +183,103 @@ def test_pink_series_windows_are_consistent():
     full = o.pink_series(s, c, 0, 600)
     part = o.pink_series(s, c, 217, 300)
     assert np.array_equal(full[:, 217:517], part)
+
+
+# ---- Timmer & Koenig pink noise (the paper's own method; R21) ----
+def _tk_workload(n_samples, n_chan=6, alpha=1.0, seed=5):
+    from paper_2604_23305_b200 import workloads as W
+    w = W.random_workload(seed, n_samples=n_samples, n_spaxel=2, n_chan=n_chan, n_freq=8, pink_noise=True)
+    return w.replace(pink_method=1, pink_A=np.full(2 * n_chan, 3e-34), pink_alpha=np.full(2 * n_chan, alpha))
+
+
+@pytest.mark.parametrize("N", [1000, 1001])
+def test_tk_series_spectrum_roundtrip_and_parseval(N):
+    """rfft of the series gives back exactly the drawn coefficients (X_0 = 0, Hermitian extension), so the
+    periodogram IS the requested PSD times the squared normals; mean zero; Parseval."""
+    w = _tk_workload(N)
+    o = O.Oracle(w)
+    s_idx, c_idx = np.array([0, 1, 1], dtype=np.int32), np.array([0, 3, 5], dtype=np.int32)
+    x = o.pink_tk_series(s_idx, c_idx)
+    assert x.shape == (3, N) and np.all(np.abs(x.mean(axis=1)) < 1e-12 * np.abs(x).max())
+    K = N // 2
+    fk = np.arange(K + 1) * w.f_sample_hz / N
+    for i, (s, c) in enumerate(zip(s_idx, c_idx)):
+        X = np.fft.rfft(x[i])
+        z = O.normals_bulk(w.seed, 0, K + 1, int(s), int(c), 3)
+        P = 3e-34 / fk[1:]
+        top = K if N % 2 == 1 else K - 1
+        want = np.sqrt(P[:top] * w.f_sample_hz * N / 4.0) * (z[1:top + 1, 0] + 1j * z[1:top + 1, 1])
+        assert np.allclose(X[1:top + 1], want, rtol=1e-9, atol=1e-12 * np.abs(want).max())
+        assert abs(X[0]) < 1e-9 * np.abs(want).max()
+        if N % 2 == 0:
+            assert np.isclose(X[K].real, np.sqrt(P[K - 1] * w.f_sample_hz * N) * z[K, 0], rtol=1e-9)
+        # Parseval: sum x^2 = (1/N) (2 sum |X_k|^2 + |X_{N/2}|^2)
+        rhs = (2 * np.sum(np.abs(X[1:top + 1]) ** 2) + (abs(X[K]) ** 2 if N % 2 == 0 else 0.0)) / N
+        assert np.isclose(np.sum(x[i] ** 2), rhs, rtol=1e-10)
+
+
+@pytest.mark.parametrize("alpha", [1.0, 1.5])
+def test_tk_average_periodogram_follows_the_power_law(alpha):
+    """One-sided periodogram (2 / (f_s N)) |X_k|^2 averaged over many detectors = A f^-alpha."""
+    N, n_chan = 512, 200
+    w = _tk_workload(N, n_chan=n_chan, alpha=alpha)
+    o = O.Oracle(w)
+    s_idx = np.repeat(np.arange(2), n_chan).astype(np.int32)
+    c_idx = np.tile(np.arange(n_chan), 2).astype(np.int32)
+    x = o.pink_tk_series(s_idx, c_idx)
+    S = 2.0 / (w.f_sample_hz * N) * np.abs(np.fft.rfft(x, axis=1)[:, 1:N // 2]) ** 2
+    fk = np.arange(1, N // 2) * w.f_sample_hz / N
+    ratio = S.mean(axis=0) / (3e-34 * fk ** (-alpha))
+    # each |X_k|^2 / (2 sigma^2) is chi^2_2 / 2: the mean over 400 detectors has relative std 1/20
+    assert abs(ratio.mean() - 1.0) < 0.02 and np.all(np.abs(ratio - 1.0) < 0.25)
+
+
+@pytest.mark.parametrize("N", [16, 17])
+def test_tk_series_is_the_direct_fourier_sum(N):
+    """Tiny N, the definition written out as cosines and sines (no FFT): x_n = (2/N) sum_{0<k<N/2} sigma_k
+    (z0 cos(2 pi k n / N) - z1 sin(2 pi k n / N)) + (1/N) sqrt(P f_s N) z0 (-1)^n, sigma_k = sqrt(P(f_k) f_s N / 4)."""
+    w = _tk_workload(N, alpha=1.3)
+    o = O.Oracle(w)
+    x = o.pink_tk_series(np.array([1], dtype=np.int32), np.array([2], dtype=np.int32))[0]
+    K = N // 2
+    z = O.normals_bulk(w.seed, 0, K + 1, 1, 2, 3)
+    want = np.zeros(N)
+    for n in range(N):
+        acc = 0.0
+        for k in range(1, K + 1):
+            fk = k * w.f_sample_hz / N
+            P = 3e-34 * fk ** (-1.3)
+            if 2 * k == N:
+                acc += np.sqrt(P * w.f_sample_hz * N) * z[k, 0] * (-1.0) ** n / N
+            else:
+                ph = 2.0 * np.pi * k * n / N
+                acc += 2.0 / N * np.sqrt(P * w.f_sample_hz * N / 4.0) * (z[k, 0] * np.cos(ph) - z[k, 1] * np.sin(ph))
+        want[n] = acc
+    assert np.allclose(x, want, rtol=1e-10, atol=1e-12 * np.abs(want).max())
+
+
+def test_tk_slope_variance_and_independence():
+    """Fitted log-log slope of the averaged periodogram is -alpha; the series variance is the integral of the
+    one-sided PSD over the resolved band, sum_k P(f_k) f_s / N; different detectors / seeds are uncorrelated."""
+    N, n_chan, alpha = 1024, 150, 1.2
+    w = _tk_workload(N, n_chan=n_chan, alpha=alpha)
+    o = O.Oracle(w)
+    s_idx = np.repeat(np.arange(2), n_chan).astype(np.int32)
+    c_idx = np.tile(np.arange(n_chan), 2).astype(np.int32)
+    x = o.pink_tk_series(s_idx, c_idx)
+    S = (2.0 / (w.f_sample_hz * N) * np.abs(np.fft.rfft(x, axis=1)[:, 1:N // 2]) ** 2).mean(axis=0)
+    fk = np.arange(1, N // 2) * w.f_sample_hz / N
+    slope = np.polyfit(np.log(fk), np.log(S), 1)[0]
+    assert abs(slope + alpha) < 0.03
+    fall = np.arange(1, N // 2 + 1) * w.f_sample_hz / N
+    var_want = np.sum(3e-34 * fall ** (-alpha)) * w.f_sample_hz / N
+    assert abs(x.var(axis=1).mean() / var_want - 1.0) < 0.1
+    # whitened coefficients of different detectors are uncorrelated unit normals (1022 of them per detector)
+    X = np.fft.rfft(x, axis=1)[:, 1:N // 2] / np.sqrt(3e-34 * fk ** (-alpha) * w.f_sample_hz * N / 4.0)
+    g = np.concatenate([X.real, X.imag], axis=1)
+    assert abs(g.mean()) < 0.01 and abs(g.var() - 1.0) < 0.01
+    cc = g @ g.T / g.shape[1]
+    np.fill_diagonal(cc, 0.0)
+    assert np.abs(cc).max() < 6.0 / np.sqrt(g.shape[1])
+    x2 = O.Oracle(w.replace(seed=w.seed + 1)).pink_tk_series(s_idx[:4], c_idx[:4])
+    assert np.abs(x2 - x[:4]).max() > 0.5 * np.abs(x[:4]).max()
