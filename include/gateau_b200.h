@@ -107,6 +107,16 @@ typedef struct {
        with PSD A f^-alpha and transformed back at plan creation (R21; needs
        n_spaxel*n_chan*n_samples*4 B of device memory; any sample range may then be simulated in any order) */
     int32_t pink_method;
+    /* output unit (R22): 0 = detected power [W]; 1 = brightness temperature [K].
+       For 1 the plan simulates a skydip at plan creation -- blank sky on the boresight at elevation el0, the
+       zenith PWV taking skydip_n (2..64) evenly spaced values in [skydip_pwv_lo_mm, skydip_pwv_hi_mm] -- records
+       the noiseless P_KID[c] and the filter-weighted line-of-sight temperature
+       T_b[c] = sum_nu Fm[c][nu] ((1 - eta_atm) T_atm + eta_atm T_cmb) / sum_nu Fm[c][nu], fits the least-squares
+       line T_b = a_c + b_c P_KID per channel, and gt_simulate returns a_c + b_c * (Eq. 21 total).
+       GT_ERR_VALUE if a channel's filter sums to zero or its P_KID does not vary over the skydip. */
+    int32_t output_unit;
+    int32_t skydip_n;
+    double skydip_pwv_lo_mm, skydip_pwv_hi_mm;
 } gt_config;
 
 /* Per-row geometry record returned by gt_debug_geometry: the integers are the quantities
@@ -172,6 +182,9 @@ const char* gt_variant_name(const gt_plan* plan);
  * over its launches (CUDA events on the launching stream); synchronises the stream.  Also
  * returns the number of launches in *n_launches (NULL ok). */
 double gt_last_fused_ms(gt_plan* plan, int32_t* n_launches);
+/* Test hook: the per-channel skydip map T_b = a + b P_KID of a plan with output_unit = 1, copied to the HOST
+ * arrays a_out, b_out [n_chan] (double).  GT_ERR_UNSUPPORTED if the plan's output unit is W. */
+gt_status gt_debug_kelvin_map(gt_plan* plan, double* a_out, double* b_out);
 
 #ifdef __cplusplus
 }

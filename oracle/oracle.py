@@ -241,6 +241,39 @@ class Oracle:
             out[i] = np.fft.irfft(X, n=N) if N > 1 else 0.0
         return out
 
+    # ---- brightness-temperature output (R22) ----
+    def skydip(self):
+        """The simulated skydip: a blank-sky stare of one on-axis detector row at the boresight elevation while
+        the PWV takes skydip_n evenly spaced values in [lo, hi] (a flat zero screen plus the drift a + b t carries
+        them), simulated noiseless with this oracle's own chain.  Returns (P_KID [k][c] in W, T_b [k][c] in K,
+        pwv [k]);  T_b = sum_nu Fm T_los / sum_nu Fm,  T_los = (1 - eta_atm) T_atm + eta_atm T_cmb."""
+        w = self.w
+        K = int(w.skydip_n)
+        step = (w.skydip_pwv_hi_mm - w.skydip_pwv_lo_mm) / (K - 1)
+        sd = w.replace(n_samples=K, az_rad=np.zeros(K), el_rad=np.zeros(K), daz_rad=np.zeros(1), del_rad=np.zeros(1),
+                       cube=None, screen=np.zeros((2, 2), dtype=np.float32), pwv0_a_mm=w.skydip_pwv_lo_mm,
+                       pwv0_b_mm_per_s=step * w.f_sample_hz, photon_noise=False, pink_noise=False, output_unit=0,
+                       pink_A=None, pink_alpha=None, pink_f_corner_hz=None, chunk_samples=0)
+        o = Oracle(sd)
+        res = o.simulate(want=("pkid", "pwv"))
+        P = res["pkid"][:, 0, :]
+        F = np.asarray(w.filt, dtype=np.float64)
+        T = np.zeros((K, w.n_chan))
+        for k in range(K):
+            _, eta, _ = o.row_spectrum(k, 0, intermediates=True)
+            T_los = (1.0 - eta) * w.T_atm_K + eta * w.T_cmb_K
+            T[k] = (F @ T_los) / F.sum(axis=1)
+        return P, T, res["pwv"][:, 0]
+
+    def kelvin_map(self):
+        """Least-squares line T_b = a_c + b_c P_KID per channel over the skydip ('a linear mapping
+        is set up between P_KID^tot and T_b')."""
+        P, T, _ = self.skydip()
+        Pm, Tm = P.mean(axis=0), T.mean(axis=0)
+        b = ((P - Pm) * (T - Tm)).sum(axis=0) / ((P - Pm) ** 2).sum(axis=0)
+        a = Tm - b * Pm
+        return a, b
+
     def dnu_eff(self):
         out = np.zeros(self.w.n_chan)
         self.L.go_dnu_eff(C.byref(self.cfg), C.c_void_p(out.ctypes.data))

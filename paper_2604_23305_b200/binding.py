@@ -20,7 +20,8 @@ STATUS_NAMES = {0: "GT_OK", 1: "GT_ERR_NULL", 2: "GT_ERR_SHAPE", 3: "GT_ERR_VALU
 VARIANT_DEFAULT, VARIANT_FP32, VARIANT_TENSOR = 0, 1, 2
 
 EXPORTS = ("gt_plan_create", "gt_simulate", "gt_plan_destroy", "gt_last_error", "gt_debug_geometry",
-           "gt_debug_philox", "gt_debug_pkid", "gt_launch_count", "gt_variant_name", "gt_last_fused_ms")
+           "gt_debug_philox", "gt_debug_pkid", "gt_launch_count", "gt_variant_name", "gt_last_fused_ms",
+           "gt_debug_kelvin_map")
 
 
 class GtStage(C.Structure):
@@ -53,6 +54,8 @@ class GtConfig(C.Structure):
         ("chunk_samples", C.c_int64),
         ("variant", C.c_int32),
         ("pink_method", C.c_int32),
+        ("output_unit", C.c_int32), ("skydip_n", C.c_int32),
+        ("skydip_pwv_lo_mm", C.c_double), ("skydip_pwv_hi_mm", C.c_double),
     ]
 
 
@@ -97,6 +100,8 @@ def lib() -> C.CDLL:
         L.gt_variant_name.argtypes = [C.c_void_p]
         L.gt_last_fused_ms.restype = C.c_double
         L.gt_last_fused_ms.argtypes = [C.c_void_p, C.POINTER(C.c_int32)]
+        L.gt_debug_kelvin_map.restype = C.c_int
+        L.gt_debug_kelvin_map.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         _lib = L
     return _lib
 
@@ -157,6 +162,10 @@ def fill_config(w, dev: dict, keep: dict, variant: int = VARIANT_DEFAULT, chunk_
     c.chunk_samples = int(w.chunk_samples if chunk_samples is None else chunk_samples)
     c.variant = int(variant)
     c.pink_method = int(getattr(w, "pink_method", 0))
+    c.output_unit = int(getattr(w, "output_unit", 0))
+    c.skydip_n = int(getattr(w, "skydip_n", 16))
+    c.skydip_pwv_lo_mm = float(getattr(w, "skydip_pwv_lo_mm", 0.5))
+    c.skydip_pwv_hi_mm = float(getattr(w, "skydip_pwv_hi_mm", 1.5))
     return c
 
 
@@ -219,6 +228,12 @@ class Plan:
         n = C.c_int32(0)
         ms = self.L.gt_last_fused_ms(self.handle, C.byref(n))
         return float(ms), int(n.value)
+
+    def kelvin_map(self):
+        """gt_debug_kelvin_map: (a [n_chan], b [n_chan]) of T_b = a + b P_KID, float64."""
+        a, b = np.zeros(self.w.n_chan), np.zeros(self.w.n_chan)
+        self._check(self.L.gt_debug_kelvin_map(self.handle, C.c_void_p(a.ctypes.data), C.c_void_p(b.ctypes.data)))
+        return a, b
 
     # ---- the three calls ----
     def simulate(self, t_begin=0, t_count=None, out=None, pwv_out=None, device_out=True, want_pwv=False):

@@ -21,6 +21,7 @@
 #include "gt_fused_tc.cuh"
 #include "gt_pink.cuh"
 #include "gt_pink_tk.cuh"
+#include "gt_kelvin.cuh"
 #include <cufft.h>
 
 namespace {
@@ -72,6 +73,9 @@ struct gt_plan {
     // fused-kernel tables
     DevBuf<float> d_Xn, d_Gs, d_lut_r, d_filt_t, d_bias, d_c1, d_c2;
     DevBuf<float4> d_chan4;
+    int32_t output_unit = 0;                    // 1: brightness temperature through the skydip map (R22)
+    DevBuf<double> d_kelvin_ab;                 // [2][n_chan] a, b
+    DevBuf<float2> d_kelvin_abf;                // [n_chan] (a, b)
     gt::TcTables tc;                 // tensor-kernel operand images
     // pink
     gt::PinkParams pink{};
@@ -141,6 +145,13 @@ gt_status validate(const gt_config* c) {
             return fail(nullptr, GT_ERR_VALUE, "stage %d: eta_scalar outside [0,1]", k + 1);
     }
     if (c->pink_method != 0 && c->pink_method != 1) return fail(nullptr, GT_ERR_VALUE, "unknown pink_method %d", c->pink_method);
+    if (c->output_unit != 0 && c->output_unit != 1) return fail(nullptr, GT_ERR_VALUE, "unknown output_unit %d", c->output_unit);
+    if (c->output_unit == 1) {
+        if (c->skydip_n < 2 || c->skydip_n > 64) return fail(nullptr, GT_ERR_SHAPE, "skydip_n = %d is outside 2..64", c->skydip_n);
+        if (!(c->skydip_pwv_hi_mm > c->skydip_pwv_lo_mm) || !std::isfinite(c->skydip_pwv_lo_mm) || !std::isfinite(c->skydip_pwv_hi_mm))
+            return fail(nullptr, GT_ERR_VALUE, "skydip PWV range [%g, %g] mm is empty", c->skydip_pwv_lo_mm, c->skydip_pwv_hi_mm);
+        if (!(std::sin(c->el0_rad) > 0.0)) return fail(nullptr, GT_ERR_VALUE, "skydip: boresight elevation is not above the horizon");
+    }
     if (c->pink_noise && c->pink_method == 0) {
         if (c->pink_n_stage < 1 || c->pink_n_stage > gt::kPinkMaxJ)
             return fail(nullptr, GT_ERR_SHAPE, "pink_n_stage must be in 1..8");
@@ -245,6 +256,12 @@ gt_status run_chunk(gt_plan* p, int64_t t0, int64_t T, float* dst, float* pwv_ds
         GT_CUDA(p, cudaFuncSetAttribute(gt::pink_chain_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         if (p->J <= 4) gt::pink_chain_kernel<4><<<(unsigned)(n_seg * n_dblk), 256, smem, st>>>(p->pink, t0, T, dst);
         else           gt::pink_chain_kernel<8><<<(unsigned)(n_seg * n_dblk), 256, smem, st>>>(p->pink, t0, T, dst);
+        GT_CUDA(p, cudaGetLastError());
+        p->launches += 1;
+    }
+    if (noise && p->output_unit == 1) {          // the gt_simulate path; gt_debug_pkid stays in W
+        const int64_t n_span = (n_rows + gt::kKelvinRows - 1) / gt::kKelvinRows;
+        gt::kelvin_kernel<<<(unsigned)std::min<int64_t>(n_span, 16 * p->num_sms), 256, 0, st>>>(dst, n_rows, p->n_chan, p->d_kelvin_abf.p);
         GT_CUDA(p, cudaGetLastError());
         p->launches += 1;
     }
@@ -374,7 +391,7 @@ gt_status gt_plan_create(const gt_config* cfg, void* cuda_stream, gt_plan** out_
     //   coupled stage k:       a *= eta_k; b1 = eta_k b1 + (1-eta_k)(B_cmb - B_atm); b0 = eta_k b0 + (1-eta_k) B_atm
     // With eps = 1 - eta_atm:  P_final = eps*(-b1) + eta_atm*(a*S) + (b0 + b1);  all three terms >= 0.
     std::vector<float> Xn(nfp, 0.f), Gs(nfp, 0.f);
-    std::vector<double> Y(nf);
+    std::vector<double> Y(nf), Xd(nf);
     for (int i = 0; i < nf; ++i) {
         const double nu = c.nu0_hz + (double)i * c.dnu_hz;
         const double Bc = jn_power(nu, c.T_cmb_K), Ba = jn_power(nu, c.T_atm_K);
@@ -387,6 +404,7 @@ gt_status gt_plan_create(const gt_config* cfg, void* cuda_stream, gt_plan** out_
             else                     { b1 = e * b1;                         b0 = e * b0 + (1.0 - e) * jn_power(nu, s.T_K); }
         }
         Xn[i] = (float)(-b1 / kPref);
+        Xd[i] = -b1;
         Gs[i] = (float)(a / kPref);
         Y[i] = b0 + b1;
     }
@@ -479,6 +497,33 @@ gt_status gt_plan_create(const gt_config* cfg, void* cuda_stream, gt_plan** out_
         g.n_pwv = c.n_pwv; g.lut_pwv0 = c.lut_pwv0_mm; g.lut_dpwv = c.lut_dpwv_mm;
         g.has_cube = c.cube != nullptr; g.n_az = c.n_az; g.n_el = c.n_el;
         g.az_min = c.az_min_rad; g.daz_grid = c.daz_grid_rad; g.el_min = c.el_min_rad; g.del_grid = c.del_grid_rad;
+    }
+
+    // ---- brightness-temperature output: the skydip and its linear map (R22) ----
+    p->output_unit = c.output_unit;
+    if (c.output_unit == 1) {
+        const int K = c.skydip_n;
+        DevBuf<double> d_Xd, d_Yd, d_P, d_T; DevBuf<int32_t> d_bad;
+        GT_CUDA0(d_Xd.upload(Xd, st)); GT_CUDA0(d_Yd.upload(Y, st));
+        GT_CUDA0(d_P.alloc((size_t)K * nc)); GT_CUDA0(d_T.alloc((size_t)K * nc)); GT_CUDA0(d_bad.alloc(1));
+        GT_CUDA0(p->d_kelvin_ab.alloc((size_t)2 * nc)); GT_CUDA0(p->d_kelvin_abf.alloc((size_t)nc));
+        GT_CUDA0(cudaMemsetAsync(d_bad.p, 0, sizeof(int32_t), st));
+        gt::SkydipParams k{};
+        k.n_chan = nc; k.n_freq = nf; k.n_freq_pad = nfp; k.n_pwv = c.n_pwv; k.K = K;
+        k.dnu = c.dnu_hz; k.lut_pwv0 = c.lut_pwv0_mm; k.lut_dpwv = c.lut_dpwv_mm;
+        k.pwv_lo = c.skydip_pwv_lo_mm; k.pwv_step = (c.skydip_pwv_hi_mm - c.skydip_pwv_lo_mm) / (double)(K - 1);
+        k.csc0 = 1.0 / std::sin(c.el0_rad); k.T_atm = c.T_atm_K; k.T_cmb = c.T_cmb_K;
+        k.lut_r = p->d_lut_r.p; k.filt = c.filt; k.Xd = d_Xd.p; k.Yd = d_Yd.p; k.P = d_P.p; k.T = d_T.p;
+        k.ab = p->d_kelvin_ab.p; k.abf = p->d_kelvin_abf.p; k.bad = d_bad.p;
+        gt::skydip_kernel<<<dim3((unsigned)nc, (unsigned)K), 256, 0, st>>>(k);
+        GT_CUDA0(cudaGetLastError());
+        gt::skydip_fit_kernel<<<(unsigned)((nc + 127) / 128), 128, 0, st>>>(k);
+        GT_CUDA0(cudaGetLastError());
+        int32_t bad = 0;
+        GT_CUDA0(cudaMemcpyAsync(&bad, d_bad.p, sizeof(bad), cudaMemcpyDeviceToHost, st));
+        GT_CUDA0(cudaStreamSynchronize(st));
+        p->launches += 2;
+        if (bad) return fail(nullptr, GT_ERR_VALUE, "skydip: channel %d cannot be calibrated (its filter sums to zero or its power does not vary with PWV)", bad - 1);
     }
 
     p->pink_method = c.pink_method;
@@ -644,6 +689,16 @@ int64_t gt_launch_count(const gt_plan* plan) { return plan ? plan->launches : 0;
 const char* gt_variant_name(const gt_plan* plan) {
     if (!plan) return "";
     return plan->variant == GT_VARIANT_FP32 ? "fp32-ffma" : "tcgen05-3xf16-split";
+}
+
+gt_status gt_debug_kelvin_map(gt_plan* plan, double* a_out, double* b_out) {
+    if (!plan || !a_out || !b_out) return fail(plan, GT_ERR_NULL, "gt_debug_kelvin_map: NULL argument");
+    if (plan->output_unit != 1) return fail(plan, GT_ERR_UNSUPPORTED, "the plan's output unit is W: no skydip map");
+    const size_t nb = (size_t)plan->n_chan * sizeof(double);
+    if (cudaMemcpy(a_out, plan->d_kelvin_ab.p, nb, cudaMemcpyDeviceToHost) != cudaSuccess ||
+        cudaMemcpy(b_out, plan->d_kelvin_ab.p + plan->n_chan, nb, cudaMemcpyDeviceToHost) != cudaSuccess)
+        return fail(plan, GT_ERR_CUDA, "gt_debug_kelvin_map: copy failed");
+    return GT_OK;
 }
 
 double gt_last_fused_ms(gt_plan* plan, int32_t* n_launches) {

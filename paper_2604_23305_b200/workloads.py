@@ -95,6 +95,12 @@ class Workload:
     pink_A: Optional[np.ndarray] = None
     pink_alpha: Optional[np.ndarray] = None
     pink_f_corner_hz: Optional[np.ndarray] = None
+    # output unit: 0 = detected power [W], 1 = brightness temperature [K] through the linear map of a
+    # simulated skydip over skydip_n PWV values in [skydip_pwv_lo_mm, skydip_pwv_hi_mm] (R22)
+    output_unit: int = 0
+    skydip_n: int = 16
+    skydip_pwv_lo_mm: float = 0.5
+    skydip_pwv_hi_mm: float = 1.5
     # streaming
     chunk_samples: int = 0
 

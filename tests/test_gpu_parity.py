@@ -417,3 +417,50 @@ def test_tod_with_timmer_koenig_pink_noise(variant, n_samples):
             nop = p0.simulate().cpu().numpy().astype(np.float64)
         pn = got.astype(np.float64) - nop
         assert np.max(np.abs(pn - tk)) <= 2e-4 * np.std(tk) + 1.3e-7 * np.max(np.abs(nop))
+
+
+# --------------------------------------------------------------------------------------
+# brightness-temperature output (R22)
+def _kelvin_workload(seed=91, **kw):
+    w = W.random_workload(seed, n_samples=300, n_spaxel=3, n_chan=37, n_freq=144, photon_noise=True, pink_noise=True, **kw)
+    return w.replace(output_unit=1, skydip_n=12, skydip_pwv_lo_mm=0.4, skydip_pwv_hi_mm=1.7)
+
+
+@pytest.mark.parametrize("variant", VARIANTS, ids=VARIANT_IDS)
+def test_kelvin_output_through_the_skydip_map(variant):
+    """tod_K = a_c + b_c (P_KID + wn + pn): the skydip runs in double on the GPU at plan creation, the map is
+    applied to the finished TOD.  Tolerance: the 2e-5 gate of the noisy TOD carried through the map, i.e.
+    2e-5 |b tod_W|, plus fp32 rounding of the two terms of the line."""
+    w = _kelvin_workload()
+    o = O.Oracle(w)
+    a, b = o.kelvin_map()
+    tod_w = o.simulate(want=("tod",))["tod"]
+    ref = a + b * tod_w
+    with _plan(w, variant) as p:
+        ga, gb = p.kelvin_map()
+        got = p.simulate().cpu().numpy().astype(np.float64)
+        host = p.simulate(device_out=False)
+        pk = p.pkid().cpu().numpy()                                   # the noiseless hook stays in W
+    assert np.max(np.abs(gb / b - 1.0)) <= 1e-6 and np.max(np.abs(ga - a)) <= 1e-6 * np.max(np.abs(ref))
+    tol = 2e-5 * np.abs(b * tod_w) + 3e-7 * (np.abs(a) + np.abs(b * tod_w))
+    assert np.all(np.abs(got - ref) <= tol)
+    assert np.array_equal(np.asarray(host, dtype=np.float64), got)
+    assert rel_err(pk, o.simulate(want=("pkid",))["pkid"]) <= TOL_PKID
+    # the brightness scale is sensible: between the CMB and the atmosphere's physical temperature
+    assert ref.min() > 0 and np.median(got) < w.T_atm_K
+
+
+def test_kelvin_output_rejects_what_it_cannot_calibrate():
+    w = _kelvin_workload()
+    for bad, status in ((dict(skydip_n=1), 2), (dict(skydip_pwv_hi_mm=0.4), 3), (dict(output_unit=2), 3)):
+        with pytest.raises(B.GateauError) as e:
+            B.Plan(w.replace(**bad), variant=B.VARIANT_FP32)
+        assert e.value.status == status
+    filt = np.array(w.filt, copy=True)
+    filt[5] = 0.0
+    with pytest.raises(B.GateauError) as e:
+        B.Plan(w.replace(filt=filt), variant=B.VARIANT_FP32)
+    assert e.value.status == 3 and "channel 5" in str(e.value)
+    with _plan(w.replace(output_unit=0), B.VARIANT_FP32) as p:
+        with pytest.raises(B.GateauError):
+            p.kelvin_map()
