@@ -241,6 +241,25 @@ class Oracle:
             out[i] = np.fft.irfft(X, n=N) if N > 1 else 0.0
         return out
 
+    # ---- exact photon noise, Eq. 17-19 (R23) ----
+    def simulate_rows_exact(self, t_idx, s_idx):
+        """For the rows (t_idx[i], s_idx[i]): noiseless P_KID [i][c] (Eq. 16) and the white-noise draw
+        P_wn = sigma z [i][c], sigma from Eq. 17-18 on the row's own spectrum, z = normal 0 of
+        Philox(seed; n, spaxel, channel, 0) as in the narrow-band mode."""
+        w = self.w
+        F = np.asarray(w.filt, dtype=np.float64)
+        nu = w.nu_hz
+        pk = np.zeros((len(t_idx), w.n_chan))
+        wn = np.zeros((len(t_idx), w.n_chan))
+        for i, (n, s) in enumerate(zip(t_idx, s_idx)):
+            P_nu = self.row_spectrum(int(n), int(s))
+            pk[i] = w.dnu_hz * (F @ P_nu)
+            nep2 = nep2_exact(F, P_nu, nu, w.dnu_hz, w.kid_gap_J, w.eta_pb)
+            sigma = np.sqrt(nep2 * 0.5 * w.f_sample_hz)                                  # Eq. 18
+            z = np.array([normals4(w.seed, int(n), int(s), c, 0)[0] for c in range(w.n_chan)])
+            wn[i] = sigma * z                                                            # Eq. 19
+        return pk, wn
+
     # ---- brightness-temperature output (PAPER.md:231, DESIGN.md R22) ----
     def skydip(self):
         """The simulated skydip: a blank-sky stare of one on-axis detector row at the boresight elevation while
@@ -321,6 +340,15 @@ def normals_bulk(seed, c0_begin, count, c1=0, c2=0, c3=0):
 
 def photon_sigma(P_W, f_center_hz, dnu_eff_hz, f_sample_hz):
     return lib().go_photon_sigma(float(P_W), float(f_center_hz), float(dnu_eff_hz), float(f_sample_hz))
+
+
+def nep2_exact(F, P_nu, nu_hz, dnu_hz, kid_gap_J, eta_pb):
+    """Eq. 17, rectangle rule on the uniform grid (R16):
+    NEP^2[c] = 2 sum_nu Fm[c][nu] P_nu (h nu + Fm[c][nu] P_nu + 2 Delta_Al / eta_pb) dnu."""
+    h = 6.62607015e-34
+    F = np.asarray(F, dtype=np.float64)
+    FP = F * np.asarray(P_nu, dtype=np.float64)[None, :]
+    return 2.0 * dnu_hz * np.sum(FP * (h * np.asarray(nu_hz)[None, :] + FP + 2.0 * kid_gap_J / eta_pb), axis=1)
 
 
 def num_threads():

@@ -91,6 +91,11 @@ class Workload:
     seed: int = 0
     photon_noise: bool = False
     pink_noise: bool = False
+    # 0: north_star's narrow-band photon noise (R17); 1: the paper's Eq. 17 with the generation-
+    # recombination term 2 Delta_Al / eta_pb (Delta_Al = 188 micro-eV, eta_pb = 0.4) (R23)
+    photon_mode: int = 0
+    kid_gap_J: float = 188e-6 * 1.602176634e-19
+    eta_pb: float = 0.4
     pink_method: int = 0                   # 0: AR(1) cascade (north_star), 1: Timmer & Koenig FFT
     pink_A: Optional[np.ndarray] = None
     pink_alpha: Optional[np.ndarray] = None
