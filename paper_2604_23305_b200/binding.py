@@ -56,6 +56,7 @@ class GtConfig(C.Structure):
         ("pink_method", C.c_int32),
         ("output_unit", C.c_int32), ("skydip_n", C.c_int32),
         ("skydip_pwv_lo_mm", C.c_double), ("skydip_pwv_hi_mm", C.c_double),
+        ("photon_mode", C.c_int32), ("kid_gap_J", C.c_double), ("eta_pb", C.c_double),
     ]
 
 
@@ -166,6 +167,9 @@ def fill_config(w, dev: dict, keep: dict, variant: int = VARIANT_DEFAULT, chunk_
     c.skydip_n = int(getattr(w, "skydip_n", 16))
     c.skydip_pwv_lo_mm = float(getattr(w, "skydip_pwv_lo_mm", 0.5))
     c.skydip_pwv_hi_mm = float(getattr(w, "skydip_pwv_hi_mm", 1.5))
+    c.photon_mode = int(getattr(w, "photon_mode", 0))
+    c.kid_gap_J = float(getattr(w, "kid_gap_J", 188e-6 * 1.602176634e-19))
+    c.eta_pb = float(getattr(w, "eta_pb", 0.4))
     return c
 
 

@@ -22,6 +22,7 @@
 #include "gt_pink.cuh"
 #include "gt_pink_tk.cuh"
 #include "gt_kelvin.cuh"
+#include "gt_photon_exact.cuh"
 #include <cufft.h>
 
 namespace {
@@ -73,6 +74,12 @@ struct gt_plan {
     // fused-kernel tables
     DevBuf<float> d_Xn, d_Gs, d_lut_r, d_filt_t, d_bias, d_c1, d_c2;
     DevBuf<float4> d_chan4;
+    // exact Eq. 17 photon noise (R23): two more filter sets for the tensor kernel and their outputs
+    int32_t photon_mode = 0;
+    gt::TcTables tc_lin, tc_sq;
+    DevBuf<float4> d_chan4_lin, d_chan4_zero;
+    DevBuf<float> d_nep_lin, d_nep_sq;          // [launch rows][n_chan]
+    float scale_sq = 0.f, sqrt_e0 = 0.f, f_sample = 0.f;
     int32_t output_unit = 0;                    // 1: brightness temperature through the skydip map (R22)
     DevBuf<double> d_kelvin_ab;                 // [2][n_chan] a, b
     DevBuf<float2> d_kelvin_abf;                // [n_chan] (a, b)
@@ -145,6 +152,12 @@ gt_status validate(const gt_config* c) {
             return fail(nullptr, GT_ERR_VALUE, "stage %d: eta_scalar outside [0,1]", k + 1);
     }
     if (c->pink_method != 0 && c->pink_method != 1) return fail(nullptr, GT_ERR_VALUE, "unknown pink_method %d", c->pink_method);
+    if (c->photon_mode != 0 && c->photon_mode != 1) return fail(nullptr, GT_ERR_VALUE, "unknown photon_mode %d", c->photon_mode);
+    if (c->photon_noise && c->photon_mode == 1) {
+        if (c->variant == GT_VARIANT_FP32) return fail(nullptr, GT_ERR_UNSUPPORTED, "photon_mode = 1 (Eq. 17) runs on the tensor variant only");
+        if (!(c->kid_gap_J >= 0.0) || !(c->eta_pb > 0.0) || !std::isfinite(c->kid_gap_J) || !std::isfinite(c->eta_pb))
+            return fail(nullptr, GT_ERR_VALUE, "kid_gap_J = %g, eta_pb = %g are not a valid pair-breaking energy and efficiency", c->kid_gap_J, c->eta_pb);
+    }
     if (c->output_unit != 0 && c->output_unit != 1) return fail(nullptr, GT_ERR_VALUE, "unknown output_unit %d", c->output_unit);
     if (c->output_unit == 1) {
         if (c->skydip_n < 2 || c->skydip_n > 64) return fail(nullptr, GT_ERR_SHAPE, "skydip_n = %d is outside 2..64", c->skydip_n);
@@ -219,7 +232,8 @@ gt_status run_chunk(gt_plan* p, int64_t t0, int64_t T, float* dst, float* pwv_ds
     fp.cube = p->cube; fp.n_az = p->n_az;
     fp.filt_t = p->d_filt_t.p; fp.n_chan_pad = p->n_chan_pad;
     fp.scale = p->scale; fp.bias = p->d_bias.p; fp.noise_c1 = p->d_c1.p; fp.noise_c2 = p->d_c2.p; fp.chan4 = p->d_chan4.p;
-    fp.photon_noise = noise ? p->photon_noise : 0;
+    const bool exact = noise && p->photon_noise && p->photon_mode == 1;
+    fp.photon_noise = (noise && !exact) ? p->photon_noise : 0;
     fp.seed_lo = (uint32_t)(p->seed & 0xffffffffu); fp.seed_hi = (uint32_t)(p->seed >> 32);
     fp.out = dst;
 
@@ -231,6 +245,25 @@ gt_status run_chunk(gt_plan* p, int64_t t0, int64_t T, float* dst, float* pwv_ds
         GT_CUDA(p, launch_fused_fp32(p, fp, st));
     } else {
         GT_CUDA(p, gt::launch_fused_tc(fp, p->tc, p->num_sms, st));
+    }
+    if (exact) {
+        // Eq. 17: the contraction linear in the spectrum and the one of its square, then sigma z (gt_photon_exact.cuh)
+        const size_t need = (size_t)n_rows * p->n_chan;
+        if (need > p->d_nep_lin.n) { GT_CUDA(p, p->d_nep_lin.alloc(need)); GT_CUDA(p, p->d_nep_sq.alloc(need)); }
+        gt::FusedParams fl = fp, fq = fp;
+        fl.chan4 = p->d_chan4_lin.p; fl.out = p->d_nep_lin.p;
+        fq.chan4 = p->d_chan4_zero.p; fq.out = p->d_nep_sq.p; fq.scale = p->scale_sq;
+        p->tc_lin.scratch = p->tc.scratch; p->tc_sq.scratch = p->tc.scratch;     // the passes run one after another
+        GT_CUDA(p, gt::launch_fused_tc(fl, p->tc_lin, p->num_sms, st));
+        GT_CUDA(p, gt::launch_fused_tc(fq, p->tc_sq, p->num_sms, st, true));
+        gt::PhotonExactParams pe{};
+        pe.tod = dst; pe.lin = p->d_nep_lin.p; pe.sq = p->d_nep_sq.p; pe.n_rows = n_rows; pe.t0 = t0;
+        pe.n_chan = p->n_chan; pe.n_spaxel = p->n_spaxel; pe.f_sample = p->f_sample; pe.sqrt_e0 = p->sqrt_e0;
+        pe.seed_lo = fp.seed_lo; pe.seed_hi = fp.seed_hi;
+        const int64_t n_span = (n_rows + 31) / 32;
+        gt::photon_exact_kernel<<<(unsigned)std::min<int64_t>(n_span, 16 * p->num_sms), 256, 0, st>>>(pe);
+        GT_CUDA(p, cudaGetLastError());
+        p->launches += 3;
     }
     GT_CUDA(p, cudaEventRecord(p->ev_fused[2 * fused_slot + 1], st));
     p->launches++;
@@ -452,9 +485,35 @@ gt_status gt_plan_create(const gt_config* cfg, void* cuda_stream, gt_plan** out_
             return fail(nullptr, s, "tensor variant: %s", gt::tc_error());
         }
         if (gt_status s = gt::alloc_tc_scratch(p->tc, p->num_sms)) return fail(nullptr, s, "tensor variant: %s", gt::tc_error());
+        if (c.photon_noise && c.photon_mode == 1) {
+            // Eq. 17 with P_nu = kPref v + Y (v = the generated element):
+            //   NEP^2 / (2 dnu) = sum Fm (h nu + g) P + sum Fm^2 P^2
+            //                   = kPref sum [Fm (h nu + g) + 2 Fm^2 Y] v + kPref^2 sum Fm^2 v^2 + sum [Fm (h nu + g) Y + Fm^2 Y^2]
+            const double g = 2.0 * c.kid_gap_J / c.eta_pb;
+            const double E0 = kH * (c.nu0_hz + (double)(nf - 1) * c.dnu_hz) + g;
+            std::vector<float> L((size_t)nc * nf), Q((size_t)nc * nf);
+            std::vector<float4> c4l(ncp, make_float4(0.f, 0.f, 0.f, 0.f)), c4z(ncp, make_float4(0.f, 0.f, 0.f, 0.f));
+            for (int ch = 0; ch < nc; ++ch) {
+                double sb = 0.0;
+                for (int i = 0; i < nf; ++i) {
+                    const double f = h_filt[(size_t)ch * nf + i], e = kH * (c.nu0_hz + (double)i * c.dnu_hz) + g;
+                    L[(size_t)ch * nf + i] = (float)((f * e + 2.0 * f * f * Y[i]) / E0);
+                    Q[(size_t)ch * nf + i] = (float)(f * f);
+                    sb += f * e * Y[i] + f * f * Y[i] * Y[i];
+                }
+                c4l[ch].x = (float)(c.dnu_hz * sb / E0);
+            }
+            if (gt_status s = gt::build_tc_tables(L, nc, nf, nfp, p->tc_lin, st)) return fail(nullptr, s, "tensor variant (Eq. 17 linear filter): %s", gt::tc_error());
+            if (gt_status s = gt::build_tc_tables(Q, nc, nf, nfp, p->tc_sq, st)) return fail(nullptr, s, "tensor variant (Eq. 17 squared filter): %s", gt::tc_error());
+            GT_CUDA0(p->d_chan4_lin.upload(c4l, st)); GT_CUDA0(p->d_chan4_zero.upload(c4z, st));
+            GT_CUDA0(cudaStreamSynchronize(st));
+            p->scale_sq = (float)(kPref * kPref * c.dnu_hz / ((double)gt::kTcSqScale * E0));
+            p->sqrt_e0 = (float)std::sqrt(E0);
+            p->f_sample = (float)c.f_sample_hz;
+        }
         if (const char* e = std::getenv("GATEAU_TC_SEG")) {          // tuning/diagnostic knob: slabs per accumulation segment
             const int v = std::atoi(e);
-            if (v > 0) p->tc.seg = v;
+            if (v > 0) p->tc.seg = p->tc_lin.seg = p->tc_sq.seg = v;
         }
     }
     GT_CUDA0(p->d_Xn.upload(Xn, st)); GT_CUDA0(p->d_Gs.upload(Gs, st)); GT_CUDA0(p->d_lut_r.upload(lut_r, st));
@@ -501,6 +560,7 @@ gt_status gt_plan_create(const gt_config* cfg, void* cuda_stream, gt_plan** out_
 
     // ---- brightness-temperature output: the skydip and its linear map (R22) ----
     p->output_unit = c.output_unit;
+    p->photon_mode = c.photon_mode;
     if (c.output_unit == 1) {
         const int K = c.skydip_n;
         DevBuf<double> d_Xd, d_Yd, d_P, d_T; DevBuf<int32_t> d_bad;
@@ -639,6 +699,8 @@ gt_status gt_plan_destroy(gt_plan* plan) {
         if (plan->ev_copied[i]) cudaEventDestroy(plan->ev_copied[i]);
     }
     for (cudaEvent_t e : plan->ev_fused) cudaEventDestroy(e);
+    plan->tc_lin.scratch = nullptr; plan->tc_sq.scratch = nullptr;      // aliases of tc.scratch
+    gt::free_tc_tables(plan->tc_lin); gt::free_tc_tables(plan->tc_sq);
     gt::free_tc_tables(plan->tc);
     delete plan;
     return GT_OK;

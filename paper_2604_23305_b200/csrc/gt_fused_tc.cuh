@@ -43,6 +43,7 @@ namespace gt {
 
 constexpr int kTcBM = 128;                 // rows per tile (UMMA M)
 constexpr int kTcBK = 64;                  // frequencies per A stage / B unit: one 128-byte swizzle row of 64 fp16
+constexpr float kTcSqScale = 1.0f / 256.0f;   // squared elements (v = O(256)) are scaled back into fp16 range
 constexpr int kTcHB = 32;                  // frequencies per generator step group (8 lanes x 4): half a slab
 constexpr int kTcKSteps = 4;               // K = 16 MMAs per 128-byte operand row
 // operand scaling into the fp16 range (exact powers of two, undone in the output scale): spectrum values are
@@ -285,7 +286,7 @@ __device__ __forceinline__ size_t tc_scratch_index(int col, int row) {
 
 __device__ __forceinline__ float4 ldg4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
 
-template <bool VEC>
+template <bool VEC, bool SQ>
 __global__ void __launch_bounds__(kTcThreads, 1)
 fused_tc_kernel(const TcParams p) {
     extern __shared__ unsigned char smem_raw[];
@@ -435,6 +436,7 @@ fused_tc_kernel(const TcParams p) {
                     v.y = element_value_fast(fmaf(fc.x, cur.L1.y - cur.L0.y, cur.L0.y), fc.y, X.y, G.y, S.y);
                     v.z = element_value_fast(fmaf(fc.x, cur.L1.z - cur.L0.z, cur.L0.z), fc.y, X.z, G.z, S.z);
                     v.w = element_value_fast(fmaf(fc.x, cur.L1.w - cur.L0.w, cur.L0.w), fc.y, X.w, G.w, S.w);
+                    if constexpr (SQ) { v.x *= v.x * kTcSqScale; v.y *= v.y * kTcSqScale; v.z *= v.z * kTcSqScale; v.w *= v.w * kTcSqScale; }
                     store_split(smem_raw + (sm.a - raw) + stage * kTcAStageBytes, rsub + kTcRowStride * j, chunk, h, v);
                 };
                 Tap t0, t1;
@@ -536,6 +538,7 @@ fused_tc_kernel(const TcParams p) {
                     v.y = element_value_fast(fmaf(fp[j], L1[j].y - L0[j].y, L0[j].y), csc[j], X.y, G.y, S[j].y);
                     v.z = element_value_fast(fmaf(fp[j], L1[j].z - L0[j].z, L0[j].z), csc[j], X.z, G.z, S[j].z);
                     v.w = element_value_fast(fmaf(fp[j], L1[j].w - L0[j].w, L0[j].w), csc[j], X.w, G.w, S[j].w);
+                    if constexpr (SQ) { v.x *= v.x * kTcSqScale; v.y *= v.y * kTcSqScale; v.z *= v.z * kTcSqScale; v.w *= v.w * kTcSqScale; }
                     store_split(a_hi, rsub + kTcRowStride * j, chunk, h, v);
                 }
                 }
@@ -792,7 +795,9 @@ fused_tc_kernel(const TcParams p) {
     }
 }
 
-inline cudaError_t launch_fused_tc(const FusedParams& fp, const TcTables& t, int num_sms, cudaStream_t st) {
+// square = true: the generator writes kTcSqScale v^2 instead of v (the bunching contraction sum Fm^2 P^2 of Eq. 17,
+// DESIGN.md R23); the caller's scale carries 1 / kTcSqScale.
+inline cudaError_t launch_fused_tc(const FusedParams& fp, const TcTables& t, int num_sms, cudaStream_t st, bool square = false) {
     TcParams p{};
     p.f = fp; p.filt_img = t.filt_img;
     // Truncation compensation: the tensor core drops up to ~1e-7 of the running sum
@@ -812,7 +817,8 @@ inline cudaError_t launch_fused_tc(const FusedParams& fp, const TcTables& t, int
     const int64_t n_tiles = kTcPair ? (int64_t)((p.n_row_tiles + 1) / 2) * p.n_groups : (int64_t)p.n_row_tiles * p.n_groups;
     const int64_t workers = kTcPair ? num_sms / 2 : num_sms;
     const unsigned grid = (unsigned)(std::min<int64_t>(n_tiles, workers) * (kTcPair ? 2 : 1));
-    auto kern = p.cube_vec ? fused_tc_kernel<true> : fused_tc_kernel<false>;
+    auto kern = square ? (p.cube_vec ? fused_tc_kernel<true, true> : fused_tc_kernel<false, true>)
+                       : (p.cube_vec ? fused_tc_kernel<true, false> : fused_tc_kernel<false, false>);
     // set on every launch: the attribute is per device
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, t.smem_bytes);
     if (e != cudaSuccess) return e;

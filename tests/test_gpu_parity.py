@@ -464,3 +464,70 @@ def test_kelvin_output_rejects_what_it_cannot_calibrate():
     with _plan(w.replace(output_unit=0), B.VARIANT_FP32) as p:
         with pytest.raises(B.GateauError):
             p.kelvin_map()
+
+
+# --------------------------------------------------------------------------------------
+# exact photon noise, Eq. 17 (R23)
+@pytest.mark.parametrize("case", ["random", "lorentzian", "nocube"])
+def test_exact_photon_noise_eq17(case):
+    """photon_mode = 1: sigma from the full Eq. 17 on each row's own spectrum (three contractions through the
+    tensor kernel), same normals as the narrow-band mode.  The TOD meets the 2e-5 gate; sigma itself, isolated
+    with the GPU's own noiseless power, agrees with the oracle's to 1e-3 (it only scales a noise draw)."""
+    if case == "random":
+        w = W.random_workload(101, n_samples=260, n_spaxel=3, n_chan=37, n_freq=144, photon_noise=True)
+    elif case == "nocube":
+        w = W.random_workload(102, n_samples=131, n_spaxel=2, n_chan=20, n_freq=70, photon_noise=True, with_cube=False)
+    else:
+        w = W.random_workload(103, n_samples=200, n_spaxel=2, n_chan=30, n_freq=512, photon_noise=True)
+        fc = np.linspace(w.nu_hz[40], w.nu_hz[-40], 30)
+        w = w.replace(filt=W.lorentzian_filterbank(w.nu_hz, fc, 200.0, 0.16), f_center_hz=fc, dnu_eff_hz=None)
+    w = w.replace(photon_mode=1)
+    o = O.Oracle(w)
+    t_idx = np.repeat(np.arange(w.n_samples), w.n_spaxel)
+    s_idx = np.tile(np.arange(w.n_spaxel), w.n_samples)
+    pk, wn = o.simulate_rows_exact(t_idx, s_idx)
+    ref = (pk + wn).reshape(w.n_samples, w.n_spaxel, w.n_chan)
+    with _plan(w, B.VARIANT_TENSOR) as p:
+        got = p.simulate().cpu().numpy().astype(np.float64)
+        nop = p.pkid().cpu().numpy().astype(np.float64)
+        part = p.simulate(57, 40).cpu().numpy()
+    assert rel_err(got, ref) <= TOL_TOD
+    assert np.array_equal(part, got[57:97].astype(np.float32))
+    wn_g = (got - nop).reshape(-1, w.n_chan)
+    big = np.abs(wn) > 0.3 * np.abs(wn).std()                       # ratios are meaningful where the draw is not ~0
+    ratio = wn_g[big] / wn[big]
+    assert np.max(np.abs(ratio - 1.0)) <= 1e-3 + 4e-7 * np.max(np.abs(pk)) / np.min(np.abs(wn[big]))
+    # and it is not the narrow-band sigma: the generation-recombination term raises it
+    _, wn0 = o.simulate_rows(t_idx, s_idx, noise=True)
+    assert np.median(np.abs(wn[big] / wn0[big])) > 1.02
+
+
+def test_exact_photon_noise_needs_the_tensor_variant():
+    w = W.random_workload(104, n_samples=8, n_spaxel=1, n_chan=4, n_freq=16, photon_noise=True).replace(photon_mode=1)
+    with pytest.raises(B.GateauError) as e:
+        B.Plan(w, variant=B.VARIANT_FP32)
+    assert e.value.status == 7
+    with pytest.raises(B.GateauError) as e:
+        B.Plan(w.replace(eta_pb=0.0), variant=B.VARIANT_TENSOR)
+    assert e.value.status == 3
+
+
+def test_C2_full_size_exact_photon_noise_and_kelvin():
+    """BASELINE.json configs[1] at full size with the paper's own options switched on: Eq. 17 photon noise (R23) and
+    brightness-temperature output (R22), on sampled rows."""
+    w = W.make_workload("C2").replace(photon_noise=True, photon_mode=1, output_unit=1,
+                                      skydip_pwv_lo_mm=0.6, skydip_pwv_hi_mm=1.4)
+    rng = np.random.default_rng(11)
+    t_idx = np.sort(rng.choice(w.n_samples, 64, replace=False)).astype(np.int64)
+    t_idx[0] = 0; t_idx[-1] = w.n_samples - 1
+    s_idx = rng.integers(0, w.n_spaxel, t_idx.size).astype(np.int32)
+    o = O.Oracle(w)
+    pk, wn = o.simulate_rows_exact(t_idx, s_idx)
+    a, b = o.kelvin_map()
+    ref = a + b * (pk + wn)
+    with B.Plan(w) as p:
+        tod = p.simulate()
+        got = tod[t_idx, s_idx.astype(np.int64)].cpu().numpy().astype(np.float64)
+        del tod
+    tol = 2e-5 * np.abs(b * (pk + wn)) + 3e-7 * (np.abs(a) + np.abs(b * (pk + wn)))
+    assert np.all(np.abs(got - ref) <= tol)
