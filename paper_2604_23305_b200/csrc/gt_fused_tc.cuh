@@ -25,7 +25,7 @@
 //                           last segment the finisher warps (4) transpose the scratch tile into the TOD:
 //                           P = sum*scale + bias[c], photon noise (Eq. 18-19), coalesced stores.
 //
-// Pipelines: A ring (3 stages, generators of both CTAs -> leader's MMA thread), B ring (loader -> MMA, the
+// Pipelines: A ring (2 stages, generators of both CTAs -> leader's MMA thread), B ring (loader -> MMA, the
 // peer's halves relayed by a forwarder), accumulator buffers flush_full / buf_free (MMA <-> flush), scratch
 // tiles tile_done / scratch_free (flush <-> finisher); all mbarrier based, CTA-scope waits.
 #pragma once
@@ -50,7 +50,7 @@ constexpr int kTcKSteps = 4;               // K = 16 MMAs per 128-byte operand r
 // O(1) (P_nu / (k_B 300 K)), filter transmissions are <= 1
 constexpr float kTcScaleA = 256.0f, kTcScaleB = 16384.0f;
 #ifndef GT_TC_A_STAGES
-#define GT_TC_A_STAGES 3
+#define GT_TC_A_STAGES 2
 #endif
 constexpr int kTcAStages = GT_TC_A_STAGES;   // <= 4
 #ifndef GT_TC_PAIR
@@ -96,7 +96,7 @@ constexpr int kTcBufCols = 128, kTcNumBuf = 4, kTcMaxCg = 3;
 constexpr int kTcSegDefault = 8;           // slabs (of 64 frequencies) per accumulation segment
 constexpr float kTcTruncPerMma = 4.0e-8f;  // measured mean relative truncation loss per chained kind::f16 MMA (about half the worst case)
 #ifndef GT_TC_MAX_B_STAGES
-#define GT_TC_MAX_B_STAGES 4
+#define GT_TC_MAX_B_STAGES 3
 #endif
 constexpr int kTcMaxBStages = GT_TC_MAX_B_STAGES;   // <= 4 (barrier slots)
 constexpr int kTcSmemLimit = 227 * 1024;
@@ -196,8 +196,8 @@ struct TcParams {
 };
 
 // shared-memory map relative to the 1024-byte aligned base:
-//   [0, 64 KB)                      A ring: stage s at s*32 KB = {hi 16 KB, lo 16 KB}
-//   [64 KB, 64 KB + NBS*unit)       B ring
+//   [0, NAS*32 KB)                  A ring: stage s at s*32 KB = {hi 16 KB, lo 16 KB}
+//   [NAS*32 KB, .. + NBS*unit)      B ring
 //   then barriers: a_full[2] a_empty[2] b_full[4] b_empty[4] flush_full[4] buf_free[4] tile_done[2]
 //   scratch_free[2], tensor-memory slot
 struct TcSmem {
