@@ -351,5 +351,33 @@ def nep2_exact(F, P_nu, nu_hz, dnu_hz, kid_gap_J, eta_pb):
     return 2.0 * dnu_hz * np.sum(FP * (h * np.asarray(nu_hz)[None, :] + FP + 2.0 * kid_gap_J / eta_pb), axis=1)
 
 
+def footprint_weights(dx_m, dy_m, R_tel_m, t_edge_db):
+    """Aperture footprint on the screen grid (PAPER.md:92 with the illumination of Eq. 2 :76, R24):
+    A(r) = 10^(-|t_edge| / 20 * r^2 / R_tel^2) inside r < R_tel (Gaussian, |t_edge| dB down at the rim), 0 outside,
+    sampled at (i dx, j dy), normalised to unit sum.  Returns K[j + ry][i + rx]."""
+    rx, ry = int(np.floor(R_tel_m / dx_m)), int(np.floor(R_tel_m / dy_m))
+    K = np.zeros((2 * ry + 1, 2 * rx + 1))
+    for j in range(-ry, ry + 1):
+        for i in range(-rx, rx + 1):
+            r2 = (i * dx_m) ** 2 + (j * dy_m) ** 2
+            if r2 < R_tel_m ** 2:
+                K[j + ry, i + rx] = 10.0 ** (-abs(t_edge_db) / 20.0 * r2 / R_tel_m ** 2)
+    return K / K.sum()
+
+
+def screen_line_of_sight(epl, dx_m, dy_m, R_tel_m, t_edge_db, pwv0_mm):
+    """Eq. 4 and the footprint smoothing (:92) on a periodic screen (R7):
+    PWV[y][x] = PWV_0 + (1 / 6.587) sum_{i,j} K[j][i] EPL[(y + j) mod ny][(x + i) mod nx]."""
+    epl = np.asarray(epl, dtype=np.float64)
+    K = footprint_weights(dx_m, dy_m, R_tel_m, t_edge_db)
+    ry, rx = K.shape[0] // 2, K.shape[1] // 2
+    acc = np.zeros_like(epl)
+    for j in range(-ry, ry + 1):
+        for i in range(-rx, rx + 1):
+            if K[j + ry, i + rx] != 0.0:
+                acc += K[j + ry, i + rx] * np.roll(epl, (-j, -i), axis=(0, 1))
+    return pwv0_mm + acc / 6.587
+
+
 def num_threads():
     return lib().go_num_threads()
