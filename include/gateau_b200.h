@@ -164,6 +164,17 @@ gt_status gt_simulate(gt_plan* plan, int64_t t_begin, int64_t t_count,
 /* Frees everything the plan owns.  NULL-safe. */
 gt_status gt_plan_destroy(gt_plan* plan);
 
+/* Pre-processing utility (R24; not part of a plan): turns an extra-path-length screen
+ * into the line-of-sight PWV screen that gt_config.screen expects.
+ *   pwv[y][x] = pwv0_mm + (1 / 6.587) sum_{i,j} K[j][i] epl[(y + j) mod ny][(x + i) mod nx]      (Eq. 4, then :92)
+ * K = the aperture footprint on the screen grid: 10^(-|t_edge_db| / 20 * r^2 / R_tel^2) for r < R_tel (the Gaussian
+ * illumination of Eq. 2 with the given edge taper), 0 outside, r^2 = (i dx)^2 + (j dy)^2, normalised to unit sum.
+ * epl_dev, pwv_dev: DEVICE [ny][nx] fp32, distinct buffers, caller-owned.  Asynchronous on cuda_stream.
+ * GT_ERR_SHAPE for non-positive sizes, GT_ERR_VALUE for non-positive dx, dy, R_tel,
+ * GT_ERR_UNSUPPORTED if R_tel spans more than 64 pixels in x or y. */
+gt_status gt_prepare_screen(const float* epl_dev, int32_t nx, int32_t ny, double dx_m, double dy_m,
+                            double R_tel_m, double t_edge_db, double pwv0_mm, float* pwv_dev, void* cuda_stream);
+
 /* Message of the last error on this plan; plan == NULL => the calling thread's last
  * gt_plan_create error.  Never NULL. */
 const char* gt_last_error(const gt_plan* plan);

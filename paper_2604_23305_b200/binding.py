@@ -21,7 +21,7 @@ VARIANT_DEFAULT, VARIANT_FP32, VARIANT_TENSOR = 0, 1, 2
 
 EXPORTS = ("gt_plan_create", "gt_simulate", "gt_plan_destroy", "gt_last_error", "gt_debug_geometry",
            "gt_debug_philox", "gt_debug_pkid", "gt_launch_count", "gt_variant_name", "gt_last_fused_ms",
-           "gt_debug_kelvin_map")
+           "gt_debug_kelvin_map", "gt_prepare_screen")
 
 
 class GtStage(C.Structure):
@@ -101,6 +101,9 @@ def lib() -> C.CDLL:
         L.gt_variant_name.argtypes = [C.c_void_p]
         L.gt_last_fused_ms.restype = C.c_double
         L.gt_last_fused_ms.argtypes = [C.c_void_p, C.POINTER(C.c_int32)]
+        L.gt_prepare_screen.restype = C.c_int
+        L.gt_prepare_screen.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_double, C.c_double, C.c_double,
+                                        C.c_double, C.c_double, C.c_void_p, C.c_void_p]
         L.gt_debug_kelvin_map.restype = C.c_int
         L.gt_debug_kelvin_map.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         _lib = L
@@ -324,3 +327,18 @@ def gt_plan_destroy(handle):
 
 def gt_last_error(handle=None) -> str:
     return lib().gt_last_error(handle).decode()
+
+
+def gt_prepare_screen(epl, dx_m, dy_m, R_tel_m, t_edge_db, pwv0_mm, out=None):
+    """gt_prepare_screen: `epl` a contiguous float32 CUDA tensor [ny][nx]; returns the PWV screen (a new CUDA tensor
+    unless `out` is given).  Argument marshalling only."""
+    import torch
+    if not (epl.is_cuda and epl.dtype == torch.float32 and epl.dim() == 2 and epl.is_contiguous()):
+        raise ValueError("epl must be a contiguous float32 CUDA tensor [ny][nx]")
+    out = torch.empty_like(epl) if out is None else out
+    st = lib().gt_prepare_screen(_ptr(epl), int(epl.shape[1]), int(epl.shape[0]), float(dx_m), float(dy_m),
+                                 float(R_tel_m), float(t_edge_db), float(pwv0_mm), _ptr(out),
+                                 C.c_void_p(torch.cuda.current_stream().cuda_stream))
+    if st != GT_OK:
+        raise GateauError(st, lib().gt_last_error(None).decode())
+    return out

@@ -23,6 +23,7 @@
 #include "gt_pink_tk.cuh"
 #include "gt_kelvin.cuh"
 #include "gt_photon_exact.cuh"
+#include "gt_screen.cuh"
 #include <cufft.h>
 
 namespace {
@@ -743,6 +744,40 @@ gt_status gt_debug_philox(uint64_t seed, uint32_t c0_begin, int64_t count, uint3
                                                                   c0_begin, count, c1, c2, c3, out.p);
     GT_CUDA(nullptr, cudaGetLastError());
     GT_CUDA(nullptr, cudaMemcpy(host_out_words, out.p, (size_t)count * sizeof(uint4), cudaMemcpyDeviceToHost));
+    return GT_OK;
+}
+
+gt_status gt_prepare_screen(const float* epl_dev, int32_t nx, int32_t ny, double dx_m, double dy_m,
+                            double R_tel_m, double t_edge_db, double pwv0_mm, float* pwv_dev, void* cuda_stream) {
+    if (!epl_dev || !pwv_dev) return fail(nullptr, GT_ERR_NULL, "gt_prepare_screen: NULL screen pointer");
+    if (epl_dev == pwv_dev) return fail(nullptr, GT_ERR_VALUE, "gt_prepare_screen: input and output must be distinct buffers");
+    if (nx <= 0 || ny <= 0) return fail(nullptr, GT_ERR_SHAPE, "gt_prepare_screen: screen size %d x %d", nx, ny);
+    if (!(dx_m > 0) || !(dy_m > 0) || !(R_tel_m > 0) || !std::isfinite(t_edge_db) || !std::isfinite(pwv0_mm))
+        return fail(nullptr, GT_ERR_VALUE, "gt_prepare_screen: dx, dy and R_tel must be positive, t_edge and pwv0 finite");
+    const double qx = std::floor(R_tel_m / dx_m), qy = std::floor(R_tel_m / dy_m);
+    if (qx > 64.0 || qy > 64.0) return fail(nullptr, GT_ERR_UNSUPPORTED, "gt_prepare_screen: the aperture spans more than 64 pixels");
+    const int rx = (int)qx, ry = (int)qy, kw = 2 * rx + 1, kh = 2 * ry + 1;
+    std::vector<double> Kd((size_t)kw * kh, 0.0);
+    double sum = 0.0;
+    for (int j = -ry; j <= ry; ++j)
+        for (int i = -rx; i <= rx; ++i) {
+            const double r2 = (i * dx_m) * (i * dx_m) + (j * dy_m) * (j * dy_m);
+            if (r2 < R_tel_m * R_tel_m) sum += Kd[(size_t)(j + ry) * kw + (i + rx)] = std::pow(10.0, -std::fabs(t_edge_db) / 20.0 * r2 / (R_tel_m * R_tel_m));
+        }
+    std::vector<float> Kf(Kd.size());
+    for (size_t i = 0; i < Kd.size(); ++i) Kf[i] = (float)(Kd[i] / sum);
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    DevBuf<float> d_K;
+    GT_CUDA(nullptr, d_K.upload(Kf, st));
+    gt::ScreenParams sp{};
+    sp.epl = epl_dev; sp.pwv = pwv_dev; sp.K = d_K.p; sp.nx = nx; sp.ny = ny; sp.rx = rx; sp.ry = ry;
+    sp.scale = (float)(1.0 / 6.587); sp.pwv0 = (float)pwv0_mm;
+    const size_t smem = ((size_t)(gt::kScreenTile + 2 * rx) * (gt::kScreenTile + 2 * ry) + (size_t)kw * kh) * sizeof(float);
+    GT_CUDA(nullptr, cudaFuncSetAttribute(gt::screen_los_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    dim3 grid((unsigned)((nx + gt::kScreenTile - 1) / gt::kScreenTile), (unsigned)((ny + gt::kScreenTile - 1) / gt::kScreenTile));
+    gt::screen_los_kernel<<<grid, 256, smem, st>>>(sp);
+    GT_CUDA(nullptr, cudaGetLastError());
+    GT_CUDA(nullptr, cudaStreamSynchronize(st));          // d_K and Kf go out of scope
     return GT_OK;
 }
 

@@ -531,3 +531,32 @@ def test_C2_full_size_exact_photon_noise_and_kelvin():
         del tod
     tol = 2e-5 * np.abs(b * (pk + wn)) + 3e-7 * (np.abs(a) + np.abs(b * (pk + wn)))
     assert np.all(np.abs(got - ref) <= tol)
+
+
+# --------------------------------------------------------------------------------------
+# screen pre-processing (R24)
+@pytest.mark.parametrize("shape,dx,dy,R,taper", [((37, 53), 0.7, 0.9, 3.0, -11.0), ((200, 131), 0.25, 0.25, 5.0, -10.0),
+                                                 ((5, 4), 1.0, 1.0, 7.5, -3.0), ((64, 64), 2.0, 2.0, 1.0, -10.0),
+                                                 ((96, 160), 0.5, 1.0, 30.0, -12.0)])
+def test_screen_preprocessing(shape, dx, dy, R, taper):
+    """Eq. 4 + footprint smoothing through gt_prepare_screen against the oracle: ragged tiles, a screen smaller than
+    the footprint (wraps several times), a footprint of one pixel, an anisotropic grid, a 60-pixel radius."""
+    import torch
+    rng = np.random.default_rng(5)
+    epl = rng.normal(0.0, 0.4, shape).astype(np.float32)
+    ref = O.screen_line_of_sight(epl, dx, dy, R, taper, 1.1)
+    got = B.gt_prepare_screen(torch.from_numpy(epl).cuda(), dx, dy, R, taper, 1.1).cpu().numpy()
+    assert got.dtype == np.float32 and got.shape == shape
+    assert np.max(np.abs(got - ref)) <= 3e-7 * 1.1 + 2e-6 * np.max(np.abs(ref - 1.1))
+
+
+def test_screen_preprocessing_rejects_bad_arguments():
+    import torch
+    epl = torch.zeros((8, 8), dtype=torch.float32, device="cuda")
+    for args, status in (((0.0, 1.0, 2.0, -10.0, 1.0), 3), ((1.0, 1.0, -2.0, -10.0, 1.0), 3), ((0.01, 1.0, 2.0, -10.0, 1.0), 7)):
+        with pytest.raises(B.GateauError) as e:
+            B.gt_prepare_screen(epl, *args)
+        assert e.value.status == status
+    with pytest.raises(B.GateauError) as e:
+        B.gt_prepare_screen(epl, 1.0, 1.0, 2.0, -10.0, 1.0, out=epl)
+    assert e.value.status == 3
