@@ -379,5 +379,49 @@ def screen_line_of_sight(epl, dx_m, dy_m, R_tel_m, t_edge_db, pwv0_mm):
     return pwv0_mm + acc / 6.587
 
 
+def far_field(rho_rad, nu_hz, R_tel_m, t_edge_db):
+    """Eq. 2-3 (R25): far-field power pattern of the circular aperture with the Gaussian
+    illumination A(r) = 10^(-|t_edge|/20 r^2/R^2), r < R_tel, normalised to 1 on axis.  The 2-D Fourier transform of
+    a circularly symmetric A is the Hankel transform: F(rho) = |int_0^R A(r) J0(2 pi r rho / lambda) r dr|^2 / F(0)."""
+    from scipy import integrate, special
+    lam = 299792458.0 / nu_hz
+    k = abs(t_edge_db) / 20.0 * np.log(10.0) / R_tel_m ** 2
+    g = lambda rho: integrate.quad(lambda r: np.exp(-k * r * r) * special.j0(2 * np.pi * r * rho / lam) * r,
+                                   0.0, R_tel_m, epsabs=1e-16 * R_tel_m ** 2, epsrel=1e-11, limit=400)[0]
+    g0 = g(0.0)
+    rho = np.atleast_1d(np.asarray(rho_rad, dtype=np.float64))
+    return np.array([(g(x) / g0) ** 2 for x in rho.ravel()]).reshape(rho.shape)
+
+
+def beam_weights(nu_hz, daz_rad, del_rad, r_pix, R_tel_m, t_edge_db):
+    """F sampled at the cube's pixel offsets (i daz, j del), |i|, |j| <= r_pix: W[j + r][i + r]."""
+    off = np.arange(-r_pix, r_pix + 1)
+    rho = np.hypot(off[None, :] * daz_rad, off[:, None] * del_rad)
+    u, inv = np.unique(np.round(rho / 1e-15).astype(np.int64), return_inverse=True)
+    return far_field(u * 1e-15, nu_hz, R_tel_m, t_edge_db)[inv].reshape(rho.shape)
+
+
+def source_power(I_cube, nu_hz, daz_rad, del_rad, el_first_rad, r_pix, R_tel_m, t_edge_db):
+    """Eq. 1 on the cube's grid, rectangle rule, zero intensity outside the cube (:137):
+    P[j][i][nu] = A_p sum_{j',i'} I[j'][i'][nu] F_nu((i - i') daz, (j - j') del) cos(theta_j') daz del,
+    A_p = pi R_tel^2, theta_j' = el_first + j' del, offsets limited to |i - i'|, |j - j'| <= r_pix."""
+    I = np.asarray(I_cube, dtype=np.float64)
+    n_el, n_az, n_f = I.shape
+    cosw = np.cos(el_first_rad + del_rad * np.arange(n_el))[:, None]
+    out = np.zeros_like(I)
+    for f in range(n_f):
+        W = beam_weights(nu_hz[f], daz_rad, del_rad, r_pix, R_tel_m, t_edge_db)
+        src = I[:, :, f] * cosw
+        pad = np.zeros((n_el + 2 * r_pix, n_az + 2 * r_pix))
+        pad[r_pix:r_pix + n_el, r_pix:r_pix + n_az] = src
+        acc = np.zeros((n_el, n_az))
+        for dj in range(-r_pix, r_pix + 1):
+            for di in range(-r_pix, r_pix + 1):
+                # pixel (j, i) receives source pixel (j - dj, i - di) through F(di daz, dj del)
+                acc += W[dj + r_pix, di + r_pix] * pad[r_pix - dj:r_pix - dj + n_el, r_pix - di:r_pix - di + n_az]
+        out[:, :, f] = np.pi * R_tel_m ** 2 * daz_rad * del_rad * acc
+    return out
+
+
 def num_threads():
     return lib().go_num_threads()
