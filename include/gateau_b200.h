@@ -172,6 +172,20 @@ gt_status gt_plan_destroy(gt_plan* plan);
  * epl_dev, pwv_dev: DEVICE [ny][nx] fp32, distinct buffers, caller-owned.  Asynchronous on cuda_stream.
  * GT_ERR_SHAPE for non-positive sizes, GT_ERR_VALUE for non-positive dx, dy, R_tel,
  * GT_ERR_UNSUPPORTED if R_tel spans more than 64 pixels in x or y. */
+/* Pre-processing utility (R25; not part of a plan): turns a specific-intensity cube
+ * I_nu [W m^-2 Hz^-1 sr^-1] into the spectral power cube P_nu,src [W/Hz] that gt_config.cube expects.
+ *   F_nu(rho) = |int_0^R A(r) J0(2 pi r rho / lambda) r dr|^2 / F_nu(0)        the far field of the circular aperture
+ *               with A(r) = 10^(-|t_edge_db| / 20 * r^2 / R_tel^2), r < R_tel (Eq. 2-3: the 2-D Fourier transform of
+ *               a circularly symmetric illumination is this Hankel transform), peak 1
+ *   P[j][i][nu] = pi R_tel^2 daz del sum_{|dj|,|di| <= r_pix} F_nu(di daz, dj del) I[j - dj][i - di][nu]
+ *                 cos(el_first + (j - dj) del)                                  (Eq. 1, rectangle rule; I = 0 outside)
+ * I_dev, P_dev: DEVICE [n_el][n_az][n_freq] fp32 (the cube layout of gt_config), distinct, caller-owned.
+ * nu = nu0_hz + k dnu_hz; daz_rad, del_rad = the cube's pixel pitch; el_first_rad = absolute elevation of row 0.
+ * Needs (2 r_pix + 1)^2 n_freq * 4 B of device scratch for the beam table.  Synchronises cuda_stream.
+ * GT_ERR_SHAPE for non-positive sizes or r_pix outside 0..64, GT_ERR_VALUE for non-positive nu0, pitch or R_tel. */
+gt_status gt_prepare_source(const float* I_dev, int32_t n_az, int32_t n_el, int32_t n_freq, double nu0_hz, double dnu_hz,
+                            double daz_rad, double del_rad, double el_first_rad, double R_tel_m, double t_edge_db,
+                            int32_t r_pix, float* P_dev, void* cuda_stream);
 gt_status gt_prepare_screen(const float* epl_dev, int32_t nx, int32_t ny, double dx_m, double dy_m,
                             double R_tel_m, double t_edge_db, double pwv0_mm, float* pwv_dev, void* cuda_stream);
 

@@ -387,7 +387,7 @@ def far_field(rho_rad, nu_hz, R_tel_m, t_edge_db):
     lam = 299792458.0 / nu_hz
     k = abs(t_edge_db) / 20.0 * np.log(10.0) / R_tel_m ** 2
     g = lambda rho: integrate.quad(lambda r: np.exp(-k * r * r) * special.j0(2 * np.pi * r * rho / lam) * r,
-                                   0.0, R_tel_m, epsabs=1e-16 * R_tel_m ** 2, epsrel=1e-11, limit=400)[0]
+                                   0.0, R_tel_m, epsabs=1e-13 * R_tel_m ** 2, epsrel=1e-11, limit=400)[0]
     g0 = g(0.0)
     rho = np.atleast_1d(np.asarray(rho_rad, dtype=np.float64))
     return np.array([(g(x) / g0) ** 2 for x in rho.ravel()]).reshape(rho.shape)

@@ -21,7 +21,7 @@ VARIANT_DEFAULT, VARIANT_FP32, VARIANT_TENSOR = 0, 1, 2
 
 EXPORTS = ("gt_plan_create", "gt_simulate", "gt_plan_destroy", "gt_last_error", "gt_debug_geometry",
            "gt_debug_philox", "gt_debug_pkid", "gt_launch_count", "gt_variant_name", "gt_last_fused_ms",
-           "gt_debug_kelvin_map", "gt_prepare_screen")
+           "gt_debug_kelvin_map", "gt_prepare_screen", "gt_prepare_source")
 
 
 class GtStage(C.Structure):
@@ -104,6 +104,9 @@ def lib() -> C.CDLL:
         L.gt_prepare_screen.restype = C.c_int
         L.gt_prepare_screen.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_double, C.c_double, C.c_double,
                                         C.c_double, C.c_double, C.c_void_p, C.c_void_p]
+        L.gt_prepare_source.restype = C.c_int
+        L.gt_prepare_source.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_double, C.c_double, C.c_double,
+                                        C.c_double, C.c_double, C.c_double, C.c_double, C.c_int32, C.c_void_p, C.c_void_p]
         L.gt_debug_kelvin_map.restype = C.c_int
         L.gt_debug_kelvin_map.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         _lib = L
@@ -339,6 +342,22 @@ def gt_prepare_screen(epl, dx_m, dy_m, R_tel_m, t_edge_db, pwv0_mm, out=None):
     st = lib().gt_prepare_screen(_ptr(epl), int(epl.shape[1]), int(epl.shape[0]), float(dx_m), float(dy_m),
                                  float(R_tel_m), float(t_edge_db), float(pwv0_mm), _ptr(out),
                                  C.c_void_p(torch.cuda.current_stream().cuda_stream))
+    if st != GT_OK:
+        raise GateauError(st, lib().gt_last_error(None).decode())
+    return out
+
+
+def gt_prepare_source(I_cube, nu0_hz, dnu_hz, daz_rad, del_rad, el_first_rad, R_tel_m, t_edge_db, r_pix, out=None):
+    """gt_prepare_source: `I_cube` a contiguous float32 CUDA tensor [n_el][n_az][n_freq]; returns P_nu,src (a new CUDA
+    tensor unless `out` is given).  Argument marshalling only."""
+    import torch
+    if not (I_cube.is_cuda and I_cube.dtype == torch.float32 and I_cube.dim() == 3 and I_cube.is_contiguous()):
+        raise ValueError("I_cube must be a contiguous float32 CUDA tensor [n_el][n_az][n_freq]")
+    out = torch.empty_like(I_cube) if out is None else out
+    n_el, n_az, n_freq = (int(x) for x in I_cube.shape)
+    st = lib().gt_prepare_source(_ptr(I_cube), n_az, n_el, n_freq, float(nu0_hz), float(dnu_hz), float(daz_rad),
+                                 float(del_rad), float(el_first_rad), float(R_tel_m), float(t_edge_db), int(r_pix),
+                                 _ptr(out), C.c_void_p(torch.cuda.current_stream().cuda_stream))
     if st != GT_OK:
         raise GateauError(st, lib().gt_last_error(None).decode())
     return out

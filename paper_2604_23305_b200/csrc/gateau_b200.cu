@@ -24,6 +24,7 @@
 #include "gt_kelvin.cuh"
 #include "gt_photon_exact.cuh"
 #include "gt_screen.cuh"
+#include "gt_beam.cuh"
 #include <cufft.h>
 
 namespace {
@@ -744,6 +745,36 @@ gt_status gt_debug_philox(uint64_t seed, uint32_t c0_begin, int64_t count, uint3
                                                                   c0_begin, count, c1, c2, c3, out.p);
     GT_CUDA(nullptr, cudaGetLastError());
     GT_CUDA(nullptr, cudaMemcpy(host_out_words, out.p, (size_t)count * sizeof(uint4), cudaMemcpyDeviceToHost));
+    return GT_OK;
+}
+
+gt_status gt_prepare_source(const float* I_dev, int32_t n_az, int32_t n_el, int32_t n_freq, double nu0_hz, double dnu_hz,
+                            double daz_rad, double del_rad, double el_first_rad, double R_tel_m, double t_edge_db,
+                            int32_t r_pix, float* P_dev, void* cuda_stream) {
+    if (!I_dev || !P_dev) return fail(nullptr, GT_ERR_NULL, "gt_prepare_source: NULL cube pointer");
+    if (I_dev == P_dev) return fail(nullptr, GT_ERR_VALUE, "gt_prepare_source: input and output must be distinct buffers");
+    if (n_az <= 0 || n_el <= 0 || n_freq <= 0 || n_az > 65535 || n_el > 65535)
+        return fail(nullptr, GT_ERR_SHAPE, "gt_prepare_source: cube size %d x %d x %d", n_el, n_az, n_freq);
+    if (r_pix < 0 || r_pix > 64) return fail(nullptr, GT_ERR_SHAPE, "gt_prepare_source: r_pix = %d is outside 0..64", r_pix);
+    if (!(nu0_hz > 0) || !(nu0_hz + (n_freq - 1) * dnu_hz > 0) || !(daz_rad > 0) || !(del_rad > 0) || !(R_tel_m > 0) ||
+        !std::isfinite(t_edge_db) || !std::isfinite(el_first_rad))
+        return fail(nullptr, GT_ERR_VALUE, "gt_prepare_source: frequencies, pixel pitch and R_tel must be positive");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const int kw = 2 * r_pix + 1;
+    DevBuf<float> d_W;
+    GT_CUDA(nullptr, d_W.alloc((size_t)kw * kw * n_freq));
+    gt::BeamParams b{};
+    b.n_az = n_az; b.n_el = n_el; b.n_freq = n_freq; b.r_pix = r_pix;
+    b.nu0 = nu0_hz; b.dnu = dnu_hz; b.daz = daz_rad; b.del = del_rad; b.el_first = el_first_rad; b.R_tel = R_tel_m;
+    b.k_taper = std::fabs(t_edge_db) / 20.0 * std::log(10.0) / (R_tel_m * R_tel_m);
+    b.scale = 3.14159265358979323846 * R_tel_m * R_tel_m * daz_rad * del_rad;
+    b.I = I_dev; b.P = P_dev; b.W = d_W.p;
+    const unsigned gf = (unsigned)((n_freq + 127) / 128);
+    gt::beam_weights_kernel<<<dim3(gf, (unsigned)(r_pix + 1), (unsigned)(r_pix + 1)), 128, 0, st>>>(b);
+    GT_CUDA(nullptr, cudaGetLastError());
+    gt::beam_conv_kernel<<<dim3(gf, (unsigned)n_az, (unsigned)n_el), 128, 0, st>>>(b);
+    GT_CUDA(nullptr, cudaGetLastError());
+    GT_CUDA(nullptr, cudaStreamSynchronize(st));          // the beam table goes out of scope
     return GT_OK;
 }
 

@@ -560,3 +560,36 @@ def test_screen_preprocessing_rejects_bad_arguments():
     with pytest.raises(B.GateauError) as e:
         B.gt_prepare_screen(epl, 1.0, 1.0, 2.0, -10.0, 1.0, out=epl)
     assert e.value.status == 3
+
+
+# --------------------------------------------------------------------------------------
+# source pre-processing: far field + beam convolution (R25)
+@pytest.mark.parametrize("n_el,n_az,n_freq,r,taper,pitch", [(9, 11, 5, 3, -10.0, 6.0), (20, 7, 130, 2, 0.0, 4.0),
+                                                           (3, 4, 3, 6, -14.0, 3.5), (6, 6, 2, 0, -10.0, 5.0)])
+def test_source_preprocessing(n_el, n_az, n_freq, r, taper, pitch):
+    """gt_prepare_source against the oracle: Hankel-transform far field (Simpson on the GPU, adaptive quadrature in
+    the oracle) and the direct convolution with zero intensity outside the cube; kernels wider than the cube, more
+    than one frequency block, no taper (Airy), r_pix = 0 (beam = on-axis value only)."""
+    import torch
+    rng = np.random.default_rng(8)
+    I = (1e-18 * rng.random((n_el, n_az, n_freq))).astype(np.float32)
+    nu0, dnu = 230e9, 1.7e9
+    nu = nu0 + dnu * np.arange(n_freq)
+    d = pitch * np.pi / 180 / 3600
+    el_first = np.deg2rad(58.0)
+    f_idx = np.unique(np.linspace(0, n_freq - 1, 4).astype(int))          # the oracle's quadrature is slow: sampled frequencies
+    ref = O.source_power(I[:, :, f_idx], nu[f_idx], d, 1.25 * d, el_first, r, 5.0, taper)
+    got = B.gt_prepare_source(torch.from_numpy(I).cuda(), nu0, dnu, d, 1.25 * d, el_first, 5.0, taper, r).cpu().numpy()
+    assert got.shape == I.shape and got.dtype == np.float32
+    assert np.max(np.abs(got[:, :, f_idx] - ref)) <= 5e-7 * np.max(np.abs(ref))
+
+
+def test_source_preprocessing_rejects_bad_arguments():
+    import torch
+    I = torch.zeros((4, 4, 4), dtype=torch.float32, device="cuda")
+    for kw, status in ((dict(r_pix=65), 2), (dict(R_tel_m=0.0), 3), (dict(daz_rad=-1e-5), 3)):
+        a = dict(nu0_hz=2e11, dnu_hz=1e9, daz_rad=2e-5, del_rad=2e-5, el_first_rad=1.0, R_tel_m=5.0, t_edge_db=-10.0, r_pix=2)
+        a.update(kw)
+        with pytest.raises(B.GateauError) as e:
+            B.gt_prepare_source(I, **a)
+        assert e.value.status == status
