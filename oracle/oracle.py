@@ -3,6 +3,12 @@
 TEST INFRASTRUCTURE, NOT THE PRODUCT: imported only by tests/, __graft_entry__.smoke()
 and bench.py's cpu_baseline / --impl reference legs.  Nothing here touches the CUDA
 path; it marshals a `Workload` (the shared seeded inputs) into the oracle's own struct.
+
+The options of SURVEY rows f1-f4 are written here in NumPy, in double precision, each from the passage it cites
+and each pinned in tests/test_oracle_*.py: Timmer & Koenig pink noise (pink_tk_series, R21),
+the skydip and its Kelvin map (skydip, kelvin_map, R22), the exact NEP of Eq. 17 (nep2_exact, simulate_rows_exact,
+R23), the screen and source pre-processing (footprint_weights, screen_line_of_sight, R24; far_field, beam_weights,
+source_power, R25).  Parity unpinned: only the absolute physical realism of the synthetic inputs (out of scope).
 """
 from __future__ import annotations
 
