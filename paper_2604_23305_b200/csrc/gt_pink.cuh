@@ -13,7 +13,10 @@
 
 namespace gt {
 
-constexpr int kPinkSeg = 64;
+#ifndef GT_PINK_SEG
+#define GT_PINK_SEG 64
+#endif
+constexpr int kPinkSeg = GT_PINK_SEG;
 constexpr int kPinkBatch = 8;      // TOD values fetched ahead per thread
 constexpr int kPinkMaxJ = 8;
 
