@@ -373,12 +373,13 @@ fused_tc_kernel(const TcParams p) {
         const size_t nf = (size_t)f.n_freq, nfp = (size_t)f.n_freq_pad;
         uint32_t a_st = 0, a_ph = 0;           // A-ring stage and its phase parity
         if constexpr (VEC) {
-            // One step = one row of this thread (4 frequencies of it): 2 LUT rows + 4 cube taps as
-            // 16-byte loads, steps 2-4, tf32 split, two 16-byte shared stores.  The loads of the
+            // One step = one row of this thread (4 frequencies of it): 4 cube taps (and, once per pair of
+            // rows, the 2 LUT rows) as 16-byte loads, steps 2-4, fp16 split, two 8-byte shared stores.  The loads of the
             // next step are issued before the current one is computed; the other three warps of the
             // scheduler cover the rest of the latency.  The per-row constants live in shared
             // memory (each warp only reads rows it wrote itself).
-            struct Tap { float4 L0, L1, c00, c01, c10, c11; };
+            struct Tap { float4 c00, c01, c10, c11; };
+            struct Lut { float4 L0, L1; };
             RowParam* rowp = reinterpret_cast<RowParam*>(smem_raw + (sm.rowp - raw));
             for (int64_t tl = worker; tl < n_tiles; tl += n_workers) {
                 const int64_t rt = tile_rt(tl);
@@ -415,15 +416,22 @@ fused_tc_kernel(const TcParams p) {
                 const uint32_t tap01 = f.cube != nullptr ? (uint32_t)nf : 0u;
                 const uint32_t tap10 = f.cube != nullptr ? (uint32_t)f.n_az * (uint32_t)nf : 0u;
                 const uint32_t nu_last = (uint32_t)(max(f.n_freq, 4) - 4) & ~3u;     // 16-byte aligned (n_freq % 4 == 0 with a cube)
-                auto issue = [&](int hb, int j, Tap& t) {                 // hb = half-slab (32 frequencies)
+                // The two LUT rows are looked up per SAMPLE, but the PWV moves by ~1e-4 of a LUT step per sample: the
+                // two rows of a thread nearly always share them.  They are therefore fetched once per half-slab
+                // (for row 0, one half-slab ahead, alternating between two register sets) and re-fetched for row 1
+                // only where its LUT row differs.
+                const bool same_lut = lut_off[1] == lut_off[0];
+                auto issue_lut = [&](int hb, int j, Lut& l) {
                     const uint32_t lo = lut_off[j] + (uint32_t)hb * kTcHB;
-                    t.L0 = ldg4(f.lut_r + lo); t.L1 = ldg4(f.lut_r + (lo + (uint32_t)nfp));
+                    l.L0 = ldg4(f.lut_r + lo); l.L1 = ldg4(f.lut_r + (lo + (uint32_t)nfp));
+                };
+                auto issue = [&](int hb, int j, Tap& t) {                 // hb = half-slab (32 frequencies)
                     if (GT_DIAG(p, 16)) return;
                     const uint32_t co = cube_off[j] + min((uint32_t)hb * kTcHB + (uint32_t)chunk * 4u, nu_last);
                     t.c00 = ldg4(cube_base + co);           t.c01 = ldg4(cube_base + (co + tap01));
                     t.c10 = ldg4(cube_base + (co + tap10)); t.c11 = ldg4(cube_base + (co + tap10 + tap01));
                 };
-                auto compute = [&](int j, int h, const Tap& cur, const float4& X, const float4& G, uint32_t stage) {
+                auto compute = [&](int j, int h, const Tap& cur, const Lut& lut, const float4& X, const float4& G, uint32_t stage) {
                     const RowParam* rp = rowp + gw * 8 + j * 4 + q4;
                     const float2 fc = *reinterpret_cast<const float2*>(rp);                    // fp, csc
                     const float4 w = *reinterpret_cast<const float4*>(&rp->w00);
@@ -432,14 +440,16 @@ fused_tc_kernel(const TcParams p) {
                     S.y = w.x * cur.c00.y + w.y * cur.c01.y + w.z * cur.c10.y + w.w * cur.c11.y;
                     S.z = w.x * cur.c00.z + w.y * cur.c01.z + w.z * cur.c10.z + w.w * cur.c11.z;
                     S.w = w.x * cur.c00.w + w.y * cur.c01.w + w.z * cur.c10.w + w.w * cur.c11.w;
-                    v.x = element_value_fast(fmaf(fc.x, cur.L1.x - cur.L0.x, cur.L0.x), fc.y, X.x, G.x, S.x);
-                    v.y = element_value_fast(fmaf(fc.x, cur.L1.y - cur.L0.y, cur.L0.y), fc.y, X.y, G.y, S.y);
-                    v.z = element_value_fast(fmaf(fc.x, cur.L1.z - cur.L0.z, cur.L0.z), fc.y, X.z, G.z, S.z);
-                    v.w = element_value_fast(fmaf(fc.x, cur.L1.w - cur.L0.w, cur.L0.w), fc.y, X.w, G.w, S.w);
+                    v.x = element_value_fast(fmaf(fc.x, lut.L1.x - lut.L0.x, lut.L0.x), fc.y, X.x, G.x, S.x);
+                    v.y = element_value_fast(fmaf(fc.x, lut.L1.y - lut.L0.y, lut.L0.y), fc.y, X.y, G.y, S.y);
+                    v.z = element_value_fast(fmaf(fc.x, lut.L1.z - lut.L0.z, lut.L0.z), fc.y, X.z, G.z, S.z);
+                    v.w = element_value_fast(fmaf(fc.x, lut.L1.w - lut.L0.w, lut.L0.w), fc.y, X.w, G.w, S.w);
                     if constexpr (SQ) { v.x *= v.x * kTcSqScale; v.y *= v.y * kTcSqScale; v.z *= v.z * kTcSqScale; v.w *= v.w * kTcSqScale; }
                     store_split(smem_raw + (sm.a - raw) + stage * kTcAStageBytes, rsub + kTcRowStride * j, chunk, h, v);
                 };
                 Tap t0, t1;
+                Lut la, lb;
+                issue_lut(0, 0, la);
                 issue(0, 0, t0);
                 const int n_hb = 2 * p.n_kb;
                 for (int kb = 0; kb < p.n_kb; ++kb, a_ph ^= (++a_st == kTcAStages), a_st = a_st == kTcAStages ? 0u : a_st) {
@@ -450,16 +460,19 @@ fused_tc_kernel(const TcParams p) {
                         if (lane == 0) arrive_leader(sm.a_full + 8 * stage);
                         continue;
                     }
-#pragma unroll
-                    for (int h = 0; h < 2; ++h) {
+                    auto half = [&](int h, Lut& cur, Lut& nxt) {
                         const int hb = 2 * kb + h;
                         const float4 X = ldg4(f.Xn + hb * kTcHB + chunk * 4), G = ldg4(f.Gs + hb * kTcHB + chunk * 4);
                         issue(hb, 1, t1);
+                        if (hb + 1 < n_hb) issue_lut(hb + 1, 0, nxt);
                         if (h == 0) wait_pair(sm.a_empty + 8 * stage, ph ^ 1u);
-                        compute(0, h, t0, X, G, stage);
+                        compute(0, h, t0, cur, X, G, stage);
                         if (hb + 1 < n_hb) issue(hb + 1, 0, t0);
-                        compute(1, h, t1, X, G, stage);
-                    }
+                        if (!same_lut) issue_lut(hb, 1, cur);
+                        compute(1, h, t1, cur, X, G, stage);
+                    };
+                    half(0, la, lb);
+                    half(1, lb, la);
                     // one arrival per warp: 512 per-thread arrivals on one mbarrier serialise (~5 cycles each)
                     ptx::fence_proxy_async_smem();
                     __syncwarp();
