@@ -593,3 +593,29 @@ def test_source_preprocessing_rejects_bad_arguments():
         with pytest.raises(B.GateauError) as e:
             B.gt_prepare_source(I, **a)
         assert e.value.status == status
+
+
+def test_all_paper_options_together_streamed():
+    """The paper's own choices at once -- Eq. 7 filterbank, Eq. 17 photon noise, Timmer & Koenig pink noise, Kelvin
+    output -- streamed to host memory in ragged chunks; device and host outputs are identical."""
+    w = W.random_workload(111, n_samples=333, n_spaxel=2, n_chan=24, n_freq=160, photon_noise=True, pink_noise=True)
+    fc = np.geomspace(w.nu_hz[30], w.nu_hz[-30], 24)
+    w = w.replace(filt=W.filterbank_upstream_absorption(w.nu_hz, fc, 80.0, 0.16), f_center_hz=fc, dnu_eff_hz=None,
+                  photon_mode=1, pink_method=1, pink_A=w.pink_A * 3e3, output_unit=1,
+                  skydip_pwv_lo_mm=0.5, skydip_pwv_hi_mm=1.6, chunk_samples=64)
+    o = O.Oracle(w)
+    t_idx = np.repeat(np.arange(w.n_samples), w.n_spaxel)
+    s_idx = np.tile(np.arange(w.n_spaxel), w.n_samples)
+    pk, wn = o.simulate_rows_exact(t_idx, s_idx)
+    d_s = np.repeat(np.arange(w.n_spaxel), w.n_chan).astype(np.int32)
+    d_c = np.tile(np.arange(w.n_chan), w.n_spaxel).astype(np.int32)
+    tk = o.pink_tk_series(d_s, d_c).T.reshape(w.n_samples, w.n_spaxel, w.n_chan)
+    a, b = o.kelvin_map()
+    tod_w = (pk + wn).reshape(w.n_samples, w.n_spaxel, w.n_chan) + tk
+    ref = a + b * tod_w
+    with _plan(w, B.VARIANT_TENSOR) as p:
+        dev = p.simulate().cpu().numpy()
+        host = np.asarray(p.simulate(device_out=False))
+    assert np.array_equal(dev, host)
+    tol = 2e-5 * np.abs(b * tod_w) + 3e-7 * (np.abs(a) + np.abs(b * tod_w))
+    assert np.all(np.abs(dev.astype(np.float64) - ref) <= tol)
