@@ -70,27 +70,41 @@ constexpr int kTcAPartBytes = kTcBM * 128;                  // 16 KB (hi or lo p
 constexpr int kTcAStageBytes = 2 * kTcAPartBytes;           // 32 KB
 constexpr int kTcEpiWarps = 4, kTcGenWarps = 16;
 // warp roles, aligned to warpgroups of 4 warps so that setmaxnreg can move registers between them:
-//   WG0 = warps 0-3 flush (tensor-memory lane quarter = warp), WG1-4 = generators, WG5 = finishers,
-//   WG6 = 2 idle, loader, MMA.  Generators (4 warps per scheduler: the per-element dependency chain lg2 -> ex2 -> split
-//   only fills the issue slots with thread-level parallelism), WG6 = finishers.  The kernel starts
-//   with 72 registers per thread (896 threads); setmaxnreg can only redistribute that pool:
-//   128 x (56 + 40 + 4*80 + 88) = 128 x 7*72.
+//   WG0 = warps 0-3 flush (tensor-memory lane quarter = warp), WG1-4 = generators (4 warps per scheduler: the
+//   per-element dependency chain lg2 -> ex2 -> split only fills the issue slots with thread-level parallelism),
+//   WG5-6 = finishers (two warps per scheduler: the ten dependent Philox rounds of one warp leave its scheduler
+//   idle, measured 9.87 -> 9.45 ms on a 16 000-sample C4 launch against one finisher warpgroup with 88 registers),
+//   WG7 = 2 idle, loader, MMA.  The kernel starts with 64 registers per thread (1024 threads); setmaxnreg can only
+//   redistribute that pool: 128 x (56 + 4*80 + 2*48 + 40) = 128 x 8*64.  GT_TC_FIN_WARPS = 4 is the earlier
+//   896-thread layout (72 registers at start, one finisher warpgroup with 88).
 // The warp scheduler favours the highest warp id among eligible warps: the two single-thread control
 // roles sit in the LAST warpgroup so that the MMA issue stream is never starved by generator warps.
 constexpr int kTcWarpGen0 = 4;
 constexpr int kTcRowsPerThread = kTcBM / (4 * kTcGenWarps), kTcRowStride = 4 * kTcGenWarps;   // 2 rows, 64 apart
-constexpr int kTcFinWarps = 4, kTcWarpFin0 = kTcWarpGen0 + kTcGenWarps;            // 20
-constexpr int kTcWarpCtl0 = kTcWarpFin0 + kTcFinWarps;                              // 24
-constexpr int kTcWarpLoader = kTcWarpCtl0 + 2, kTcWarpMma = kTcWarpCtl0 + 3;        // 26, 27
-constexpr int kTcThreads = 32 * (kTcWarpCtl0 + 4);                                  // 896
+#ifndef GT_TC_FIN_WARPS
+#define GT_TC_FIN_WARPS 8
+#endif
+constexpr int kTcFinWarps = GT_TC_FIN_WARPS, kTcWarpFin0 = kTcWarpGen0 + kTcGenWarps;   // 4 or 8 finisher warps from warp 20
+static_assert(kTcFinWarps == 4 || kTcFinWarps == 8, "finishers fill whole warpgroups");
+constexpr int kTcWarpCtl0 = kTcWarpFin0 + kTcFinWarps;                              // 24 (28)
+constexpr int kTcWarpLoader = kTcWarpCtl0 + 2, kTcWarpMma = kTcWarpCtl0 + 3;        // 26, 27 (30, 31)
+constexpr int kTcThreads = 32 * (kTcWarpCtl0 + 4);                                  // 896 (1024)
+constexpr int kTcRegsBase = (65536 / kTcThreads) / 8 * 8;                           // 72 (64): registers per thread at kernel start
 #ifndef GT_TC_REGS_FLUSH
 #define GT_TC_REGS_FLUSH 56
 #endif
 #ifndef GT_TC_REGS_FIN
-#define GT_TC_REGS_FIN 88
+#define GT_TC_REGS_FIN (GT_TC_FIN_WARPS == 8 ? 48 : 88)
+#endif
+// finisher: channels in flight per lane, and whether the next row's partial sums are fetched a row ahead
+#ifndef GT_TC_FIN_W
+#define GT_TC_FIN_W (GT_TC_FIN_WARPS == 8 ? 3 : 4)
+#endif
+#ifndef GT_TC_FIN_PREFETCH
+#define GT_TC_FIN_PREFETCH (GT_TC_FIN_WARPS == 8 ? 0 : 1)
 #endif
 constexpr int kTcRegsFlush = GT_TC_REGS_FLUSH, kTcRegsCtl = 40, kTcRegsGen = 80, kTcRegsFin = GT_TC_REGS_FIN;
-static_assert(kTcRegsFlush + kTcRegsCtl + 4 * kTcRegsGen + kTcRegsFin <= 7 * 72, "setmaxnreg pool");
+static_assert(kTcRegsFlush + kTcRegsCtl + 4 * kTcRegsGen + (kTcFinWarps / 4) * kTcRegsFin <= (kTcThreads / 128) * kTcRegsBase, "setmaxnreg pool");
 constexpr int kTcMaxGroupChan = 384;       // channels per tile: 3 column groups of 128 (+ 1 spare buffer = 512 columns)
 constexpr int kTcBufCols = 128, kTcNumBuf = 4, kTcMaxCg = 3;
 constexpr int kTcSegDefault = 8;           // slabs (of 64 frequencies) per accumulation segment
@@ -681,7 +695,7 @@ fused_tc_kernel(const TcParams p) {
       }
     } else if (warp >= kTcWarpFin0 && warp < kTcWarpCtl0) {
         // ============ finisher: scratch tile -> P = sum*scale + bias, photon noise -> TOD ========
-        if constexpr (kTcRegsFin > 72) ptx::setmaxnreg_inc<kTcRegsFin>(); else if constexpr (kTcRegsFin < 72) ptx::setmaxnreg_dec<kTcRegsFin>();
+        if constexpr (kTcRegsFin > kTcRegsBase) ptx::setmaxnreg_inc<kTcRegsFin>(); else if constexpr (kTcRegsFin < kTcRegsBase) ptx::setmaxnreg_dec<kTcRegsFin>();
         const int q = warp - kTcWarpFin0;
         uint32_t ti = 0;
         for (int64_t tl = worker; tl < n_tiles; tl += n_workers, ++ti) {
@@ -694,25 +708,37 @@ fused_tc_kernel(const TcParams p) {
             const float* sc = p.scratch + ((size_t)blockIdx.x * 2 + sb) * p.nb_tot * kTcBM;
             ptx::mbar_wait_relaxed(sm.tile_done + 8 * sb, (ti >> 1) & 1u);
             constexpr int kMaxPerLane = kTcMaxGroupChan / 32;             // 12
-            float x[kMaxPerLane], xn[kMaxPerLane];
+            constexpr bool kPrefetch = GT_TC_FIN_PREFETCH != 0;
+            float x[kMaxPerLane], xn[kPrefetch ? kMaxPerLane : 1];
+            if constexpr (kPrefetch) {
 #pragma unroll
-            for (int j = 0; j < kMaxPerLane; ++j) {
-                const int c = lane + 32 * j;
-                xn[j] = c < n_valid ? __ldcg(sc + tc_scratch_index(c, q)) : 0.f;
+                for (int j = 0; j < kMaxPerLane; ++j) {
+                    const int c = lane + 32 * j;
+                    xn[j] = c < n_valid ? __ldcg(sc + tc_scratch_index(c, q)) : 0.f;
+                }
             }
             for (int r = q; r < kTcBM; r += kTcFinWarps) {
                 const int64_t t = tb * kTcBM + r;                         // sample of this row within the launch
                 if (t >= n_t || GT_DIAG(p, 8)) break;
                 const uint32_t n = (uint32_t)(f.t0 + t);
                 float* o = f.out + (size_t)(t * f.n_spaxel + s) * f.n_chan + cg0;
-                // this row's partial sums were fetched during the previous row; fetch the next row's now
+                if constexpr (kPrefetch) {
+                    // this row's partial sums were fetched during the previous row; fetch the next row's now
 #pragma unroll
-                for (int j = 0; j < kMaxPerLane; ++j) {
-                    x[j] = xn[j];
-                    const int c = lane + 32 * j;
-                    xn[j] = (c < n_valid && r + kTcFinWarps < kTcBM) ? __ldcg(sc + tc_scratch_index(c, r + kTcFinWarps)) : 0.f;
+                    for (int j = 0; j < kMaxPerLane; ++j) {
+                        x[j] = xn[j];
+                        const int c = lane + 32 * j;
+                        xn[j] = (c < n_valid && r + kTcFinWarps < kTcBM) ? __ldcg(sc + tc_scratch_index(c, r + kTcFinWarps)) : 0.f;
+                    }
+                } else {
+                    // all of this row's partial sums are requested at once; the other finisher warp of the scheduler covers the latency
+#pragma unroll
+                    for (int j = 0; j < kMaxPerLane; ++j) {
+                        const int c = lane + 32 * j;
+                        x[j] = c < n_valid ? __ldcg(sc + tc_scratch_index(c, r)) : 0.f;
+                    }
                 }
-                constexpr int W = 4;                                      // channels in flight per lane
+                constexpr int W = GT_TC_FIN_W;                            // channels in flight per lane
 #pragma unroll
                 for (int j0 = 0; j0 < kMaxPerLane; j0 += W) {
                     if (lane + 32 * j0 >= n_valid) break;
