@@ -185,6 +185,67 @@ def test_pink_series_windows_are_consistent():
     assert np.array_equal(full[:, 217:517], part)
 
 
+# ---- the J > 4 branch: stages 4-7 draw from Philox stream 2 (gateau_oracle.cpp pink_series, R19) ----
+def _pink8_workload(n_samples, n_chan):
+    """Eight corners an octave apart, 16 ... 0.125 Hz: every stage carries power inside the Welch band, so a slip
+    in the second stream (stages 4-7 re-using stream 1, or the wrong normals of stream 2) shows in the PSD."""
+    w = _pink_workload(J=8, n_samples=n_samples, n_chan=n_chan)
+    return w.replace(pink_f_corner_hz=16.0 * 2.0 ** (-np.arange(8, dtype=np.float64)))
+
+
+def test_pink_eight_stages_psd_and_variance():
+    """Welch PSD of the J = 8 cascade against the exact discrete-time sum of EIGHT independent unit-variance AR(1)
+    spectra, and the ensemble variance against sum g_j^2.  Correlated stages (x_{j+4} driven by the innovations of
+    x_j) would add the cross spectra 2 g_j g_{j+4} Re(H_j H*_{j+4}): tens of per cent here."""
+    w = _pink8_workload(1 << 16, 128)
+    o = O.Oracle(w)
+    nd, fs = w.n_chan, w.f_sample_hz
+    x = o.pink_series(np.zeros(nd, np.int32), np.arange(nd, dtype=np.int32), 0, w.n_samples)
+    phi, g = o.pink_coeffs(0, 0)
+    assert phi.shape == (8,) and g.shape == (8,)
+    np.testing.assert_allclose(phi, np.exp(-2 * np.pi * w.pink_f_corner_hz / fs), rtol=1e-15)
+    np.testing.assert_allclose(g ** 2, 2.5e-34 * math.log(2.0) * np.ones(8), rtol=1e-12)     # alpha = 1, rho = 2
+    f, pxx = signal.welch(x, fs=fs, nperseg=4096, axis=1)
+    pxx = pxx.mean(axis=0)
+
+    def H2(p):
+        return (2 / fs) * (1 - p * p) / (1 - 2 * p * np.cos(2 * np.pi * f / fs) + p * p)
+
+    exact = sum(gj ** 2 * H2(p) for gj, p in zip(g, phi))
+    band = (f > 0.2) & (f < 60)
+    n_avg = nd * (w.n_samples // 2048 - 1)
+    tol = 6 / math.sqrt(n_avg) + 0.03
+    assert np.abs(pxx[band] / exact[band] - 1).max() < tol
+    # what the test would see if stages j and j+4 shared their innovations: far outside the tolerance
+    z = np.exp(-2j * np.pi * f / fs)
+    shared = exact + sum(2 * g[j] * g[j + 4] * (2 / fs) * math.sqrt((1 - phi[j] ** 2) * (1 - phi[j + 4] ** 2))
+                         * np.real(1 / ((1 - phi[j] * z) * np.conj(1 - phi[j + 4] * z))) for j in range(4))
+    assert np.abs(shared[band] / exact[band] - 1).min() > 3 * tol
+    # every stage is stationary with unit variance from n = 0 on: ensemble variance at fixed times
+    v = x[:, ::1024].var(axis=0).mean()
+    assert v == pytest.approx(float(np.sum(g ** 2)), rel=0.08)
+
+
+def test_pink_eight_stages_two_streams_by_hand():
+    """The series rebuilt from the pinned Philox normals: stages 0-3 take the four normals of stream 1, stages 4-7
+    those of stream 2, initial states from counter 0xFFFFFFFF (R19).  The two halves are also uncorrelated."""
+    w = _pink8_workload(4096, 3)
+    o = O.Oracle(w)
+    n, ch = w.n_samples, 2
+    got = o.pink_series(np.zeros(1, np.int32), np.array([ch], dtype=np.int32), 0, n)[0]
+    phi, g = o.pink_coeffs(0, ch)
+    z = np.concatenate([O.normals_bulk(w.seed, 0, n, 0, ch, 1), O.normals_bulk(w.seed, 0, n, 0, ch, 2)], axis=1)
+    x = np.concatenate([O.normals4(w.seed, 0xFFFFFFFF, 0, ch, 1), O.normals4(w.seed, 0xFFFFFFFF, 0, ch, 2)])
+    xs = np.empty((n, 8))
+    for i in range(n):
+        x = phi * x + np.sqrt(1 - phi * phi) * z[i]
+        xs[i] = x
+    np.testing.assert_allclose(got, xs @ g, rtol=0, atol=1e-12 * np.abs(got).max())
+    # innovations of the two streams are independent draws
+    c = np.corrcoef(z.T)
+    assert np.abs(c[:4, 4:]).max() < 5 / math.sqrt(n)
+
+
 # ---- Timmer & Koenig pink noise (the paper's own method, PAPER.md:223; DESIGN.md R21) ----
 def _tk_workload(n_samples, n_chan=6, alpha=1.0, seed=5):
     from paper_2604_23305_b200 import workloads as W
