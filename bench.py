@@ -44,6 +44,10 @@ def parse():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    ap.add_argument("--peak-seconds", type=float, default=4.0, help="length of the sustained matmul runs that measure the tensor peaks")
+    ap.add_argument("--no-peaks", action="store_true", help="skip the in-run measurement of the TF32 / fp16 / FP32 / PCIe denominators")
+    ap.add_argument("--no-extras", action="store_true", help="skip the timing lines of the paper's own options (rows f1-f3)")
+    ap.add_argument("--timeline", default=None, help="write the per-chunk compute / D2H timeline of one end-to-end step to this file")
     return ap.parse_args()
 
 
@@ -171,6 +175,54 @@ def peaks():
         "fallback (B200_PROFILING.md)"
 
 
+def measure_peaks(torch, B, dev, seconds):
+    """The denominators SURVEY 8d asks to MEASURE, in this run and on this GPU: dense fp16 and TF32 matmul 8192^3
+    (torch / cuBLAS is fine for a measurement: burst = best of 10, sustained = back to back for `seconds`), the FP32 FMA
+    peak (the library's register-only loop), and the host link (1 GiB pinned cudaMemcpyAsync, both directions)."""
+    out = {}
+    n = 8192
+    old = torch.backends.cuda.matmul.allow_tf32
+    for name, dt, tf32 in (("f16", torch.float16, False), ("tf32", torch.float32, True)):
+        torch.backends.cuda.matmul.allow_tf32 = tf32
+        a = torch.randn((n, n), device=dev, dtype=dt); b = torch.randn((n, n), device=dev, dtype=dt)
+        c = torch.empty((n, n), device=dev, dtype=dt)
+        for _ in range(3):
+            torch.matmul(a, b, out=c)
+        torch.cuda.synchronize()
+        best = 0.0
+        for _ in range(10):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); torch.matmul(a, b, out=c); e1.record(); e1.synchronize()
+            best = max(best, 2.0 * n ** 3 / (e0.elapsed_time(e1) * 1e-3) / 1e12)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        k, t0 = 0, time.perf_counter()
+        e0.record()
+        while time.perf_counter() - t0 < seconds:
+            for _ in range(20):
+                torch.matmul(a, b, out=c)
+            k += 20
+            torch.cuda.synchronize()
+        e1.record(); e1.synchronize()
+        out[f"peak_{name}_measured"] = best
+        out[f"peak_{name}_sustained_measured"] = 2.0 * n ** 3 * k / (e0.elapsed_time(e1) * 1e-3) / 1e12
+        del a, b, c
+    torch.backends.cuda.matmul.allow_tf32 = old
+    out["peak_fp32_fma_measured"] = B.measure_fp32_fma()
+    nb = 1 << 30
+    host = torch.empty(nb, dtype=torch.uint8, pin_memory=True); devb = torch.empty(nb, dtype=torch.uint8, device=dev)
+    for name, src, dst in (("d2h", devb, host), ("h2d", host, devb)):
+        rates = []
+        for _ in range(10):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); dst.copy_(src, non_blocking=True); e1.record(); e1.synchronize()
+            rates.append(nb / (e0.elapsed_time(e1) * 1e-3) / 1e9)
+        out[f"pcie_{name}_gbs"] = float(np.median(rates[1:]))
+    del host, devb
+    out["how"] = (f"torch.matmul {n}^3 fp16 and TF32 (allow_tf32): best of 10 and back to back for {seconds:g} s; FP32: "
+                  "gt_measure_fp32_fma (register-only FMA loop); PCIe: median of 9 pinned 1 GiB copies per direction")
+    return out
+
+
 def ncu_traffic(kernel, rows_per_launch):
     """DRAM bytes per launch of the dominant kernel from the committed ncu capture (profiles/*_traffic.csv),
     scaled by rows when bench's launch size differs from the captured one; None if there is no capture."""
@@ -240,23 +292,37 @@ def run_ours(args):
     flops_per_launch = 2.0 * w.n_chan * w.n_freq * (w.n_samples * w.n_spaxel) / max(fused_n / args.steps, 1)
     avg_launch_s = fused_ms * 1e-3 / max(fused_n, 1)
     achieved = flops_per_launch / avg_launch_s / 1e12
+    measured = {}
+    if not args.no_peaks and rank == 0 and world == 1:
+        try:
+            measured = measure_peaks(torch, B, f"cuda:{local}", args.peak_seconds)
+        except Exception as ex:                                   # report, never fake
+            measured = {"error": repr(ex)[:200]}
     if plan.variant_name.startswith("tcgen05"):
-        peak = 0.5 * pk["bf16_tflops_sustained"]          # kernel timed inside a long step: sustained figure
+        peak = pk["bf16_tflops_sustained"]                # the MMAs run as kind::f16 (fp16 rate = bf16 rate); kernel timed inside a long step: sustained figure
         roof = {"bound": "tensor", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                 "traffic": None, "kernel": "fused_tc_kernel",
-                "peak_source": f"TF32-class dense = 0.5 x bf16 sustained, {pk_src}", "peak_burst": 0.5 * pk["bf16_tflops"],
+                "peak_source": f"dense fp16/bf16 sustained (the dtype the MMAs run in), {pk_src}", "peak_burst": pk["bf16_tflops"],
                 "mma_dtype": "f16 (three-term split of fp32 operands, fp32 accumulate)",
-                "issued_tflops": 3 * achieved, "issued_peak": pk["bf16_tflops_sustained"],
-                "issued_frac": 3 * achieved / pk["bf16_tflops_sustained"],
-                "note": "achieved = algorithmic 2*n_chan*n_freq flop/row against the TF32-class peak the metric names; the "
-                        "split issues 3 fp16 products per useful one (hi*hi + lo*hi + hi*lo as kind::f16 K=16 MMAs): "
-                        "issued_* counts those against the measured fp16/bf16 peak"}
+                "issued_tflops": 3 * achieved, "issued_frac": 3 * achieved / peak,
+                "tf32_class_peak": measured.get("peak_tf32_sustained_measured") or 0.5 * peak,
+                "tf32_class_peak_source": "measured in this run (torch TF32 matmul, sustained)" if measured.get("peak_tf32_sustained_measured")
+                                          else "0.5 x fp16/bf16 sustained (nominal ratio)",
+                "note": "achieved = algorithmic (useful) 2*n_chan*n_freq flop/row; frac = useful / fp16 peak: a three-term split can "
+                        "reach at most 1/3.  issued_* counts the 3 fp16 products the split issues per useful one (hi*hi + lo*hi + "
+                        "hi*lo as kind::f16 K=16 MMAs).  tf32_class_frac = useful flop against the TF32 dense peak, the "
+                        "denominator north_star names (a genuine 3xTF32 kernel could reach 1/3 of it, this one up to 2/3)"}
+        roof["tf32_class_frac"] = achieved / roof["tf32_class_peak"]
     else:
         mhz = clocks.get("sm_mhz") or pk.get("sm_max_mhz", 1965.0)
-        peak = 148 * 128 * 2 * mhz * 1e6 / 1e12
+        peak = measured.get("peak_fp32_fma_measured") or 148 * 128 * 2 * mhz * 1e6 / 1e12
         roof = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                 "traffic": None, "kernel": "fused_fp32_kernel",
-                "peak_source": f"FP32 FMA = 148 SM x 128 lanes x 2 x {mhz:.0f} MHz (median SM clock under load)"}
+                "peak_source": "FP32 FMA measured in this run (gt_measure_fp32_fma)" if measured.get("peak_fp32_fma_measured")
+                               else f"FP32 FMA = 148 SM x 128 lanes x 2 x {mhz:.0f} MHz (median SM clock under load)"}
+    roof.update({k: v for k, v in measured.items() if k.startswith("peak_")})
+    if measured.get("how"):
+        roof["measured_how"] = measured["how"]
     roof["traffic"], roof["traffic_source"] = ncu_traffic(roof["kernel"], (w.n_samples * w.n_spaxel) / max(fused_n / args.steps, 1))
     roof["fused_ms_per_step"] = fused_ms / args.steps
     roof["fused_share_of_step"] = fused_ms / total_ms if world == 1 else None
@@ -265,11 +331,24 @@ def run_ours(args):
     e2e = None
     if not args.no_e2e:
         try:
-            e2e = run_e2e(torch, B, w, variant, local, world, max(1, min(args.steps, 3)), barrier)
+            e2e = run_e2e(torch, B, w, variant, local, world, max(1, min(args.steps, 3)), barrier, args.timeline if rank == 0 else None)
+            if measured.get("pcie_d2h_gbs"):
+                e2e["pcie_gbs"] = measured["pcie_d2h_gbs"]
+                e2e["pcie_h2d_gbs"] = measured["pcie_h2d_gbs"]
+                e2e["achieved_d2h_gbs"] = e2e["d2h_bytes_per_step"] / (e2e["ms_per_step"] * 1e-3) / 1e9
+                e2e["frac_of_pcie"] = e2e["achieved_d2h_gbs"] / measured["pcie_d2h_gbs"]
         except Exception as ex:                                   # report, never fake
             e2e = {"value": None, "unit": UNIT, "error": repr(ex)[:200]}
+    extras = None
+    if rank == 0 and world == 1 and not args.no_extras and not args.samples:
+        try:
+            extras = run_extras(torch, B, w, local, tod)
+        except Exception as ex:
+            extras = {"error": repr(ex)[:200]}
 
+    variant_name = plan.variant_name
     plan.destroy()
+    del tod
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cpu, _, _ = oracle_sample(w, args.cpu_seconds)
@@ -277,8 +356,10 @@ def run_ours(args):
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-                "config": workload_config(w, {"variant": plan_variant_name(args, roof), "parallelism": f"replica x{world}"}),
+                "config": workload_config(w, {"variant": variant_name, "parallelism": f"replica x{world}"}),
                 "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roof, "cpu_baseline": cpu}
+        if extras:
+            line["options"] = extras
         if args.samples:
             line["invalid"] = "--samples shrinks the workload: debug only"
         print(json.dumps(line))
@@ -286,11 +367,31 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
-def plan_variant_name(args, roof):
-    return "tcgen05-3xf16-split" if roof["bound"] == "tensor" else "fp32-ffma"
+def run_extras(torch, B, w, local, tod):
+    """Device-resident step times of the paper's own options (rows f1-f3), same workload: one warm-up + two timed steps."""
+    out = {}
+    dev = f"cuda:{local}"
+    for name, kw in (("f1_exact_photon_noise_eq17", dict(photon_mode=1)),
+                     ("f2_kelvin_output", dict(output_unit=1, skydip_pwv_lo_mm=0.6, skydip_pwv_hi_mm=1.4)),
+                     ("f3_timmer_koenig_pink", dict(pink_method=1))):
+        t0 = time.perf_counter()
+        p = B.Plan(w.replace(**kw), device=dev)
+        torch.cuda.synchronize()
+        create_ms = 1e3 * (time.perf_counter() - t0)
+        p.simulate(out=tod)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(2):
+            p.simulate(out=tod)
+        e1.record(); e1.synchronize()
+        ms = e0.elapsed_time(e1) / 2
+        out[name] = {"ms_per_step": ms, "value": w.detector_samples() / (ms * 1e-3), "unit": UNIT, "plan_create_ms": create_ms}
+        p.destroy()
+        torch.cuda.empty_cache()
+    return out
 
 
-def run_e2e(torch, B, w, variant, local, world, steps, barrier):
+def run_e2e(torch, B, w, variant, local, world, steps, barrier, timeline=None):
     """Public API from HOST buffers: per step, pinned inputs -> device, gt_plan_create,
     gt_simulate streaming the TOD into pinned host memory, gt_plan_destroy."""
     dev = f"cuda:{local}"
@@ -305,13 +406,37 @@ def run_e2e(torch, B, w, variant, local, world, steps, barrier):
     # the workload's large arrays now live in pinned host memory (views of the pinned tensors)
     wp = w.replace(**{k: v.numpy() for k, v in host.items()})
 
-    def one():
-        # B.Plan copies the pinned arrays to the device (H2D) and creates the plan; simulate streams to `out`
-        p = B.Plan(wp, variant=variant, device=dev)
-        p.simulate(out=out)
-        p.destroy()
+    parts = {"h2d_and_create_ms": 0.0, "simulate_ms": 0.0, "destroy_ms": 0.0}
 
-    one()                                                        # warm-up (allocators, pinned pages)
+    def one(record=None):
+        # B.Plan copies the pinned arrays to the device (H2D) and creates the plan; simulate streams to `out`
+        t0 = time.perf_counter()
+        p = B.Plan(wp, variant=variant, device=dev)
+        t1 = time.perf_counter()
+        p.simulate(out=out)
+        t2 = time.perf_counter()
+        if record:
+            tl = p.timeline()
+            with open(record, "w") as f:
+                f.write("# per-chunk device timeline of one end-to-end gt_simulate into pinned host memory (gt_debug_timeline):\n"
+                        "# ms after the first chunk's compute begin; compute = geometry + fused + pink kernels on the caller's stream,\n"
+                        "# copy = cudaMemcpyAsync D2H of that chunk on the plan's side stream\n"
+                        f"# command: python bench.py --steps 1 --warmup 3 --timeline {record}\n"
+                        f"# workload: {w.name}, {tl.shape[0]} chunks of {p.chunking()[0]} samples, {out.numel() * 4 / tl.shape[0] / 1e6:.0f} MB each\n"
+                        "# chunk compute_begin compute_end copy_begin copy_end  copy_GB/s  copy_overlaps_next_compute\n")
+                per = out.numel() * 4 / tl.shape[0]
+                for k, r in enumerate(tl):
+                    ov = "yes" if k + 1 < tl.shape[0] and r[2] < tl[k + 1][1] and r[3] > tl[k + 1][0] else ("-" if k + 1 == tl.shape[0] else "no")
+                    f.write(f"{k:4d} {r[0]:9.3f} {r[1]:9.3f} {r[2]:9.3f} {r[3]:9.3f} {per / max(r[3] - r[2], 1e-6) / 1e6:8.1f}  {ov}\n")
+                f.write(f"# compute busy {sum(r[1] - r[0] for r in tl):.1f} ms, copy busy {sum(r[3] - r[2] for r in tl):.1f} ms, "
+                        f"span {tl[-1][3]:.1f} ms\n")
+        p.destroy()
+        t3 = time.perf_counter()
+        parts["h2d_and_create_ms"] += 1e3 * (t1 - t0); parts["simulate_ms"] += 1e3 * (t2 - t1); parts["destroy_ms"] += 1e3 * (t3 - t2)
+
+    one(record=timeline)                                         # warm-up (allocators, pinned pages)
+    for k in parts:
+        parts[k] = 0.0
     barrier()
     t0 = time.perf_counter()
     for _ in range(steps):
@@ -325,6 +450,7 @@ def run_e2e(torch, B, w, variant, local, world, steps, barrier):
     dt = float(t.item())
     return {"value": world * w.detector_samples() * steps / dt, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
             "d2h_bytes_per_step": int(d2h), "ms_per_step": 1e3 * dt / steps, "steps": steps,
+            "breakdown_ms_per_step": {k: v / steps for k, v in parts.items()},
             "what": "host arrays -> H2D -> gt_plan_create -> gt_simulate into pinned host TOD (chunked D2H on a side stream) -> gt_plan_destroy"}
 
 

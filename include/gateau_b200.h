@@ -126,7 +126,23 @@ typedef struct {
        kid_gap_J = Delta_Al (188 micro-eV in the paper, :103), eta_pb = pair-breaking efficiency (0.4). */
     int32_t photon_mode;
     double kid_gap_J, eta_pb;
+    /* Global index of this plan's spaxel 0 (default 0).  A plan may hold a sub-range of an instrument's spaxels
+       (spaxel-sharded runs): the Philox counter word 1 is spaxel_index_base + s, so that the shard
+       reproduces the TOD of the same spaxels in a plan that holds them all, bit for bit.  >= 0. */
+    int32_t spaxel_index_base;
 } gt_config;
+
+/* Value ranges (tensor variant).  The fused kernel contracts fp16 (hi, lo) operand pairs:
+ *   - filt: any finite values (negative lobes of an Eq. 7 filterbank included).  Every channel is scaled by its own
+ *     power of two, so a delta filter 1/dnu, a row-normalised filter and a transmission of peak 1 are equally accurate;
+ *     inside one channel, values below 2^-39 of the channel's largest are rounded to multiples of 2^-39 of it.
+ *   - spectrum: the plan takes the largest element it can meet (max over nu of |(B_atm - B_cmb) prod eta_k| and
+ *     |eta_front prod eta_k| max |cube|, one device reduction over the cube) and scales by a power of two; elements
+ *     below 2^-36 of that maximum are rounded to multiples of it.  NaN / Inf in cube, screen, filt, LUT or the
+ *     per-frequency efficiencies: GT_ERR_VALUE.  A spectrum whose scale leaves the fp32 range: GT_ERR_RANGE.
+ * Threads and streams: a plan owns one set of work buffers.  It may be used by one thread and one stream at a time;
+ * calls on the same plan must be ordered by the caller (same stream, or events).  A plan belongs to the device that was
+ * current at gt_plan_create; calling it with another device current returns GT_ERR_VALUE. */
 
 /* Per-row geometry record returned by gt_debug_geometry: the integers are the quantities
  * "index, scan and RNG counters" that must match the oracle bit for bit. */
@@ -161,17 +177,10 @@ gt_status gt_plan_create(const gt_config* cfg, void* cuda_stream, gt_plan** out_
 gt_status gt_simulate(gt_plan* plan, int64_t t_begin, int64_t t_count,
                       float* tod_out, float* pwv_out, void* cuda_stream);
 
-/* Frees everything the plan owns.  NULL-safe. */
+/* Frees everything the plan owns, after waiting for the work the plan itself enqueued (the stream of its last call
+ * and its internal copy stream).  NULL-safe. */
 gt_status gt_plan_destroy(gt_plan* plan);
 
-/* Pre-processing utility (PAPER.md:84-92, DESIGN.md R24; not part of a plan): turns an extra-path-length screen
- * into the line-of-sight PWV screen that gt_config.screen expects.
- *   pwv[y][x] = pwv0_mm + (1 / 6.587) sum_{i,j} K[j][i] epl[(y + j) mod ny][(x + i) mod nx]      (Eq. 4, then :92)
- * K = the aperture footprint on the screen grid: 10^(-|t_edge_db| / 20 * r^2 / R_tel^2) for r < R_tel (the Gaussian
- * illumination of Eq. 2 with the given edge taper), 0 outside, r^2 = (i dx)^2 + (j dy)^2, normalised to unit sum.
- * epl_dev, pwv_dev: DEVICE [ny][nx] fp32, distinct buffers, caller-owned.  Asynchronous on cuda_stream.
- * GT_ERR_SHAPE for non-positive sizes, GT_ERR_VALUE for non-positive dx, dy, R_tel,
- * GT_ERR_UNSUPPORTED if R_tel spans more than 64 pixels in x or y. */
 /* Pre-processing utility (R25; not part of a plan): turns a specific-intensity cube
  * I_nu [W m^-2 Hz^-1 sr^-1] into the spectral power cube P_nu,src [W/Hz] that gt_config.cube expects.
  *   F_nu(rho) = |int_0^R A(r) J0(2 pi r rho / lambda) r dr|^2 / F_nu(0)        the far field of the circular aperture
@@ -186,6 +195,15 @@ gt_status gt_plan_destroy(gt_plan* plan);
 gt_status gt_prepare_source(const float* I_dev, int32_t n_az, int32_t n_el, int32_t n_freq, double nu0_hz, double dnu_hz,
                             double daz_rad, double del_rad, double el_first_rad, double R_tel_m, double t_edge_db,
                             int32_t r_pix, float* P_dev, void* cuda_stream);
+/* Pre-processing utility (PAPER.md:84-92, DESIGN.md R24; not part of a plan): turns an extra-path-length screen
+ * into the line-of-sight PWV screen that gt_config.screen expects.
+ *   pwv[y][x] = pwv0_mm + (1 / 6.587) sum_{i,j} K[j][i] epl[(y + j) mod ny][(x + i) mod nx]      (Eq. 4, then :92)
+ * K = the aperture footprint on the screen grid: 10^(-|t_edge_db| / 20 * r^2 / R_tel^2) for r < R_tel (the Gaussian
+ * illumination of Eq. 2 with the given edge taper), 0 outside, r^2 = (i dx)^2 + (j dy)^2, normalised to unit sum.
+ * epl_dev, pwv_dev: DEVICE [ny][nx] fp32, distinct buffers, caller-owned.  Synchronises cuda_stream before returning
+ * (the footprint weights are a temporary of the call).
+ * GT_ERR_SHAPE for non-positive sizes, GT_ERR_VALUE for non-positive dx, dy, R_tel,
+ * GT_ERR_UNSUPPORTED if R_tel spans more than 64 pixels in x or y. */
 gt_status gt_prepare_screen(const float* epl_dev, int32_t nx, int32_t ny, double dx_m, double dy_m,
                             double R_tel_m, double t_edge_db, double pwv0_mm, float* pwv_dev, void* cuda_stream);
 
@@ -208,14 +226,38 @@ gt_status gt_debug_philox(uint64_t seed, uint32_t c0_begin, int64_t count,
  * pink-noise state. */
 gt_status gt_debug_pkid(gt_plan* plan, int64_t t_begin, int64_t t_count,
                         float* pkid_out, void* cuda_stream);
+/* Samples per kernel launch: *host_chunk when the output is host memory (= chunk_samples, or the library's pick),
+ * *device_chunk when it is device memory.  The parity tests place sampled rows on both sides of these seams. */
+gt_status gt_debug_chunking(const gt_plan* plan, int64_t* host_chunk, int64_t* device_chunk);
 /* Number of kernels this library launched since the plan was created. */
 int64_t gt_launch_count(const gt_plan* plan);
+/* Diagnostic counters since plan creation (any pointer may be NULL): rows = (sample, spaxel) pairs the
+ * geometry kernel processed for gt_simulate / gt_debug_pkid; rows_outside_cube = rows whose pointing fell outside the
+ * source cube (they see blank sky); pwv_below_lut / pwv_above_lut = rows whose line-of-sight PWV was
+ * clamped to the first / last row of the lookup table (R13).  Synchronises the plan's last stream. */
+gt_status gt_plan_counters(gt_plan* plan, int64_t* rows, int64_t* rows_outside_cube,
+                           int64_t* pwv_below_lut, int64_t* pwv_above_lut);
+/* Checkpoint / restart at call granularity: everything but the AR(1) pink-noise state is a pure function
+ * of the sample index (counter-based RNG), so a run can be resumed by another plan of the same configuration.
+ *   export: host_state [n_spaxel * n_chan * pink_n_stage] fp32 = x_j of every detector at the last simulated sample
+ *           (detector-major, stage fastest), *next_t = the sample the next gt_simulate must start at.
+ *   import: sets both; the next gt_simulate must start at next_t (1 <= next_t <= n_samples; 0 needs no import).
+ * GT_ERR_UNSUPPORTED unless the plan has pink_noise != 0 with pink_method = 0.  Both synchronise the plan's last stream. */
+gt_status gt_pink_state_export(gt_plan* plan, float* host_state, int64_t* next_t);
+gt_status gt_pink_state_import(gt_plan* plan, const float* host_state, int64_t next_t);
 /* Name of the fused-kernel variant the plan resolved to ("tcgen05-3xf16-split", "fp32-ffma"). */
 const char* gt_variant_name(const gt_plan* plan);
 /* Device time [ms] the fused kernel took in the last gt_simulate / gt_debug_pkid call, summed
  * over its launches (CUDA events on the launching stream); synchronises the stream.  Also
  * returns the number of launches in *n_launches (NULL ok). */
 double gt_last_fused_ms(gt_plan* plan, int32_t* n_launches);
+/* Measurement hooks (bench.py).  gt_debug_timeline: device timeline of the last HOST-output gt_simulate call, per chunk
+ * k < *n_chunks <= capacity: ms_out[4 k + {0,1,2,3}] = {compute begin, compute end, copy begin, copy end} in ms after the
+ * first chunk's compute begin (CUDA events on the compute stream and on the internal copy stream): shows the D2H copy
+ * of chunk k running under the kernels of chunk k+1.  gt_measure_fp32_fma: FP32 FMA peak of the current device in
+ * TFLOP/s from a register-only FMA loop (8 chains per thread, every thread slot resident), best of 5. */
+gt_status gt_debug_timeline(gt_plan* plan, int32_t capacity, int32_t* n_chunks, double* ms_out);
+gt_status gt_measure_fp32_fma(void* cuda_stream, double* tflops_out);
 /* Test hook: the per-channel skydip map T_b = a + b P_KID of a plan with output_unit = 1, copied to the HOST
  * arrays a_out, b_out [n_chan] (double).  GT_ERR_UNSUPPORTED if the plan's output unit is W. */
 gt_status gt_debug_kelvin_map(gt_plan* plan, double* a_out, double* b_out);

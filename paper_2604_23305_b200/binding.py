@@ -21,7 +21,9 @@ VARIANT_DEFAULT, VARIANT_FP32, VARIANT_TENSOR = 0, 1, 2
 
 EXPORTS = ("gt_plan_create", "gt_simulate", "gt_plan_destroy", "gt_last_error", "gt_debug_geometry",
            "gt_debug_philox", "gt_debug_pkid", "gt_launch_count", "gt_variant_name", "gt_last_fused_ms",
-           "gt_debug_kelvin_map", "gt_prepare_screen", "gt_prepare_source")
+           "gt_debug_kelvin_map", "gt_prepare_screen", "gt_prepare_source", "gt_plan_counters",
+           "gt_pink_state_export", "gt_pink_state_import", "gt_debug_chunking", "gt_debug_timeline",
+           "gt_measure_fp32_fma")
 
 
 class GtStage(C.Structure):
@@ -57,6 +59,7 @@ class GtConfig(C.Structure):
         ("output_unit", C.c_int32), ("skydip_n", C.c_int32),
         ("skydip_pwv_lo_mm", C.c_double), ("skydip_pwv_hi_mm", C.c_double),
         ("photon_mode", C.c_int32), ("kid_gap_J", C.c_double), ("eta_pb", C.c_double),
+        ("spaxel_index_base", C.c_int32),
     ]
 
 
@@ -109,6 +112,18 @@ def lib() -> C.CDLL:
                                         C.c_double, C.c_double, C.c_double, C.c_double, C.c_int32, C.c_void_p, C.c_void_p]
         L.gt_debug_kelvin_map.restype = C.c_int
         L.gt_debug_kelvin_map.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.gt_plan_counters.restype = C.c_int
+        L.gt_plan_counters.argtypes = [C.c_void_p] + [C.POINTER(C.c_int64)] * 4
+        L.gt_debug_timeline.restype = C.c_int
+        L.gt_debug_timeline.argtypes = [C.c_void_p, C.c_int32, C.POINTER(C.c_int32), C.c_void_p]
+        L.gt_measure_fp32_fma.restype = C.c_int
+        L.gt_measure_fp32_fma.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
+        L.gt_debug_chunking.restype = C.c_int
+        L.gt_debug_chunking.argtypes = [C.c_void_p, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
+        L.gt_pink_state_export.restype = C.c_int
+        L.gt_pink_state_export.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_int64)]
+        L.gt_pink_state_import.restype = C.c_int
+        L.gt_pink_state_import.argtypes = [C.c_void_p, C.c_void_p, C.c_int64]
         _lib = L
     return _lib
 
@@ -176,6 +191,7 @@ def fill_config(w, dev: dict, keep: dict, variant: int = VARIANT_DEFAULT, chunk_
     c.photon_mode = int(getattr(w, "photon_mode", 0))
     c.kid_gap_J = float(getattr(w, "kid_gap_J", 188e-6 * 1.602176634e-19))
     c.eta_pb = float(getattr(w, "eta_pb", 0.4))
+    c.spaxel_index_base = int(getattr(w, "spaxel_index_base", 0))
     return c
 
 
@@ -245,6 +261,37 @@ class Plan:
         self._check(self.L.gt_debug_kelvin_map(self.handle, C.c_void_p(a.ctypes.data), C.c_void_p(b.ctypes.data)))
         return a, b
 
+    def chunking(self):
+        """gt_debug_chunking: (samples per launch for host output, for device output)."""
+        h, d = C.c_int64(0), C.c_int64(0)
+        self._check(self.L.gt_debug_chunking(self.handle, C.byref(h), C.byref(d)))
+        return int(h.value), int(d.value)
+
+    def timeline(self, capacity=4096):
+        """gt_debug_timeline: [n_chunks, 4] ms = compute begin, compute end, copy begin, copy end of the last host-output call."""
+        n = C.c_int32(0)
+        ms = np.zeros((capacity, 4), dtype=np.float64)
+        self._check(self.L.gt_debug_timeline(self.handle, capacity, C.byref(n), C.c_void_p(ms.ctypes.data)))
+        return ms[:int(n.value)].copy()
+
+    def counters(self) -> dict:
+        """gt_plan_counters: rows processed, rows outside the cube, PWV clamps below / above the LUT."""
+        v = [C.c_int64(0) for _ in range(4)]
+        self._check(self.L.gt_plan_counters(self.handle, *[C.byref(x) for x in v]))
+        return dict(zip(("rows", "rows_outside_cube", "pwv_below_lut", "pwv_above_lut"), (int(x.value) for x in v)))
+
+    def pink_state_export(self):
+        """gt_pink_state_export: (state [n_spaxel * n_chan, J] float32, next_t)."""
+        J = int(np.size(self.w.pink_f_corner_hz))
+        st = np.zeros((self.w.n_spaxel * self.w.n_chan, J), dtype=np.float32)
+        nt = C.c_int64(0)
+        self._check(self.L.gt_pink_state_export(self.handle, C.c_void_p(st.ctypes.data), C.byref(nt)))
+        return st, int(nt.value)
+
+    def pink_state_import(self, state, next_t):
+        st = np.ascontiguousarray(state, dtype=np.float32)
+        self._check(self.L.gt_pink_state_import(self.handle, C.c_void_p(st.ctypes.data), int(next_t)))
+
     # ---- the three calls ----
     def simulate(self, t_begin=0, t_count=None, out=None, pwv_out=None, device_out=True, want_pwv=False):
         """gt_simulate.  `out`: a torch CUDA tensor, a pinned/pageable torch CPU tensor or a
@@ -302,6 +349,15 @@ def _ptr(x):
         return C.c_void_p(x.ctypes.data)
     assert x.is_contiguous()
     return C.c_void_p(x.data_ptr())
+
+
+def measure_fp32_fma() -> float:
+    """gt_measure_fp32_fma: FP32 FMA peak of the current device, TFLOP/s."""
+    v = C.c_double(0.0)
+    st = lib().gt_measure_fp32_fma(None, C.byref(v))
+    if st != GT_OK:
+        raise GateauError(st, lib().gt_last_error(None).decode())
+    return float(v.value)
 
 
 def debug_philox(seed, c0_begin, count, c1=0, c2=0, c3=0) -> np.ndarray:

@@ -25,14 +25,18 @@
 #include "gt_photon_exact.cuh"
 #include "gt_screen.cuh"
 #include "gt_beam.cuh"
+#include "gt_reduce.cuh"
+#include "gt_measure.cuh"
 #include <cufft.h>
 
 namespace {
 
 // CODATA exact values (PAPER.md names h, k_B implicitly through P^JN; R4)
 constexpr double kH = 6.62607015e-34, kKB = 1.380649e-23, kPi = 3.14159265358979323846;
-constexpr double kPref = kKB * 300.0 / gt::kTcScaleA;   // spectrum scale: kernels work on P_nu / kPref = O(256), the range the
-                                                        // tensor kernel's fp16 operand split wants (exact power of two on top of k_B 300 K)
+// Spectrum scale: the kernels work on P_nu / p_ref with p_ref = k_B 300 K 2^-e, e chosen per plan so that the largest
+// element the generator can produce lands just below 2^kTcAMaxLog2, the range the tensor kernel's fp16 operand split
+// wants.
+constexpr double kPref0 = kKB * 300.0;
 
 thread_local std::string g_create_error = "";
 
@@ -65,8 +69,11 @@ struct gt_plan {
     int32_t n_freq = 0, n_freq_pad = 0, n_chan = 0, n_chan_pad = 0, n_spaxel = 0, n_pwv = 0, J = 0;
     int64_t n_samples = 0, chunk_samples = 0, chunk_dev = 0;      // samples per launch: host-output chunks / device output
     int32_t photon_noise = 0, pink_noise = 0, variant = GT_VARIANT_FP32;
+    int32_t spaxel_base = 0;         // global index of spaxel 0 of this plan (Philox counter word 1)
+    int device = 0;
     uint64_t seed = 0;
     float scale = 0.f;
+    double p_ref = kPref0;           // W/Hz per unit of the generated spectrum
     // borrowed
     const float* cube = nullptr; int32_t n_az = 0, n_el = 0;
     // geometry
@@ -101,9 +108,15 @@ struct gt_plan {
     cudaStream_t copy_stream = nullptr;
     cudaEvent_t ev_ready[2] = {nullptr, nullptr}, ev_copied[2] = {nullptr, nullptr};
     std::vector<cudaEvent_t> ev_fused;       // start/stop pairs of the last call
+    std::vector<cudaEvent_t> ev_tl;          // host-output calls: per chunk {compute begin, compute end, copy begin, copy end} (timing enabled)
+    int32_t n_tl_last = 0;
     int32_t n_fused_last = 0;
     int64_t launches = 0;
     int num_sms = 148;
+    // diagnostics (SURVEY section 5 "Metrics"): rows seen by the geometry kernel, rows outside the cube, PWV clamps
+    DevBuf<unsigned long long> d_counters;   // [3] outside cube, PWV below / above the LUT
+    int64_t rows_done = 0;
+    cudaStream_t last_stream = nullptr;
     std::string error;
 };
 
@@ -137,6 +150,24 @@ gt_status validate(const gt_config* c) {
         c->n_pwv < 2 || c->n_nu_lut < 2 || c->n_stage < 0 || c->chunk_samples < 0)
         return fail(nullptr, GT_ERR_SHAPE, "a size is non-positive (n_freq/n_samples/n_spaxel/n_chan/nx/ny/n_pwv/n_nu_lut/n_stage)");
     if (c->n_samples > 0xFFFFFFFELL) return fail(nullptr, GT_ERR_SHAPE, "n_samples exceeds the 32-bit Philox counter word");
+    if (c->spaxel_index_base < 0) return fail(nullptr, GT_ERR_VALUE, "spaxel_index_base is negative");
+    {
+        // Eq. 10 needs every line of sight above the horizon: sin(el0 + el[n] + del[s]) > 0 for all n, s
+        double e_lo = c->el_rad[0], e_hi = c->el_rad[0], d_lo = c->del_rad[0], d_hi = c->del_rad[0];
+        bool finite = std::isfinite(c->el0_rad);
+        for (int64_t n = 0; n < c->n_samples; ++n) {
+            finite = finite && std::isfinite(c->az_rad[n]) && std::isfinite(c->el_rad[n]);
+            e_lo = std::min(e_lo, c->el_rad[n]); e_hi = std::max(e_hi, c->el_rad[n]);
+        }
+        for (int s = 0; s < c->n_spaxel; ++s) {
+            finite = finite && std::isfinite(c->daz_rad[s]) && std::isfinite(c->del_rad[s]);
+            d_lo = std::min(d_lo, c->del_rad[s]); d_hi = std::max(d_hi, c->del_rad[s]);
+        }
+        if (!finite) return fail(nullptr, GT_ERR_VALUE, "the scan pattern or the spaxel offsets hold a NaN or Inf");
+        if (!(c->el0_rad + e_lo + d_lo > 0.0) || !(c->el0_rad + e_hi + d_hi < 3.14159265358979323846))
+            return fail(nullptr, GT_ERR_VALUE, "a line of sight is at or below the horizon: el0 + el + del spans [%g, %g] rad",
+                        c->el0_rad + e_lo + d_lo, c->el0_rad + e_hi + d_hi);
+    }
     if (c->n_stage > 0 && !c->stages) return fail(nullptr, GT_ERR_NULL, "stages is NULL with n_stage > 0");
     if (c->cube && (c->n_az < 2 || c->n_el < 2)) return fail(nullptr, GT_ERR_SHAPE, "source cube needs n_az, n_el >= 2");
     if (c->cube && (double)c->n_az * (double)c->n_el * (double)c->n_freq >= 4294967296.0)
@@ -223,9 +254,10 @@ gt_status run_chunk(gt_plan* p, int64_t t0, int64_t T, float* dst, float* pwv_ds
                     cudaStream_t st, int fused_slot) {
     const int64_t n_rows = T * p->n_spaxel;
     if (n_rows == 0) return GT_OK;
-    gt::geometry_kernel<<<(unsigned)((n_rows + 255) / 256), 256, 0, st>>>(p->geo, t0, n_rows, p->d_rows.p, pwv_dst, nullptr);
+    gt::geometry_kernel<<<(unsigned)((n_rows + 255) / 256), 256, 0, st>>>(p->geo, t0, n_rows, p->d_rows.p, pwv_dst, nullptr, p->d_counters.p);
     GT_CUDA(p, cudaGetLastError());
     p->launches++;
+    p->rows_done += n_rows;
 
     gt::FusedParams fp{};
     fp.rows = p->d_rows.p; fp.n_rows = n_rows; fp.t0 = t0;
@@ -237,6 +269,7 @@ gt_status run_chunk(gt_plan* p, int64_t t0, int64_t T, float* dst, float* pwv_ds
     const bool exact = noise && p->photon_noise && p->photon_mode == 1;
     fp.photon_noise = (noise && !exact) ? p->photon_noise : 0;
     fp.seed_lo = (uint32_t)(p->seed & 0xffffffffu); fp.seed_hi = (uint32_t)(p->seed >> 32);
+    fp.spaxel_base = (uint32_t)p->spaxel_base;
     fp.out = dst;
 
     while ((int)p->ev_fused.size() < 2 * (fused_slot + 1)) {
@@ -261,7 +294,7 @@ gt_status run_chunk(gt_plan* p, int64_t t0, int64_t T, float* dst, float* pwv_ds
         gt::PhotonExactParams pe{};
         pe.tod = dst; pe.lin = p->d_nep_lin.p; pe.sq = p->d_nep_sq.p; pe.n_rows = n_rows; pe.t0 = t0;
         pe.n_chan = p->n_chan; pe.n_spaxel = p->n_spaxel; pe.f_sample = p->f_sample; pe.sqrt_e0 = p->sqrt_e0;
-        pe.seed_lo = fp.seed_lo; pe.seed_hi = fp.seed_hi;
+        pe.seed_lo = fp.seed_lo; pe.seed_hi = fp.seed_hi; pe.spaxel_base = fp.spaxel_base;
         const int64_t n_span = (n_rows + 31) / 32;
         gt::photon_exact_kernel<<<(unsigned)std::min<int64_t>(n_span, 16 * p->num_sms), 256, 0, st>>>(pe);
         GT_CUDA(p, cudaGetLastError());
@@ -317,6 +350,12 @@ gt_status simulate_impl(gt_plan* p, int64_t t_begin, int64_t t_count, float* out
                     (long long)(t_begin + t_count), (long long)p->n_samples);
     if (t_count == 0) return GT_OK;
     if (!out) return fail(p, GT_ERR_NULL, "output pointer is NULL");
+    {
+        int dev = -1;
+        GT_CUDA(p, cudaGetDevice(&dev));
+        if (dev != p->device) return fail(p, GT_ERR_VALUE, "the plan lives on device %d, the current device is %d", p->device, dev);
+    }
+    p->last_stream = st;
     const bool pink = noise && p->pink_noise && p->pink_method == 0;      // the AR(1) cascade carries state between calls
     if (pink) {
         if (t_begin == 0) {
@@ -329,7 +368,7 @@ gt_status simulate_impl(gt_plan* p, int64_t t_begin, int64_t t_count, float* out
                         (long long)p->pink_next_t, (long long)t_begin);
         }
     }
-    p->n_fused_last = 0;
+    p->n_fused_last = 0; p->n_tl_last = 0;
     const bool dev_out = is_device_ptr(out);
     const bool dev_pwv = pwv_out ? is_device_ptr(pwv_out) : true;
     if (pwv_out && dev_pwv != dev_out)
@@ -349,16 +388,22 @@ gt_status simulate_impl(gt_plan* p, int64_t t_begin, int64_t t_count, float* out
             if (!p->d_chunk[slot].p) GT_CUDA(p, p->d_chunk[slot].alloc((size_t)chunk * row_floats));
             if (pwv_out && !p->d_pwv[slot].p) GT_CUDA(p, p->d_pwv[slot].alloc((size_t)chunk * p->n_spaxel));
             GT_CUDA(p, cudaStreamWaitEvent(st, p->ev_copied[slot], 0));      // buffer free again?
+            while ((int)p->ev_tl.size() < 4 * (k + 1)) { cudaEvent_t e; GT_CUDA(p, cudaEventCreate(&e)); p->ev_tl.push_back(e); }
+            GT_CUDA(p, cudaEventRecord(p->ev_tl[4 * k + 0], st));
             gt_status s = run_chunk(p, t, T, p->d_chunk[slot].p, pwv_out ? p->d_pwv[slot].p : nullptr, noise, st, k);
             if (s != GT_OK) return s;
+            GT_CUDA(p, cudaEventRecord(p->ev_tl[4 * k + 1], st));
             GT_CUDA(p, cudaEventRecord(p->ev_ready[slot], st));
             GT_CUDA(p, cudaStreamWaitEvent(p->copy_stream, p->ev_ready[slot], 0));
+            GT_CUDA(p, cudaEventRecord(p->ev_tl[4 * k + 2], p->copy_stream));
             GT_CUDA(p, cudaMemcpyAsync(out + off * row_floats, p->d_chunk[slot].p, (size_t)T * row_floats * sizeof(float),
                                        cudaMemcpyDeviceToHost, p->copy_stream));
             if (pwv_out)
                 GT_CUDA(p, cudaMemcpyAsync(pwv_out + off * p->n_spaxel, p->d_pwv[slot].p,
                                            (size_t)T * p->n_spaxel * sizeof(float), cudaMemcpyDeviceToHost, p->copy_stream));
+            GT_CUDA(p, cudaEventRecord(p->ev_tl[4 * k + 3], p->copy_stream));
             GT_CUDA(p, cudaEventRecord(p->ev_copied[slot], p->copy_stream));
+            p->n_tl_last = k + 1;
             slot ^= 1;
         }
     }
@@ -394,6 +439,7 @@ gt_status gt_plan_create(const gt_config* cfg, void* cuda_stream, gt_plan** out_
         int dev = 0; cudaDeviceProp prop{};
         GT_CUDA0(cudaGetDevice(&dev));
         GT_CUDA0(cudaGetDeviceProperties(&prop, dev));
+        p->device = dev;
         p->num_sms = prop.multiProcessorCount;
         if (prop.major != 10) return fail(nullptr, GT_ERR_UNSUPPORTED, "built for sm_100a, device is sm_%d%d", prop.major, prop.minor);
     }
@@ -403,9 +449,47 @@ gt_status gt_plan_create(const gt_config* cfg, void* cuda_stream, gt_plan** out_
     const int nfp = (nf + 63) / 64 * 64;      // the tensor kernel works in slabs of 64 frequencies
     p->n_freq = nf; p->n_freq_pad = nfp; p->n_chan = nc; p->n_spaxel = ns; p->n_pwv = c.n_pwv;
     p->n_samples = c.n_samples; p->photon_noise = c.photon_noise != 0; p->pink_noise = c.pink_noise != 0;
-    p->seed = c.seed; p->cube = c.cube; p->n_az = c.n_az; p->n_el = c.n_el;
+    p->seed = c.seed; p->cube = c.cube; p->n_az = c.n_az; p->n_el = c.n_el; p->spaxel_base = c.spaxel_index_base;
     p->variant = (c.variant == GT_VARIANT_FP32) ? GT_VARIANT_FP32 : GT_VARIANT_TENSOR;   // DEFAULT -> tensor: measured 8x faster than the FP32 kernel on C4
-    p->scale = (float)(kPref * c.dnu_hz);
+
+    // ---- statistics of the large device arrays: non-finite values are refused, the cube's per-frequency maximum
+    //      bounds the spectrum elements (operand range of the tensor kernel), the means feed the reference spectrum ----
+    std::vector<float> cube_max(nf, 0.f);
+    std::vector<double> cube_mean(nf, 0.0);
+    double screen_mean = 0.0;
+    {
+        const int64_t n_pix = c.cube ? (int64_t)c.n_az * c.n_el : 0;
+        DevBuf<uint32_t> d_max; DevBuf<double> d_sum;
+        const size_t n_stat = (size_t)nf + (size_t)c.nx;
+        GT_CUDA0(d_max.alloc(n_stat)); GT_CUDA0(d_sum.alloc(n_stat));
+        GT_CUDA0(cudaMemsetAsync(d_max.p, 0, n_stat * sizeof(uint32_t), st));
+        GT_CUDA0(cudaMemsetAsync(d_sum.p, 0, n_stat * sizeof(double), st));
+        if (c.cube) {
+            const unsigned gy = (unsigned)std::min<int64_t>(n_pix, std::max<int64_t>(1, (8 * p->num_sms) / ((nf + 255) / 256)));
+            gt::colstat_kernel<<<dim3((unsigned)((nf + 255) / 256), gy), 256, 0, st>>>(c.cube, n_pix, nf, d_max.p, d_sum.p);
+            GT_CUDA0(cudaGetLastError());
+        }
+        {
+            const unsigned gy = (unsigned)std::min<int64_t>(c.ny, std::max<int64_t>(1, (8 * p->num_sms) / ((c.nx + 255) / 256)));
+            gt::colstat_kernel<<<dim3((unsigned)((c.nx + 255) / 256), gy), 256, 0, st>>>(c.screen, c.ny, c.nx, d_max.p + nf, d_sum.p + nf);
+            GT_CUDA0(cudaGetLastError());
+        }
+        p->launches += c.cube ? 2 : 1;
+        std::vector<uint32_t> h_max(n_stat); std::vector<double> h_sum(n_stat);
+        GT_CUDA0(cudaMemcpyAsync(h_max.data(), d_max.p, n_stat * sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
+        GT_CUDA0(cudaMemcpyAsync(h_sum.data(), d_sum.p, n_stat * sizeof(double), cudaMemcpyDeviceToHost, st));
+        GT_CUDA0(cudaStreamSynchronize(st));
+        for (int i = 0; i < nf; ++i) {
+            if (h_max[i] >= 0x7F800000u) return fail(nullptr, GT_ERR_VALUE, "the source cube holds a NaN or Inf (frequency index %d)", i);
+            std::memcpy(&cube_max[i], &h_max[i], sizeof(float));
+            cube_mean[i] = n_pix ? h_sum[i] / (double)n_pix : 0.0;
+        }
+        for (int i = 0; i < c.nx; ++i) {
+            if (h_max[nf + i] >= 0x7F800000u) return fail(nullptr, GT_ERR_VALUE, "the PWV screen holds a NaN or Inf (column %d)", i);
+            screen_mean += h_sum[nf + i];
+        }
+        screen_mean /= (double)c.nx * (double)c.ny;
+    }
 
     // ---- small device arrays needed on the host ----
     std::vector<float> h_lut, h_filt, h_front;
@@ -418,6 +502,7 @@ gt_status gt_plan_create(const gt_config* cfg, void* cuda_stream, gt_plan** out_
     for (float v : h_front) if (!(v >= 0.f && v <= 1.f)) return fail(nullptr, GT_ERR_VALUE, "eta_front_nu outside [0,1]");
     for (auto& hs : h_stage) for (float v : hs) if (!(v >= 0.f && v <= 1.f)) return fail(nullptr, GT_ERR_VALUE, "stage eta_nu outside [0,1]");
     for (float v : h_lut) if (!(v > 0.f && v <= 1.f)) return fail(nullptr, GT_ERR_VALUE, "atm_lut outside (0,1]");
+    for (float v : h_filt) if (!std::isfinite(v)) return fail(nullptr, GT_ERR_VALUE, "filt holds a NaN or Inf");
 
     // ---- collapsed cascade, double precision ----
     // P_final(nu) = eta_atm * (b1 + a*S) + b0 after Eq. 11 and Eq. 12 for k = 0..n_stage:
@@ -425,8 +510,8 @@ gt_status gt_plan_create(const gt_config* cfg, void* cuda_stream, gt_plan** out_
     //   plain stage k:         a *= eta_k; b1 *= eta_k; b0 = eta_k b0 + (1-eta_k) B(T_k)
     //   coupled stage k:       a *= eta_k; b1 = eta_k b1 + (1-eta_k)(B_cmb - B_atm); b0 = eta_k b0 + (1-eta_k) B_atm
     // With eps = 1 - eta_atm:  P_final = eps*(-b1) + eta_atm*(a*S) + (b0 + b1);  all three terms >= 0.
-    std::vector<float> Xn(nfp, 0.f), Gs(nfp, 0.f);
-    std::vector<double> Y(nf), Xd(nf);
+    std::vector<double> Y(nf), Xd(nf), Gd(nf);
+    double v_max = 0.0;                        // largest |element| the generator can produce, in W/Hz
     for (int i = 0; i < nf; ++i) {
         const double nu = c.nu0_hz + (double)i * c.dnu_hz;
         const double Bc = jn_power(nu, c.T_cmb_K), Ba = jn_power(nu, c.T_atm_K);
@@ -438,11 +523,26 @@ gt_status gt_plan_create(const gt_config* cfg, void* cuda_stream, gt_plan** out_
             if (s.couple_atmosphere) { b1 = e * b1 + (1.0 - e) * (Bc - Ba); b0 = e * b0 + (1.0 - e) * Ba; }
             else                     { b1 = e * b1;                         b0 = e * b0 + (1.0 - e) * jn_power(nu, s.T_K); }
         }
-        Xn[i] = (float)(-b1 / kPref);
-        Xd[i] = -b1;
-        Gs[i] = (float)(a / kPref);
-        Y[i] = b0 + b1;
+        Xd[i] = -b1; Gd[i] = a; Y[i] = b0 + b1;
+        // an element is the convex combination (1 - eta) Xn + eta G S of its two end points, eta in [0,1]
+        v_max = std::max(v_max, std::max(std::fabs(b1), a * (double)cube_max[i]));
     }
+    if (!std::isfinite(v_max)) return fail(nullptr, GT_ERR_RANGE, "the spectrum is not finite (stage temperatures, source cube)");
+    {
+        // p_ref = k_B 300 K 2^-e with v_max / p_ref in [2^(kTcAMaxLog2 - 1), 2^kTcAMaxLog2): exact power of two on top of
+        // k_B 300 K, so the fp16 (hi, lo) pairs of the elements keep 22 bits down to ~1e-4 of the largest one
+        int e = 8;
+        if (v_max > 0.0) { int x; std::frexp(v_max / kPref0, &x); e = gt::kTcAMaxLog2 - x; }
+        e = std::max(-900, std::min(900, e));
+        p->p_ref = std::ldexp(kPref0, -e);
+        const double s = p->p_ref * c.dnu_hz;
+        if (!(s > 1e-37) || !(s < 1e37) || !(1.0 / p->p_ref < 1e37))
+            return fail(nullptr, GT_ERR_RANGE, "spectrum of at most %g W/Hz cannot be scaled into the fp32 range of the kernels", v_max);
+        p->scale = (float)s;
+    }
+    const double kPref = p->p_ref;
+    std::vector<float> Xn(nfp, 0.f), Gs(nfp, 0.f);
+    for (int i = 0; i < nf; ++i) { Xn[i] = (float)(Xd[i] / kPref); Gs[i] = (float)(Gd[i] / kPref); }
 
     // ---- LUT resampled on the frequency grid (bilinear is separable, R14) ----
     std::vector<float> lut_r((size_t)c.n_pwv * nfp, 1.0f);
@@ -459,11 +559,34 @@ gt_status gt_plan_create(const gt_config* cfg, void* cuda_stream, gt_plan** out_
         }
     }
 
+    // ---- reference spectrum (any positive multiple): the mean line of sight -- screen mean + drift at mid-run, boresight
+    //      airmass, mean cube spectrum.  Used only to shape the truncation-compensation table of the tensor kernel. ----
+    std::vector<double> a_ref(nf, 1.0);
+    {
+        const double pwv = screen_mean + c.pwv0_a_mm + c.pwv0_b_mm_per_s * 0.5 * (double)c.n_samples / c.f_sample_hz;
+        double q = (pwv - c.lut_pwv0_mm) / c.lut_dpwv_mm;
+        if (!(q >= 0.0)) q = 0.0;
+        if (q > (double)(c.n_pwv - 1)) q = (double)(c.n_pwv - 1);
+        const int ip = (int)std::min<double>(std::floor(q), c.n_pwv - 2);
+        const double fpq = q - ip, csc0 = 1.0 / std::max(std::sin(c.el0_rad), 1e-3);
+        double top = 0.0;
+        for (int i = 0; i < nf; ++i) {
+            const double ez = (1.0 - fpq) * lut_r[(size_t)ip * nfp + i] + fpq * lut_r[(size_t)(ip + 1) * nfp + i];
+            const double eta = std::pow(ez, csc0);
+            a_ref[i] = (1.0 - eta) * Xd[i] + eta * Gd[i] * cube_mean[i];
+            top = std::max(top, std::fabs(a_ref[i]));
+        }
+        bool ok = top > 0.0;
+        for (int i = 0; i < nf && ok; ++i) ok = a_ref[i] >= 0.0 && std::isfinite(a_ref[i]);
+        if (!ok) std::fill(a_ref.begin(), a_ref.end(), 1.0);              // no usable reference: flat
+        else for (double& v : a_ref) v = v / top + 1e-6;                  // keeps channels in fully transparent bands alive
+    }
+
     // ---- filter: transposed/padded copy (FP32 variant), per-channel constants ----
     const int tn = fp32_tn(nc);
     const int ncp = ((nc + 32 * tn - 1) / (32 * tn)) * 32 * tn;
     p->n_chan_pad = ncp;
-    std::vector<float> bias(ncp, 0.f), c1(ncp, 0.f), c2(ncp, 0.f);
+    std::vector<float> bias(ncp, 0.f), c1(ncp, 0.f), c2(ncp, 0.f), cw(ncp, 1.f);
     for (int ch = 0; ch < nc; ++ch) {
         double sb = 0.0, s1 = 0.0, s2 = 0.0;
         for (int i = 0; i < nf; ++i) {
@@ -483,9 +606,17 @@ gt_status gt_plan_create(const gt_config* cfg, void* cuda_stream, gt_plan** out_
         GT_CUDA0(p->d_filt_t.upload(ft, st));
         GT_CUDA0(cudaStreamSynchronize(st));
     } else {
-        if (gt_status s = gt::build_tc_tables(h_filt, nc, nf, nfp, p->tc, st)) {
+#ifdef GT_TC_DIAG
+        if (const char* e = std::getenv("GATEAU_TC_SEG")) {          // tuning builds only: slabs per accumulation segment
+            const int v = std::atoi(e);
+            if (v > 0) p->tc.seg = p->tc_lin.seg = p->tc_sq.seg = v;
+        }
+#endif
+        std::vector<float> inv;
+        if (gt_status s = gt::build_tc_tables(h_filt, nc, nf, nfp, a_ref, p->tc, inv, st)) {
             return fail(nullptr, s, "tensor variant: %s", gt::tc_error());
         }
+        for (int ch = 0; ch < nc; ++ch) cw[ch] = inv[ch];            // channel ch = column ch % nb_tot of channel group ch / nb_tot
         if (gt_status s = gt::alloc_tc_scratch(p->tc, p->num_sms)) return fail(nullptr, s, "tensor variant: %s", gt::tc_error());
         if (c.photon_noise && c.photon_mode == 1) {
             // Eq. 17 with P_nu = kPref v + Y (v = the generated element):
@@ -494,7 +625,7 @@ gt_status gt_plan_create(const gt_config* cfg, void* cuda_stream, gt_plan** out_
             const double g = 2.0 * c.kid_gap_J / c.eta_pb;
             const double E0 = kH * (c.nu0_hz + (double)(nf - 1) * c.dnu_hz) + g;
             std::vector<float> L((size_t)nc * nf), Q((size_t)nc * nf);
-            std::vector<float4> c4l(ncp, make_float4(0.f, 0.f, 0.f, 0.f)), c4z(ncp, make_float4(0.f, 0.f, 0.f, 0.f));
+            std::vector<float4> c4l(ncp, make_float4(0.f, 0.f, 0.f, 1.f)), c4z(ncp, make_float4(0.f, 0.f, 0.f, 1.f));
             for (int ch = 0; ch < nc; ++ch) {
                 double sb = 0.0;
                 for (int i = 0; i < nf; ++i) {
@@ -505,27 +636,29 @@ gt_status gt_plan_create(const gt_config* cfg, void* cuda_stream, gt_plan** out_
                 }
                 c4l[ch].x = (float)(c.dnu_hz * sb / E0);
             }
-            if (gt_status s = gt::build_tc_tables(L, nc, nf, nfp, p->tc_lin, st)) return fail(nullptr, s, "tensor variant (Eq. 17 linear filter): %s", gt::tc_error());
-            if (gt_status s = gt::build_tc_tables(Q, nc, nf, nfp, p->tc_sq, st)) return fail(nullptr, s, "tensor variant (Eq. 17 squared filter): %s", gt::tc_error());
+            std::vector<double> a_ref2(nf);
+            for (int i = 0; i < nf; ++i) a_ref2[i] = a_ref[i] * a_ref[i];
+            std::vector<float> inv_l, inv_q;
+            if (gt_status s = gt::build_tc_tables(L, nc, nf, nfp, a_ref, p->tc_lin, inv_l, st)) return fail(nullptr, s, "tensor variant (Eq. 17 linear filter): %s", gt::tc_error());
+            if (gt_status s = gt::build_tc_tables(Q, nc, nf, nfp, a_ref2, p->tc_sq, inv_q, st)) return fail(nullptr, s, "tensor variant (Eq. 17 squared filter): %s", gt::tc_error());
+            for (int ch = 0; ch < nc; ++ch) { c4l[ch].w = inv_l[ch]; c4z[ch].w = inv_q[ch]; }
             GT_CUDA0(p->d_chan4_lin.upload(c4l, st)); GT_CUDA0(p->d_chan4_zero.upload(c4z, st));
             GT_CUDA0(cudaStreamSynchronize(st));
             p->scale_sq = (float)(kPref * kPref * c.dnu_hz / ((double)gt::kTcSqScale * E0));
             p->sqrt_e0 = (float)std::sqrt(E0);
             p->f_sample = (float)c.f_sample_hz;
         }
-        if (const char* e = std::getenv("GATEAU_TC_SEG")) {          // tuning/diagnostic knob: slabs per accumulation segment
-            const int v = std::atoi(e);
-            if (v > 0) p->tc.seg = p->tc_lin.seg = p->tc_sq.seg = v;
-        }
     }
     GT_CUDA0(p->d_Xn.upload(Xn, st)); GT_CUDA0(p->d_Gs.upload(Gs, st)); GT_CUDA0(p->d_lut_r.upload(lut_r, st));
     GT_CUDA0(p->d_bias.upload(bias, st)); GT_CUDA0(p->d_c1.upload(c1, st)); GT_CUDA0(p->d_c2.upload(c2, st));
     {
         std::vector<float4> c4(ncp);
-        for (int ch = 0; ch < ncp; ++ch) c4[ch] = make_float4(bias[ch], c1[ch], c2[ch], 0.f);
+        for (int ch = 0; ch < ncp; ++ch) c4[ch] = make_float4(bias[ch], c1[ch], c2[ch], cw[ch]);
         GT_CUDA0(p->d_chan4.upload(c4, st));
         GT_CUDA0(cudaStreamSynchronize(st));
     }
+    GT_CUDA0(p->d_counters.alloc(3));
+    GT_CUDA0(cudaMemsetAsync(p->d_counters.p, 0, 3 * sizeof(unsigned long long), st));
 
     // ---- geometry tables: per-sample and per-spaxel transcendental inputs from the host libm ----
     {
@@ -605,6 +738,7 @@ gt_status gt_plan_create(const gt_config* cfg, void* cuda_stream, gt_plan** out_
         k.n_det = n_det; k.n_samples = N; k.n_chan = nc; k.f_sample = c.f_sample_hz;
         k.amp = p->d_tk_amp.p; k.half_alpha = p->d_tk_halpha.p; k.series = p->d_tk_series.p; k.ld = ld;
         k.seed_lo = (uint32_t)(c.seed & 0xffffffffu); k.seed_hi = (uint32_t)(c.seed >> 32);
+        k.spaxel_base = (uint32_t)c.spaxel_index_base;
         const int64_t n_thr = n_det * (K + 1);
         gt::tk_spectrum_kernel<<<(unsigned)((n_thr + 255) / 256), 256, 0, st>>>(k);
         GT_CUDA0(cudaGetLastError());
@@ -632,6 +766,7 @@ gt_status gt_plan_create(const gt_config* cfg, void* cuda_stream, gt_plan** out_
         gt::PinkParams& k = p->pink;
         k.J = J; k.n_chan = nc; k.n_det = (int64_t)ns * nc;
         k.seed_lo = (uint32_t)(c.seed & 0xffffffffu); k.seed_hi = (uint32_t)(c.seed >> 32);
+        k.spaxel_base = (uint32_t)c.spaxel_index_base;
         double lnrho = 1.0;
         if (J >= 2) lnrho = std::log(c.pink_f_corner_hz[0] / c.pink_f_corner_hz[J - 1]) / (double)(J - 1);
         for (int j = 0; j < gt::kPinkMaxJ; ++j) { k.phi[j] = 0.f; k.sq[j] = 0.f; }
@@ -694,13 +829,15 @@ gt_status gt_debug_pkid(gt_plan* plan, int64_t t_begin, int64_t t_count, float* 
 
 gt_status gt_plan_destroy(gt_plan* plan) {
     if (!plan) return GT_OK;
-    cudaDeviceSynchronize();
-    if (plan->copy_stream) cudaStreamDestroy(plan->copy_stream);
+    // wait for the work this plan enqueued (its last stream and its copy stream), not for the whole device
+    if (plan->last_stream != nullptr || plan->launches > 0) cudaStreamSynchronize(plan->last_stream);
+    if (plan->copy_stream) { cudaStreamSynchronize(plan->copy_stream); cudaStreamDestroy(plan->copy_stream); }
     for (int i = 0; i < 2; ++i) {
         if (plan->ev_ready[i]) cudaEventDestroy(plan->ev_ready[i]);
         if (plan->ev_copied[i]) cudaEventDestroy(plan->ev_copied[i]);
     }
     for (cudaEvent_t e : plan->ev_fused) cudaEventDestroy(e);
+    for (cudaEvent_t e : plan->ev_tl) cudaEventDestroy(e);
     plan->tc_lin.scratch = nullptr; plan->tc_sq.scratch = nullptr;      // aliases of tc.scratch
     gt::free_tc_tables(plan->tc_lin); gt::free_tc_tables(plan->tc_sq);
     gt::free_tc_tables(plan->tc);
@@ -721,7 +858,7 @@ gt_status gt_debug_geometry(gt_plan* plan, int64_t t_begin, int64_t t_count, gt_
     if (n_rows == 0) return GT_OK;
     DevBuf<gt_georec> rec;
     GT_CUDA(p, rec.alloc((size_t)n_rows));
-    gt::geometry_kernel<<<(unsigned)((n_rows + 255) / 256), 256>>>(p->geo, t_begin, n_rows, nullptr, nullptr, rec.p);
+    gt::geometry_kernel<<<(unsigned)((n_rows + 255) / 256), 256>>>(p->geo, t_begin, n_rows, nullptr, nullptr, rec.p, nullptr);
     GT_CUDA(p, cudaGetLastError());
     p->launches++;
     GT_CUDA(p, cudaMemcpy(host_records_out, rec.p, (size_t)n_rows * sizeof(gt_georec), cudaMemcpyDeviceToHost));
@@ -814,6 +951,44 @@ gt_status gt_prepare_screen(const float* epl_dev, int32_t nx, int32_t ny, double
 
 int64_t gt_launch_count(const gt_plan* plan) { return plan ? plan->launches : 0; }
 
+gt_status gt_plan_counters(gt_plan* plan, int64_t* rows, int64_t* rows_outside_cube, int64_t* pwv_below_lut, int64_t* pwv_above_lut) {
+    if (!plan) return fail(nullptr, GT_ERR_NULL, "plan is NULL");
+    unsigned long long h[3] = {0, 0, 0};
+    GT_CUDA(plan, cudaStreamSynchronize(plan->last_stream));
+    GT_CUDA(plan, cudaMemcpy(h, plan->d_counters.p, sizeof h, cudaMemcpyDeviceToHost));
+    if (rows) *rows = plan->rows_done;
+    if (rows_outside_cube) *rows_outside_cube = (int64_t)h[0];
+    if (pwv_below_lut) *pwv_below_lut = (int64_t)h[1];
+    if (pwv_above_lut) *pwv_above_lut = (int64_t)h[2];
+    return GT_OK;
+}
+
+gt_status gt_pink_state_export(gt_plan* plan, float* host_state, int64_t* next_t) {
+    if (!plan || !host_state || !next_t) return fail(plan, GT_ERR_NULL, "gt_pink_state_export: NULL argument");
+    if (!plan->pink_noise || plan->pink_method != 0) return fail(plan, GT_ERR_UNSUPPORTED, "the plan carries no AR(1) pink-noise state");
+    GT_CUDA(plan, cudaStreamSynchronize(plan->last_stream));
+    GT_CUDA(plan, cudaMemcpy(host_state, plan->d_state.p, (size_t)plan->pink.n_det * plan->J * sizeof(float), cudaMemcpyDeviceToHost));
+    *next_t = plan->pink_next_t;
+    return GT_OK;
+}
+
+gt_status gt_pink_state_import(gt_plan* plan, const float* host_state, int64_t next_t) {
+    if (!plan || !host_state) return fail(plan, GT_ERR_NULL, "gt_pink_state_import: NULL argument");
+    if (!plan->pink_noise || plan->pink_method != 0) return fail(plan, GT_ERR_UNSUPPORTED, "the plan carries no AR(1) pink-noise state");
+    if (next_t < 1 || next_t > plan->n_samples) return fail(plan, GT_ERR_RANGE, "next_t = %lld is outside 1..n_samples", (long long)next_t);
+    GT_CUDA(plan, cudaStreamSynchronize(plan->last_stream));
+    GT_CUDA(plan, cudaMemcpy(plan->d_state.p, host_state, (size_t)plan->pink.n_det * plan->J * sizeof(float), cudaMemcpyHostToDevice));
+    plan->pink_next_t = next_t;
+    return GT_OK;
+}
+
+gt_status gt_debug_chunking(const gt_plan* plan, int64_t* host_chunk, int64_t* device_chunk) {
+    if (!plan) return fail(nullptr, GT_ERR_NULL, "plan is NULL");
+    if (host_chunk) *host_chunk = plan->chunk_samples;
+    if (device_chunk) *device_chunk = plan->chunk_dev;
+    return GT_OK;
+}
+
 const char* gt_variant_name(const gt_plan* plan) {
     if (!plan) return "";
     return plan->variant == GT_VARIANT_FP32 ? "fp32-ffma" : "tcgen05-3xf16-split";
@@ -826,6 +1001,46 @@ gt_status gt_debug_kelvin_map(gt_plan* plan, double* a_out, double* b_out) {
     if (cudaMemcpy(a_out, plan->d_kelvin_ab.p, nb, cudaMemcpyDeviceToHost) != cudaSuccess ||
         cudaMemcpy(b_out, plan->d_kelvin_ab.p + plan->n_chan, nb, cudaMemcpyDeviceToHost) != cudaSuccess)
         return fail(plan, GT_ERR_CUDA, "gt_debug_kelvin_map: copy failed");
+    return GT_OK;
+}
+
+gt_status gt_debug_timeline(gt_plan* plan, int32_t capacity, int32_t* n_chunks, double* ms_out) {
+    if (!plan || !n_chunks || !ms_out) return fail(plan, GT_ERR_NULL, "gt_debug_timeline: NULL argument");
+    *n_chunks = std::min(plan->n_tl_last, capacity);
+    for (int k = 0; k < *n_chunks; ++k)
+        for (int j = 0; j < 4; ++j) {
+            GT_CUDA(plan, cudaEventSynchronize(plan->ev_tl[4 * k + j]));
+            float ms = 0.f;
+            GT_CUDA(plan, cudaEventElapsedTime(&ms, plan->ev_tl[0], plan->ev_tl[4 * k + j]));
+            ms_out[4 * k + j] = ms;
+        }
+    return GT_OK;
+}
+
+gt_status gt_measure_fp32_fma(void* cuda_stream, double* tflops_out) {
+    if (!tflops_out) return fail(nullptr, GT_ERR_NULL, "gt_measure_fp32_fma: NULL argument");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    int dev = 0; cudaDeviceProp prop{};
+    GT_CUDA(nullptr, cudaGetDevice(&dev));
+    GT_CUDA(nullptr, cudaGetDeviceProperties(&prop, dev));
+    const int blocks = 2 * prop.multiProcessorCount, iters = 1 << 14;     // 2 CTAs of 1024 threads per SM = every resident thread slot
+    DevBuf<float> out;
+    GT_CUDA(nullptr, out.alloc((size_t)blocks * 1024));
+    cudaEvent_t e0, e1;
+    GT_CUDA(nullptr, cudaEventCreate(&e0)); GT_CUDA(nullptr, cudaEventCreate(&e1));
+    double best = 0.0;
+    for (int rep = 0; rep < 6; ++rep) {                                    // first pass warms up; best of the rest
+        cudaEventRecord(e0, st);
+        gt::fma_peak_kernel<<<blocks, 1024, 0, st>>>(out.p, iters, 0.999f, 1e-3f);
+        cudaEventRecord(e1, st);
+        if (cudaEventSynchronize(e1) != cudaSuccess) break;
+        float ms = 0.f; cudaEventElapsedTime(&ms, e0, e1);
+        const double flop = 2.0 * 8.0 * 16.0 * (double)iters * 1024.0 * (double)blocks;
+        if (rep > 0 && ms > 0.f) best = std::max(best, flop / (ms * 1e-3) / 1e12);
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    GT_CUDA(nullptr, cudaGetLastError());
+    *tflops_out = best;
     return GT_OK;
 }
 

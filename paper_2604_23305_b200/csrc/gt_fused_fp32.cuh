@@ -37,6 +37,7 @@ struct FusedParams {
     const float *noise_c1, *noise_c2;   // [n_chan_pad] h f_c f_s, f_s / dnu_c
     const float4* chan4;                // [n_chan_pad] {bias, noise_c1, noise_c2, 0}: one 16-byte load per output
     int32_t photon_noise; uint32_t seed_lo, seed_hi;
+    uint32_t spaxel_base;     // global index of the plan's spaxel 0: Philox counter word 1 = spaxel_base + s
     float* out;               // [n_rows][n_chan]
 };
 
@@ -160,7 +161,7 @@ fused_fp32_kernel(const FusedParams p) {
             float P = fmaf(a, p.scale, bias);
             if (p.photon_noise) {
                 const uint32_t n = (uint32_t)(p.t0 + r / p.n_spaxel), s = (uint32_t)(r % p.n_spaxel);
-                const uint4 w = philox4x32_10(n, s, (uint32_t)c, kStreamPhoton, p.seed_lo, p.seed_hi);
+                const uint4 w = philox4x32_10(n, p.spaxel_base + s, (uint32_t)c, kStreamPhoton, p.seed_lo, p.seed_hi);
                 P = fmaf(photon_sigma(P, n1, n2), normal_cos(w.x, w.y), P);
             }
             p.out[(size_t)r * p.n_chan + c] = P;

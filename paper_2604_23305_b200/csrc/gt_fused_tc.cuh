@@ -33,6 +33,7 @@
 #include <cstring>
 #include <algorithm>
 #include <cstdlib>
+#include <cmath>
 #include <cuda_fp16.h>
 #include "gt_common.cuh"
 #include "gt_fused_fp32.cuh"
@@ -46,9 +47,13 @@ constexpr int kTcBK = 64;                  // frequencies per A stage / B unit: 
 constexpr float kTcSqScale = 1.0f / 256.0f;   // squared elements (v = O(256)) are scaled back into fp16 range
 constexpr int kTcHB = 32;                  // frequencies per generator step group (8 lanes x 4): half a slab
 constexpr int kTcKSteps = 4;               // K = 16 MMAs per 128-byte operand row
-// operand scaling into the fp16 range (exact powers of two, undone in the output scale): spectrum values are
-// O(1) (P_nu / (k_B 300 K)), filter transmissions are <= 1
-constexpr float kTcScaleA = 256.0f, kTcScaleB = 16384.0f;
+// Operand scaling into the fp16 range: exact powers of two chosen at plan time and
+// undone in the epilogue.  A (spectrum): ONE scale per plan, from the largest element the generator can produce
+// (max |Xn|, max |G| max |cube|), so that it lands in [2^kTcAMaxLog2 - 1, 2^kTcAMaxLog2).  B (filter): one scale PER
+// CHANNEL, so that the row maximum lands in [2^14, 2^15): a delta filter 1/dnu ~ 1e-8, a row-normalised filter ~ 1e-10
+// and a filter of peak 1 all keep their 22 bits.
+constexpr int kTcAMaxLog2 = 11;            // |A| < 2048: the squared elements of Eq. 17 (A^2 / 256) still fit fp16
+constexpr int kTcBMaxLog2 = 15;            // row maximum of |B| < 32768
 #ifndef GT_TC_A_STAGES
 #define GT_TC_A_STAGES 2
 #endif
@@ -69,6 +74,7 @@ constexpr bool kTcPair = GT_TC_PAIR != 0;
 constexpr int kTcAPartBytes = kTcBM * 128;                  // 16 KB (hi or lo part: 128 rows of 64 fp16)
 constexpr int kTcAStageBytes = 2 * kTcAPartBytes;           // 32 KB
 constexpr int kTcEpiWarps = 4, kTcGenWarps = 16;
+constexpr int kTcStageBytes = 16 * 32 * 4;                  // one flush batch: 16 columns x 32 rows of fp32
 // warp roles, aligned to warpgroups of 4 warps so that setmaxnreg can move registers between them:
 //   WG0 = warps 0-3 flush (tensor-memory lane quarter = warp), WG1-4 = generators (4 warps per scheduler: the
 //   per-element dependency chain lg2 -> ex2 -> split only fills the issue slots with thread-level parallelism),
@@ -107,8 +113,20 @@ constexpr int kTcRegsFlush = GT_TC_REGS_FLUSH, kTcRegsCtl = 40, kTcRegsGen = 80,
 static_assert(kTcRegsFlush + kTcRegsCtl + 4 * kTcRegsGen + (kTcFinWarps / 4) * kTcRegsFin <= (kTcThreads / 128) * kTcRegsBase, "setmaxnreg pool");
 constexpr int kTcMaxGroupChan = 384;       // channels per tile: 3 column groups of 128 (+ 1 spare buffer = 512 columns)
 constexpr int kTcBufCols = 128, kTcNumBuf = 4, kTcMaxCg = 3;
-constexpr int kTcSegDefault = 12;          // slabs (of 64 frequencies) per accumulation segment: measured max error 6.9e-6 of the 1e-5 gate (8: 5.2e-6, 16: 8.8e-6)
-constexpr float kTcTruncPerMma = 4.0e-8f;  // measured mean relative truncation loss per chained kind::f16 MMA (about half the worst case)
+constexpr int kTcSegDefault = 8;           // slabs (of 64 frequencies) per accumulation segment (measured max error 4.9e-6 of the 1e-5 gate; 12: 6.5e-6, 16: 9.4e-6)
+// The tensor core's fp32 accumulate TRUNCATES (measured): the 16 products of an MMA are aligned
+// to the running sum and cut at kTcTruncGrain of its unit in the last place (two guard bits), the new sum is cut to
+// the unit itself.  Positive products far above the grain therefore lose 16 x grain / 2 + 1/2 = 2.5 ulp per MMA;
+// products below the grain are dropped whole; the split's correction products (random signs) lose 1/2 ulp per MMA
+// once they reach the grain and nothing below it.  The plan tabulates, per (channel, segment), how many ulps of its
+// final sum a segment loses (from the channel's own filter and a reference spectrum: a narrow channel whose mass
+// arrives in the first slab of a segment loses 2.5 ulp per later 16-frequency step, one whose mass arrives last
+// loses nothing) and the flush warps add them back in units of the ulp of the partial sum they hold.
+constexpr double kTcTruncGrain = 0.25;
+#ifndef GT_TC_TRUNC_ULP
+#define GT_TC_TRUNC_ULP 1.0f
+#endif
+constexpr float kTcTruncUlp = GT_TC_TRUNC_ULP;      // overall factor on the table; tuning builds calibrate with 0 (off)
 #ifndef GT_TC_MAX_B_STAGES
 #define GT_TC_MAX_B_STAGES 3
 #endif
@@ -126,43 +144,89 @@ struct TcTables {
     int32_t unit_bytes = 0;              // nb_tot * 128
     int32_t b_stages = 0;
     int32_t smem_bytes = 0;
+    float* comp = nullptr;               // [group][n_seg][nb_tot] truncation compensation in ulp of the segment sum, times 2^-23
+    int32_t n_seg = 0;                   // segments per tile (max over the column groups)
 };
 
-inline const char*& tc_error_ref() { static const char* e = ""; return e; }
+inline const char*& tc_error_ref() { static thread_local const char* e = ""; return e; }
 inline const char* tc_error() { return tc_error_ref(); }
 
-// Splits the (scaled) filter into fp16 hi/lo parts and lays every (group, 64-frequency slab, part) out as
+// Expected number of ulps (of the FINAL segment sum S) that one chained MMA loses when the accumulator stands at
+// p S: the loss is ~1 ulp of the accumulator, ulp(p S) / ulp(S) = 2^floor(log2(p m)) for S = m 2^e; the flush warps
+// know e (they hold S) but the plan only knows the profile p, so the table carries the mean over a log-uniform
+// mantissa m in [1,2): 2^k (1 + f) with log2 p = k + f.  Signed like p (the truncation is toward zero).
+inline double tc_ulp_ratio(double p) {
+    if (p == 0.0 || !std::isfinite(p)) return 0.0;
+    const double a = std::fabs(p), l = std::log2(a), k = std::floor(l);
+    const double r = std::ldexp(1.0 + (l - k), (int)std::max(-60.0, std::min(60.0, k)));
+    return p < 0.0 ? -r : r;
+}
+
+// Splits the filter into fp16 hi/lo parts and lays every (group, 64-frequency slab, part) out as
 // the exact shared-memory image tcgen05.mma reads (K-major, SWIZZLE_128B): the loader is a flat copy.
+// Channel c is scaled by its own power of two 2^kb[c] so that its largest |value| lands in [2^14, 2^15);
+// inv_scale[c] = 2^-kb[c] goes into the epilogue constant of the channel.
+// a_ref [n_freq]: a reference spectrum in the generator's scaled units (any positive multiple will do), used only for
+// the truncation-compensation table: W[c][segment] = kTcTruncUlp 2^-23 sum over the MMAs of the segment of
+// tc_ulp_ratio(accumulator after that MMA / final segment sum), in the order the MMA thread issues them.
 inline gt_status build_tc_tables(const std::vector<float>& filt, int n_chan, int n_freq, int n_freq_pad,
-                                 TcTables& t, cudaStream_t st) {
+                                 const std::vector<double>& a_ref, TcTables& t, std::vector<float>& inv_scale,
+                                 cudaStream_t st) {
     const int G = (n_chan + kTcMaxGroupChan - 1) / kTcMaxGroupChan;
     int per = (n_chan + G - 1) / G;
     const int nbt = (per + 31) / 32 * 32;
     t.n_groups = G; t.nb_tot = nbt;
     t.n_cg = (nbt + kTcBufCols - 1) / kTcBufCols;
     t.n_kb = n_freq_pad / kTcBK;
+    if (t.seg <= 0) t.seg = kTcSegDefault;
     // one unit = the rows one CTA holds of one (slab, part): all nb_tot rows, or (CTA pair) the half of every
     // column group this CTA supplies to the M = 256 MMAs (rank r: columns [r w/2, (r+1) w/2) of a group of width w)
     constexpr int kRanks = kTcPair ? 2 : 1;
     t.unit_bytes = nbt * 128 / kRanks;
-    const int fixed = kTcAStages * kTcAStageBytes + 1024 /*alignment slack*/ + 320 /*barriers*/ + kTcBM * 32 /*row constants*/;
+    const int fixed = kTcAStages * kTcAStageBytes + 1024 /*alignment slack*/ + 320 /*barriers*/ + kTcBM * 32 /*row constants*/ + kTcEpiWarps * kTcBufCols * 4 /*compensation weights of the next flush, per flush warp*/
+                    + kTcEpiWarps * 2 * kTcStageBytes /*flush staging: two 2 KB batches per flush warp*/;
     t.b_stages = std::min(kTcMaxBStages, (kTcSmemLimit - fixed) / t.unit_bytes);
     if (t.b_stages < 2) { tc_error_ref() = "filter slab does not fit in shared memory"; return GT_ERR_UNSUPPORTED; }
     t.smem_bytes = fixed + t.b_stages * t.unit_bytes;
 
+    // segment of every slab, per column group: the host-side twin of TcRotation::boundary
+    std::vector<int> seg_of((size_t)t.n_cg * t.n_kb);
+    t.n_seg = 1;
+    for (int cg = 0; cg < t.n_cg; ++cg) {
+        int cnt = (cg * t.seg) / t.n_cg, si = 0;
+        for (int kb = 0; kb < t.n_kb; ++kb) {
+            seg_of[(size_t)cg * t.n_kb + kb] = si;
+            if (kb != t.n_kb - 1 && ++cnt == t.seg) { cnt = 0; ++si; }
+        }
+        t.n_seg = std::max(t.n_seg, si + 1);
+    }
+
+    inv_scale.assign((size_t)G * nbt, 1.0f);
     const size_t total = (size_t)G * t.n_kb * 2 * kRanks * t.unit_bytes;
     std::vector<float> img(total / 4, 0.f);
+    std::vector<float> comp((size_t)G * t.n_seg * nbt, 0.f);
+    std::vector<double> part((size_t)t.n_kb * kTcKSteps);
     uint16_t* img16 = reinterpret_cast<uint16_t*>(img.data());
     for (int g = 0; g < G; ++g)
         for (int n = 0; n < nbt; ++n) {
             const int ch = g * nbt + n;
             if (ch >= n_chan) continue;
+            const float* frow = filt.data() + (size_t)ch * n_freq;
+            float amax = 0.f;
+            for (int i = 0; i < n_freq; ++i) {
+                if (!std::isfinite(frow[i])) { tc_error_ref() = "the filter holds a NaN or Inf"; return GT_ERR_VALUE; }
+                amax = std::max(amax, std::fabs(frow[i]));
+            }
+            int kb_c = 0;
+            if (amax > 0.f) { int e; std::frexp(amax, &e); kb_c = std::max(-100, std::min(100, kTcBMaxLog2 - e)); }
+            inv_scale[(size_t)g * nbt + n] = std::ldexp(1.0f, -kb_c);
             // which CTA holds row n, and where inside its unit
             const int cg = n / kTcBufCols, col0 = cg * kTcBufCols, w = std::min(kTcBufCols, nbt - col0);
             const int rk = kTcPair ? (n - col0) / (w / 2) : 0;
             const int nl = kTcPair ? col0 / 2 + (n - col0) - rk * (w / 2) : n;        // local row
+            std::fill(part.begin(), part.end(), 0.0);
             for (int i = 0; i < n_freq; ++i) {
-                const float f = filt[(size_t)ch * n_freq + i] * kTcScaleB;
+                const float f = std::ldexp(frow[i], kb_c);
                 const __half fh = __float2half_rn(f);
                 const __half fl = __float2half_rn(f - __half2float(fh));
                 const int kb = i / kTcBK, kk = i % kTcBK;
@@ -173,12 +237,48 @@ inline gt_status build_tc_tables(const std::vector<float>& filt, int n_chan, int
                 const size_t off = (size_t)nl * 64 + (size_t)(((kk >> 3) ^ (nl & 7)) << 3) + (kk & 7);
                 img16[unit0 + off] = __half_as_ushort(fh);         // unit 0: Fm_hi
                 img16[unit1 + off] = __half_as_ushort(fl);         // unit 1: Fm_lo
+                part[(size_t)kb * kTcKSteps + kk / 16] += (double)f * a_ref[i];
+            }
+            // truncation compensation: walk the MMAs of every segment in issue order.  Per slab the MMA thread issues,
+            // for k = 0..3, A_hi.Fm_hi (moves the accumulator by part[kb][k]) and A_lo.Fm_hi, then for k = 0..3 A_hi.Fm_lo.
+            for (int s0 = 0, kb0 = 0; kb0 < t.n_kb; ++s0) {
+                int kb1 = kb0;
+                while (kb1 < t.n_kb && seg_of[(size_t)cg * t.n_kb + kb1] == s0) ++kb1;
+                double S = 0.0;
+                for (int kb = kb0; kb < kb1; ++kb) for (int k = 0; k < kTcKSteps; ++k) S += part[(size_t)kb * kTcKSteps + k];
+                double W = 0.0;
+                if (S != 0.0) {
+                    // losses in ulp of the accumulator at that moment; x = mean product of the step in those ulps
+                    // (E[1/m] = 0.72 over the mantissa m of the final sum, whose exponent the flush warps know)
+                    auto step_x = [&](double part_k, double r) { return r > 0.0 ? std::fabs(part_k / S) / 16.0 / (std::ldexp(0.72, -23) * r) : 0.0; };
+                    auto loss_main = [&](double x) { return x < kTcTruncGrain ? 16.0 * x : 16.0 * kTcTruncGrain / 2.0 + 0.5; };
+                    auto loss_corr = [&](double x) { return 0.5 * std::min(1.0, x * std::ldexp(1.0, -12) / 1.4142 / kTcTruncGrain); };
+                    double acc = 0.0;
+                    for (int kb = kb0; kb < kb1; ++kb) {
+                        for (int k = 0; k < kTcKSteps; ++k) {
+                            const double pk = part[(size_t)kb * kTcKSteps + k];
+                            acc += pk;
+                            const double r = tc_ulp_ratio(acc / S), x = step_x(pk, std::fabs(r));
+                            W += r * (loss_main(x) + loss_corr(x));
+                        }
+                        const double r = tc_ulp_ratio(acc / S);
+                        for (int k = 0; k < kTcKSteps; ++k) W += r * loss_corr(step_x(part[(size_t)kb * kTcKSteps + k], std::fabs(r)));
+                    }
+                    // a profile that overshoots or changes sign (filters with negative lobes) is not a profile the
+                    // row's own sums need follow: keep the compensation inside what a one-signed sum can lose
+                    const double w_max = (16.0 * kTcTruncGrain / 2.0 + 1.5) * kTcKSteps * (kb1 - kb0);
+                    W = std::max(0.0, std::min(W, w_max));
+                }
+                comp[((size_t)g * t.n_seg + s0) * nbt + n] = (float)(W * (double)kTcTruncUlp * std::ldexp(1.0, -23));
+                kb0 = kb1;
             }
         }
-    if (cudaMalloc(reinterpret_cast<void**>(&t.filt_img), total) != cudaSuccess) {
+    if (cudaMalloc(reinterpret_cast<void**>(&t.filt_img), total) != cudaSuccess ||
+        cudaMalloc(reinterpret_cast<void**>(&t.comp), comp.size() * sizeof(float)) != cudaSuccess) {
         cudaGetLastError(); tc_error_ref() = "cudaMalloc of the filter image failed"; return GT_ERR_OOM;
     }
     if (cudaMemcpyAsync(t.filt_img, img.data(), total, cudaMemcpyHostToDevice, st) != cudaSuccess ||
+        cudaMemcpyAsync(t.comp, comp.data(), comp.size() * sizeof(float), cudaMemcpyHostToDevice, st) != cudaSuccess ||
         cudaStreamSynchronize(st) != cudaSuccess) {
         cudaGetLastError(); tc_error_ref() = "upload of the filter image failed"; return GT_ERR_CUDA;
     }
@@ -196,13 +296,16 @@ inline gt_status alloc_tc_scratch(TcTables& t, int num_sms) {
 inline void free_tc_tables(TcTables& t) {
     if (t.filt_img) cudaFree(t.filt_img);
     if (t.scratch) cudaFree(t.scratch);
-    t.filt_img = nullptr; t.scratch = nullptr;
+    if (t.comp) cudaFree(t.comp);
+    t.filt_img = nullptr; t.scratch = nullptr; t.comp = nullptr;
 }
 
 struct TcParams {
     FusedParams f;
     const unsigned char* filt_img;
     float* scratch;
+    const float* comp;          // [group][n_seg][nb_tot] truncation compensation (build_tc_tables)
+    int32_t n_seg;
     int32_t n_groups, nb_tot, n_cg, seg, n_kb, unit_bytes, b_stages;
     int32_t n_row_tiles;
     int32_t cube_vec;           // 1: cube spectra can be read as aligned float4
@@ -215,13 +318,15 @@ struct TcParams {
 //   then barriers: a_full[2] a_empty[2] b_full[4] b_empty[4] flush_full[4] buf_free[4] tile_done[2]
 //   scratch_free[2], tensor-memory slot
 struct TcSmem {
-    uint32_t a, b, a_full, a_empty, b_full, b_empty, flush_full, buf_free, tile_done, scratch_free, b_peer, slot, rowp;
+    uint32_t a, b, a_full, a_empty, b_full, b_empty, flush_full, buf_free, tile_done, scratch_free, b_peer, slot, rowp, wcomp, stage;
     __device__ TcSmem(uint32_t base, int b_stages, int unit_bytes) {
         a = base; b = base + kTcAStages * kTcAStageBytes;
         const uint32_t bar = b + (uint32_t)b_stages * (uint32_t)unit_bytes;
         a_full = bar; a_empty = bar + 32; b_full = bar + 64; b_empty = bar + 96;
         flush_full = bar + 128; buf_free = bar + 160; tile_done = bar + 192; scratch_free = bar + 208; b_peer = bar + 224; slot = bar + 256;
         rowp = bar + 320;
+        wcomp = rowp + kTcBM * 32;
+        stage = wcomp + kTcEpiWarps * kTcBufCols * 4;
     }
 };
 
@@ -293,9 +398,10 @@ __device__ __forceinline__ void store_split(unsigned char* a_stage, int row, int
     *reinterpret_cast<uint2*>(dst + kTcAPartBytes) = lo2;
 }
 
-// element (column, row) of a scratch tile laid out [column / 4][row][column % 4]
-__device__ __forceinline__ size_t tc_scratch_index(int col, int row) {
-    return ((size_t)(col >> 2) * kTcBM + (size_t)row) * 4 + (size_t)(col & 3);
+// element (column, row) of a scratch tile laid out [row / 32][column / 4][row % 32][column % 4]: the 32 rows one flush
+// warp owns are contiguous per group of 4 columns (512 B), 16 columns of them 2 KB -- one bulk copy
+__device__ __forceinline__ size_t tc_scratch_index(int col, int row, int nb_tot) {
+    return ((size_t)(row >> 5) * (size_t)(nb_tot >> 2) + (size_t)(col >> 2)) * 128 + (size_t)(row & 31) * 4 + (size_t)(col & 3);
 }
 
 __device__ __forceinline__ float4 ldg4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
@@ -360,7 +466,7 @@ fused_tc_kernel(const TcParams p) {
         if constexpr (kTcPair) ptx::tc_commit2(bar, (uint16_t)3); else ptx::tc_commit(bar);
     };
     auto mma_f16 = [&](uint32_t d, uint64_t a, uint64_t b, uint32_t id, uint32_t acc) {       // kind::f16, K = 16
-        if constexpr (kTcPair) ptx::mma2_bf16_ss(d, a, b, id, acc); else ptx::mma_bf16_ss(d, a, b, id, acc);
+        if constexpr (kTcPair) ptx::mma2_f16_ss(d, a, b, id, acc); else ptx::mma_f16_ss(d, a, b, id, acc);
     };
     // Row tiles are TIME-MAJOR: row tile rt = (block of 128 consecutive samples tb, spaxel s), tile row r = sample
     // tb*128 + r of the launch.  Consecutive samples of one spaxel point ~1 source pixel apart, so their 2 x 2 tap
@@ -714,7 +820,7 @@ fused_tc_kernel(const TcParams p) {
 #pragma unroll
                 for (int j = 0; j < kMaxPerLane; ++j) {
                     const int c = lane + 32 * j;
-                    xn[j] = c < n_valid ? __ldcg(sc + tc_scratch_index(c, q)) : 0.f;
+                    xn[j] = c < n_valid ? __ldcg(sc + tc_scratch_index(c, q, p.nb_tot)) : 0.f;
                 }
             }
             for (int r = q; r < kTcBM; r += kTcFinWarps) {
@@ -728,14 +834,14 @@ fused_tc_kernel(const TcParams p) {
                     for (int j = 0; j < kMaxPerLane; ++j) {
                         x[j] = xn[j];
                         const int c = lane + 32 * j;
-                        xn[j] = (c < n_valid && r + kTcFinWarps < kTcBM) ? __ldcg(sc + tc_scratch_index(c, r + kTcFinWarps)) : 0.f;
+                        xn[j] = (c < n_valid && r + kTcFinWarps < kTcBM) ? __ldcg(sc + tc_scratch_index(c, r + kTcFinWarps, p.nb_tot)) : 0.f;
                     }
                 } else {
                     // all of this row's partial sums are requested at once; the other finisher warp of the scheduler covers the latency
 #pragma unroll
                     for (int j = 0; j < kMaxPerLane; ++j) {
                         const int c = lane + 32 * j;
-                        x[j] = c < n_valid ? __ldcg(sc + tc_scratch_index(c, r)) : 0.f;
+                        x[j] = c < n_valid ? __ldcg(sc + tc_scratch_index(c, r, p.nb_tot)) : 0.f;
                     }
                 }
                 constexpr int W = GT_TC_FIN_W;                            // channels in flight per lane
@@ -748,12 +854,12 @@ fused_tc_kernel(const TcParams p) {
                     for (int i = 0; i < W; ++i) {
                         const int c = min(lane + 32 * (j0 + i), n_valid - 1);
                         cc[i] = (uint32_t)(cg0 + c);
-                        const float4 k4 = __ldg(f.chan4 + cc[i]);          // bias, h f_c f_s, f_s / dnu_c
-                        P[i] = fmaf(x[j0 + i], f.scale, k4.x);
+                        const float4 k4 = __ldg(f.chan4 + cc[i]);          // bias, h f_c f_s, f_s / dnu_c, 2^-kb (the channel's filter scale)
+                        P[i] = fmaf(x[j0 + i] * k4.w, f.scale, k4.x);
                         n1[i] = k4.y; n2[i] = k4.z;
                     }
                     if (f.photon_noise) {
-                        philox4x32_10_multi<W>(n, s, cc, kStreamPhoton, f.seed_lo, f.seed_hi, w0, w1);
+                        philox4x32_10_multi<W>(n, f.spaxel_base + s, cc, kStreamPhoton, f.seed_lo, f.seed_hi, w0, w1);
 #pragma unroll
                         for (int i = 0; i < W; ++i)
                             P[i] = fmaf(photon_sigma(P[i], n1[i], n2[i]), normal_cos(w0[i], w1[i]), P[i]);
@@ -775,54 +881,85 @@ fused_tc_kernel(const TcParams p) {
         const int trow = 32 * q + lane;                        // tile row = tensor-memory lane
         TcRotation rot(p.n_cg, p.seg, p.n_kb);
         uint32_t fulls = 0u;                                   // bit b: parity of buffer b's flush count
-        uint32_t ti = 0;
+        uint32_t ti = 0, nbatch = 0;
         for (int64_t tl = worker; tl < n_tiles; tl += n_workers, ++ti) {
             const uint32_t sb = ti & 1u;
             float* const sc = p.scratch + ((size_t)blockIdx.x * 2 + sb) * p.nb_tot * kTcBM;
             if (ti >= 2) ptx::mbar_wait_relaxed(sm.scratch_free + 8 * sb, ((ti >> 1) - 1u) & 1u);   // finisher done with tile ti-2
             bool first[kTcMaxCg] = {true, true, true};
+            int segi[kTcMaxCg] = {0, 0, 0};                      // segment of the tile each group is in
+            const float* const comp_t = p.comp + (size_t)(tl % p.n_groups) * p.n_seg * p.nb_tot;
             for (int kb = 0; kb < p.n_kb; ++kb)
 #pragma unroll
                 for (int g = 0; g < kTcMaxCg; ++g) {
                     if (g >= p.n_cg || !rot.boundary(kb, g)) continue;
                     const int b = rot.rotate(g);
                     const int wg = rot.width(g, p.nb_tot);
-                    // scratch tile layout [column / 4][row][column % 4]: a thread (= row) moves 4 columns as one
-                    // 16-byte access, a warp 512 contiguous bytes
-                    float4* scg = reinterpret_cast<float4*>(sc) + (size_t)(g * (kTcBufCols / 4)) * kTcBM + trow;
+                    // truncation-compensation weights of this (group, segment): fetched into this warp's own shared-memory
+                    // strip BEFORE the wait, so that the flush itself never waits on global memory for them
+                    float4* const wsm = reinterpret_cast<float4*>(smem_raw + (sm.wcomp - raw)) + q * (kTcBufCols / 4);
+                    {
+                        const float4* const comp4 = reinterpret_cast<const float4*>(comp_t + (size_t)segi[g] * p.nb_tot + g * kTcBufCols);
+                        __syncwarp();
+                        wsm[lane] = 4 * lane < wg ? __ldg(comp4 + lane) : make_float4(0.f, 0.f, 0.f, 0.f);
+                        __syncwarp();
+                    }
+                    ++segi[g];
+                    // The partial sums go to the scratch tile through the bulk-copy engine: 16 columns x this warp's 32 rows
+                    // (2 KB, contiguous in the scratch layout) are staged in shared memory and sent with ONE
+                    // cp.async.bulk (first segment: store) or cp.reduce.async.bulk.add.f32 (later segments: the L2 adds,
+                    // round to nearest) -- the flush never waits for a load of the running sums, so its duration no longer
+                    // depends on the L2 round trip and the accumulator buffer is handed back after ~8 short batches.
+                    float* const scw = sc + tc_scratch_index(g * kTcBufCols, 32 * q, p.nb_tot);            // this warp's strip of the group
                     const uint32_t taddr = tmem_base + ((uint32_t)(32 * q) << 16) + (uint32_t)(b * kTcBufCols);
                     const bool add = !first[g];
                     uint32_t v[16];
-                    float4 pa[4];
-                    // the running sums of the first 16 columns are fetched while the MMAs still run
-                    if (add) {
-#pragma unroll
-                        for (int i = 0; i < 4; ++i) pa[i] = __ldcg(scg + (size_t)i * kTcBM);
-                    }
                     wait_pair(sm.flush_full + 8 * b, fulls >> b & 1u);
                     fulls ^= 1u << b;
                     ptx::tc_fence_after();
-                    for (int c0 = 0; c0 < wg; c0 += 16) {
+                    for (int c0 = 0; c0 < wg; c0 += 16, ++nbatch) {
                         ptx::tmem_ld_32x16(taddr + (uint32_t)c0, v);
+                        // the staging buffer of this batch was last read by the bulk copy issued two batches ago
+                        if (lane == 0) ptx::bulk_wait_read<1>();
+                        float4* const stg = reinterpret_cast<float4*>(smem_raw + (sm.stage - raw)) + (q * 2 + (nbatch & 1)) * (kTcStageBytes / 16) + lane;
                         ptx::tmem_ld_wait();
+                        if (c0 + 16 >= wg) {
+                            // all of the group's columns are in registers: the accumulator buffer can go back to the MMA thread
+                            ptx::tc_fence_before();
+                            __syncwarp();
+                            if (lane == 0) arrive_leader(sm.buf_free + 8 * b);
+                        } else __syncwarp();
 #pragma unroll
                         for (int i = 0; i < 4; ++i) {
-                            float4 sum = make_float4(__uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1]),
-                                                     __uint_as_float(v[4 * i + 2]), __uint_as_float(v[4 * i + 3]));
-                            if (add) { sum.x += pa[i].x; sum.y += pa[i].y; sum.z += pa[i].z; sum.w += pa[i].w; }
-                            __stcg(scg + (size_t)(c0 / 4 + i) * kTcBM, sum);
-                            if (add && c0 + 16 < wg) pa[i] = __ldcg(scg + (size_t)(c0 / 4 + 4 + i) * kTcBM);
+                            // truncation compensation: the segment lost w ulp of its own sum (table of the plan, per
+                            // channel and segment); +-2^e of the sum = its sign and exponent bits
+#ifndef GT_TC_NO_COMP
+                            const float4 w4 = wsm[c0 / 4 + i];
+#else
+                            const float4 w4 = make_float4(0.f, 0.f, 0.f, 0.f);      // tuning builds: cost of the table look-up
+#endif
+                            float4 sum;
+                            sum.x = fmaf(__uint_as_float(v[4 * i] & 0xFF800000u), w4.x, __uint_as_float(v[4 * i]));
+                            sum.y = fmaf(__uint_as_float(v[4 * i + 1] & 0xFF800000u), w4.y, __uint_as_float(v[4 * i + 1]));
+                            sum.z = fmaf(__uint_as_float(v[4 * i + 2] & 0xFF800000u), w4.z, __uint_as_float(v[4 * i + 2]));
+                            sum.w = fmaf(__uint_as_float(v[4 * i + 3] & 0xFF800000u), w4.w, __uint_as_float(v[4 * i + 3]));
+                            stg[i * 32] = sum;                               // [column / 4][row][column % 4], as the scratch tile
+                        }
+                        ptx::fence_proxy_async_smem();
+                        __syncwarp();
+                        if (lane == 0) {
+                            const uint32_t src = sm.stage + (uint32_t)((q * 2 + (nbatch & 1)) * kTcStageBytes);
+                            float* const dst = scw + (size_t)(c0 / 4) * (32 * 4);
+                            if (add) ptx::bulk_reduce_add_f32_s2g(dst, src, kTcStageBytes); else ptx::bulk_s2g(dst, src, kTcStageBytes);
+                            ptx::bulk_commit();
                         }
                     }
-                    ptx::tc_fence_before();
-                    __syncwarp();
-                    if (lane == 0) arrive_leader(sm.buf_free + 8 * b);
                     first[g] = false;
                 }
-            // every partial sum of the tile is in the scratch tile: hand it to the finisher warps
-            __threadfence_block();
+            // every partial sum of the tile is on its way: once this warp's bulk copies have completed, hand the
+            // tile to the finisher warps
+            if (lane == 0) { ptx::bulk_wait_all(); __threadfence(); ptx::mbar_arrive(sm.tile_done + 8 * sb); }
             __syncwarp();
-            if (lane == 0) ptx::mbar_arrive(sm.tile_done + 8 * sb);
         }
     }
 
@@ -839,19 +976,14 @@ fused_tc_kernel(const TcParams p) {
 inline cudaError_t launch_fused_tc(const FusedParams& fp, const TcTables& t, int num_sms, cudaStream_t st, bool square = false) {
     TcParams p{};
     p.f = fp; p.filt_img = t.filt_img;
-    // Truncation compensation: the tensor core drops up to ~1e-7 of the running sum
-    // per chained MMA, always toward zero, so a segment of n MMAs comes out low by between 0 and ~1e-7 n;
-    // adding half of that (folded into the output scale: nearly every segment has the same n) centres
-    // the one-sided error interval.
-    {
-        const int seg = t.seg > 0 ? t.seg : kTcSegDefault;
-        p.f.scale *= (1.0f + kTcTruncPerMma * (float)(3 * kTcKSteps * std::min(seg, (int)t.n_kb))) / kTcScaleB;      // kTcScaleA is part of FusedParams::scale (plan)
-    }
-    p.scratch = t.scratch;
+    // FusedParams::scale carries the spectrum scale of the plan; the per-channel filter scale is chan4.w
+    p.scratch = t.scratch; p.comp = t.comp; p.n_seg = t.n_seg;
     p.n_groups = t.n_groups; p.nb_tot = t.nb_tot; p.n_cg = t.n_cg; p.seg = t.seg > 0 ? t.seg : kTcSegDefault; p.n_kb = t.n_kb;
     p.unit_bytes = t.unit_bytes; p.b_stages = t.b_stages;
     p.n_row_tiles = (int32_t)(((fp.n_rows / fp.n_spaxel + kTcBM - 1) / kTcBM) * fp.n_spaxel);      // time-major: blocks of 128 samples x spaxels
-    if (const char* e = std::getenv("GATEAU_TC_DEBUG")) p.debug = std::atoi(e);
+#ifdef GT_TC_DIAG
+    if (const char* e = std::getenv("GATEAU_TC_DEBUG")) p.debug = std::atoi(e);      // tuning builds only
+#endif
     p.cube_vec = (fp.cube == nullptr) || ((fp.n_freq % 4 == 0) && ((reinterpret_cast<uintptr_t>(fp.cube) & 15u) == 0));
     const int64_t n_tiles = kTcPair ? (int64_t)((p.n_row_tiles + 1) / 2) * p.n_groups : (int64_t)p.n_row_tiles * p.n_groups;
     const int64_t workers = kTcPair ? num_sms / 2 : num_sms;

@@ -40,9 +40,11 @@ __device__ __forceinline__ int64_t pmod64(int64_t a, int64_t m) {
 // rows r = 0 .. n_rows-1 of the chunk starting at sample t0: n = t0 + r / n_spaxel, s = r % n_spaxel.
 __global__ void __launch_bounds__(256)
 geometry_kernel(GeoParams g, int64_t t0, int64_t n_rows, RowParam* __restrict__ rows,
-                float* __restrict__ pwv_out, gt_georec* __restrict__ rec_out) {
+                float* __restrict__ pwv_out, gt_georec* __restrict__ rec_out,
+                unsigned long long* __restrict__ counters) {       // [3] rows outside the cube, PWV below / above the LUT (NULL ok)
     const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (r >= n_rows) return;
+    const unsigned active = __activemask();
     const int64_t n = t0 + r / g.n_spaxel;
     const int s = (int)(r % g.n_spaxel);
 
@@ -78,10 +80,12 @@ geometry_kernel(GeoParams g, int64_t t0, int64_t n_rows, RowParam* __restrict__ 
 
     // LUT cell in PWV, clamped (R13)
     double q = __ddiv_rn(__dsub_rn(pwv, g.lut_pwv0), g.lut_dpwv);
-    if (q < 0.0) q = 0.0;
-    if (q > (double)(g.n_pwv - 1)) q = (double)(g.n_pwv - 1);
+    const bool clamp_lo = !(q >= 0.0), clamp_hi = q > (double)(g.n_pwv - 1);     // a NaN is clamped to row 0 as well: every index stays in bounds
+    if (clamp_lo) q = 0.0;
+    if (clamp_hi) q = (double)(g.n_pwv - 1);
     int64_t ip = (int64_t)floor(q);
     if (ip > g.n_pwv - 2) ip = g.n_pwv - 2;
+    if (ip < 0) ip = 0;
     const double fp = __dsub_rn(q, (double)ip);
 
     // Eq. 10 airmass: sin(E + dtheta_s) by the addition formula
@@ -118,6 +122,15 @@ geometry_kernel(GeoParams g, int64_t t0, int64_t n_rows, RowParam* __restrict__ 
         rows[r] = rp;
     }
     if (pwv_out) pwv_out[r] = (float)pwv;
+    if (counters) {
+        // diagnostics: one atomic per warp and event kind, only where the event occurs (both are rare)
+        const unsigned b0 = __ballot_sync(active, g.has_cube && ju < 0), b1 = __ballot_sync(active, clamp_lo), b2 = __ballot_sync(active, clamp_hi);
+        if ((threadIdx.x & 31) == __ffs(active) - 1) {
+            if (b0) atomicAdd(counters + 0, (unsigned long long)__popc(b0));
+            if (b1) atomicAdd(counters + 1, (unsigned long long)__popc(b1));
+            if (b2) atomicAdd(counters + 2, (unsigned long long)__popc(b2));
+        }
+    }
     if (rec_out) {
         gt_georec o;
         o.n = n; o.iu0 = (int32_t)iu0; o.iv0 = (int32_t)iv0; o.ju = ju; o.jv = jv;

@@ -16,7 +16,7 @@ struct PhotonExactParams {
     int64_t n_rows, t0;
     int32_t n_chan, n_spaxel;
     float f_sample, sqrt_e0;
-    uint32_t seed_lo, seed_hi;
+    uint32_t seed_lo, seed_hi, spaxel_base;
 };
 
 // block = 256 threads walking spans of 32 whole rows, as kelvin_kernel
@@ -30,7 +30,7 @@ __global__ void __launch_bounds__(256) photon_exact_kernel(PhotonExactParams p) 
         for (uint32_t j = threadIdx.x; j < len; j += 256) {
             const uint32_t rl = j / (uint32_t)p.n_chan, c = j - rl * (uint32_t)p.n_chan;
             const int64_t r = r0 + rl;
-            const uint32_t n = (uint32_t)(p.t0 + r / p.n_spaxel), s = (uint32_t)(r % p.n_spaxel);
+            const uint32_t n = (uint32_t)(p.t0 + r / p.n_spaxel), s = p.spaxel_base + (uint32_t)(r % p.n_spaxel);
             const uint4 w = philox4x32_10(n, s, c, kStreamPhoton, p.seed_lo, p.seed_hi);
             const float half_nep2 = fmaxf(__ldcs(p.lin + base + j) + __ldcs(p.sq + base + j), 0.f);
             const float sigma = sqrt_fast(half_nep2 * p.f_sample) * p.sqrt_e0;

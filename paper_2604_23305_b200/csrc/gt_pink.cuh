@@ -30,6 +30,7 @@ struct PinkParams {
     uint32_t* flags;               // [n_seg][n_det / 256] end state published; zeroed before every launch
     uint32_t* ticket;              // block ticket counter; zeroed before every launch
     uint32_t seed_lo, seed_hi;
+    uint32_t spaxel_base;          // global index of the plan's spaxel 0 (Philox counter word 1)
 };
 
 __device__ __forceinline__ void pink_normals(const PinkParams& p, uint32_t c0, uint32_t s, uint32_t c,
@@ -51,7 +52,7 @@ __global__ void __launch_bounds__(256) pink_init_kernel(PinkParams p) {
     const int64_t d = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (d >= p.n_det) return;
     float z[kPinkMaxJ];
-    pink_normals(p, kCounterInit, (uint32_t)(d / p.n_chan), (uint32_t)(d % p.n_chan), z);
+    pink_normals(p, kCounterInit, p.spaxel_base + (uint32_t)(d / p.n_chan), (uint32_t)(d % p.n_chan), z);
 #pragma unroll
     for (int j = 0; j < kPinkMaxJ; ++j)
         if (j < p.J) p.state[d * p.J + j] = z[j];
@@ -87,7 +88,7 @@ pink_chain_kernel(PinkParams p, int64_t t0, int64_t T, float* __restrict__ tod) 
 #pragma unroll
     for (int j = 0; j < JM; ++j) { g[j] = (valid && j < p.J) ? p.gain[d * p.J + j] : 0.f; x[j] = 0.f; }
     if (valid) {
-        const uint32_t s = (uint32_t)(d / p.n_chan), c = (uint32_t)(d % p.n_chan);
+        const uint32_t s = p.spaxel_base + (uint32_t)(d / p.n_chan), c = (uint32_t)(d % p.n_chan);
         for (int m = 0; m < len; ++m) {
             float z[kPinkMaxJ];
             pink_normals(p, (uint32_t)(t0 + m0 + m), s, c, z);

@@ -24,6 +24,7 @@ struct TkParams {
     float* series;           // [n_det][ld] fp32, ld = 2 (N/2 + 1): half spectrum (complex) before, real series after the FFT
     int64_t ld;
     uint32_t seed_lo, seed_hi;
+    uint32_t spaxel_base;    // global index of the plan's spaxel 0 (Philox counter word 1)
 };
 
 // thread = (detector, frequency index k), k fastest
@@ -34,7 +35,7 @@ __global__ void __launch_bounds__(256) tk_spectrum_kernel(TkParams p) {
     const int64_t d = idx / (K + 1), k = idx - d * (K + 1);
     float re = 0.f, im = 0.f;
     if (k > 0) {
-        const uint4 w = philox4x32_10((uint32_t)k, (uint32_t)(d / p.n_chan), (uint32_t)(d % p.n_chan), kStreamPinkTk,
+        const uint4 w = philox4x32_10((uint32_t)k, p.spaxel_base + (uint32_t)(d / p.n_chan), (uint32_t)(d % p.n_chan), kStreamPinkTk,
                                       p.seed_lo, p.seed_hi);
         float z0, z1;
         normal_pair(w.x, w.y, z0, z1);

@@ -108,6 +108,8 @@ class Workload:
     skydip_pwv_hi_mm: float = 1.5
     # streaming
     chunk_samples: int = 0
+    # global index of spaxel 0 when the workload holds a sub-range of an instrument's spaxels (RNG counter word 1)
+    spaxel_index_base: int = 0
 
     # derived sizes
     @property
