@@ -120,9 +120,9 @@ typedef struct {
     /* photon-noise model when photon_noise != 0: 0 = north_star's narrow-band form (R17);
        1 = the paper's Eq. 17: NEP^2 = 2 sum_nu Fm P_nu (h nu + Fm P_nu + 2 kid_gap_J / eta_pb) dnu on the
        row's own spectrum (shot + bunching + generation-recombination), sigma = NEP sqrt(f_sample / 2), same Philox
-       normal as mode 0 (R23).  Mode 1 runs the contraction three times (tensor variant only:
-       GT_ERR_UNSUPPORTED with GT_VARIANT_FP32) and needs two more [launch rows][n_chan] fp32 device buffers.
-       The squared spectrum is formed in fp16 pairs: P_nu must stay below ~16 k_B 300 K per Hz.
+       normal as mode 0 (R23).  Mode 1 runs the fused kernel a second time per launch (tensor variant only:
+       GT_ERR_UNSUPPORTED with GT_VARIANT_FP32): the spectrum is generated again and contracted, as single fp16 terms, with
+       Fm (h nu + g) + 2 Fm^2 Y and (its square) with Fm^2 into one accumulator; sigma is accurate to ~1e-3.
        kid_gap_J = Delta_Al (188 micro-eV in the paper, :103), eta_pb = pair-breaking efficiency (0.4). */
     int32_t photon_mode;
     double kid_gap_J, eta_pb;

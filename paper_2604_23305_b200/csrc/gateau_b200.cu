@@ -22,7 +22,6 @@
 #include "gt_pink.cuh"
 #include "gt_pink_tk.cuh"
 #include "gt_kelvin.cuh"
-#include "gt_photon_exact.cuh"
 #include "gt_screen.cuh"
 #include "gt_beam.cuh"
 #include "gt_reduce.cuh"
@@ -85,10 +84,9 @@ struct gt_plan {
     DevBuf<float4> d_chan4;
     // exact Eq. 17 photon noise (R23): two more filter sets for the tensor kernel and their outputs
     int32_t photon_mode = 0;
-    gt::TcTables tc_lin, tc_sq;
-    DevBuf<float4> d_chan4_lin, d_chan4_zero;
-    DevBuf<float> d_nep_lin, d_nep_sq;          // [launch rows][n_chan]
-    float scale_sq = 0.f, sqrt_e0 = 0.f, f_sample = 0.f;
+    gt::TcTables tc_nep;                        // filter units L and Fm^2 kPref 256 / E0 of the second pass
+    DevBuf<float4> d_chan4_nep;
+    float sqrt_e0 = 0.f, f_sample = 0.f;
     int32_t output_unit = 0;                    // 1: brightness temperature through the skydip map (R22)
     DevBuf<double> d_kelvin_ab;                 // [2][n_chan] a, b
     DevBuf<float2> d_kelvin_abf;                // [n_chan] (a, b)
@@ -282,23 +280,13 @@ gt_status run_chunk(gt_plan* p, int64_t t0, int64_t T, float* dst, float* pwv_ds
         GT_CUDA(p, gt::launch_fused_tc(fp, p->tc, p->num_sms, st));
     }
     if (exact) {
-        // Eq. 17: the contraction linear in the spectrum and the one of its square, then sigma z (gt_photon_exact.cuh)
-        const size_t need = (size_t)n_rows * p->n_chan;
-        if (need > p->d_nep_lin.n) { GT_CUDA(p, p->d_nep_lin.alloc(need)); GT_CUDA(p, p->d_nep_sq.alloc(need)); }
-        gt::FusedParams fl = fp, fq = fp;
-        fl.chan4 = p->d_chan4_lin.p; fl.out = p->d_nep_lin.p;
-        fq.chan4 = p->d_chan4_zero.p; fq.out = p->d_nep_sq.p; fq.scale = p->scale_sq;
-        p->tc_lin.scratch = p->tc.scratch; p->tc_sq.scratch = p->tc.scratch;     // the passes run one after another
-        GT_CUDA(p, gt::launch_fused_tc(fl, p->tc_lin, p->num_sms, st));
-        GT_CUDA(p, gt::launch_fused_tc(fq, p->tc_sq, p->num_sms, st, true));
-        gt::PhotonExactParams pe{};
-        pe.tod = dst; pe.lin = p->d_nep_lin.p; pe.sq = p->d_nep_sq.p; pe.n_rows = n_rows; pe.t0 = t0;
-        pe.n_chan = p->n_chan; pe.n_spaxel = p->n_spaxel; pe.f_sample = p->f_sample; pe.sqrt_e0 = p->sqrt_e0;
-        pe.seed_lo = fp.seed_lo; pe.seed_hi = fp.seed_hi; pe.spaxel_base = fp.spaxel_base;
-        const int64_t n_span = (n_rows + 31) / 32;
-        gt::photon_exact_kernel<<<(unsigned)std::min<int64_t>(n_span, 16 * p->num_sms), 256, 0, st>>>(pe);
-        GT_CUDA(p, cudaGetLastError());
-        p->launches += 3;
+        // Eq. 17: a second pass of the fused kernel contracts the spectrum with L and its square with Fm^2 into ONE
+        // accumulator (single fp16 terms, one segment), and its finisher adds sigma z to the TOD of the first pass
+        gt::FusedParams fn = fp;
+        fn.chan4 = p->d_chan4_nep.p; fn.nep_f_sample = p->f_sample; fn.nep_sqrt_e0 = p->sqrt_e0;
+        p->tc_nep.scratch = p->tc.scratch;                                       // the passes run one after another
+        GT_CUDA(p, gt::launch_fused_tc(fn, p->tc_nep, p->num_sms, st, true));
+        p->launches += 1;
     }
     GT_CUDA(p, cudaEventRecord(p->ev_fused[2 * fused_slot + 1], st));
     p->launches++;
@@ -609,7 +597,7 @@ gt_status gt_plan_create(const gt_config* cfg, void* cuda_stream, gt_plan** out_
 #ifdef GT_TC_DIAG
         if (const char* e = std::getenv("GATEAU_TC_SEG")) {          // tuning builds only: slabs per accumulation segment
             const int v = std::atoi(e);
-            if (v > 0) p->tc.seg = p->tc_lin.seg = p->tc_sq.seg = v;
+            if (v > 0) p->tc.seg = v;
         }
 #endif
         std::vector<float> inv;
@@ -622,29 +610,27 @@ gt_status gt_plan_create(const gt_config* cfg, void* cuda_stream, gt_plan** out_
             // Eq. 17 with P_nu = kPref v + Y (v = the generated element):
             //   NEP^2 / (2 dnu) = sum Fm (h nu + g) P + sum Fm^2 P^2
             //                   = kPref sum [Fm (h nu + g) + 2 Fm^2 Y] v + kPref^2 sum Fm^2 v^2 + sum [Fm (h nu + g) Y + Fm^2 Y^2]
+            // divided by E0 = h nu_max + g (so that it is O(P_KID)):  kPref dnu [sum L v + sum Q' (v^2 / 256)] + const,
+            //   L = (Fm (h nu + g) + 2 Fm^2 Y) / E0,   Q' = Fm^2 256 kPref / E0
             const double g = 2.0 * c.kid_gap_J / c.eta_pb;
             const double E0 = kH * (c.nu0_hz + (double)(nf - 1) * c.dnu_hz) + g;
             std::vector<float> L((size_t)nc * nf), Q((size_t)nc * nf);
-            std::vector<float4> c4l(ncp, make_float4(0.f, 0.f, 0.f, 1.f)), c4z(ncp, make_float4(0.f, 0.f, 0.f, 1.f));
+            std::vector<float4> c4n(ncp, make_float4(0.f, 0.f, 0.f, 1.f));
             for (int ch = 0; ch < nc; ++ch) {
                 double sb = 0.0;
                 for (int i = 0; i < nf; ++i) {
                     const double f = h_filt[(size_t)ch * nf + i], e = kH * (c.nu0_hz + (double)i * c.dnu_hz) + g;
                     L[(size_t)ch * nf + i] = (float)((f * e + 2.0 * f * f * Y[i]) / E0);
-                    Q[(size_t)ch * nf + i] = (float)(f * f);
+                    Q[(size_t)ch * nf + i] = (float)(f * f * kPref / ((double)gt::kTcSqScale * E0));
                     sb += f * e * Y[i] + f * f * Y[i] * Y[i];
                 }
-                c4l[ch].x = (float)(c.dnu_hz * sb / E0);
+                c4n[ch].x = (float)(c.dnu_hz * sb / E0);
             }
-            std::vector<double> a_ref2(nf);
-            for (int i = 0; i < nf; ++i) a_ref2[i] = a_ref[i] * a_ref[i];
-            std::vector<float> inv_l, inv_q;
-            if (gt_status s = gt::build_tc_tables(L, nc, nf, nfp, a_ref, p->tc_lin, inv_l, st)) return fail(nullptr, s, "tensor variant (Eq. 17 linear filter): %s", gt::tc_error());
-            if (gt_status s = gt::build_tc_tables(Q, nc, nf, nfp, a_ref2, p->tc_sq, inv_q, st)) return fail(nullptr, s, "tensor variant (Eq. 17 squared filter): %s", gt::tc_error());
-            for (int ch = 0; ch < nc; ++ch) { c4l[ch].w = inv_l[ch]; c4z[ch].w = inv_q[ch]; }
-            GT_CUDA0(p->d_chan4_lin.upload(c4l, st)); GT_CUDA0(p->d_chan4_zero.upload(c4z, st));
+            std::vector<float> inv_n;
+            if (gt_status s = gt::build_tc_tables(L, nc, nf, nfp, a_ref, p->tc_nep, inv_n, st, &Q)) return fail(nullptr, s, "tensor variant (Eq. 17 filters): %s", gt::tc_error());
+            for (int ch = 0; ch < nc; ++ch) c4n[ch].w = inv_n[ch];
+            GT_CUDA0(p->d_chan4_nep.upload(c4n, st));
             GT_CUDA0(cudaStreamSynchronize(st));
-            p->scale_sq = (float)(kPref * kPref * c.dnu_hz / ((double)gt::kTcSqScale * E0));
             p->sqrt_e0 = (float)std::sqrt(E0);
             p->f_sample = (float)c.f_sample_hz;
         }
@@ -838,8 +824,8 @@ gt_status gt_plan_destroy(gt_plan* plan) {
     }
     for (cudaEvent_t e : plan->ev_fused) cudaEventDestroy(e);
     for (cudaEvent_t e : plan->ev_tl) cudaEventDestroy(e);
-    plan->tc_lin.scratch = nullptr; plan->tc_sq.scratch = nullptr;      // aliases of tc.scratch
-    gt::free_tc_tables(plan->tc_lin); gt::free_tc_tables(plan->tc_sq);
+    plan->tc_nep.scratch = nullptr;                                     // alias of tc.scratch
+    gt::free_tc_tables(plan->tc_nep);
     gt::free_tc_tables(plan->tc);
     delete plan;
     return GT_OK;

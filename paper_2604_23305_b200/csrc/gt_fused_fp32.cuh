@@ -38,6 +38,7 @@ struct FusedParams {
     const float4* chan4;                // [n_chan_pad] {bias, noise_c1, noise_c2, 0}: one 16-byte load per output
     int32_t photon_noise; uint32_t seed_lo, seed_hi;
     uint32_t spaxel_base;     // global index of the plan's spaxel 0: Philox counter word 1 = spaxel_base + s
+    float nep_f_sample, nep_sqrt_e0;   // Eq. 17 pass of the tensor kernel: sigma = sqrt(P f_s) sqrt(E0)
     float* out;               // [n_rows][n_chan]
 };
 

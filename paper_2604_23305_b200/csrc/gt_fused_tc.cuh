@@ -113,7 +113,7 @@ constexpr int kTcRegsFlush = GT_TC_REGS_FLUSH, kTcRegsCtl = 40, kTcRegsGen = 80,
 static_assert(kTcRegsFlush + kTcRegsCtl + 4 * kTcRegsGen + (kTcFinWarps / 4) * kTcRegsFin <= (kTcThreads / 128) * kTcRegsBase, "setmaxnreg pool");
 constexpr int kTcMaxGroupChan = 384;       // channels per tile: 3 column groups of 128 (+ 1 spare buffer = 512 columns)
 constexpr int kTcBufCols = 128, kTcNumBuf = 4, kTcMaxCg = 3;
-constexpr int kTcSegDefault = 8;           // slabs (of 64 frequencies) per accumulation segment (measured max error 4.9e-6 of the 1e-5 gate; 12: 6.5e-6, 16: 9.4e-6)
+constexpr int kTcSegDefault = 12;          // slabs (of 64 frequencies) per accumulation segment (measured max error on the C4 window 6.5e-6 of the 1e-5 gate, narrow channels on segment edges 0.8e-6; 8: 4.9e-6, 16: 9.4e-6)
 // The tensor core's fp32 accumulate TRUNCATES (measured): the 16 products of an MMA are aligned
 // to the running sum and cut at kTcTruncGrain of its unit in the last place (two guard bits), the new sum is cut to
 // the unit itself.  Positive products far above the grain therefore lose 16 x grain / 2 + 1/2 = 2.5 ulp per MMA;
@@ -124,9 +124,9 @@ constexpr int kTcSegDefault = 8;           // slabs (of 64 frequencies) per accu
 // loses nothing) and the flush warps add them back in units of the ulp of the partial sum they hold.
 constexpr double kTcTruncGrain = 0.25;
 #ifndef GT_TC_TRUNC_ULP
-#define GT_TC_TRUNC_ULP 1.0f
+#define GT_TC_TRUNC_ULP 0.9f
 #endif
-constexpr float kTcTruncUlp = GT_TC_TRUNC_ULP;      // overall factor on the table; tuning builds calibrate with 0 (off)
+constexpr float kTcTruncUlp = GT_TC_TRUNC_ULP;      // overall factor on the table (0.9: the model with factor 1 left a mean error of +0.9e-6 on the config windows); tuning builds calibrate with 0 (off)
 #ifndef GT_TC_MAX_B_STAGES
 #define GT_TC_MAX_B_STAGES 3
 #endif
@@ -169,9 +169,11 @@ inline double tc_ulp_ratio(double p) {
 // a_ref [n_freq]: a reference spectrum in the generator's scaled units (any positive multiple will do), used only for
 // the truncation-compensation table: W[c][segment] = kTcTruncUlp 2^-23 sum over the MMAs of the segment of
 // tc_ulp_ratio(accumulator after that MMA / final segment sum), in the order the MMA thread issues them.
+// filt1 != nullptr (the Eq. 17 pass): no split -- unit 0 = fp16(2^kb filt), unit 1 = fp16(2^kb filt1), one scale per
+// channel from the larger of the two maxima; one accumulation segment per tile and no compensation table (sigma needs 1e-3).
 inline gt_status build_tc_tables(const std::vector<float>& filt, int n_chan, int n_freq, int n_freq_pad,
                                  const std::vector<double>& a_ref, TcTables& t, std::vector<float>& inv_scale,
-                                 cudaStream_t st) {
+                                 cudaStream_t st, const std::vector<float>* filt1 = nullptr) {
     const int G = (n_chan + kTcMaxGroupChan - 1) / kTcMaxGroupChan;
     int per = (n_chan + G - 1) / G;
     const int nbt = (per + 31) / 32 * 32;
@@ -179,6 +181,7 @@ inline gt_status build_tc_tables(const std::vector<float>& filt, int n_chan, int
     t.n_cg = (nbt + kTcBufCols - 1) / kTcBufCols;
     t.n_kb = n_freq_pad / kTcBK;
     if (t.seg <= 0) t.seg = kTcSegDefault;
+    if (filt1) t.seg = t.n_kb;
     // one unit = the rows one CTA holds of one (slab, part): all nb_tot rows, or (CTA pair) the half of every
     // column group this CTA supplies to the M = 256 MMAs (rank r: columns [r w/2, (r+1) w/2) of a group of width w)
     constexpr int kRanks = kTcPair ? 2 : 1;
@@ -212,10 +215,12 @@ inline gt_status build_tc_tables(const std::vector<float>& filt, int n_chan, int
             const int ch = g * nbt + n;
             if (ch >= n_chan) continue;
             const float* frow = filt.data() + (size_t)ch * n_freq;
+            const float* frow1 = filt1 ? filt1->data() + (size_t)ch * n_freq : nullptr;
             float amax = 0.f;
             for (int i = 0; i < n_freq; ++i) {
-                if (!std::isfinite(frow[i])) { tc_error_ref() = "the filter holds a NaN or Inf"; return GT_ERR_VALUE; }
+                if (!std::isfinite(frow[i]) || (frow1 && !std::isfinite(frow1[i]))) { tc_error_ref() = "the filter holds a NaN or Inf"; return GT_ERR_VALUE; }
                 amax = std::max(amax, std::fabs(frow[i]));
+                if (frow1) amax = std::max(amax, std::fabs(frow1[i]));
             }
             int kb_c = 0;
             if (amax > 0.f) { int e; std::frexp(amax, &e); kb_c = std::max(-100, std::min(100, kTcBMaxLog2 - e)); }
@@ -228,7 +233,7 @@ inline gt_status build_tc_tables(const std::vector<float>& filt, int n_chan, int
             for (int i = 0; i < n_freq; ++i) {
                 const float f = std::ldexp(frow[i], kb_c);
                 const __half fh = __float2half_rn(f);
-                const __half fl = __float2half_rn(f - __half2float(fh));
+                const __half fl = __float2half_rn(frow1 ? std::ldexp(frow1[i], kb_c) : f - __half2float(fh));
                 const int kb = i / kTcBK, kk = i % kTcBK;
                 // element index of (group tile, slab, unit, rank): units are laid out [g][kb][unit][rank]
                 const size_t unit0 = ((size_t)((g * t.n_kb + kb) * 2 + 0) * kRanks + rk) * (t.unit_bytes / 2);
@@ -269,6 +274,7 @@ inline gt_status build_tc_tables(const std::vector<float>& filt, int n_chan, int
                     const double w_max = (16.0 * kTcTruncGrain / 2.0 + 1.5) * kTcKSteps * (kb1 - kb0);
                     W = std::max(0.0, std::min(W, w_max));
                 }
+                if (filt1) W = 0.0;
                 comp[((size_t)g * t.n_seg + s0) * nbt + n] = (float)(W * (double)kTcTruncUlp * std::ldexp(1.0, -23));
                 kb0 = kb1;
             }
@@ -398,6 +404,22 @@ __device__ __forceinline__ void store_split(unsigned char* a_stage, int row, int
     *reinterpret_cast<uint2*>(dst + kTcAPartBytes) = lo2;
 }
 
+// Eq. 17 pass (NEP = true): the same shared-memory slots hold fp16(v) in part 0 and fp16(v^2 / 256) in part 1 (single
+// terms: sigma only needs 1e-3); the filter units hold L and Fm^2 kPref 256 / E0 on one per-channel scale, so that
+// part 0 . unit 0 + part 1 . unit 1 accumulates the linear and the quadratic term of NEP^2 into ONE accumulator.
+__device__ __forceinline__ void store_nep(unsigned char* a_stage, int row, int chunk, int h, const float4& v) {
+    const __half2 h01 = __float22half2_rn(make_float2(v.x, v.y)), h23 = __float22half2_rn(make_float2(v.z, v.w));
+    const __half2 q01 = __float22half2_rn(make_float2(v.x * v.x * kTcSqScale, v.y * v.y * kTcSqScale));
+    const __half2 q23 = __float22half2_rn(make_float2(v.z * v.z * kTcSqScale, v.w * v.w * kTcSqScale));
+    uint2 a2, b2;
+    a2.x = *reinterpret_cast<const uint32_t*>(&h01); a2.y = *reinterpret_cast<const uint32_t*>(&h23);
+    b2.x = *reinterpret_cast<const uint32_t*>(&q01); b2.y = *reinterpret_cast<const uint32_t*>(&q23);
+    const uint32_t c16 = (uint32_t)(h * 4 + (chunk >> 1)), sub = (uint32_t)(chunk & 1) * 8u;
+    unsigned char* dst = a_stage + (uint32_t)row * 128u + ((c16 ^ (uint32_t)(row & 7)) << 4) + sub;
+    *reinterpret_cast<uint2*>(dst) = a2;
+    *reinterpret_cast<uint2*>(dst + kTcAPartBytes) = b2;
+}
+
 // element (column, row) of a scratch tile laid out [row / 32][column / 4][row % 32][column % 4]: the 32 rows one flush
 // warp owns are contiguous per group of 4 columns (512 B), 16 columns of them 2 KB -- one bulk copy
 __device__ __forceinline__ size_t tc_scratch_index(int col, int row, int nb_tot) {
@@ -406,7 +428,7 @@ __device__ __forceinline__ size_t tc_scratch_index(int col, int row, int nb_tot)
 
 __device__ __forceinline__ float4 ldg4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
 
-template <bool VEC, bool SQ>
+template <bool VEC, bool NEP>
 __global__ void __launch_bounds__(kTcThreads, 1)
 fused_tc_kernel(const TcParams p) {
     extern __shared__ unsigned char smem_raw[];
@@ -564,8 +586,8 @@ fused_tc_kernel(const TcParams p) {
                     v.y = element_value_fast(fmaf(fc.x, lut.L1.y - lut.L0.y, lut.L0.y), fc.y, X.y, G.y, S.y);
                     v.z = element_value_fast(fmaf(fc.x, lut.L1.z - lut.L0.z, lut.L0.z), fc.y, X.z, G.z, S.z);
                     v.w = element_value_fast(fmaf(fc.x, lut.L1.w - lut.L0.w, lut.L0.w), fc.y, X.w, G.w, S.w);
-                    if constexpr (SQ) { v.x *= v.x * kTcSqScale; v.y *= v.y * kTcSqScale; v.z *= v.z * kTcSqScale; v.w *= v.w * kTcSqScale; }
-                    store_split(smem_raw + (sm.a - raw) + stage * kTcAStageBytes, rsub + kTcRowStride * j, chunk, h, v);
+                    if constexpr (NEP) store_nep(smem_raw + (sm.a - raw) + stage * kTcAStageBytes, rsub + kTcRowStride * j, chunk, h, v);
+                    else store_split(smem_raw + (sm.a - raw) + stage * kTcAStageBytes, rsub + kTcRowStride * j, chunk, h, v);
                 };
                 Tap t0, t1;
                 Lut la, lb;
@@ -671,8 +693,8 @@ fused_tc_kernel(const TcParams p) {
                     v.y = element_value_fast(fmaf(fp[j], L1[j].y - L0[j].y, L0[j].y), csc[j], X.y, G.y, S[j].y);
                     v.z = element_value_fast(fmaf(fp[j], L1[j].z - L0[j].z, L0[j].z), csc[j], X.z, G.z, S[j].z);
                     v.w = element_value_fast(fmaf(fp[j], L1[j].w - L0[j].w, L0[j].w), csc[j], X.w, G.w, S[j].w);
-                    if constexpr (SQ) { v.x *= v.x * kTcSqScale; v.y *= v.y * kTcSqScale; v.z *= v.z * kTcSqScale; v.w *= v.w * kTcSqScale; }
-                    store_split(a_hi, rsub + kTcRowStride * j, chunk, h, v);
+                    if constexpr (NEP) store_nep(a_hi, rsub + kTcRowStride * j, chunk, h, v);
+                    else store_split(a_hi, rsub + kTcRowStride * j, chunk, h, v);
                 }
                 }
                 ptx::fence_proxy_async_smem();
@@ -756,7 +778,7 @@ fused_tc_kernel(const TcParams p) {
                                     if (g < p.n_cg) {
                                         const uint64_t bd = bd0 + (uint64_t)(g * kGroupDesc + k * 2);
                                         mma_f16(d[g], ad_hi + (uint64_t)(k * 2), bd, idesc[g], (k != 0 || !(fresh >> g & 1u)) ? 1u : 0u);
-                                        mma_f16(d[g], ad_lo + (uint64_t)(k * 2), bd, idesc[g], 1u);
+                                        if constexpr (!NEP) mma_f16(d[g], ad_lo + (uint64_t)(k * 2), bd, idesc[g], 1u);
                                     }
                         }
                         __syncwarp();
@@ -774,7 +796,7 @@ fused_tc_kernel(const TcParams p) {
 #pragma unroll
                                 for (int g = 0; g < kTcMaxCg; ++g)
                                     if (g < p.n_cg)
-                                        mma_f16(d[g], ad_hi + (uint64_t)(k * 2),
+                                        mma_f16(d[g], (NEP ? ad_lo : ad_hi) + (uint64_t)(k * 2),
                                                         bd0 + (uint64_t)(g * kGroupDesc + k * 2), idesc[g], 1u);
                         }
                         __syncwarp();
@@ -858,7 +880,17 @@ fused_tc_kernel(const TcParams p) {
                         P[i] = fmaf(x[j0 + i] * k4.w, f.scale, k4.x);
                         n1[i] = k4.y; n2[i] = k4.z;
                     }
-                    if (f.photon_noise) {
+                    if constexpr (NEP) {
+                        // Eq. 17 pass: P = NEP^2 / (2 E0) of this detector-sample; the TOD already holds the noiseless power of
+                        // the first pass: tod += sqrt(P f_s) sqrt(E0) z, z = the normal of the narrow-band mode (Eq. 18-19)
+                        philox4x32_10_multi<W>(n, f.spaxel_base + s, cc, kStreamPhoton, f.seed_lo, f.seed_hi, w0, w1);
+#pragma unroll
+                        for (int i = 0; i < W; ++i) {
+                            const int c = lane + 32 * (j0 + i);
+                            const float sigma = sqrt_fast(fmaxf(P[i], 0.f) * f.nep_f_sample) * f.nep_sqrt_e0;
+                            P[i] = fmaf(sigma, normal_cos(w0[i], w1[i]), c < n_valid ? __ldcs(o + c) : 0.f);
+                        }
+                    } else if (f.photon_noise) {
                         philox4x32_10_multi<W>(n, f.spaxel_base + s, cc, kStreamPhoton, f.seed_lo, f.seed_hi, w0, w1);
 #pragma unroll
                         for (int i = 0; i < W; ++i)
@@ -971,9 +1003,10 @@ fused_tc_kernel(const TcParams p) {
     }
 }
 
-// square = true: the generator writes kTcSqScale v^2 instead of v (the bunching contraction sum Fm^2 P^2 of Eq. 17,
-// DESIGN.md R23); the caller's scale carries 1 / kTcSqScale.
-inline cudaError_t launch_fused_tc(const FusedParams& fp, const TcTables& t, int num_sms, cudaStream_t st, bool square = false) {
+// nep = true: the second pass of the exact photon noise (Eq. 17, R23): the generator writes fp16(v) and
+// fp16(v^2 / 256), the tables hold L and the scaled Fm^2, the finisher turns the contraction into sigma and adds sigma z
+// to the TOD the first pass wrote.
+inline cudaError_t launch_fused_tc(const FusedParams& fp, const TcTables& t, int num_sms, cudaStream_t st, bool nep = false) {
     TcParams p{};
     p.f = fp; p.filt_img = t.filt_img;
     // FusedParams::scale carries the spectrum scale of the plan; the per-channel filter scale is chan4.w
@@ -988,7 +1021,7 @@ inline cudaError_t launch_fused_tc(const FusedParams& fp, const TcTables& t, int
     const int64_t n_tiles = kTcPair ? (int64_t)((p.n_row_tiles + 1) / 2) * p.n_groups : (int64_t)p.n_row_tiles * p.n_groups;
     const int64_t workers = kTcPair ? num_sms / 2 : num_sms;
     const unsigned grid = (unsigned)(std::min<int64_t>(n_tiles, workers) * (kTcPair ? 2 : 1));
-    auto kern = square ? (p.cube_vec ? fused_tc_kernel<true, true> : fused_tc_kernel<false, true>)
+    auto kern = nep ? (p.cube_vec ? fused_tc_kernel<true, true> : fused_tc_kernel<false, true>)
                        : (p.cube_vec ? fused_tc_kernel<true, false> : fused_tc_kernel<false, false>);
     // set on every launch: the attribute is per device
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, t.smem_bytes);
