@@ -429,5 +429,39 @@ def source_power(I_cube, nu_hz, daz_rad, del_rad, el_first_rad, r_pix, R_tel_m, 
     return out
 
 
+def eta_zenith_at(w, f_hz, pwv_mm):
+    """Zenith transmission eta_atm,z(f) of the workload's lookup table at frequencies f_hz and one PWV: bilinear on the
+    table's own grid, PWV clamped to the table (R13) -- the per-channel transmission Eq. 25 starts from (PAPER.md:366:
+    "the zenith PWV ... averaged over the entire observation and used to calculate eta_atm,z(f)")."""
+    lut = np.asarray(w.atm_lut, dtype=np.float64)
+    n_pwv, n_nu = lut.shape
+    q = min(max((pwv_mm - w.lut_pwv0_mm) / w.lut_dpwv_mm, 0.0), n_pwv - 1.0)
+    ip = min(int(np.floor(q)), n_pwv - 2)
+    fp = q - ip
+    r = (np.asarray(f_hz, dtype=np.float64) - w.lut_nu0_hz) / w.lut_dnu_hz
+    ir = np.clip(np.floor(r).astype(int), 0, n_nu - 2)
+    fr = r - ir
+    row0 = (1 - fr) * lut[ip, ir] + fr * lut[ip, ir + 1]
+    row1 = (1 - fr) * lut[ip + 1, ir] + fr * lut[ip + 1, ir + 1]
+    return (1 - fp) * row0 + fp * row1
+
+
+def common_mode_subtract(T_b, eta_z, csc, daz_rad, del_rad, r_out_rad):
+    """Eq. 25-26, literally, in double.  T_b [t][spaxel][chan] brightness temperature, eta_z [chan]
+    zenith transmission, csc [t][spaxel] = 1 / sin(elevation) (Eq. 10: eta_j(t,f) = eta_z(f)^csc_j(t)), spaxel offsets
+    daz, del [spaxel]:
+        S_j = 1 if sqrt(daz_j^2 + del_j^2) > r_out else 0,   N_out = sum_j S_j,
+        T*_a,i = T_b,i / eta_i - (1 - eta_i) / (eta_i N_out) sum_j S_j T_b,j / (1 - eta_j).
+    Returns (T*_a, S, common) with common[t][chan] = sum_j S_j T_b,j / (1 - eta_j)."""
+    T_b = np.asarray(T_b, dtype=np.float64)
+    eta = np.asarray(eta_z, dtype=np.float64)[None, None, :] ** np.asarray(csc, dtype=np.float64)[:, :, None]
+    S = (np.sqrt(np.asarray(daz_rad, dtype=np.float64) ** 2 + np.asarray(del_rad, dtype=np.float64) ** 2) > r_out_rad).astype(np.float64)
+    n_out = S.sum()
+    if n_out < 1:
+        raise ValueError("Eq. 25: no spaxel lies outside r_out")
+    common = (S[None, :, None] * T_b / (1.0 - eta)).sum(axis=1)
+    return T_b / eta - (1.0 - eta) / (eta * n_out) * common[:, None, :], S, common
+
+
 def num_threads():
     return lib().go_num_threads()
