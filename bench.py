@@ -41,6 +41,10 @@ def parse():
     ap.add_argument("--workload", default="C4")
     ap.add_argument("--variant", default="default", choices=["default", "fp32", "tensor"])
     ap.add_argument("--samples", type=int, default=None, help="shrink n_samples (debug only; marks the line invalid)")
+    ap.add_argument("--shard", default="replica", choices=["replica", "spaxel"],
+                    help="N > 1: 'replica' = independent observations per rank (weak scaling, the default); 'spaxel' = the "
+                         "workload's spaxels split over the ranks, Kelvin output and the common-mode subtraction of Eq. 25 "
+                         "with its one all-reduce over [t x chan] inside the step (strong scaling)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
@@ -259,8 +263,10 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     w = W.make_workload(args.workload, n_samples=args.samples)
-    w = w.replace(seed=shard.replica_seed(w.seed, rank))          # independent observation per rank
     variant = {"default": B.VARIANT_DEFAULT, "fp32": B.VARIANT_FP32, "tensor": B.VARIANT_TENSOR}[args.variant]
+    if args.shard == "spaxel":
+        return run_spaxel_sharded(args, torch, dist, B, W, shard, w, variant, rank, world, local, barrier)
+    w = w.replace(seed=shard.replica_seed(w.seed, rank))          # independent observation per rank
     plan = B.Plan(w, variant=variant, device=f"cuda:{local}")
     units = w.detector_samples()
     tod = torch.empty((w.n_samples, w.n_spaxel, w.n_chan), dtype=torch.float32, device=f"cuda:{local}")
@@ -367,6 +373,59 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_spaxel_sharded(args, torch, dist, B, W, shard, w, variant, rank, world, local, barrier):
+    """Strong scaling over spaxels: rank r simulates spaxels [b_r, e_r) of the SAME observation in
+    kelvin (RNG counters keep the global spaxel index), then the common-mode subtraction of Eq. 25: per-rank partial sums
+    over [t x chan] (gt_common_mode_partial), ONE all-reduce (NCCL), gt_common_mode_apply on the rank's own slab."""
+    dev = f"cuda:{local}"
+    b, e = shard.partition_spaxels(w.n_spaxel, world)[rank]
+    wk = w.replace(output_unit=1, skydip_pwv_lo_mm=0.6, skydip_pwv_hi_mm=1.4)
+    r_out = 0.6 * float(np.max(np.hypot(w.daz_rad, w.del_rad))) if w.n_spaxel > 1 else -1.0
+    plan = B.Plan(shard.shard_workload(wk, b, e), variant=variant, device=dev)
+    tod = torch.empty((w.n_samples, e - b, w.n_chan), dtype=torch.float32, device=dev)
+    pwv = torch.empty((w.n_samples, e - b), dtype=torch.float32, device=dev)
+    grp = dist if world > 1 else None
+
+    def step():
+        plan.simulate(out=tod, pwv_out=pwv)
+        acc = torch.stack([pwv.double().sum(), torch.tensor(float(pwv.numel()), dtype=torch.float64, device=dev)])
+        if world > 1:
+            dist.all_reduce(acc)
+        pwv_mean = float((acc[0] / acc[1]).item())                 # PAPER.md:366: the zenith PWV averaged over the observation
+        partial, n_out = plan.common_mode_partial(tod, pwv_mean, r_out)
+        total, n_tot = shard.common_mode_allreduce(partial, n_out, grp)
+        plan.common_mode_apply(tod, pwv_mean, total, n_tot)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    sampler = ClockSampler(local); sampler.start()
+    launches0 = plan.launch_count
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record(); e1.synchronize()
+    barrier()
+    total_ms = shard.max_over_ranks(e0.elapsed_time(e1), grp, device=dev)
+    clocks = sampler.stop()
+    launches = plan.launch_count - launches0
+    name = plan.variant_name
+    plan.destroy()
+    if rank == 0:
+        line = {"metric": METRIC, "value": w.detector_samples() * args.steps / (total_ms * 1e-3), "unit": UNIT, "n_gpus": world,
+                "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+                "scaling": "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": workload_config(w, {"variant": name, "parallelism": f"spaxel-shard x{world}",
+                                              "step": "gt_simulate in kelvin + Eq. 25 common-mode subtraction (per-rank partial sums, "
+                                                      "one all-reduce over [t x chan], apply)", "rank0_spaxels": [b, e]}),
+                "clocks": clocks, "gpu_launches": int(launches), "e2e": None, "roofline": None, "cpu_baseline": None}
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def run_extras(torch, B, w, local, tod):
     """Device-resident step times of the paper's own options (rows f1-f3), same workload: one warm-up + two timed steps."""
     out = {}
@@ -403,10 +462,10 @@ def run_e2e(torch, B, w, variant, local, world, steps, barrier, timeline=None):
     out = torch.empty((w.n_samples, w.n_spaxel, w.n_chan), dtype=torch.float32, pin_memory=True)
     d2h = out.numel() * 4
 
-    # the workload's large arrays now live in pinned host memory (views of the pinned tensors)
-    wp = w.replace(**{k: v.numpy() for k, v in host.items()})
+    # the workload's large arrays now live in pinned host memory: the binding copies the pinned tensors as they are
+    wp = w.replace(**host)
 
-    parts = {"h2d_and_create_ms": 0.0, "simulate_ms": 0.0, "destroy_ms": 0.0}
+    parts = {"h2d_ms": 0.0, "plan_create_ms": 0.0, "simulate_ms": 0.0, "destroy_ms": 0.0}
 
     def one(record=None):
         # B.Plan copies the pinned arrays to the device (H2D) and creates the plan; simulate streams to `out`
@@ -432,7 +491,8 @@ def run_e2e(torch, B, w, variant, local, world, steps, barrier, timeline=None):
                         f"span {tl[-1][3]:.1f} ms\n")
         p.destroy()
         t3 = time.perf_counter()
-        parts["h2d_and_create_ms"] += 1e3 * (t1 - t0); parts["simulate_ms"] += 1e3 * (t2 - t1); parts["destroy_ms"] += 1e3 * (t3 - t2)
+        parts["h2d_ms"] += p.upload_ms; parts["plan_create_ms"] += p.create_ms
+        parts["simulate_ms"] += 1e3 * (t2 - t1); parts["destroy_ms"] += 1e3 * (t3 - t2)
 
     one(record=timeline)                                         # warm-up (allocators, pinned pages)
     for k in parts:

@@ -177,6 +177,11 @@ gt_status gt_plan_create(const gt_config* cfg, void* cuda_stream, gt_plan** out_
 gt_status gt_simulate(gt_plan* plan, int64_t t_begin, int64_t t_count,
                       float* tod_out, float* pwv_out, void* cuda_stream);
 
+/* Device memory of the plans comes from a library-owned stream-ordered pool that keeps what destroyed plans return, so
+ * that creating plans back to back (one observation per plan) does not pay cudaMalloc / cudaFree every time.  This call
+ * returns the cached blocks of the current device to the driver (it synchronises the device). */
+gt_status gt_release_cached_memory(void);
+
 /* Frees everything the plan owns, after waiting for the work the plan itself enqueued (the stream of its last call
  * and its internal copy stream).  NULL-safe. */
 gt_status gt_plan_destroy(gt_plan* plan);
@@ -206,6 +211,26 @@ gt_status gt_prepare_source(const float* I_dev, int32_t n_az, int32_t n_el, int3
  * GT_ERR_UNSUPPORTED if R_tel spans more than 64 pixels in x or y. */
 gt_status gt_prepare_screen(const float* epl_dev, int32_t nx, int32_t ny, double dx_m, double dy_m,
                             double R_tel_m, double t_edge_db, double pwv0_mm, float* pwv_dev, void* cuda_stream);
+
+/* Common-mode subtraction, Eq. 25-26, on a TOD in brightness temperature (output_unit = 1):
+ *   T*_a,i(t,f) = T_b,i / eta_i - (1 - eta_i) / (eta_i N_out) sum_j S_j T_b,j / (1 - eta_j),
+ *   eta_j(t,f) = eta_atm,z(f)^csc(el0 + el[t] + del[j]) (Eq. 10), eta_atm,z(f) = the plan's lookup table, bilinear at
+ *   (f_center[f], pwv_mean_mm) (the zenith PWV averaged over the observation; clamped to the table),
+ *   S_j = 1 where sqrt(daz_j^2 + del_j^2) > r_out_rad, N_out = sum_j S_j.
+ * The sum over spaxels is the only cross-spaxel term of the paper, so it is split for spaxel-sharded runs (one plan per
+ * spaxel sub-range, spaxel_index_base):
+ *   gt_common_mode_partial: partial_dev[t][chan] (DEVICE, fp32, overwritten) = sum over THIS plan's spaxels of
+ *       S_j T_b,j / (1 - eta_j), and *n_out = this plan's number of spaxels with S_j = 1.  tod_K_dev DEVICE
+ *       [t_count][n_spaxel][n_chan], read only.
+ *   -- the caller adds partial sums and n_out over the plans (one all-reduce over [t x chan]) --
+ *   gt_common_mode_apply: tod_K_dev <- T*_a in place, given sum_dev[t][chan] over ALL spaxels and n_out_total >= 1.
+ * A single plan holding every spaxel calls both with its own partial sum.  Asynchronous on cuda_stream (after a short
+ * synchronous upload of per-channel constants).  GT_ERR_RANGE if a channel centre lies outside the table,
+ * GT_ERR_VALUE if a channel is fully transparent (1 - eta = 0) or n_out_total < 1. */
+gt_status gt_common_mode_partial(gt_plan* plan, int64_t t_begin, int64_t t_count, const float* tod_K_dev, double pwv_mean_mm,
+                                 double r_out_rad, float* partial_dev, int32_t* n_out, void* cuda_stream);
+gt_status gt_common_mode_apply(gt_plan* plan, int64_t t_begin, int64_t t_count, float* tod_K_dev, double pwv_mean_mm,
+                               const float* sum_dev, int32_t n_out_total, void* cuda_stream);
 
 /* Message of the last error on this plan; plan == NULL => the calling thread's last
  * gt_plan_create error.  Never NULL. */

@@ -23,7 +23,7 @@ EXPORTS = ("gt_plan_create", "gt_simulate", "gt_plan_destroy", "gt_last_error", 
            "gt_debug_philox", "gt_debug_pkid", "gt_launch_count", "gt_variant_name", "gt_last_fused_ms",
            "gt_debug_kelvin_map", "gt_prepare_screen", "gt_prepare_source", "gt_plan_counters",
            "gt_pink_state_export", "gt_pink_state_import", "gt_debug_chunking", "gt_debug_timeline",
-           "gt_measure_fp32_fma")
+           "gt_measure_fp32_fma", "gt_common_mode_partial", "gt_common_mode_apply", "gt_release_cached_memory")
 
 
 class GtStage(C.Structure):
@@ -118,6 +118,13 @@ def lib() -> C.CDLL:
         L.gt_debug_timeline.argtypes = [C.c_void_p, C.c_int32, C.POINTER(C.c_int32), C.c_void_p]
         L.gt_measure_fp32_fma.restype = C.c_int
         L.gt_measure_fp32_fma.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
+        L.gt_common_mode_partial.restype = C.c_int
+        L.gt_common_mode_partial.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_void_p, C.c_double, C.c_double, C.c_void_p,
+                                             C.POINTER(C.c_int32), C.c_void_p]
+        L.gt_common_mode_apply.restype = C.c_int
+        L.gt_common_mode_apply.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_void_p, C.c_double, C.c_void_p, C.c_int32, C.c_void_p]
+        L.gt_release_cached_memory.restype = C.c_int
+        L.gt_release_cached_memory.argtypes = []
         L.gt_debug_chunking.restype = C.c_int
         L.gt_debug_chunking.argtypes = [C.c_void_p, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
         L.gt_pink_state_export.restype = C.c_int
@@ -211,8 +218,15 @@ class Plan:
         self._dev = {}
         ptrs = {}
 
+        import time
+        t_start = time.perf_counter()
+
         def up(name, arr):
-            t = torch.from_numpy(np.ascontiguousarray(arr, dtype=np.float32)).to(self.device)
+            # a torch tensor (e.g. pinned host memory) is copied as it is; NumPy arrays go through from_numpy
+            if isinstance(arr, torch.Tensor):
+                t = arr.to(device=self.device, dtype=torch.float32, non_blocking=True).contiguous()
+            else:
+                t = torch.from_numpy(np.ascontiguousarray(arr, dtype=np.float32)).to(self.device)
             self._dev[name] = t
             ptrs[name] = t.data_ptr()
 
@@ -227,12 +241,14 @@ class Plan:
             if np.ndim(s.eta) != 0:
                 up(f"stage{i}", s.eta)
         torch.cuda.synchronize()
+        t_up = time.perf_counter()
         keep = {}
         cfg = fill_config(w, ptrs, keep, variant, chunk_samples)
         self.handle = C.c_void_p()
         st = self.L.gt_plan_create(C.byref(cfg), None, C.byref(self.handle))
         if st != GT_OK:
             raise GateauError(st, self.L.gt_last_error(None).decode())
+        self.upload_ms, self.create_ms = 1e3 * (t_up - t_start), 1e3 * (time.perf_counter() - t_up)
 
     # ---- helpers ----
     def _check(self, st):
@@ -273,6 +289,21 @@ class Plan:
         ms = np.zeros((capacity, 4), dtype=np.float64)
         self._check(self.L.gt_debug_timeline(self.handle, capacity, C.byref(n), C.c_void_p(ms.ctypes.data)))
         return ms[:int(n.value)].copy()
+
+    def common_mode_partial(self, tod_K, pwv_mean_mm, r_out_rad, t_begin=0):
+        """gt_common_mode_partial: (partial [t, chan] CUDA tensor, this plan's N_out)."""
+        t_count = int(tod_K.shape[0])
+        partial = self.torch.empty((t_count, self.w.n_chan), dtype=self.torch.float32, device=self.device)
+        n = C.c_int32(0)
+        self._check(self.L.gt_common_mode_partial(self.handle, t_begin, t_count, _ptr(tod_K), float(pwv_mean_mm), float(r_out_rad),
+                                                  _ptr(partial), C.byref(n), self._stream()))
+        return partial, int(n.value)
+
+    def common_mode_apply(self, tod_K, pwv_mean_mm, total, n_out_total, t_begin=0):
+        """gt_common_mode_apply: tod_K <- T*_a (Eq. 25) in place."""
+        self._check(self.L.gt_common_mode_apply(self.handle, t_begin, int(tod_K.shape[0]), _ptr(tod_K), float(pwv_mean_mm),
+                                                _ptr(total), int(n_out_total), self._stream()))
+        return tod_K
 
     def counters(self) -> dict:
         """gt_plan_counters: rows processed, rows outside the cube, PWV clamps below / above the LUT."""
@@ -349,6 +380,13 @@ def _ptr(x):
         return C.c_void_p(x.ctypes.data)
     assert x.is_contiguous()
     return C.c_void_p(x.data_ptr())
+
+
+def release_cached_memory() -> None:
+    """gt_release_cached_memory: returns the plan pool's cached device memory to the driver."""
+    st = lib().gt_release_cached_memory()
+    if st != GT_OK:
+        raise GateauError(st, lib().gt_last_error(None).decode())
 
 
 def measure_fp32_fma() -> float:

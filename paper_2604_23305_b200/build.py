@@ -11,7 +11,7 @@ INCLUDE = _HERE.parent / "include"
 LIB = _HERE / "libgateau_b200.so"
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-              "-shared", "-Xcompiler", "-fPIC", "-Xptxas", "-v", "-lcuda", "-lcufft"]
+              "-shared", "-Xcompiler", "-fPIC", "-Xcompiler", "-pthread", "-Xptxas", "-v", "-lcuda", "-lcufft"]
 
 
 def _nvcc() -> str:

@@ -14,6 +14,7 @@
 #include <string>
 #include <vector>
 #include <new>
+#include <atomic>
 
 #include "gt_common.cuh"
 #include "gt_geometry.cuh"
@@ -26,6 +27,7 @@
 #include "gt_beam.cuh"
 #include "gt_reduce.cuh"
 #include "gt_measure.cuh"
+#include "gt_common_mode.cuh"
 #include <cufft.h>
 
 namespace {
@@ -45,19 +47,58 @@ double jn_power(double nu, double T) {
     return kH * nu / std::expm1(kH * nu / (kKB * T));
 }
 
+// Device memory of the plans comes from ONE library-owned stream-ordered pool per device that keeps what plans return
+// (release threshold = everything): creating and destroying plans back to back -- an observation per plan, as bench.py's
+// end-to-end leg does -- does not pay cudaMalloc / cudaFree of the 0.5 GB chunk buffers each time.
+// gt_release_cached_memory() gives the cached blocks back to the driver.
+cudaStream_t g_pool_stream[64] = {};      // the pool's own (non-blocking) stream: allocations and releases are ordered on it
+cudaMemPool_t plan_pool(int dev) {
+    static cudaMemPool_t pools[64] = {};
+    if (dev < 0 || dev >= 64) return nullptr;
+    if (!pools[dev]) {
+        if (cudaStreamCreateWithFlags(&g_pool_stream[dev], cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+        cudaMemPoolProps props{};
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev;
+        cudaMemPool_t pool = nullptr;
+        if (cudaMemPoolCreate(&pool, &props) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+        uint64_t keep = UINT64_MAX;
+        cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+        pools[dev] = pool;
+    }
+    return pools[dev];
+}
+
 template <class T>
 struct DevBuf {
-    T* p = nullptr; size_t n = 0;
+    T* p = nullptr; size_t n = 0; int pool_dev = -1;
+    // allocation and release are ordered on the pool's own stream; an allocation is synchronised before it is handed out,
+    // a release happens only after the plan's streams have been synchronised (gt_plan_destroy) or before first use
     cudaError_t alloc(size_t count) {
         release(); n = count;
-        return cudaMalloc(reinterpret_cast<void**>(&p), std::max<size_t>(count, 1) * sizeof(T));
+        const size_t bytes = std::max<size_t>(count, 1) * sizeof(T);
+        int dev = 0;
+        cudaMemPool_t pool = cudaGetDevice(&dev) == cudaSuccess ? plan_pool(dev) : nullptr;
+        if (pool) {
+            cudaError_t e = cudaMallocFromPoolAsync(reinterpret_cast<void**>(&p), bytes, pool, g_pool_stream[dev]);
+            if (e == cudaSuccess) e = cudaStreamSynchronize(g_pool_stream[dev]);
+            if (e == cudaSuccess) { pool_dev = dev; return e; }
+            cudaGetLastError(); p = nullptr;
+        }
+        pool_dev = -1;
+        return cudaMalloc(reinterpret_cast<void**>(&p), bytes);
     }
     cudaError_t upload(const std::vector<T>& h, cudaStream_t st) {
         cudaError_t e = alloc(h.size());
         if (e != cudaSuccess || h.empty()) return e;
         return cudaMemcpyAsync(p, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice, st);
     }
-    void release() { if (p) cudaFree(p); p = nullptr; n = 0; }
+    void release() {
+        if (p) { if (pool_dev >= 0) cudaFreeAsync(p, g_pool_stream[pool_dev]); else cudaFree(p); }
+        p = nullptr; n = 0; pool_dev = -1;
+    }
     ~DevBuf() { release(); }
 };
 
@@ -111,6 +152,11 @@ struct gt_plan {
     int32_t n_fused_last = 0;
     int64_t launches = 0;
     int num_sms = 148;
+    // common-mode subtraction (Eq. 25-26): what the plan keeps of its inputs for it
+    std::vector<float> h_lut;  int32_t n_nu_lut = 0;
+    double lut_nu0 = 0, lut_dnu = 0, lut_pwv0 = 0, lut_dpwv = 0;
+    std::vector<double> h_daz, h_del, h_fc;
+    DevBuf<double> d_ln_eta_z;  DevBuf<float> d_cm_weight;
     // diagnostics (SURVEY section 5 "Metrics"): rows seen by the geometry kernel, rows outside the cube, PWV clamps
     DevBuf<unsigned long long> d_counters;   // [3] outside cube, PWV below / above the LUT
     int64_t rows_done = 0;
@@ -575,17 +621,21 @@ gt_status gt_plan_create(const gt_config* cfg, void* cuda_stream, gt_plan** out_
     const int ncp = ((nc + 32 * tn - 1) / (32 * tn)) * 32 * tn;
     p->n_chan_pad = ncp;
     std::vector<float> bias(ncp, 0.f), c1(ncp, 0.f), c2(ncp, 0.f), cw(ncp, 1.f);
-    for (int ch = 0; ch < nc; ++ch) {
-        double sb = 0.0, s1 = 0.0, s2 = 0.0;
-        for (int i = 0; i < nf; ++i) {
-            const double f = h_filt[(size_t)ch * nf + i];
-            sb += f * Y[i]; s1 += f * c.dnu_hz; s2 += f * f * c.dnu_hz;
-        }
-        bias[ch] = (float)(c.dnu_hz * sb);
-        const double dnu_c = c.dnu_eff_hz ? c.dnu_eff_hz[ch] : (s2 > 0 ? s1 * s1 / s2 : 1.0);
-        if (!(dnu_c > 0)) return fail(nullptr, GT_ERR_VALUE, "dnu_eff[%d] is not positive", ch);
-        c1[ch] = (float)(kH * c.f_center_hz[ch] * c.f_sample_hz);
-        c2[ch] = (float)(c.f_sample_hz / dnu_c);
+    {
+        std::atomic<int> bad_ch{-1};
+        gt::host_parallel_for(nc, [&](int64_t ch) {
+            double sb = 0.0, s1 = 0.0, s2 = 0.0;
+            for (int i = 0; i < nf; ++i) {
+                const double f = h_filt[(size_t)ch * nf + i];
+                sb += f * Y[i]; s1 += f * c.dnu_hz; s2 += f * f * c.dnu_hz;
+            }
+            bias[ch] = (float)(c.dnu_hz * sb);
+            const double dnu_c = c.dnu_eff_hz ? c.dnu_eff_hz[ch] : (s2 > 0 ? s1 * s1 / s2 : 1.0);
+            if (!(dnu_c > 0)) { bad_ch = (int)ch; return; }
+            c1[ch] = (float)(kH * c.f_center_hz[ch] * c.f_sample_hz);
+            c2[ch] = (float)(c.f_sample_hz / dnu_c);
+        });
+        if (bad_ch >= 0) return fail(nullptr, GT_ERR_VALUE, "dnu_eff[%d] is not positive", (int)bad_ch);
     }
     if (p->variant == GT_VARIANT_FP32) {
         std::vector<float> ft((size_t)nfp * ncp, 0.f);
@@ -643,6 +693,11 @@ gt_status gt_plan_create(const gt_config* cfg, void* cuda_stream, gt_plan** out_
         GT_CUDA0(p->d_chan4.upload(c4, st));
         GT_CUDA0(cudaStreamSynchronize(st));
     }
+    p->h_lut = h_lut; p->n_nu_lut = c.n_nu_lut; p->lut_nu0 = c.lut_nu0_hz; p->lut_dnu = c.lut_dnu_hz;
+    p->lut_pwv0 = c.lut_pwv0_mm; p->lut_dpwv = c.lut_dpwv_mm;
+    p->h_daz.assign(c.daz_rad, c.daz_rad + ns); p->h_del.assign(c.del_rad, c.del_rad + ns);
+    p->h_fc.assign(c.f_center_hz, c.f_center_hz + nc);
+    GT_CUDA0(p->d_ln_eta_z.alloc((size_t)nc)); GT_CUDA0(p->d_cm_weight.alloc((size_t)ns));
     GT_CUDA0(p->d_counters.alloc(3));
     GT_CUDA0(cudaMemsetAsync(p->d_counters.p, 0, 3 * sizeof(unsigned long long), st));
 
@@ -650,11 +705,11 @@ gt_status gt_plan_create(const gt_config* cfg, void* cuda_stream, gt_plan** out_
     {
         const int64_t nt = c.n_samples;
         std::vector<double> ta(nt), te(nt), sE(nt), cE(nt), az(c.az_rad, c.az_rad + nt), el(c.el_rad, c.el_rad + nt);
-        for (int64_t n = 0; n < nt; ++n) {
+        gt::host_parallel_for(nt, [&](int64_t n) {
             ta[n] = std::tan(c.az_rad[n]); te[n] = std::tan(c.el_rad[n]);
             const double E = c.el0_rad + c.el_rad[n];
             sE[n] = std::sin(E); cE[n] = std::cos(E);
-        }
+        });
         GT_CUDA0(p->d_tan_az.upload(ta, st)); GT_CUDA0(p->d_tan_el.upload(te, st));
         GT_CUDA0(p->d_sinE.upload(sE, st)); GT_CUDA0(p->d_cosE.upload(cE, st));
         GT_CUDA0(p->d_az.upload(az, st)); GT_CUDA0(p->d_el.upload(el, st));
@@ -937,6 +992,16 @@ gt_status gt_prepare_screen(const float* epl_dev, int32_t nx, int32_t ny, double
 
 int64_t gt_launch_count(const gt_plan* plan) { return plan ? plan->launches : 0; }
 
+gt_status gt_release_cached_memory(void) {
+    int dev = 0;
+    GT_CUDA(nullptr, cudaGetDevice(&dev));
+    if (cudaMemPool_t pool = plan_pool(dev)) {
+        GT_CUDA(nullptr, cudaDeviceSynchronize());
+        GT_CUDA(nullptr, cudaMemPoolTrimTo(pool, 0));
+    }
+    return GT_OK;
+}
+
 gt_status gt_plan_counters(gt_plan* plan, int64_t* rows, int64_t* rows_outside_cube, int64_t* pwv_below_lut, int64_t* pwv_above_lut) {
     if (!plan) return fail(nullptr, GT_ERR_NULL, "plan is NULL");
     unsigned long long h[3] = {0, 0, 0};
@@ -987,6 +1052,75 @@ gt_status gt_debug_kelvin_map(gt_plan* plan, double* a_out, double* b_out) {
     if (cudaMemcpy(a_out, plan->d_kelvin_ab.p, nb, cudaMemcpyDeviceToHost) != cudaSuccess ||
         cudaMemcpy(b_out, plan->d_kelvin_ab.p + plan->n_chan, nb, cudaMemcpyDeviceToHost) != cudaSuccess)
         return fail(plan, GT_ERR_CUDA, "gt_debug_kelvin_map: copy failed");
+    return GT_OK;
+}
+
+namespace {
+// ln eta_atm,z at the channel centres: bilinear on the lookup table's own grid at (f_c, mean PWV), PWV clamped to the
+// table (R13); uploads it and the Eq. 26 weights S_j.  Returns N_out of this plan's spaxels.
+gt_status cm_setup(gt_plan* p, double pwv_mean_mm, double r_out_rad, gt::CmParams& k, int32_t* n_out, cudaStream_t st) {
+    if (!(pwv_mean_mm == pwv_mean_mm) || !(r_out_rad >= 0.0)) return fail(p, GT_ERR_VALUE, "common mode: pwv_mean and r_out must be a number and non-negative");
+    const int n_pwv = p->n_pwv, nn = p->n_nu_lut;
+    double q = (pwv_mean_mm - p->lut_pwv0) / p->lut_dpwv;
+    if (!(q >= 0.0)) q = 0.0;
+    if (q > (double)(n_pwv - 1)) q = (double)(n_pwv - 1);
+    const int ip = (int)std::min<double>(std::floor(q), n_pwv - 2);
+    const double fpq = q - ip;
+    std::vector<double> le((size_t)p->n_chan);
+    for (int c = 0; c < p->n_chan; ++c) {
+        const double r = (p->h_fc[c] - p->lut_nu0) / p->lut_dnu;
+        if (r < -1e-9 || r > (nn - 1) + 1e-9) return fail(p, GT_ERR_RANGE, "common mode: channel centre %d lies outside the lookup table", c);
+        int ir = (int)std::floor(r);
+        ir = std::max(0, std::min(ir, nn - 2));
+        const double fr = r - ir;
+        const float* L0 = p->h_lut.data() + (size_t)ip * nn + ir;
+        const float* L1 = L0 + nn;
+        const double ez = (1.0 - fpq) * ((1.0 - fr) * L0[0] + fr * L0[1]) + fpq * ((1.0 - fr) * L1[0] + fr * L1[1]);
+        le[c] = std::log(ez);
+        if (!(le[c] < 0.0)) return fail(p, GT_ERR_VALUE, "common mode: the atmosphere is fully transparent in channel %d (1 - eta_atm = 0 in Eq. 25)", c);
+    }
+    std::vector<float> w((size_t)p->n_spaxel);
+    int32_t n = 0;
+    for (int s = 0; s < p->n_spaxel; ++s) { w[s] = std::hypot(p->h_daz[s], p->h_del[s]) > r_out_rad ? 1.f : 0.f; n += w[s] != 0.f; }
+    GT_CUDA(p, cudaMemcpyAsync(p->d_ln_eta_z.p, le.data(), le.size() * sizeof(double), cudaMemcpyHostToDevice, st));
+    GT_CUDA(p, cudaMemcpyAsync(p->d_cm_weight.p, w.data(), w.size() * sizeof(float), cudaMemcpyHostToDevice, st));
+    GT_CUDA(p, cudaStreamSynchronize(st));                 // the host vectors go out of scope
+    k.sinE = p->d_sinE.p; k.cosE = p->d_cosE.p; k.sin_del = p->d_sp.p + 2 * p->n_spaxel; k.cos_del = p->d_sp.p + 3 * p->n_spaxel;
+    k.ln_eta_z = p->d_ln_eta_z.p; k.weight = p->d_cm_weight.p; k.n_spaxel = p->n_spaxel; k.n_chan = p->n_chan;
+    if (n_out) *n_out = n;
+    return GT_OK;
+}
+}  // namespace
+
+gt_status gt_common_mode_partial(gt_plan* plan, int64_t t_begin, int64_t t_count, const float* tod_K_dev, double pwv_mean_mm,
+                                 double r_out_rad, float* partial_dev, int32_t* n_out, void* cuda_stream) {
+    if (!plan || !tod_K_dev || !partial_dev || !n_out) return fail(plan, GT_ERR_NULL, "gt_common_mode_partial: NULL argument");
+    if (t_begin < 0 || t_count < 0 || t_begin + t_count > plan->n_samples) return fail(plan, GT_ERR_RANGE, "sample range outside the plan");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    gt::CmParams k{};
+    if (gt_status s = cm_setup(plan, pwv_mean_mm, r_out_rad, k, n_out, st)) return s;
+    if (t_count == 0) return GT_OK;
+    k.t0 = t_begin; k.T = t_count;
+    gt::cm_partial_kernel<<<(unsigned)t_count, 128, 0, st>>>(k, tod_K_dev, partial_dev);
+    GT_CUDA(plan, cudaGetLastError());
+    plan->launches++; plan->last_stream = st;
+    return GT_OK;
+}
+
+gt_status gt_common_mode_apply(gt_plan* plan, int64_t t_begin, int64_t t_count, float* tod_K_dev, double pwv_mean_mm,
+                               const float* sum_dev, int32_t n_out_total, void* cuda_stream) {
+    if (!plan || !tod_K_dev || !sum_dev) return fail(plan, GT_ERR_NULL, "gt_common_mode_apply: NULL argument");
+    if (t_begin < 0 || t_count < 0 || t_begin + t_count > plan->n_samples) return fail(plan, GT_ERR_RANGE, "sample range outside the plan");
+    if (n_out_total < 1) return fail(plan, GT_ERR_VALUE, "common mode: no spaxel lies outside r_out (N_out = 0 in Eq. 25)");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    gt::CmParams k{};
+    if (gt_status s = cm_setup(plan, pwv_mean_mm, 0.0, k, nullptr, st)) return s;
+    if (t_count == 0) return GT_OK;
+    k.t0 = t_begin; k.T = t_count; k.inv_n_out = 1.0 / (double)n_out_total;
+    if (t_count * plan->n_spaxel > 0x7fffffffLL) return fail(plan, GT_ERR_SHAPE, "common mode: more than 2^31 rows in one call");
+    gt::cm_apply_kernel<<<(unsigned)(t_count * plan->n_spaxel), 128, 0, st>>>(k, tod_K_dev, sum_dev);
+    GT_CUDA(plan, cudaGetLastError());
+    plan->launches++; plan->last_stream = st;
     return GT_OK;
 }
 

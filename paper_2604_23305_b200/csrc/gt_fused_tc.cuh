@@ -34,6 +34,8 @@
 #include <algorithm>
 #include <cstdlib>
 #include <cmath>
+#include <atomic>
+#include <thread>
 #include <cuda_fp16.h>
 #include "gt_common.cuh"
 #include "gt_fused_fp32.cuh"
@@ -148,6 +150,18 @@ struct TcTables {
     int32_t n_seg = 0;                   // segments per tile (max over the column groups)
 };
 
+// plan-time host loops over channels / samples are independent: a plain thread pool per call (plan creation is part of
+// the end-to-end time bench.py reports)
+template <class F>
+inline void host_parallel_for(int64_t n, F&& f) {
+    const int64_t nt = std::max<int64_t>(1, std::min<int64_t>({(int64_t)std::thread::hardware_concurrency(), (int64_t)16, n}));
+    if (nt == 1) { for (int64_t i = 0; i < n; ++i) f(i); return; }
+    std::vector<std::thread> th;
+    for (int64_t k = 0; k < nt; ++k)
+        th.emplace_back([=, &f]() { for (int64_t i = k * n / nt; i < (k + 1) * n / nt; ++i) f(i); });
+    for (auto& t : th) t.join();
+}
+
 inline const char*& tc_error_ref() { static thread_local const char* e = ""; return e; }
 inline const char* tc_error() { return tc_error_ref(); }
 
@@ -208,17 +222,19 @@ inline gt_status build_tc_tables(const std::vector<float>& filt, int n_chan, int
     const size_t total = (size_t)G * t.n_kb * 2 * kRanks * t.unit_bytes;
     std::vector<float> img(total / 4, 0.f);
     std::vector<float> comp((size_t)G * t.n_seg * nbt, 0.f);
-    std::vector<double> part((size_t)t.n_kb * kTcKSteps);
     uint16_t* img16 = reinterpret_cast<uint16_t*>(img.data());
-    for (int g = 0; g < G; ++g)
-        for (int n = 0; n < nbt; ++n) {
+    std::atomic<int> bad{0};
+    host_parallel_for((int64_t)G * nbt, [&](int64_t gn) {
+        {
+            const int g = (int)(gn / nbt), n = (int)(gn % nbt);
             const int ch = g * nbt + n;
-            if (ch >= n_chan) continue;
+            if (ch >= n_chan) return;
+            std::vector<double> part((size_t)t.n_kb * kTcKSteps);
             const float* frow = filt.data() + (size_t)ch * n_freq;
             const float* frow1 = filt1 ? filt1->data() + (size_t)ch * n_freq : nullptr;
             float amax = 0.f;
             for (int i = 0; i < n_freq; ++i) {
-                if (!std::isfinite(frow[i]) || (frow1 && !std::isfinite(frow1[i]))) { tc_error_ref() = "the filter holds a NaN or Inf"; return GT_ERR_VALUE; }
+                if (!std::isfinite(frow[i]) || (frow1 && !std::isfinite(frow1[i]))) { bad = 1; return; }
                 amax = std::max(amax, std::fabs(frow[i]));
                 if (frow1) amax = std::max(amax, std::fabs(frow1[i]));
             }
@@ -279,6 +295,8 @@ inline gt_status build_tc_tables(const std::vector<float>& filt, int n_chan, int
                 kb0 = kb1;
             }
         }
+    });
+    if (bad) { tc_error_ref() = "the filter holds a NaN or Inf"; return GT_ERR_VALUE; }
     if (cudaMalloc(reinterpret_cast<void**>(&t.filt_img), total) != cudaSuccess ||
         cudaMalloc(reinterpret_cast<void**>(&t.comp), comp.size() * sizeof(float)) != cudaSuccess) {
         cudaGetLastError(); tc_error_ref() = "cudaMalloc of the filter image failed"; return GT_ERR_OOM;

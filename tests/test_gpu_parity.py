@@ -841,6 +841,51 @@ def test_source_preprocessing_rejects_bad_arguments():
         assert e.value.status == status
 
 
+def test_common_mode_subtraction_sharded_and_single_plan_against_the_oracle():
+    """Eq. 25-26 on the Kelvin TOD: one plan holding every spaxel, and three plans holding spaxel
+    sub-ranges whose partial sums are added (the all-reduce of a sharded run), against the oracle's literal formula
+    evaluated on the same TOD.  The shards' TODs are bit-identical slices of the full plan's."""
+    import torch
+    from paper_2604_23305_b200 import shard
+    w = W.random_workload(121, n_samples=150, n_spaxel=7, n_chan=21, n_freq=80, photon_noise=True)
+    w = w.replace(output_unit=1, skydip_n=10, skydip_pwv_lo_mm=0.6, skydip_pwv_hi_mm=1.7)
+    r_out = 8 * np.pi / 180 / 3600                                  # offsets are +-10 arcsec: some spaxels inside, some outside
+    o = O.Oracle(w)
+    with B.Plan(w) as p:
+        tod, pwv = p.simulate(want_pwv=True)
+        pwv_mean = float(pwv.double().mean().item())
+        partial, n_out = p.common_mode_partial(tod, pwv_mean, r_out)
+        got = p.common_mode_apply(tod.clone(), pwv_mean, partial, n_out).cpu().numpy().astype(np.float64)
+        tod_np = tod.cpu().numpy()
+    eta_z = O.eta_zenith_at(w, w.f_center_hz, pwv_mean)
+    csc = o.geometry()["csc"]
+    ref, S, common = O.common_mode_subtract(tod_np.astype(np.float64), eta_z, csc, w.daz_rad, w.del_rad, r_out)
+    assert 0 < S.sum() < w.n_spaxel and n_out == int(S.sum())
+    scale = np.max(np.abs(tod_np / (eta_z[None, None, :] ** csc[:, :, None])))
+    assert np.max(np.abs(partial.cpu().numpy() - common)) <= 3e-7 * np.max(np.abs(common))
+    assert np.max(np.abs(got - ref)) <= 3e-7 * scale
+    # spaxel shards: partial sums and counts added over the plans, then each finishes its own slab
+    parts = shard.partition_spaxels(w.n_spaxel, 3)
+    plans = [B.Plan(shard.shard_workload(w, b, e)) for b, e in parts]
+    try:
+        tods = [q.simulate() for q in plans]
+        for (b, e), t in zip(parts, tods):
+            assert np.array_equal(t.cpu().numpy(), tod_np[:, b:e])
+        ps = [q.common_mode_partial(t, pwv_mean, r_out) for q, t in zip(plans, tods)]
+        total = torch.stack([x[0] for x in ps]).sum(dim=0)
+        n_tot = sum(x[1] for x in ps)
+        assert n_tot == n_out
+        outs = [q.common_mode_apply(t, pwv_mean, total, n_tot).cpu().numpy() for q, t in zip(plans, tods)]
+    finally:
+        for q in plans:
+            q.destroy()
+    assert np.max(np.abs(np.concatenate(outs, axis=1) - ref)) <= 3e-7 * scale
+    with B.Plan(w) as p:
+        with pytest.raises(B.GateauError) as e:
+            p.common_mode_apply(tod, pwv_mean, partial, 0)
+        assert e.value.status == 3
+
+
 def test_all_paper_options_together_streamed():
     """The paper's own choices at once -- Eq. 7 filterbank, Eq. 17 photon noise, Timmer & Koenig pink noise, Kelvin
     output -- streamed to host memory in ragged chunks; device and host outputs are identical."""
