@@ -838,11 +838,11 @@ gt_status gt_plan_create(const gt_config* cfg, void* cuda_stream, gt_plan** out_
         chunk = std::min(chunk, c.n_samples);
         if (c.chunk_samples == 0 && chunk > gt::kPinkSeg) chunk = chunk / gt::kPinkSeg * gt::kPinkSeg;
         p->chunk_samples = chunk;
-        // device output needs no staging buffers: larger launches (about 2^20 rows) keep the persistent kernel's
-        // tail (the last partial wave of tiles) near 1 % instead of 3 %
+        // device output needs no staging buffers: larger launches (about 2^22 rows, 134 MB of RowParam) keep the persistent
+        // kernel's tail (the last partial wave of tiles, and the cluster barrier the pairs end on) below half a per cent
         int64_t chunk_dev = chunk;
         if (c.chunk_samples == 0) {
-            chunk_dev = std::max<int64_t>(chunk, std::min<int64_t>(c.n_samples, (1 << 20) / std::max(ns, 1)));
+            chunk_dev = std::max<int64_t>(chunk, std::min<int64_t>(c.n_samples, (1 << 22) / std::max(ns, 1)));
             if (chunk_dev > gt::kPinkSeg) chunk_dev = chunk_dev / gt::kPinkSeg * gt::kPinkSeg;
         }
         p->chunk_dev = chunk_dev;

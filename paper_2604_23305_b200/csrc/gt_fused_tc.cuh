@@ -525,11 +525,13 @@ fused_tc_kernel(const TcParams p) {
         // =========================== generator: steps 2-4 -> A ring ===========================
         ptx::setmaxnreg_inc<kTcRegsGen>();
         const int gw = warp - kTcWarpGen0;
-        // rows of this thread: rsub and rsub + 64.  A warp's four rows are {0,1,4,5} or {2,3,6,7} of an 8-row
-        // swizzle group: the 64-byte pieces it stores per row then spread over all 32 banks (two rows whose 16-byte
-        // chunks land in banks 0-15, two in banks 16-31) instead of 4-way conflicting in one half.
+        // rows of this thread: rsub and rsub + 64.  A warp's four rows are {0,4,1,5} or {2,6,3,7} of an 8-row swizzle
+        // group, in lane order: an 8-byte shared store is served per HALF warp, and the two rows of a half warp ({0,4}, {1,5},
+        // ...) differ in bit 2 of the row, so the swizzle puts their 64-byte pieces into different halves of the 128-byte
+        // bank line: no conflict (rows {0,1} shared a half: 2-way, measured 96.1 -> 93.9 ms per C4 step once the kernel had
+        // become bound by the L1's wavefront pipe).
         const int q4 = lane >> 3;
-        const int rsub = (gw >> 1) * 8 + (gw & 1) * 2 + (q4 & 1) + (q4 >> 1) * 4, chunk = lane & 7;
+        const int rsub = (gw >> 1) * 8 + (gw & 1) * 2 + (q4 >> 1) + (q4 & 1) * 4, chunk = lane & 7;
         const size_t nf = (size_t)f.n_freq, nfp = (size_t)f.n_freq_pad;
         uint32_t a_st = 0, a_ph = 0;           // A-ring stage and its phase parity
         if constexpr (VEC) {
@@ -593,7 +595,7 @@ fused_tc_kernel(const TcParams p) {
                 };
                 auto compute = [&](int j, int h, const Tap& cur, const Lut& lut, const float4& X, const float4& G, uint32_t stage) {
                     const RowParam* rp = rowp + gw * 8 + j * 4 + q4;
-                    const float2 fc = *reinterpret_cast<const float2*>(rp);                    // fp, csc
+                    const float2 fc = *reinterpret_cast<const float2*>(rp);                    // fp, csc (registers for them cost spills: measured 91 -> 108 ms)
                     const float4 w = *reinterpret_cast<const float4*>(&rp->w00);
                     float4 S, v;
                     S.x = w.x * cur.c00.x + w.y * cur.c01.x + w.z * cur.c10.x + w.w * cur.c11.x;
@@ -620,6 +622,23 @@ fused_tc_kernel(const TcParams p) {
                         if (lane == 0) arrive_leader(sm.a_full + 8 * stage);
                         continue;
                     }
+#ifndef GT_TC_LUT_DOUBLE
+                    // the LUT rows are L1 hits (two rows shared by the whole tile): fetched at the head of the half slab they
+                    // are used in, in ONE register set (8 registers fewer than the double-buffered form: fewer spills)
+                    auto half = [&](int h, Lut& cur, Lut&) {
+                        const int hb = 2 * kb + h;
+                        issue_lut(hb, 0, cur);
+                        const float4 X = ldg4(f.Xn + hb * kTcHB + chunk * 4), G = ldg4(f.Gs + hb * kTcHB + chunk * 4);
+                        issue(hb, 1, t1);
+                        if (h == 0) wait_pair(sm.a_empty + 8 * stage, ph ^ 1u);
+                        compute(0, h, t0, cur, X, G, stage);
+                        if (hb + 1 < n_hb) issue(hb + 1, 0, t0);
+                        if (!same_lut) issue_lut(hb, 1, cur);
+                        compute(1, h, t1, cur, X, G, stage);
+                    };
+                    half(0, la, la);
+                    half(1, la, la);
+#else
                     auto half = [&](int h, Lut& cur, Lut& nxt) {
                         const int hb = 2 * kb + h;
                         const float4 X = ldg4(f.Xn + hb * kTcHB + chunk * 4), G = ldg4(f.Gs + hb * kTcHB + chunk * 4);
@@ -633,6 +652,7 @@ fused_tc_kernel(const TcParams p) {
                     };
                     half(0, la, lb);
                     half(1, lb, la);
+#endif
                     // one arrival per warp: 512 per-thread arrivals on one mbarrier serialise (~5 cycles each)
                     ptx::fence_proxy_async_smem();
                     __syncwarp();

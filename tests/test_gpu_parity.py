@@ -512,7 +512,7 @@ def test_C4_bench_configuration_full_size_sampled():
         assert p.variant_name.startswith("tcgen05")
         _, launch = p.chunking()
         assert 0 < launch < w.n_samples                       # several launches: there are seams to look at
-        t_idx, s_idx = _sampled_tiles(w, launch, rng, 0.01)
+        t_idx, s_idx = _sampled_tiles(w, launch, rng, 0.0105)
         assert t_idx.size >= 0.01 * w.n_samples * w.n_spaxel
         tod = p.simulate()
         got_t = tod[t_idx, s_idx.astype(np.int64)].cpu().numpy()
@@ -544,7 +544,7 @@ def test_C5_long_survey_streamed_in_60s_chunks():
     rng = np.random.default_rng(23)
     seams = rng.choice(np.arange(1, n_chunks), 12, replace=False) * chunk
     around = np.concatenate([np.arange(sm - 128, sm + 128) for sm in seams])
-    t_idx, s_idx = _sampled_tiles(w, chunk, rng, 0.01, extra_t=around)
+    t_idx, s_idx = _sampled_tiles(w, chunk, rng, 0.0105, extra_t=around)
     assert t_idx.size >= 0.01 * w.n_samples * w.n_spaxel
     chans = np.array([0, 127, 128, 255, 256, 346], dtype=np.int32)
     got = np.empty((t_idx.size, w.n_chan), dtype=np.float32)
@@ -575,7 +575,7 @@ def test_C3_full_size_sampled_rows():
     rng = np.random.default_rng(7)
     with B.Plan(w) as p:
         _, launch = p.chunking()
-        t_idx, s_idx = _sampled_tiles(w, launch, rng, 0.01)
+        t_idx, s_idx = _sampled_tiles(w, launch, rng, 0.0105)
         assert t_idx.size >= 0.01 * w.n_samples * w.n_spaxel
         tod = p.simulate()
         got_t = tod[t_idx, s_idx.astype(np.int64)].cpu().numpy()
