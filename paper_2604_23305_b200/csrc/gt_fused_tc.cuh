@@ -438,10 +438,14 @@ __device__ __forceinline__ void store_nep(unsigned char* a_stage, int row, int c
     *reinterpret_cast<uint2*>(dst + kTcAPartBytes) = b2;
 }
 
-// element (column, row) of a scratch tile laid out [row / 32][column / 4][row % 32][column % 4]: the 32 rows one flush
-// warp owns are contiguous per group of 4 columns (512 B), 16 columns of them 2 KB -- one bulk copy
+// element (column, row) of a scratch tile laid out [row / 32][column / 16][row % 32][16 columns]: the 16 columns x 32 rows one
+// flush batch moves are 2 KB contiguous (one bulk copy), and inside them a row's 16 columns are 64 contiguous bytes, so a
+// finisher warp (lane = channel, one row) touches two 64-byte pieces per load instead of eight 16-byte ones.  The four
+// 16-byte chunks of a row are XOR-swizzled with bits 1-2 of the row: the flush warps' 16-byte shared stores (lane = row) are
+// then conflict-free, and the bulk copy carries the permutation into the scratch tile unchanged.
 __device__ __forceinline__ size_t tc_scratch_index(int col, int row, int nb_tot) {
-    return ((size_t)(row >> 5) * (size_t)(nb_tot >> 2) + (size_t)(col >> 2)) * 128 + (size_t)(row & 31) * 4 + (size_t)(col & 3);
+    return ((size_t)(row >> 5) * (size_t)(nb_tot >> 4) + (size_t)(col >> 4)) * 512 + (size_t)(row & 31) * 16
+         + (size_t)((((col >> 2) & 3) ^ ((row >> 1) & 3)) << 2) + (size_t)(col & 3);
 }
 
 __device__ __forceinline__ float4 ldg4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
@@ -991,7 +995,7 @@ fused_tc_kernel(const TcParams p) {
                         ptx::tmem_ld_32x16(taddr + (uint32_t)c0, v);
                         // the staging buffer of this batch was last read by the bulk copy issued two batches ago
                         if (lane == 0) ptx::bulk_wait_read<1>();
-                        float4* const stg = reinterpret_cast<float4*>(smem_raw + (sm.stage - raw)) + (q * 2 + (nbatch & 1)) * (kTcStageBytes / 16) + lane;
+                        float4* const stg = reinterpret_cast<float4*>(smem_raw + (sm.stage - raw)) + (q * 2 + (nbatch & 1)) * (kTcStageBytes / 16) + lane * 4;
                         ptx::tmem_ld_wait();
                         if (c0 + 16 >= wg) {
                             // all of the group's columns are in registers: the accumulator buffer can go back to the MMA thread
@@ -1013,13 +1017,13 @@ fused_tc_kernel(const TcParams p) {
                             sum.y = fmaf(__uint_as_float(v[4 * i + 1] & 0xFF800000u), w4.y, __uint_as_float(v[4 * i + 1]));
                             sum.z = fmaf(__uint_as_float(v[4 * i + 2] & 0xFF800000u), w4.z, __uint_as_float(v[4 * i + 2]));
                             sum.w = fmaf(__uint_as_float(v[4 * i + 3] & 0xFF800000u), w4.w, __uint_as_float(v[4 * i + 3]));
-                            stg[i * 32] = sum;                               // [column / 4][row][column % 4], as the scratch tile
+                            stg[i ^ ((lane >> 1) & 3)] = sum;                // [row][16 columns, chunks swizzled], as the scratch tile
                         }
                         ptx::fence_proxy_async_smem();
                         __syncwarp();
                         if (lane == 0) {
                             const uint32_t src = sm.stage + (uint32_t)((q * 2 + (nbatch & 1)) * kTcStageBytes);
-                            float* const dst = scw + (size_t)(c0 / 4) * (32 * 4);
+                            float* const dst = scw + (size_t)(c0 / 16) * (32 * 16);
                             if (add) ptx::bulk_reduce_add_f32_s2g(dst, src, kTcStageBytes); else ptx::bulk_s2g(dst, src, kTcStageBytes);
                             ptx::bulk_commit();
                         }
