@@ -481,10 +481,11 @@ def run_e2e(torch, B, w, variant, local, world, steps, barrier, timeline=None):
                         "# ms after the first chunk's compute begin; compute = geometry + fused + pink kernels on the caller's stream,\n"
                         "# copy = cudaMemcpyAsync D2H of that chunk on the plan's side stream\n"
                         f"# command: python bench.py --steps 1 --warmup 3 --timeline {record}\n"
-                        f"# workload: {w.name}, {tl.shape[0]} chunks of {p.chunking()[0]} samples, {out.numel() * 4 / tl.shape[0] / 1e6:.0f} MB each\n"
+                        f"# workload: {w.name}, {tl.shape[0]} chunks of {p.chunking()[0]} samples ({p.chunking()[0] * w.n_spaxel * w.n_chan * 4 / 1e6:.0f} MB; the last one is shorter)\n"
                         "# chunk compute_begin compute_end copy_begin copy_end  copy_GB/s  copy_overlaps_next_compute\n")
-                per = out.numel() * 4 / tl.shape[0]
+                chunk_s, row_b = p.chunking()[0], w.n_spaxel * w.n_chan * 4
                 for k, r in enumerate(tl):
+                    per = min(chunk_s, w.n_samples - k * chunk_s) * row_b
                     ov = "yes" if k + 1 < tl.shape[0] and r[2] < tl[k + 1][1] and r[3] > tl[k + 1][0] else ("-" if k + 1 == tl.shape[0] else "no")
                     f.write(f"{k:4d} {r[0]:9.3f} {r[1]:9.3f} {r[2]:9.3f} {r[3]:9.3f} {per / max(r[3] - r[2], 1e-6) / 1e6:8.1f}  {ov}\n")
                 f.write(f"# compute busy {sum(r[1] - r[0] for r in tl):.1f} ms, copy busy {sum(r[3] - r[2] for r in tl):.1f} ms, "
