@@ -71,6 +71,20 @@ cudaMemPool_t plan_pool(int dev) {
     return pools[dev];
 }
 
+// the same pool for the tensor kernel's tables (gt_fused_tc.cuh): plain pointers, so the device of the pool is looked up
+cudaError_t pool_alloc_raw(void** p, size_t bytes) {
+    int dev = 0;
+    cudaMemPool_t pool = cudaGetDevice(&dev) == cudaSuccess ? plan_pool(dev) : nullptr;
+    if (!pool) return cudaMalloc(p, bytes);
+    cudaError_t e = cudaMallocFromPoolAsync(p, std::max<size_t>(bytes, 1), pool, g_pool_stream[dev]);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(g_pool_stream[dev]);
+    return e;
+}
+void pool_free_raw(void* p) {
+    int dev = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess && plan_pool(dev)) cudaFreeAsync(p, g_pool_stream[dev]); else cudaFree(p);
+}
+
 template <class T>
 struct DevBuf {
     T* p = nullptr; size_t n = 0; int pool_dev = -1;
@@ -478,6 +492,7 @@ gt_status gt_plan_create(const gt_config* cfg, void* cuda_stream, gt_plan** out_
         if (prop.major != 10) return fail(nullptr, GT_ERR_UNSUPPORTED, "built for sm_100a, device is sm_%d%d", prop.major, prop.minor);
     }
     GT_CUDA0(cudaStreamSynchronize(st));
+    gt::tc_alloc_fn() = pool_alloc_raw; gt::tc_free_fn() = pool_free_raw;
 
     const int nf = c.n_freq, nc = c.n_chan, ns = c.n_spaxel;
     const int nfp = (nf + 63) / 64 * 64;      // the tensor kernel works in slabs of 64 frequencies

@@ -162,6 +162,14 @@ inline void host_parallel_for(int64_t n, F&& f) {
     for (auto& t : th) t.join();
 }
 
+// device memory of the tables: the plan layer installs its pool allocator here (gateau_b200.cu); plain cudaMalloc otherwise
+using TcAllocFn = cudaError_t (*)(void**, size_t);
+using TcFreeFn = void (*)(void*);
+inline cudaError_t tc_default_alloc(void** p, size_t n) { return cudaMalloc(p, n); }
+inline void tc_default_free(void* p) { cudaFree(p); }
+inline TcAllocFn& tc_alloc_fn() { static TcAllocFn f = tc_default_alloc; return f; }
+inline TcFreeFn& tc_free_fn() { static TcFreeFn f = tc_default_free; return f; }
+
 inline const char*& tc_error_ref() { static thread_local const char* e = ""; return e; }
 inline const char* tc_error() { return tc_error_ref(); }
 
@@ -297,8 +305,8 @@ inline gt_status build_tc_tables(const std::vector<float>& filt, int n_chan, int
         }
     });
     if (bad) { tc_error_ref() = "the filter holds a NaN or Inf"; return GT_ERR_VALUE; }
-    if (cudaMalloc(reinterpret_cast<void**>(&t.filt_img), total) != cudaSuccess ||
-        cudaMalloc(reinterpret_cast<void**>(&t.comp), comp.size() * sizeof(float)) != cudaSuccess) {
+    if (tc_alloc_fn()(reinterpret_cast<void**>(&t.filt_img), total) != cudaSuccess ||
+        tc_alloc_fn()(reinterpret_cast<void**>(&t.comp), comp.size() * sizeof(float)) != cudaSuccess) {
         cudaGetLastError(); tc_error_ref() = "cudaMalloc of the filter image failed"; return GT_ERR_OOM;
     }
     if (cudaMemcpyAsync(t.filt_img, img.data(), total, cudaMemcpyHostToDevice, st) != cudaSuccess ||
@@ -312,15 +320,15 @@ inline gt_status build_tc_tables(const std::vector<float>& filt, int n_chan, int
 inline gt_status alloc_tc_scratch(TcTables& t, int num_sms) {
     if (t.scratch) return GT_OK;
     const size_t bytes = (size_t)num_sms * 2 * t.nb_tot * kTcBM * sizeof(float);     // two tiles per CTA
-    if (cudaMalloc(reinterpret_cast<void**>(&t.scratch), bytes) != cudaSuccess) {
+    if (tc_alloc_fn()(reinterpret_cast<void**>(&t.scratch), bytes) != cudaSuccess) {
         cudaGetLastError(); tc_error_ref() = "cudaMalloc of the partial-sum scratch failed"; return GT_ERR_OOM;
     }
     return GT_OK;
 }
 inline void free_tc_tables(TcTables& t) {
-    if (t.filt_img) cudaFree(t.filt_img);
-    if (t.scratch) cudaFree(t.scratch);
-    if (t.comp) cudaFree(t.comp);
+    if (t.filt_img) tc_free_fn()(t.filt_img);
+    if (t.scratch) tc_free_fn()(t.scratch);
+    if (t.comp) tc_free_fn()(t.comp);
     t.filt_img = nullptr; t.scratch = nullptr; t.comp = nullptr;
 }
 
