@@ -963,7 +963,7 @@ fused_tc_kernel(const TcParams p) {
         const int trow = 32 * q + lane;                        // tile row = tensor-memory lane
         TcRotation rot(p.n_cg, p.seg, p.n_kb);
         uint32_t fulls = 0u;                                   // bit b: parity of buffer b's flush count
-        uint32_t ti = 0, nbatch = 0;
+        uint32_t ti = 0;
         for (int64_t tl = worker; tl < n_tiles; tl += n_workers, ++ti) {
             const uint32_t sb = ti & 1u;
             float* const sc = p.scratch + ((size_t)blockIdx.x * 2 + sb) * p.nb_tot * kTcBM;
@@ -999,40 +999,50 @@ fused_tc_kernel(const TcParams p) {
                     wait_pair(sm.flush_full + 8 * b, fulls >> b & 1u);
                     fulls ^= 1u << b;
                     ptx::tc_fence_after();
-                    for (int c0 = 0; c0 < wg; c0 += 16, ++nbatch) {
+                    // 32 columns (two tcgen05.ld of 16) per round: both halves go into this warp's 4 KB staging strip, ONE
+                    // proxy fence and ONE 4 KB bulk copy per round.  wg is a multiple of 32.
+                    float4* const stg = reinterpret_cast<float4*>(smem_raw + (sm.stage - raw)) + q * (2 * kTcStageBytes / 16) + lane * 4;
+                    const uint32_t stg_s = sm.stage + (uint32_t)(q * 2 * kTcStageBytes);
+                    for (int c0 = 0; c0 < wg; c0 += 32) {
                         ptx::tmem_ld_32x16(taddr + (uint32_t)c0, v);
-                        // the staging buffer of this batch was last read by the bulk copy issued two batches ago
-                        if (lane == 0) ptx::bulk_wait_read<1>();
-                        float4* const stg = reinterpret_cast<float4*>(smem_raw + (sm.stage - raw)) + (q * 2 + (nbatch & 1)) * (kTcStageBytes / 16) + lane * 4;
+                        // the strip was last read by the bulk copy of the previous round
+                        if (lane == 0) ptx::bulk_wait_read<0>();
                         ptx::tmem_ld_wait();
-                        if (c0 + 16 >= wg) {
-                            // all of the group's columns are in registers: the accumulator buffer can go back to the MMA thread
-                            ptx::tc_fence_before();
-                            __syncwarp();
-                            if (lane == 0) arrive_leader(sm.buf_free + 8 * b);
-                        } else __syncwarp();
+                        __syncwarp();
 #pragma unroll
-                        for (int i = 0; i < 4; ++i) {
-                            // truncation compensation: the segment lost w ulp of its own sum (table of the plan, per
-                            // channel and segment); +-2^e of the sum = its sign and exponent bits
+                        for (int hh = 0; hh < 2; ++hh) {
+                            if (hh == 1) {
+                                ptx::tmem_ld_32x16(taddr + (uint32_t)(c0 + 16), v);
+                                ptx::tmem_ld_wait();
+                                if (c0 + 32 >= wg) {
+                                    // all of the group's columns are in registers: the accumulator buffer can go back to the MMA thread
+                                    ptx::tc_fence_before();
+                                    __syncwarp();
+                                    if (lane == 0) arrive_leader(sm.buf_free + 8 * b);
+                                }
+                            }
+#pragma unroll
+                            for (int i = 0; i < 4; ++i) {
+                                // truncation compensation: the segment lost w ulp of its own sum (table of the plan, per
+                                // channel and segment); +-2^e of the sum = its sign and exponent bits
 #ifndef GT_TC_NO_COMP
-                            const float4 w4 = wsm[c0 / 4 + i];
+                                const float4 w4 = wsm[(c0 + 16 * hh) / 4 + i];
 #else
-                            const float4 w4 = make_float4(0.f, 0.f, 0.f, 0.f);      // tuning builds: cost of the table look-up
+                                const float4 w4 = make_float4(0.f, 0.f, 0.f, 0.f);      // tuning builds: cost of the table look-up
 #endif
-                            float4 sum;
-                            sum.x = fmaf(__uint_as_float(v[4 * i] & 0xFF800000u), w4.x, __uint_as_float(v[4 * i]));
-                            sum.y = fmaf(__uint_as_float(v[4 * i + 1] & 0xFF800000u), w4.y, __uint_as_float(v[4 * i + 1]));
-                            sum.z = fmaf(__uint_as_float(v[4 * i + 2] & 0xFF800000u), w4.z, __uint_as_float(v[4 * i + 2]));
-                            sum.w = fmaf(__uint_as_float(v[4 * i + 3] & 0xFF800000u), w4.w, __uint_as_float(v[4 * i + 3]));
-                            stg[i ^ ((lane >> 1) & 3)] = sum;                // [row][16 columns, chunks swizzled], as the scratch tile
+                                float4 sum;
+                                sum.x = fmaf(__uint_as_float(v[4 * i] & 0xFF800000u), w4.x, __uint_as_float(v[4 * i]));
+                                sum.y = fmaf(__uint_as_float(v[4 * i + 1] & 0xFF800000u), w4.y, __uint_as_float(v[4 * i + 1]));
+                                sum.z = fmaf(__uint_as_float(v[4 * i + 2] & 0xFF800000u), w4.z, __uint_as_float(v[4 * i + 2]));
+                                sum.w = fmaf(__uint_as_float(v[4 * i + 3] & 0xFF800000u), w4.w, __uint_as_float(v[4 * i + 3]));
+                                stg[hh * (kTcStageBytes / 16) + (i ^ ((lane >> 1) & 3))] = sum;      // [16-column batch][row][16 columns, chunks swizzled], as the scratch tile
+                            }
                         }
                         ptx::fence_proxy_async_smem();
                         __syncwarp();
                         if (lane == 0) {
-                            const uint32_t src = sm.stage + (uint32_t)((q * 2 + (nbatch & 1)) * kTcStageBytes);
                             float* const dst = scw + (size_t)(c0 / 16) * (32 * 16);
-                            if (add) ptx::bulk_reduce_add_f32_s2g(dst, src, kTcStageBytes); else ptx::bulk_s2g(dst, src, kTcStageBytes);
+                            if (add) ptx::bulk_reduce_add_f32_s2g(dst, stg_s, 2 * kTcStageBytes); else ptx::bulk_s2g(dst, stg_s, 2 * kTcStageBytes);
                             ptx::bulk_commit();
                         }
                     }

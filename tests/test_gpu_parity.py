@@ -886,6 +886,25 @@ def test_common_mode_subtraction_sharded_and_single_plan_against_the_oracle():
         assert e.value.status == 3
 
 
+def test_measurement_hooks_and_plan_pool():
+    """gt_debug_timeline (per-chunk compute / copy events of a host-output call: every copy starts after its chunk's
+    kernels and ends after it started), gt_measure_fp32_fma (tens of TFLOP/s on a B200), gt_release_cached_memory
+    (plans created after the pool was trimmed still work and give the same TOD)."""
+    w = W.random_workload(131, n_samples=400, n_spaxel=3, n_chan=40, n_freq=64, photon_noise=True)
+    with B.Plan(w, chunk_samples=64) as p:
+        host = p.simulate(device_out=False).numpy().copy()
+        tl = p.timeline()
+        assert p.chunking()[0] == 64
+    assert tl.shape == (7, 4)                                   # 400 samples in chunks of 64
+    assert np.all(tl[:, 1] >= tl[:, 0]) and np.all(tl[:, 2] >= tl[:, 1]) and np.all(tl[:, 3] >= tl[:, 2])
+    assert np.all(np.diff(tl[:, 0]) >= 0) and np.all(np.diff(tl[:, 3]) >= 0)
+    B.release_cached_memory()
+    with B.Plan(w, chunk_samples=64) as p:
+        again = p.simulate(device_out=False).numpy()
+    assert np.array_equal(host, again)
+    assert 20.0 < B.measure_fp32_fma() < 100.0
+
+
 def test_all_paper_options_together_streamed():
     """The paper's own choices at once -- Eq. 7 filterbank, Eq. 17 photon noise, Timmer & Koenig pink noise, Kelvin
     output -- streamed to host memory in ragged chunks; device and host outputs are identical."""
