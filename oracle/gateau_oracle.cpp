@@ -74,7 +74,8 @@ void philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]
 double uniform01(uint32_t w) { return ((double)(w >> 9) + 0.5) * (1.0 / 8388608.0); }
 
 /* Four standard normals from one Philox block: Box-Muller on (w0,w1) and on (w2,w3).
- * Counter layout (reading R19): c0 = sample index n, c1 = spaxel, c2 = channel,
+ * Counter layout (reading R19): c0 = sample index n, c1 = spaxel, c2 = channel (pink noise) or
+ * channel block (photon noise, see photon_normal),
  * c3 = stream; key = (seed low 32, seed high 32). */
 void normals4(uint64_t seed, uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, double z[4]) {
     const uint32_t ctr[4] = {c0, c1, c2, c3};
@@ -93,6 +94,16 @@ void normals4(uint64_t seed, uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
 
 constexpr uint32_t STREAM_PHOTON = 0, STREAM_PINK_LO = 1, STREAM_PINK_HI = 2;
 constexpr uint32_t COUNTER_INIT  = 0xFFFFFFFFu;    /* c0 used for the AR(1) initial states */
+
+/* The photon-noise normal of detector-sample (n, spaxel s, channel ch) (reading R19): one Philox block of
+ * stream 0 yields four independent normals (Box-Muller's cosine and sine branches of both word pairs) and serves
+ * the four channels b + 128 q + {0, 32, 64, 96}, b = ch mod 32, q = ch div 128:
+ *   counter = (n, s, 32 q + b, 0),  normal index k = (ch div 32) mod 4. */
+double photon_normal(uint64_t seed, uint32_t n, uint32_t s, uint32_t ch) {
+    double z[4];
+    normals4(seed, n, s, 32u * (ch / 128u) + ch % 32u, STREAM_PHOTON, z);
+    return z[(ch / 32u) % 4u];
+}
 
 /* Eq. 17-18 in north_star's narrow-band form (reading R17):
  * sigma^2 = (2 h f_c P + 2 P^2 / dnu_c) * f_sample / 2. */
@@ -339,6 +350,8 @@ void go_normals4(uint64_t seed, uint32_t c0, uint32_t c1, uint32_t c2, uint32_t 
     normals4(seed, c0, c1, c2, c3, z);
 }
 
+double go_photon_normal(uint64_t seed, uint32_t n, uint32_t s, uint32_t ch) { return photon_normal(seed, n, s, ch); }
+
 void go_normals_bulk(uint64_t seed, uint32_t c0_begin, int64_t count, uint32_t c1, uint32_t c2,
                      uint32_t c3, double* z) {
     for (int64_t k = 0; k < count; ++k) normals4(seed, c0_begin + (uint32_t)k, c1, c2, c3, z + 4 * k);
@@ -401,10 +414,8 @@ int go_simulate_rows(const go_config* cfg, int64_t n_rows, const int64_t* t_idx,
                 const double pk = contract_channel(c, ch, P.data());
                 pkid[(size_t)r * c.n_chan + ch] = pk;
                 if (wn) {
-                    double z[4];
-                    normals4(c.seed, (uint32_t)n, (uint32_t)s, (uint32_t)ch, STREAM_PHOTON, z);
-                    wn[(size_t)r * c.n_chan + ch] =
-                        photon_sigma(pk, c.f_center_hz[ch], dnu_c[ch], c.f_sample_hz) * z[0];
+                    wn[(size_t)r * c.n_chan + ch] = photon_sigma(pk, c.f_center_hz[ch], dnu_c[ch], c.f_sample_hz)
+                                                  * photon_normal(c.seed, (uint32_t)n, (uint32_t)s, (uint32_t)ch);
                 }
             }
         }
@@ -449,9 +460,8 @@ int go_simulate(const go_config* cfg, int64_t t_begin, int64_t t_count,
                 if (tod) {
                     double wn = 0.0;
                     if (c.photon_noise) {                                      /* Eq. 18-19 */
-                        double z[4];
-                        normals4(c.seed, (uint32_t)n, (uint32_t)s, (uint32_t)ch, STREAM_PHOTON, z);
-                        wn = photon_sigma(pk, c.f_center_hz[ch], dnu_c[ch], c.f_sample_hz) * z[0];
+                        wn = photon_sigma(pk, c.f_center_hz[ch], dnu_c[ch], c.f_sample_hz)
+                           * photon_normal(c.seed, (uint32_t)n, (uint32_t)s, (uint32_t)ch);
                     }
                     tod[(size_t)r * nc + ch] = pk + wn;
                 }

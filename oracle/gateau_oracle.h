@@ -84,6 +84,7 @@ void   go_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t o
 double go_uniform(uint32_t w);                                    /* (0,1), 23 bits + half    */
 void   go_normals4(uint64_t seed, uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
                    double z[4]);                                  /* Box-Muller x2            */
+double go_photon_normal(uint64_t seed, uint32_t n, uint32_t s, uint32_t ch);   /* R19: block 32 (ch div 128) + ch mod 32, normal (ch div 32) mod 4 */
 void   go_normals_bulk(uint64_t seed, uint32_t c0_begin, int64_t count, uint32_t c1, uint32_t c2,
                        uint32_t c3, double* z /*[count][4]*/);
 double go_photon_sigma(double P_W, double f_center_hz, double dnu_eff_hz, double f_sample_hz);

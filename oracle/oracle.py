@@ -90,6 +90,8 @@ def lib() -> C.CDLL:
         L.go_photon_sigma.argtypes = [C.c_double] * 4
         L.go_philox4x32_10.restype = None
         L.go_normals4.restype = None
+        L.go_photon_normal.restype = C.c_double
+        L.go_photon_normal.argtypes = [C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32]
         L.go_normals4.argtypes = [C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint32, C.c_void_p]
         for name in ("go_geometry", "go_row_spectrum", "go_simulate", "go_simulate_rows",
                      "go_pink_series", "go_num_threads"):
@@ -262,7 +264,7 @@ class Oracle:
             pk[i] = w.dnu_hz * (F @ P_nu)
             nep2 = nep2_exact(F, P_nu, nu, w.dnu_hz, w.kid_gap_J, w.eta_pb)
             sigma = np.sqrt(nep2 * 0.5 * w.f_sample_hz)                                  # Eq. 18
-            z = np.array([normals4(w.seed, int(n), int(s), c, 0)[0] for c in range(w.n_chan)])
+            z = np.array([photon_normal(w.seed, int(n), int(s), c) for c in range(w.n_chan)])
             wn[i] = sigma * z                                                            # Eq. 19
         return pk, wn
 
@@ -333,6 +335,12 @@ def normals4(seed, c0, c1, c2, c3):
     z = np.zeros(4)
     lib().go_normals4(int(seed), int(c0) & 0xffffffff, int(c1), int(c2), int(c3), C.c_void_p(z.ctypes.data))
     return z
+
+
+def photon_normal(seed, n, s, ch):
+    """The photon-noise normal of (sample n, spaxel s, channel ch) (R19): normal (ch div 32) mod 4 of the
+    Philox block with counter (n, s, 32 (ch div 128) + ch mod 32, stream 0)."""
+    return lib().go_photon_normal(int(seed), int(n) & 0xffffffff, int(s), int(ch))
 
 
 def normals_bulk(seed, c0_begin, count, c1=0, c2=0, c3=0):

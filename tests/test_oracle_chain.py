@@ -351,13 +351,15 @@ def test_simulate_is_sum_of_its_parts_and_chunk_invariant():
 
 
 def test_photon_noise_counter_layout():
-    """wn of row (n, s), channel c uses z0 of Philox(counter = (n, s, c, 0), key = seed)."""
-    w = W.random_workload(18, n_samples=5, n_spaxel=2, n_chan=3, n_freq=8, photon_noise=True)
+    """wn of row (n, s), channel c uses normal (c div 32) mod 4 of Philox(counter = (n, s, 32 (c div 128) + c mod 32, 0),
+    key = seed) (R19; the block and normal are written out per channel here)."""
+    w = W.random_workload(18, n_samples=5, n_spaxel=2, n_chan=131, n_freq=8, photon_noise=True)
     o = O.Oracle(w)
     pk, wn = o.simulate_rows([4, 2], [1, 0], noise=True)
     d = o.dnu_eff()
+    where = {0: (0, 0), 2: (2, 0), 33: (1, 1), 70: (6, 2), 100: (4, 3), 127: (31, 3), 128: (32, 0), 130: (34, 0)}
     for r, (n, s) in enumerate([(4, 1), (2, 0)]):
-        for c in range(3):
-            z0 = O.normals4(w.seed, n, s, c, 0)[0]
+        for c, (blk, k) in where.items():
+            z0 = O.normals4(w.seed, n, s, blk, 0)[k]
             sig = O.photon_sigma(pk[r, c], w.f_center_hz[c], d[c], w.f_sample_hz)
             assert wn[r, c] == pytest.approx(sig * z0, rel=1e-14)

@@ -96,6 +96,45 @@ def test_normals_distribution():
     assert np.abs(c - np.eye(4)).max() < 5 / math.sqrt(n / 4)
 
 
+def test_photon_normal_channel_mapping():
+    """R19: one stream-0 block serves the four channels b + 128 q + {0, 32, 64, 96}.  Checked without the formula's own
+    index arithmetic: every channel of a 300-channel row must find its normal among the four of exactly one of the
+    blocks 0..95 of that (n, s), each (block, normal) pair is used by exactly one channel, and the table below lists the
+    expected (block, normal) of hand-picked channels."""
+    seed, n, s = 0xfeedfacecafe, 1234, 17
+    blocks = np.array([O.normals4(seed, n, s, b, 0) for b in range(96)])          # [block][normal]
+    used = {}
+    for ch in range(300):
+        z = O.photon_normal(seed, n, s, ch)
+        hit = np.argwhere(blocks == z)
+        assert len(hit) == 1
+        used[ch] = tuple(int(v) for v in hit[0])
+    assert len(set(used.values())) == 300
+    by_hand = {0: (0, 0), 31: (31, 0), 32: (0, 1), 63: (31, 1), 64: (0, 2), 97: (1, 3), 127: (31, 3),
+               128: (32, 0), 160: (32, 1), 255: (63, 3), 256: (64, 0), 299: (75, 1)}
+    for ch, bk in by_hand.items():
+        assert used[ch] == bk
+    # other samples, spaxels and seeds give other values
+    z0 = O.photon_normal(seed, n, s, 5)
+    assert len({z0, O.photon_normal(seed, n + 1, s, 5), O.photon_normal(seed, n, s + 1, 5), O.photon_normal(seed + 1, n, s, 5)}) == 4
+
+
+def test_photon_normals_of_a_row_are_independent_standard_normals():
+    """The four channels that share a block use the cosine and sine branches of two Box-Muller pairs: jointly independent
+    N(0,1).  Moments over 347 channels x 3000 samples, and the correlation between the channels of a block."""
+    seed, s, nc, ns = 99, 3, 347, 3000
+    z = np.array([[O.photon_normal(seed, n, s, ch) for ch in range(nc)] for n in range(ns)])
+    m = z.size
+    assert abs(z.mean()) < 4 / math.sqrt(m)
+    assert abs(z.var() - 1) < 4 * math.sqrt(2 / m)
+    assert abs(stats.kurtosis(z.ravel())) < 4 * math.sqrt(24 / m)
+    assert stats.kstest(z.ravel()[:200_000], "norm").pvalue > 1e-3
+    c = np.corrcoef(z[:, [5, 37, 69, 101, 133, 6]].T)             # channels 5, 37, 69, 101 share block 5
+    assert np.abs(c - np.eye(6)).max() < 5 / math.sqrt(ns)
+    q = np.corrcoef((z[:, [5, 37, 69, 101]] ** 2).T)               # and their squares (radius shared by cos / sin branches)
+    assert np.abs(q - np.eye(4)).max() < 5 / math.sqrt(ns)
+
+
 # ---------------------------------------------------------------- photon noise (Eq. 17-19)
 def test_photon_sigma_formula_and_limits():
     P, fc, dn, fs = 1.3e-13, 300e9, 1.9e9, 160.0
