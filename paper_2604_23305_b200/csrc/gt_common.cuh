@@ -58,7 +58,26 @@ __device__ __forceinline__ void philox4x32_10_multi(uint32_t c0, uint32_t c1, co
         k0 += kPhiloxW0; k1 += kPhiloxW1;
     }
 #pragma unroll
-    for (int i = 0; i < W; ++i) { o0[i] = a[i]; o1[i] = b[i]; }      // words 0 and 1 (the photon-noise normal uses only these)
+    for (int i = 0; i < W; ++i) { o0[i] = a[i]; o1[i] = b[i]; }      // words 0 and 1
+}
+template <int W>
+__device__ __forceinline__ void philox4x32_10_multi4(uint32_t c0, uint32_t c1, const uint32_t (&c2)[W], uint32_t c3,
+                                                     uint32_t k0, uint32_t k1, uint4 (&o)[W]) {
+    uint32_t a[W], b[W], c[W], d[W];
+#pragma unroll
+    for (int i = 0; i < W; ++i) { a[i] = c0; b[i] = c1; c[i] = c2[i]; d[i] = c3; }
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+#pragma unroll
+        for (int i = 0; i < W; ++i) {
+            const uint32_t hi0 = __umulhi(kPhiloxM0, a[i]), lo0 = kPhiloxM0 * a[i];
+            const uint32_t hi1 = __umulhi(kPhiloxM1, c[i]), lo1 = kPhiloxM1 * c[i];
+            a[i] = hi1 ^ b[i] ^ k0; b[i] = lo1; c[i] = hi0 ^ d[i] ^ k1; d[i] = lo0;
+        }
+        k0 += kPhiloxW0; k1 += kPhiloxW1;
+    }
+#pragma unroll
+    for (int i = 0; i < W; ++i) o[i] = make_uint4(a[i], b[i], c[i], d[i]);
 }
 
 // U(w) = ((w >> 9) + 1/2) 2^-23 in (0,1): exact in fp32 (R19).
@@ -81,6 +100,23 @@ __device__ __forceinline__ void normal_pair(uint32_t w0, uint32_t w1, float& z0,
     float s, c;
     __sincosf(6.28318530717958647692f * uniform01(w1), &s, &c);
     z0 = r * c; z1 = r * s;
+}
+
+// Photon noise (stream 0, R19): one block yields four normals and serves the channels b + 128 q + {0, 32, 64, 96}:
+// channel c uses normal photon_slot(c) of the block with counter word 2 = photon_block(c).
+__device__ __forceinline__ uint32_t photon_block(uint32_t c) { return ((c >> 7) << 5) | (c & 31u); }
+__device__ __forceinline__ uint32_t photon_slot(uint32_t c) { return (c >> 5) & 3u; }
+__device__ __forceinline__ void normals_of_block(const uint4& w, float (&z)[4]) {
+    normal_pair(w.x, w.y, z[0], z[1]);
+    normal_pair(w.z, w.w, z[2], z[3]);
+}
+// one channel on its own (FP32 kernel: the whole block for one normal; the tensor kernel's finisher uses all four)
+__device__ __forceinline__ float photon_normal(uint32_t n, uint32_t spaxel, uint32_t c, uint32_t seed_lo, uint32_t seed_hi) {
+    const uint4 w = philox4x32_10(n, spaxel, photon_block(c), kStreamPhoton, seed_lo, seed_hi);
+    const uint32_t k = photon_slot(c);
+    const float r = sqrt_fast(-2.0f * __logf(uniform01(k < 2u ? w.x : w.z)));
+    const float a = 6.28318530717958647692f * uniform01(k < 2u ? w.y : w.w);
+    return r * ((k & 1u) ? __sinf(a) : __cosf(a));
 }
 
 // sigma of Eq. 18 in north_star's narrow-band form (R17):

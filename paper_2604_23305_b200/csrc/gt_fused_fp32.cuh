@@ -162,8 +162,7 @@ fused_fp32_kernel(const FusedParams p) {
             float P = fmaf(a, p.scale, bias);
             if (p.photon_noise) {
                 const uint32_t n = (uint32_t)(p.t0 + r / p.n_spaxel), s = (uint32_t)(r % p.n_spaxel);
-                const uint4 w = philox4x32_10(n, p.spaxel_base + s, (uint32_t)c, kStreamPhoton, p.seed_lo, p.seed_hi);
-                P = fmaf(photon_sigma(P, n1, n2), normal_cos(w.x, w.y), P);
+                P = fmaf(photon_sigma(P, n1, n2), photon_normal(n, p.spaxel_base + s, (uint32_t)c, p.seed_lo, p.seed_hi), P);
             }
             p.out[(size_t)r * p.n_chan + c] = P;
         }

@@ -105,8 +105,8 @@ constexpr int kTcRegsBase = (65536 / kTcThreads) / 8 * 8;                       
 #define GT_TC_REGS_FIN (GT_TC_FIN_WARPS == 8 ? 48 : 88)
 #endif
 // finisher: channels in flight per lane, and whether the next row's partial sums are fetched a row ahead
-#ifndef GT_TC_FIN_W
-#define GT_TC_FIN_W (GT_TC_FIN_WARPS == 8 ? 3 : 4)
+#ifndef GT_TC_FIN_QW
+#define GT_TC_FIN_QW 3      // Philox blocks (quads of channels) in flight per finisher lane: 1 or 3
 #endif
 #ifndef GT_TC_FIN_PREFETCH
 #define GT_TC_FIN_PREFETCH (GT_TC_FIN_WARPS == 8 ? 0 : 1)
@@ -198,7 +198,9 @@ inline gt_status build_tc_tables(const std::vector<float>& filt, int n_chan, int
                                  cudaStream_t st, const std::vector<float>* filt1 = nullptr) {
     const int G = (n_chan + kTcMaxGroupChan - 1) / kTcMaxGroupChan;
     int per = (n_chan + G - 1) / G;
-    const int nbt = (per + 31) / 32 * 32;
+    // several groups: every group starts on a multiple of 128 channels, so that a finisher lane's quads of channels
+    // (lane + 128 m + {0, 32, 64, 96}: one Philox block each, R19) never straddle two groups
+    const int nbt = G > 1 ? (per + 127) / 128 * 128 : (per + 31) / 32 * 32;
     t.n_groups = G; t.nb_tot = nbt;
     t.n_cg = (nbt + kTcBufCols - 1) / kTcBufCols;
     t.n_kb = n_freq_pad / kTcBK;
@@ -419,8 +421,13 @@ __device__ __forceinline__ void store_split(unsigned char* a_stage, int row, int
     const float2 s01 = make_float2(v.x, v.y), s23 = make_float2(v.z, v.w);      // v is already scaled: the plan folds kTcScaleA into Xn and Gs
     const __half2 h01 = __float22half2_rn(s01), h23 = __float22half2_rn(s23);
     const float2 b01 = __half22float2(h01), b23 = __half22float2(h23);
+#ifndef GT_TC_SCALAR_GEN
+    const __half2 l01 = __float22half2_rn(ptx::upk2(ptx::sub2(ptx::pk2(s01.x, s01.y), ptx::pk2(b01.x, b01.y))));
+    const __half2 l23 = __float22half2_rn(ptx::upk2(ptx::sub2(ptx::pk2(s23.x, s23.y), ptx::pk2(b23.x, b23.y))));
+#else
     const __half2 l01 = __float22half2_rn(make_float2(s01.x - b01.x, s01.y - b01.y));
     const __half2 l23 = __float22half2_rn(make_float2(s23.x - b23.x, s23.y - b23.y));
+#endif
     uint2 hi2, lo2;
     hi2.x = *reinterpret_cast<const uint32_t*>(&h01); hi2.y = *reinterpret_cast<const uint32_t*>(&h23);
     lo2.x = *reinterpret_cast<const uint32_t*>(&l01); lo2.y = *reinterpret_cast<const uint32_t*>(&l23);
@@ -610,6 +617,36 @@ fused_tc_kernel(const TcParams p) {
                     const float2 fc = *reinterpret_cast<const float2*>(rp);                    // fp, csc (registers for them cost spills: measured 91 -> 108 ms)
                     const float4 w = *reinterpret_cast<const float4*>(&rp->w00);
                     float4 S, v;
+#ifndef GT_TC_SCALAR_GEN
+                    // steps 2-4 on pairs of frequencies: every fp32 operation below is one FFMA2 / FMUL2 / FADD2 for two
+                    // elements (same IEEE operations, same order as the scalar form: bit-identical results, half the
+                    // issue slots -- the generator is bound by issue slots and the L1, not by the FMA pipe)
+                    {
+                        using namespace ptx;
+                        const f32x2 w00 = pk2(w.x, w.x), w01 = pk2(w.y, w.y), w10 = pk2(w.z, w.z), w11 = pk2(w.w, w.w);
+                        const f32x2 fp2 = pk2(fc.x, fc.x), csc2 = pk2(fc.y, fc.y);
+                        auto pair = [&](float c00x, float c00y, float c01x, float c01y, float c10x, float c10y, float c11x, float c11y,
+                                        float l0x, float l0y, float l1x, float l1y, float Xx, float Xy, float Gx, float Gy,
+                                        float& vx, float& vy) {
+                            f32x2 S2 = mul2(w00, pk2(c00x, c00y));
+                            S2 = fma2(w01, pk2(c01x, c01y), S2);
+                            S2 = fma2(w10, pk2(c10x, c10y), S2);
+                            S2 = fma2(w11, pk2(c11x, c11y), S2);
+                            const f32x2 L0 = pk2(l0x, l0y);
+                            const float2 ez = upk2(fma2(fp2, sub2(pk2(l1x, l1y), L0), L0));
+                            const float2 lg = upk2(mul2(csc2, pk2(lg2_ftz(ez.x), lg2_ftz(ez.y))));
+                            const f32x2 eta = pk2(ex2_ftz(lg.x), ex2_ftz(lg.y));
+                            const f32x2 X2 = pk2(Xx, Xy);
+                            const float2 r = upk2(fma2(eta, fma2(pk2(Gx, Gy), S2, pk2(-Xx, -Xy)), X2));
+                            vx = r.x; vy = r.y;
+                        };
+                        pair(cur.c00.x, cur.c00.y, cur.c01.x, cur.c01.y, cur.c10.x, cur.c10.y, cur.c11.x, cur.c11.y,
+                             lut.L0.x, lut.L0.y, lut.L1.x, lut.L1.y, X.x, X.y, G.x, G.y, v.x, v.y);
+                        pair(cur.c00.z, cur.c00.w, cur.c01.z, cur.c01.w, cur.c10.z, cur.c10.w, cur.c11.z, cur.c11.w,
+                             lut.L0.z, lut.L0.w, lut.L1.z, lut.L1.w, X.z, X.w, G.z, G.w, v.z, v.w);
+                        (void)S;
+                    }
+#else
                     S.x = w.x * cur.c00.x + w.y * cur.c01.x + w.z * cur.c10.x + w.w * cur.c11.x;
                     S.y = w.x * cur.c00.y + w.y * cur.c01.y + w.z * cur.c10.y + w.w * cur.c11.y;
                     S.z = w.x * cur.c00.z + w.y * cur.c01.z + w.z * cur.c10.z + w.w * cur.c11.z;
@@ -618,6 +655,7 @@ fused_tc_kernel(const TcParams p) {
                     v.y = element_value_fast(fmaf(fc.x, lut.L1.y - lut.L0.y, lut.L0.y), fc.y, X.y, G.y, S.y);
                     v.z = element_value_fast(fmaf(fc.x, lut.L1.z - lut.L0.z, lut.L0.z), fc.y, X.z, G.z, S.z);
                     v.w = element_value_fast(fmaf(fc.x, lut.L1.w - lut.L0.w, lut.L0.w), fc.y, X.w, G.w, S.w);
+#endif
                     if constexpr (NEP) store_nep(smem_raw + (sm.a - raw) + stage * kTcAStageBytes, rsub + kTcRowStride * j, chunk, h, v);
                     else store_split(smem_raw + (sm.a - raw) + stage * kTcAStageBytes, rsub + kTcRowStride * j, chunk, h, v);
                 };
@@ -916,40 +954,47 @@ fused_tc_kernel(const TcParams p) {
                         x[j] = c < n_valid ? __ldcg(sc + tc_scratch_index(c, r, p.nb_tot)) : 0.f;
                     }
                 }
-                constexpr int W = GT_TC_FIN_W;                            // channels in flight per lane
+                // One Philox block per FOUR channels (R19): the lane owns channels lane + 32 j, and the four channels
+                // lane + 128 m + {0, 32, 64, 96} of quad m share the block 32 (cg0 / 128 + m) + lane (group starts are
+                // multiples of 128, build_tc_tables), whose four normals are the cosine and sine branches of two
+                // Box-Muller pairs.  QW blocks are interleaved: the ten rounds of one block are a serial chain.
+                constexpr int kQuads = kMaxPerLane / 4, QW = GT_TC_FIN_QW;
+                const uint32_t blk0 = (((uint32_t)cg0 >> 7) << 5) + (uint32_t)lane;
 #pragma unroll
-                for (int j0 = 0; j0 < kMaxPerLane; j0 += W) {
-                    if (lane + 32 * j0 >= n_valid) break;
-                    float P[W], n1[W], n2[W];
-                    uint32_t cc[W], w0[W], w1[W];
+                for (int m0 = 0; m0 < kQuads; m0 += QW) {
+                    if (lane + 128 * m0 >= n_valid) break;
+                    float z[QW][4];
+                    if (NEP || f.photon_noise) {
+                        uint32_t cc[QW];
+                        uint4 w[QW];
 #pragma unroll
-                    for (int i = 0; i < W; ++i) {
-                        const int c = min(lane + 32 * (j0 + i), n_valid - 1);
-                        cc[i] = (uint32_t)(cg0 + c);
-                        const float4 k4 = __ldg(f.chan4 + cc[i]);          // bias, h f_c f_s, f_s / dnu_c, 2^-kb (the channel's filter scale)
-                        P[i] = fmaf(x[j0 + i] * k4.w, f.scale, k4.x);
-                        n1[i] = k4.y; n2[i] = k4.z;
+                        for (int i = 0; i < QW; ++i) cc[i] = blk0 + 32u * (uint32_t)(m0 + i);
+                        philox4x32_10_multi4<QW>(n, f.spaxel_base + s, cc, kStreamPhoton, f.seed_lo, f.seed_hi, w);
+#pragma unroll
+                        for (int i = 0; i < QW; ++i) normals_of_block(w[i], z[i]);
+                    } else {
+#pragma unroll
+                        for (int i = 0; i < QW; ++i) z[i][0] = z[i][1] = z[i][2] = z[i][3] = 0.f;
                     }
-                    if constexpr (NEP) {
-                        // Eq. 17 pass: P = NEP^2 / (2 E0) of this detector-sample; the TOD already holds the noiseless power of
-                        // the first pass: tod += sqrt(P f_s) sqrt(E0) z, z = the normal of the narrow-band mode (Eq. 18-19)
-                        philox4x32_10_multi<W>(n, f.spaxel_base + s, cc, kStreamPhoton, f.seed_lo, f.seed_hi, w0, w1);
 #pragma unroll
-                        for (int i = 0; i < W; ++i) {
-                            const int c = lane + 32 * (j0 + i);
-                            const float sigma = sqrt_fast(fmaxf(P[i], 0.f) * f.nep_f_sample) * f.nep_sqrt_e0;
-                            P[i] = fmaf(sigma, normal_cos(w0[i], w1[i]), c < n_valid ? __ldcs(o + c) : 0.f);
+                    for (int i = 0; i < QW; ++i) {
+#pragma unroll
+                        for (int k = 0; k < 4; ++k) {
+                            const int j = 4 * (m0 + i) + k, c = lane + 32 * j;
+                            if (j < kMaxPerLane && c < n_valid) {
+                                const float4 k4 = __ldg(f.chan4 + cg0 + c);   // bias, h f_c f_s, f_s / dnu_c, 2^-kb (the channel's filter scale)
+                                float P = fmaf(x[j] * k4.w, f.scale, k4.x);
+                                if constexpr (NEP) {
+                                    // Eq. 17 pass: P = NEP^2 / (2 E0) of this detector-sample; the TOD already holds the noiseless power of
+                                    // the first pass: tod += sqrt(P f_s) sqrt(E0) z, z = the normal of the narrow-band mode (Eq. 18-19)
+                                    const float sigma = sqrt_fast(fmaxf(P, 0.f) * f.nep_f_sample) * f.nep_sqrt_e0;
+                                    P = fmaf(sigma, z[i][k], __ldcs(o + c));
+                                } else if (f.photon_noise) {
+                                    P = fmaf(photon_sigma(P, k4.y, k4.z), z[i][k], P);
+                                }
+                                __stcs(o + c, P);                          // streaming store: the TOD must not evict the scratch tiles from L2
+                            }
                         }
-                    } else if (f.photon_noise) {
-                        philox4x32_10_multi<W>(n, f.spaxel_base + s, cc, kStreamPhoton, f.seed_lo, f.seed_hi, w0, w1);
-#pragma unroll
-                        for (int i = 0; i < W; ++i)
-                            P[i] = fmaf(photon_sigma(P[i], n1[i], n2[i]), normal_cos(w0[i], w1[i]), P[i]);
-                    }
-#pragma unroll
-                    for (int i = 0; i < W; ++i) {
-                        const int c = lane + 32 * (j0 + i);
-                        if (c < n_valid) __stcs(o + c, P[i]);      // streaming store: the TOD must not evict the scratch tiles from L2
                     }
                 }
             }
