@@ -421,13 +421,8 @@ __device__ __forceinline__ void store_split(unsigned char* a_stage, int row, int
     const float2 s01 = make_float2(v.x, v.y), s23 = make_float2(v.z, v.w);      // v is already scaled: the plan folds kTcScaleA into Xn and Gs
     const __half2 h01 = __float22half2_rn(s01), h23 = __float22half2_rn(s23);
     const float2 b01 = __half22float2(h01), b23 = __half22float2(h23);
-#ifndef GT_TC_SCALAR_GEN
-    const __half2 l01 = __float22half2_rn(ptx::upk2(ptx::sub2(ptx::pk2(s01.x, s01.y), ptx::pk2(b01.x, b01.y))));
+    const __half2 l01 = __float22half2_rn(ptx::upk2(ptx::sub2(ptx::pk2(s01.x, s01.y), ptx::pk2(b01.x, b01.y))));    // FADD2
     const __half2 l23 = __float22half2_rn(ptx::upk2(ptx::sub2(ptx::pk2(s23.x, s23.y), ptx::pk2(b23.x, b23.y))));
-#else
-    const __half2 l01 = __float22half2_rn(make_float2(s01.x - b01.x, s01.y - b01.y));
-    const __half2 l23 = __float22half2_rn(make_float2(s23.x - b23.x, s23.y - b23.y));
-#endif
     uint2 hi2, lo2;
     hi2.x = *reinterpret_cast<const uint32_t*>(&h01); hi2.y = *reinterpret_cast<const uint32_t*>(&h23);
     lo2.x = *reinterpret_cast<const uint32_t*>(&l01); lo2.y = *reinterpret_cast<const uint32_t*>(&l23);
@@ -544,30 +539,32 @@ fused_tc_kernel(const TcParams p) {
         // =========================== generator: steps 2-4 -> A ring ===========================
         ptx::setmaxnreg_inc<kTcRegsGen>();
         const int gw = warp - kTcWarpGen0;
-        // rows of this thread: rsub and rsub + 64.  A warp's four rows are {0,4,1,5} or {2,6,3,7} of an 8-row swizzle
-        // group, in lane order: an 8-byte shared store is served per HALF warp, and the two rows of a half warp ({0,4}, {1,5},
-        // ...) differ in bit 2 of the row, so the swizzle puts their 64-byte pieces into different halves of the 128-byte
-        // bank line: no conflict (rows {0,1} shared a half: 2-way, measured 96.1 -> 93.9 ms per C4 step once the kernel had
-        // become bound by the L1's wavefront pipe).
+        // general path (any n_freq, no 16-byte loads): rows of this thread rsub and rsub + 64; a warp's four rows are
+        // {0,4,1,5} or {2,6,3,7} of an 8-row swizzle group, in lane order (conflict-free 8-byte shared stores per half warp)
         const int q4 = lane >> 3;
         const int rsub = (gw >> 1) * 8 + (gw & 1) * 2 + (q4 >> 1) + (q4 & 1) * 4, chunk = lane & 7;
         const size_t nf = (size_t)f.n_freq, nfp = (size_t)f.n_freq_pad;
         uint32_t a_st = 0, a_ph = 0;           // A-ring stage and its phase parity
         if constexpr (VEC) {
-            // One step = one row of this thread (4 frequencies of it): 4 cube taps (and, once per pair of
-            // rows, the 2 LUT rows) as 16-byte loads, steps 2-4, fp16 split, two 8-byte shared stores.  The loads of the
-            // next step are issued before the current one is computed; the other three warps of the
-            // scheduler cover the rest of the latency.  The per-row constants live in shared
-            // memory (each warp only reads rows it wrote itself).
+            // Warp = TWO rows x the whole 64-frequency slab (half warp = one row, lane = 4 frequencies); a thread walks FOUR
+            // rows (32 apart) per slab.  Against the earlier map (warp = four rows x half a slab, two rows per thread) the
+            // per-frequency vectors Xn, G and the LUT rows, which every row of the tile shares, are fetched once per slab
+            // and four rows instead of once per half slab and two rows: half the 16-byte loads whose 512 bytes per warp hold
+            // only 128-256 distinct ones (the L1's wavefront pipe is this kernel's busiest unit, profiles/r02b), and a half
+            // warp's 8-byte shared stores cover one whole 128-byte row: conflict-free by construction.
+            // The loads of the next row are issued before the current one is computed; the per-row constants live in
+            // shared memory (each warp only reads rows it wrote itself).
             struct Tap { float4 c00, c01, c10, c11; };
             struct Lut { float4 L0, L1; };
+            constexpr int kRows = 4, kStride = 2 * kTcGenWarps;          // rows of a thread: r0 + 32 j
+            static_assert(kRows * kStride == kTcBM, "generator rows");
+            const int q2 = lane >> 4, c16 = lane & 15, r0 = 2 * gw + q2;
             RowParam* rowp = reinterpret_cast<RowParam*>(smem_raw + (sm.rowp - raw));
             for (int64_t tl = worker; tl < n_tiles; tl += n_workers) {
                 const int64_t rt = tile_rt(tl);
                 __syncwarp();
-                if (chunk < kTcRowsPerThread) {
-                    const int rr = rsub + kTcRowStride * chunk;
-                    const int64_t R = tile_row(rt, rr);
+                if (c16 < kRows) {
+                    const int64_t R = tile_row(rt, r0 + kStride * c16);
                     RowParam rp;
                     if (R >= 0) {
                         const int4* src = reinterpret_cast<const int4*>(f.rows + R);
@@ -579,18 +576,17 @@ fused_tc_kernel(const TcParams p) {
                         rp.fp = 0.f; rp.csc = 1.f; rp.ip = 0; rp.pix = -1; rp.w00 = rp.w01 = rp.w10 = rp.w11 = 0.f;
                     }
                     if (f.cube == nullptr || rp.pix < 0) { rp.pix = 0; rp.w00 = rp.w01 = rp.w10 = rp.w11 = 0.f; }
-                    rowp[gw * 8 + chunk * 4 + q4] = rp;     // slot of row (q4, j = chunk): the warp's rows of one j are contiguous (conflict-free reads)
+                    rowp[gw * 8 + c16 * 2 + q2] = rp;      // slot of row (j = c16, q2): the warp's two rows of one j are adjacent
                 }
                 __syncwarp();
-                // 32-bit element offsets of this thread's two rows (plan creation rejects tables of 2^32 elements
-                // or more): one IMAD.WIDE per load instead of 64-bit pointer chains.  Rows outside the cube
-                // carry zero weights and read pixel 0; padded frequencies read the last real chunk (their
-                // filter entries are zero), so every load is unconditional and in bounds.
-                uint32_t lut_off[kTcRowsPerThread], cube_off[kTcRowsPerThread];
+                // 32-bit element offsets of this thread's rows (plan creation rejects tables of 2^32 elements or more).
+                // Rows outside the cube carry zero weights and read pixel 0; padded frequencies read the last real
+                // chunk (their filter entries are zero), so every load is unconditional and in bounds.
+                uint32_t lut_off[kRows], cube_off[kRows];
 #pragma unroll
-                for (int j = 0; j < kTcRowsPerThread; ++j) {
-                    const int4 a = *reinterpret_cast<const int4*>(rowp + gw * 8 + j * 4 + q4);   // fp, csc, ip, pix
-                    lut_off[j] = (uint32_t)a.z * (uint32_t)nfp + (uint32_t)chunk * 4u;
+                for (int j = 0; j < kRows; ++j) {
+                    const int4 a = *reinterpret_cast<const int4*>(rowp + gw * 8 + j * 2 + q2);   // fp, csc, ip, pix
+                    lut_off[j] = (uint32_t)a.z * (uint32_t)nfp + (uint32_t)c16 * 4u;
                     cube_off[j] = (uint32_t)a.w * (uint32_t)nf;
                 }
                 const float* const cube_base = f.cube != nullptr ? f.cube : f.lut_r;
@@ -598,29 +594,28 @@ fused_tc_kernel(const TcParams p) {
                 const uint32_t tap10 = f.cube != nullptr ? (uint32_t)f.n_az * (uint32_t)nf : 0u;
                 const uint32_t nu_last = (uint32_t)(max(f.n_freq, 4) - 4) & ~3u;     // 16-byte aligned (n_freq % 4 == 0 with a cube)
                 // The two LUT rows are looked up per SAMPLE, but the PWV moves by ~1e-4 of a LUT step per sample: the
-                // two rows of a thread nearly always share them.  They are therefore fetched once per half-slab
-                // (for row 0, one half-slab ahead, alternating between two register sets) and re-fetched for row 1
-                // only where its LUT row differs.
-                const bool same_lut = lut_off[1] == lut_off[0];
-                auto issue_lut = [&](int hb, int j, Lut& l) {
-                    const uint32_t lo = lut_off[j] + (uint32_t)hb * kTcHB;
+                // rows of a thread nearly always share them.  They are fetched for row 0 of every slab and re-fetched for
+                // a later row only where its LUT row differs from the one before.
+                bool new_lut[kRows];
+#pragma unroll
+                for (int j = 1; j < kRows; ++j) new_lut[j] = lut_off[j] != lut_off[j - 1];
+                auto issue_lut = [&](int kb, int j, Lut& l) {
+                    const uint32_t lo = lut_off[j] + (uint32_t)kb * kTcBK;
                     l.L0 = ldg4(f.lut_r + lo); l.L1 = ldg4(f.lut_r + (lo + (uint32_t)nfp));
                 };
-                auto issue = [&](int hb, int j, Tap& t) {                 // hb = half-slab (32 frequencies)
+                auto issue = [&](int kb, int j, Tap& t) {
                     if (GT_DIAG(p, 16)) return;
-                    const uint32_t co = cube_off[j] + min((uint32_t)hb * kTcHB + (uint32_t)chunk * 4u, nu_last);
+                    const uint32_t co = cube_off[j] + min((uint32_t)kb * kTcBK + (uint32_t)c16 * 4u, nu_last);
                     t.c00 = ldg4(cube_base + co);           t.c01 = ldg4(cube_base + (co + tap01));
                     t.c10 = ldg4(cube_base + (co + tap10)); t.c11 = ldg4(cube_base + (co + tap10 + tap01));
                 };
-                auto compute = [&](int j, int h, const Tap& cur, const Lut& lut, const float4& X, const float4& G, uint32_t stage) {
-                    const RowParam* rp = rowp + gw * 8 + j * 4 + q4;
+                auto compute = [&](int j, const Tap& cur, const Lut& lut, const float4& X, const float4& G, uint32_t stage) {
+                    const RowParam* rp = rowp + gw * 8 + j * 2 + q2;
                     const float2 fc = *reinterpret_cast<const float2*>(rp);                    // fp, csc (registers for them cost spills: measured 91 -> 108 ms)
                     const float4 w = *reinterpret_cast<const float4*>(&rp->w00);
-                    float4 S, v;
-#ifndef GT_TC_SCALAR_GEN
+                    float4 v;
                     // steps 2-4 on pairs of frequencies: every fp32 operation below is one FFMA2 / FMUL2 / FADD2 for two
-                    // elements (same IEEE operations, same order as the scalar form: bit-identical results, half the
-                    // issue slots -- the generator is bound by issue slots and the L1, not by the FMA pipe)
+                    // elements (the same IEEE operations in the same order as the scalar form, half the issue slots)
                     {
                         using namespace ptx;
                         const f32x2 w00 = pk2(w.x, w.x), w01 = pk2(w.y, w.y), w10 = pk2(w.z, w.z), w11 = pk2(w.w, w.w);
@@ -636,34 +631,21 @@ fused_tc_kernel(const TcParams p) {
                             const float2 ez = upk2(fma2(fp2, sub2(pk2(l1x, l1y), L0), L0));
                             const float2 lg = upk2(mul2(csc2, pk2(lg2_ftz(ez.x), lg2_ftz(ez.y))));
                             const f32x2 eta = pk2(ex2_ftz(lg.x), ex2_ftz(lg.y));
-                            const f32x2 X2 = pk2(Xx, Xy);
-                            const float2 r = upk2(fma2(eta, fma2(pk2(Gx, Gy), S2, pk2(-Xx, -Xy)), X2));
+                            const float2 r = upk2(fma2(eta, fma2(pk2(Gx, Gy), S2, pk2(-Xx, -Xy)), pk2(Xx, Xy)));
                             vx = r.x; vy = r.y;
                         };
                         pair(cur.c00.x, cur.c00.y, cur.c01.x, cur.c01.y, cur.c10.x, cur.c10.y, cur.c11.x, cur.c11.y,
                              lut.L0.x, lut.L0.y, lut.L1.x, lut.L1.y, X.x, X.y, G.x, G.y, v.x, v.y);
                         pair(cur.c00.z, cur.c00.w, cur.c01.z, cur.c01.w, cur.c10.z, cur.c10.w, cur.c11.z, cur.c11.w,
                              lut.L0.z, lut.L0.w, lut.L1.z, lut.L1.w, X.z, X.w, G.z, G.w, v.z, v.w);
-                        (void)S;
                     }
-#else
-                    S.x = w.x * cur.c00.x + w.y * cur.c01.x + w.z * cur.c10.x + w.w * cur.c11.x;
-                    S.y = w.x * cur.c00.y + w.y * cur.c01.y + w.z * cur.c10.y + w.w * cur.c11.y;
-                    S.z = w.x * cur.c00.z + w.y * cur.c01.z + w.z * cur.c10.z + w.w * cur.c11.z;
-                    S.w = w.x * cur.c00.w + w.y * cur.c01.w + w.z * cur.c10.w + w.w * cur.c11.w;
-                    v.x = element_value_fast(fmaf(fc.x, lut.L1.x - lut.L0.x, lut.L0.x), fc.y, X.x, G.x, S.x);
-                    v.y = element_value_fast(fmaf(fc.x, lut.L1.y - lut.L0.y, lut.L0.y), fc.y, X.y, G.y, S.y);
-                    v.z = element_value_fast(fmaf(fc.x, lut.L1.z - lut.L0.z, lut.L0.z), fc.y, X.z, G.z, S.z);
-                    v.w = element_value_fast(fmaf(fc.x, lut.L1.w - lut.L0.w, lut.L0.w), fc.y, X.w, G.w, S.w);
-#endif
-                    if constexpr (NEP) store_nep(smem_raw + (sm.a - raw) + stage * kTcAStageBytes, rsub + kTcRowStride * j, chunk, h, v);
-                    else store_split(smem_raw + (sm.a - raw) + stage * kTcAStageBytes, rsub + kTcRowStride * j, chunk, h, v);
+                    const int row = r0 + kStride * j;
+                    if constexpr (NEP) store_nep(smem_raw + (sm.a - raw) + stage * kTcAStageBytes, row, c16 & 7, c16 >> 3, v);
+                    else store_split(smem_raw + (sm.a - raw) + stage * kTcAStageBytes, row, c16 & 7, c16 >> 3, v);
                 };
                 Tap t0, t1;
-                Lut la, lb;
-                issue_lut(0, 0, la);
+                Lut lut;
                 issue(0, 0, t0);
-                const int n_hb = 2 * p.n_kb;
                 for (int kb = 0; kb < p.n_kb; ++kb, a_ph ^= (++a_st == kTcAStages), a_st = a_st == kTcAStages ? 0u : a_st) {
                     const uint32_t stage = a_st, ph = a_ph;
                     if (GT_DIAG(p, 1)) {
@@ -672,37 +654,20 @@ fused_tc_kernel(const TcParams p) {
                         if (lane == 0) arrive_leader(sm.a_full + 8 * stage);
                         continue;
                     }
-#ifndef GT_TC_LUT_DOUBLE
-                    // the LUT rows are L1 hits (two rows shared by the whole tile): fetched at the head of the half slab they
-                    // are used in, in ONE register set (8 registers fewer than the double-buffered form: fewer spills)
-                    auto half = [&](int h, Lut& cur, Lut&) {
-                        const int hb = 2 * kb + h;
-                        issue_lut(hb, 0, cur);
-                        const float4 X = ldg4(f.Xn + hb * kTcHB + chunk * 4), G = ldg4(f.Gs + hb * kTcHB + chunk * 4);
-                        issue(hb, 1, t1);
-                        if (h == 0) wait_pair(sm.a_empty + 8 * stage, ph ^ 1u);
-                        compute(0, h, t0, cur, X, G, stage);
-                        if (hb + 1 < n_hb) issue(hb + 1, 0, t0);
-                        if (!same_lut) issue_lut(hb, 1, cur);
-                        compute(1, h, t1, cur, X, G, stage);
-                    };
-                    half(0, la, la);
-                    half(1, la, la);
-#else
-                    auto half = [&](int h, Lut& cur, Lut& nxt) {
-                        const int hb = 2 * kb + h;
-                        const float4 X = ldg4(f.Xn + hb * kTcHB + chunk * 4), G = ldg4(f.Gs + hb * kTcHB + chunk * 4);
-                        issue(hb, 1, t1);
-                        if (hb + 1 < n_hb) issue_lut(hb + 1, 0, nxt);
-                        if (h == 0) wait_pair(sm.a_empty + 8 * stage, ph ^ 1u);
-                        compute(0, h, t0, cur, X, G, stage);
-                        if (hb + 1 < n_hb) issue(hb + 1, 0, t0);
-                        if (!same_lut) issue_lut(hb, 1, cur);
-                        compute(1, h, t1, cur, X, G, stage);
-                    };
-                    half(0, la, lb);
-                    half(1, lb, la);
-#endif
+                    issue_lut(kb, 0, lut);
+                    const float4 X = ldg4(f.Xn + kb * kTcBK + c16 * 4), G = ldg4(f.Gs + kb * kTcBK + c16 * 4);
+                    issue(kb, 1, t1);
+                    wait_pair(sm.a_empty + 8 * stage, ph ^ 1u);
+                    compute(0, t0, lut, X, G, stage);
+                    issue(kb, 2, t0);
+                    if (new_lut[1]) issue_lut(kb, 1, lut);
+                    compute(1, t1, lut, X, G, stage);
+                    issue(kb, 3, t1);
+                    if (new_lut[2]) issue_lut(kb, 2, lut);
+                    compute(2, t0, lut, X, G, stage);
+                    if (kb + 1 < p.n_kb) issue(kb + 1, 0, t0);
+                    if (new_lut[3]) issue_lut(kb, 3, lut);
+                    compute(3, t1, lut, X, G, stage);
                     // one arrival per warp: 512 per-thread arrivals on one mbarrier serialise (~5 cycles each)
                     ptx::fence_proxy_async_smem();
                     __syncwarp();
