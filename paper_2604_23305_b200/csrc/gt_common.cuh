@@ -80,9 +80,10 @@ __device__ __forceinline__ void philox4x32_10_multi4(uint32_t c0, uint32_t c1, c
     for (int i = 0; i < W; ++i) o[i] = make_uint4(a[i], b[i], c[i], d[i]);
 }
 
-// U(w) = ((w >> 9) + 1/2) 2^-23 in (0,1): exact in fp32 (R19).
+// U(w) = ((w >> 9) + 1/2) 2^-23 in (0,1): exact in fp32 (R19), as ONE fused multiply-add (the product and the
+// sum are both exact, so this equals the two-step form bit for bit).
 __device__ __forceinline__ float uniform01(uint32_t w) {
-    return ((float)(w >> 9) + 0.5f) * (1.0f / 8388608.0f);
+    return fmaf((float)(w >> 9), 1.0f / 8388608.0f, 0.5f / 8388608.0f);
 }
 
 // Box-Muller: z0 = sqrt(-2 ln U(w0)) cos(2 pi U(w1)), z1 = ... sin(...).  MUFU log/sin/cos: the
@@ -91,14 +92,23 @@ __device__ __forceinline__ float uniform01(uint32_t w) {
 __device__ __forceinline__ float sqrt_fast(float x) {
     float r; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r;
 }
+// radius sqrt(-2 ln U(w)) = sqrt(-2 ln2 log2 U): U >= 2^-24 is a normal number, so the bare MUFU.LG2 serves (__logf adds a
+// denormal branch of three instructions) and the two constants fold into one multiply
+__device__ __forceinline__ float bm_radius(uint32_t w) {
+    float l; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(l) : "f"(uniform01(w)));
+    return sqrt_fast(-1.38629436111989061883f * l);
+}
+// angle 2 pi U(w) in one fused multiply-add (one rounding instead of two: 2^-24 relative, far inside MUFU.SIN's own error)
+__device__ __forceinline__ float bm_angle(uint32_t w) {
+    return fmaf((float)(w >> 9), 6.28318530717958647692f / 8388608.0f, 3.14159265358979323846f / 8388608.0f);
+}
 __device__ __forceinline__ float normal_cos(uint32_t w0, uint32_t w1) {
-    const float r = sqrt_fast(-2.0f * __logf(uniform01(w0)));
-    return r * __cosf(6.28318530717958647692f * uniform01(w1));
+    return bm_radius(w0) * __cosf(bm_angle(w1));
 }
 __device__ __forceinline__ void normal_pair(uint32_t w0, uint32_t w1, float& z0, float& z1) {
-    const float r = sqrt_fast(-2.0f * __logf(uniform01(w0)));
+    const float r = bm_radius(w0);
     float s, c;
-    __sincosf(6.28318530717958647692f * uniform01(w1), &s, &c);
+    __sincosf(bm_angle(w1), &s, &c);
     z0 = r * c; z1 = r * s;
 }
 
@@ -114,8 +124,7 @@ __device__ __forceinline__ void normals_of_block(const uint4& w, float (&z)[4]) 
 __device__ __forceinline__ float photon_normal(uint32_t n, uint32_t spaxel, uint32_t c, uint32_t seed_lo, uint32_t seed_hi) {
     const uint4 w = philox4x32_10(n, spaxel, photon_block(c), kStreamPhoton, seed_lo, seed_hi);
     const uint32_t k = photon_slot(c);
-    const float r = sqrt_fast(-2.0f * __logf(uniform01(k < 2u ? w.x : w.z)));
-    const float a = 6.28318530717958647692f * uniform01(k < 2u ? w.y : w.w);
+    const float r = bm_radius(k < 2u ? w.x : w.z), a = bm_angle(k < 2u ? w.y : w.w);
     return r * ((k & 1u) ? __sinf(a) : __cosf(a));
 }
 

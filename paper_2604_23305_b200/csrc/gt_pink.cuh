@@ -10,6 +10,7 @@
 // fused kernel's 4 B, one Philox call per detector-sample.
 #pragma once
 #include "gt_common.cuh"
+#include "gt_tc_ptx.cuh"     // packed fp32 pairs (FFMA2 / FMUL2 / FADD2)
 
 namespace gt {
 
@@ -84,23 +85,51 @@ pink_chain_kernel(PinkParams p, int64_t t0, int64_t T, float* __restrict__ tod) 
     const bool valid = d < p.n_det;
     const int64_t m0 = sg * kPinkSeg;
     const int len = (int)min((int64_t)kPinkSeg, T - m0);
-    float g[JM], x[JM];
+    // The stages are worked in PAIRS (2i, 2i + 1) on packed fp32 (FFMA2 / FMUL2: two IEEE operations per issue slot; the
+    // kernel is bound by instruction issue, profiles/r02a_pink.md): a pair shares one Box-Muller radius, its normals are
+    // the cosine and the sine branch, so  x2 <- phi2 x2 + r (sq2 * (cos, sin)).
+    using ptx::f32x2; using ptx::pk2; using ptx::upk2; using ptx::fma2; using ptx::mul2; using ptx::add2;
+    float g[JM];
+    f32x2 x2[JM / 2], g2[JM / 2], phi2[JM / 2], sq2[JM / 2];
 #pragma unroll
-    for (int j = 0; j < JM; ++j) { g[j] = (valid && j < p.J) ? p.gain[d * p.J + j] : 0.f; x[j] = 0.f; }
+    for (int j = 0; j < JM; ++j) g[j] = (valid && j < p.J) ? p.gain[d * p.J + j] : 0.f;
+#pragma unroll
+    for (int i = 0; i < JM / 2; ++i) {
+        x2[i] = pk2(0.f, 0.f); g2[i] = pk2(g[2 * i], g[2 * i + 1]);
+        phi2[i] = pk2(p.phi[2 * i], p.phi[2 * i + 1]); sq2[i] = pk2(p.sq[2 * i], p.sq[2 * i + 1]);
+    }
     if (valid) {
         const uint32_t s = p.spaxel_base + (uint32_t)(d / p.n_chan), c = (uint32_t)(d % p.n_chan);
         for (int m = 0; m < len; ++m) {
-            float z[kPinkMaxJ];
-            pink_normals(p, (uint32_t)(t0 + m0 + m), s, c, z);
-            float pn = 0.f;
-#pragma unroll
-            for (int j = 0; j < JM; ++j) {
-                x[j] = fmaf(p.phi[j], x[j], p.sq[j] * z[j]);
-                pn = fmaf(g[j], x[j], pn);
+            uint32_t w[JM];
+            {
+                const uint4 a = philox4x32_10((uint32_t)(t0 + m0 + m), s, c, kStreamPinkLo, p.seed_lo, p.seed_hi);
+                w[0] = a.x; w[1] = a.y; w[2] = a.z; w[3] = a.w;
             }
-            s_pn[m * 256 + tid] = pn;
+            if constexpr (JM > 4) {
+                if (p.J > 4) {
+                    const uint4 b = philox4x32_10((uint32_t)(t0 + m0 + m), s, c, kStreamPinkHi, p.seed_lo, p.seed_hi);
+                    w[4] = b.x; w[5] = b.y; w[6] = b.z; w[7] = b.w;
+                } else {
+                    w[4] = w[5] = w[6] = w[7] = 0u;       // stages 4-7 carry zero gains and zero states
+                }
+            }
+            f32x2 pn2 = pk2(0.f, 0.f);
+#pragma unroll
+            for (int i = 0; i < JM / 2; ++i) {
+                const float r = bm_radius(w[2 * i]);
+                float sn, cs;
+                __sincosf(bm_angle(w[2 * i + 1]), &sn, &cs);
+                x2[i] = fma2(pk2(r, r), mul2(sq2[i], pk2(cs, sn)), mul2(phi2[i], x2[i]));
+                pn2 = fma2(g2[i], x2[i], pn2);
+            }
+            const float2 pn = upk2(pn2);
+            s_pn[m * 256 + tid] = pn.x + pn.y;
         }
     }
+    float x[JM];
+#pragma unroll
+    for (int i = 0; i < JM / 2; ++i) { const float2 v = upk2(x2[i]); x[2 * i] = v.x; x[2 * i + 1] = v.y; }
     // state at the segment start
     if (sg > 0) {
         if (tid == 0) {
@@ -138,9 +167,9 @@ pink_chain_kernel(PinkParams p, int64_t t0, int64_t T, float* __restrict__ tod) 
     }
     // one read-modify-write of the TOD
     if (valid) {
-        float a[JM];
+        f32x2 a2[JM / 2];
 #pragma unroll
-        for (int j = 0; j < JM; ++j) a[j] = g[j] * cin[j];
+        for (int i = 0; i < JM / 2; ++i) a2[i] = mul2(g2[i], pk2(cin[2 * i], cin[2 * i + 1]));
         float* col = tod + m0 * p.n_det + d;
         for (int mb = 0; mb < len; mb += kPinkBatch) {
             float cur[kPinkBatch];
@@ -150,10 +179,11 @@ pink_chain_kernel(PinkParams p, int64_t t0, int64_t T, float* __restrict__ tod) 
             for (int b = 0; b < kPinkBatch; ++b) {
                 const int m = mb + b;
                 if (m < len) {
-                    float add = 0.f;
+                    f32x2 add2v = pk2(0.f, 0.f);
 #pragma unroll
-                    for (int j = 0; j < JM; ++j) { a[j] *= p.phi[j]; add += a[j]; }
-                    col[(int64_t)m * p.n_det] = cur[b] + (s_pn[m * 256 + tid] + add);
+                    for (int i = 0; i < JM / 2; ++i) { a2[i] = mul2(a2[i], phi2[i]); add2v = add2(add2v, a2[i]); }
+                    const float2 add = upk2(add2v);
+                    col[(int64_t)m * p.n_det] = cur[b] + (s_pn[m * 256 + tid] + (add.x + add.y));
                 }
             }
         }
