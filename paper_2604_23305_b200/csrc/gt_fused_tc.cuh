@@ -589,7 +589,16 @@ fused_tc_kernel(const TcParams p) {
                     lut_off[j] = (uint32_t)a.z * (uint32_t)nfp + (uint32_t)c16 * 4u;
                     cube_off[j] = (uint32_t)a.w * (uint32_t)nf;
                 }
-                const float* const cube_base = f.cube != nullptr ? f.cube : f.lut_r;
+                // The base pointer lives in a per-thread register pair (it gets an opaque zero added): "base + 4 * offset" then
+                // compiles to LEA + LEA.HI.X on the integer pipe.  With the base in a uniform register it is IMAD.MOV (the
+                // constant 4) + IMAD.WIDE on the FMA pipe, which the packed FFMA2 stream already keeps busy: 78.0-79.2 ->
+                // 76.5 ms per C4 step.
+                const float* cube_base = f.cube != nullptr ? f.cube : f.lut_r;
+                {
+                    uint32_t zero;                                    // lane >> 5: always 0, opaque to the compiler
+                    asm volatile("mov.u32 %0, %%laneid;" : "=r"(zero));
+                    cube_base += zero >> 5;
+                }
                 const uint32_t tap01 = f.cube != nullptr ? (uint32_t)nf : 0u;
                 const uint32_t tap10 = f.cube != nullptr ? (uint32_t)f.n_az * (uint32_t)nf : 0u;
                 const uint32_t nu_last = (uint32_t)(max(f.n_freq, 4) - 4) & ~3u;     // 16-byte aligned (n_freq % 4 == 0 with a cube)
