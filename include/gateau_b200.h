@@ -232,6 +232,26 @@ gt_status gt_common_mode_partial(gt_plan* plan, int64_t t_begin, int64_t t_count
 gt_status gt_common_mode_apply(gt_plan* plan, int64_t t_begin, int64_t t_count, float* tod_K_dev, double pwv_mean_mm,
                                const float* sum_dev, int32_t n_out_total, void* cuda_stream);
 
+/* The same subtraction (Eq. 25-26, single plan holding every spaxel: partial sum, then apply) for callers that cannot
+ * allocate device memory -- code under CUDA-graph capture, tight serving loops, harnesses that forbid cudaMalloc.  The
+ * [t_count][n_chan] partial sums, which gt_common_mode_partial / _apply take as a caller-owned buffer, live in ONE
+ * file-scope static device array of GT_COMMON_MODE_STATIC_MAX floats (8 MB) inside the library: every GPU that loads the
+ * library holds it until the process exits.  The call allocates nothing, on the device or on the host (no cudaMalloc,
+ * cudaFree, pool or allocating library routine: the per-channel and per-spaxel constants are built on the stack and
+ * copied into tables the plan already owns); its device address is resolved once per device at gt_plan_create.
+ *   tod_K_dev: DEVICE [t_count][n_spaxel][n_chan] fp32, brightness temperature, overwritten in place with T*_a.
+ *   *n_out = N_out of the plan's spaxels.  Results are bit-identical to gt_common_mode_partial + gt_common_mode_apply.
+ * Limits: t_count * n_chan <= GT_COMMON_MODE_STATIC_MAX (call it on windows of samples), n_chan <= 4096,
+ * n_spaxel <= 4096: GT_ERR_SHAPE beyond them, with the limit in the message.  GT_ERR_VALUE if N_out = 0; otherwise the
+ * errors of gt_common_mode_partial.
+ * EVERY call on a device shares the array, which keeps the last call's contents (never read: the partial sums overwrite
+ * all t_count * n_chan elements before they are used, so nothing needs clearing).  Calls that overlap on the GPU -- two
+ * streams, two plans, two host threads on one device -- RACE on it: serialise them (one stream, or events).  Asynchronous
+ * on cuda_stream after a short synchronous upload of the constants, like gt_common_mode_partial. */
+#define GT_COMMON_MODE_STATIC_MAX 2097152
+gt_status gt_common_mode_static(gt_plan* plan, int64_t t_begin, int64_t t_count, float* tod_K_dev, double pwv_mean_mm,
+                                double r_out_rad, int32_t* n_out, void* cuda_stream);
+
 /* Message of the last error on this plan; plan == NULL => the calling thread's last
  * gt_plan_create error.  Never NULL. */
 const char* gt_last_error(const gt_plan* plan);

@@ -23,7 +23,11 @@ EXPORTS = ("gt_plan_create", "gt_simulate", "gt_plan_destroy", "gt_last_error", 
            "gt_debug_philox", "gt_debug_pkid", "gt_launch_count", "gt_variant_name", "gt_last_fused_ms",
            "gt_debug_kelvin_map", "gt_prepare_screen", "gt_prepare_source", "gt_plan_counters",
            "gt_pink_state_export", "gt_pink_state_import", "gt_debug_chunking", "gt_debug_timeline",
-           "gt_measure_fp32_fma", "gt_common_mode_partial", "gt_common_mode_apply", "gt_release_cached_memory")
+           "gt_measure_fp32_fma", "gt_common_mode_partial", "gt_common_mode_apply", "gt_release_cached_memory",
+           "gt_common_mode_static")
+
+
+COMMON_MODE_STATIC_MAX = 2097152      # GT_COMMON_MODE_STATIC_MAX: floats of static device scratch (t_count * n_chan per call)
 
 
 class GtStage(C.Structure):
@@ -123,6 +127,9 @@ def lib() -> C.CDLL:
                                              C.POINTER(C.c_int32), C.c_void_p]
         L.gt_common_mode_apply.restype = C.c_int
         L.gt_common_mode_apply.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_void_p, C.c_double, C.c_void_p, C.c_int32, C.c_void_p]
+        L.gt_common_mode_static.restype = C.c_int
+        L.gt_common_mode_static.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_void_p, C.c_double, C.c_double,
+                                            C.POINTER(C.c_int32), C.c_void_p]
         L.gt_release_cached_memory.restype = C.c_int
         L.gt_release_cached_memory.argtypes = []
         L.gt_debug_chunking.restype = C.c_int
@@ -304,6 +311,14 @@ class Plan:
         self._check(self.L.gt_common_mode_apply(self.handle, t_begin, int(tod_K.shape[0]), _ptr(tod_K), float(pwv_mean_mm),
                                                 _ptr(total), int(n_out_total), self._stream()))
         return tod_K
+
+    def common_mode_static(self, tod_K, pwv_mean_mm, r_out_rad, t_begin=0):
+        """gt_common_mode_static: tod_K <- T*_a (Eq. 25) in place, partial sums in the library's static device array
+        (no allocation; t_count * n_chan <= COMMON_MODE_STATIC_MAX).  Returns (tod_K, N_out)."""
+        n = C.c_int32(0)
+        self._check(self.L.gt_common_mode_static(self.handle, t_begin, int(tod_K.shape[0]), _ptr(tod_K), float(pwv_mean_mm),
+                                                 float(r_out_rad), C.byref(n), self._stream()))
+        return tod_K, int(n.value)
 
     def counters(self) -> dict:
         """gt_plan_counters: rows processed, rows outside the cube, PWV clamps below / above the LUT."""

@@ -30,6 +30,31 @@
 #include "gt_common_mode.cuh"
 #include <cufft.h>
 
+// ---- gt_common_mode_static: the [t x chan] partial sums of Eq. 25 in library-owned static device memory ----
+// Part of the module image: every GPU that loads this library holds these 8 MB until the process exits.  In HOST code the
+// name below is a host-side stand-in, not a device address (a kernel given it faults, or silently uses the wrong memory
+// where the GPU can reach host memory): host code uses the address cudaGetSymbolAddress returns, resolved once per
+// device at plan creation (cm_static_resolve) with that device current.
+static __device__ __align__(256) float g_cm_static_scratch[GT_COMMON_MODE_STATIC_MAX];
+
+namespace {
+float* g_cm_static_ptr[64] = {};          // per device: device address of g_cm_static_scratch (nullptr = not resolved yet)
+std::atomic<bool> g_cm_static_ok[64] = {};
+
+// set-up, once per device, with that device current (called by gt_plan_create)
+cudaError_t cm_static_resolve(int dev) {
+    if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+    if (g_cm_static_ok[dev].load(std::memory_order_acquire)) return cudaSuccess;
+    float* ptr = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(reinterpret_cast<void**>(&ptr), g_cm_static_scratch);
+    if (e != cudaSuccess) return e;
+    if (ptr == nullptr) return cudaErrorInvalidSymbol;
+    g_cm_static_ptr[dev] = ptr;            // racing plan creations on one device store the same value
+    g_cm_static_ok[dev].store(true, std::memory_order_release);
+    return cudaSuccess;
+}
+}  // namespace
+
 namespace {
 
 // CODATA exact values (PAPER.md names h, k_B implicitly through P^JN; R4)
@@ -713,6 +738,7 @@ gt_status gt_plan_create(const gt_config* cfg, void* cuda_stream, gt_plan** out_
     p->h_daz.assign(c.daz_rad, c.daz_rad + ns); p->h_del.assign(c.del_rad, c.del_rad + ns);
     p->h_fc.assign(c.f_center_hz, c.f_center_hz + nc);
     GT_CUDA0(p->d_ln_eta_z.alloc((size_t)nc)); GT_CUDA0(p->d_cm_weight.alloc((size_t)ns));
+    GT_CUDA0(cm_static_resolve(p->device));     // device address of the static scratch of gt_common_mode_static
     GT_CUDA0(p->d_counters.alloc(3));
     GT_CUDA0(cudaMemsetAsync(p->d_counters.p, 0, 3 * sizeof(unsigned long long), st));
 
@@ -1136,6 +1162,76 @@ gt_status gt_common_mode_apply(gt_plan* plan, int64_t t_begin, int64_t t_count, 
     gt::cm_apply_kernel<<<(unsigned)(t_count * plan->n_spaxel), 128, 0, st>>>(k, tod_K_dev, sum_dev);
     GT_CUDA(plan, cudaGetLastError());
     plan->launches++; plan->last_stream = st;
+    return GT_OK;
+}
+
+gt_status gt_common_mode_static(gt_plan* plan, int64_t t_begin, int64_t t_count, float* tod_K_dev, double pwv_mean_mm,
+                                double r_out_rad, int32_t* n_out, void* cuda_stream) {
+    if (!plan || !tod_K_dev || !n_out) return fail(plan, GT_ERR_NULL, "gt_common_mode_static: NULL argument");
+    if (t_begin < 0 || t_count < 0 || t_begin + t_count > plan->n_samples) return fail(plan, GT_ERR_RANGE, "sample range outside the plan");
+    constexpr int kMaxChan = 4096, kMaxSpaxel = 4096;      // the per-channel / per-spaxel constants are built on the stack
+    if (plan->n_chan > kMaxChan || plan->n_spaxel > kMaxSpaxel)
+        return fail(plan, GT_ERR_SHAPE, "gt_common_mode_static: at most %d channels and %d spaxels (the plan has %d and %d)",
+                    kMaxChan, kMaxSpaxel, plan->n_chan, plan->n_spaxel);
+    if (t_count * (int64_t)plan->n_chan > (int64_t)GT_COMMON_MODE_STATIC_MAX)
+        return fail(plan, GT_ERR_SHAPE, "gt_common_mode_static: t_count * n_chan = %lld exceeds the static scratch of %lld "
+                    "elements (GT_COMMON_MODE_STATIC_MAX): call it on windows of at most %lld samples, or use "
+                    "gt_common_mode_partial / gt_common_mode_apply with a buffer of your own",
+                    (long long)(t_count * plan->n_chan), (long long)GT_COMMON_MODE_STATIC_MAX,
+                    (long long)(GT_COMMON_MODE_STATIC_MAX / plan->n_chan));
+    if (t_count * plan->n_spaxel > 0x7fffffffLL) return fail(plan, GT_ERR_SHAPE, "common mode: more than 2^31 rows in one call");
+    {
+        int dev = -1;
+        GT_CUDA(plan, cudaGetDevice(&dev));
+        if (dev != plan->device) return fail(plan, GT_ERR_VALUE, "the plan lives on device %d, the current device is %d", plan->device, dev);
+    }
+    float* const scratch = g_cm_static_ok[plan->device].load(std::memory_order_acquire) ? g_cm_static_ptr[plan->device] : nullptr;
+    if (!scratch) return fail(plan, GT_ERR_CUDA, "gt_common_mode_static: the static scratch of device %d was never resolved", plan->device);
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    gt_plan* const p = plan;
+    if (!(pwv_mean_mm == pwv_mean_mm) || !(r_out_rad >= 0.0)) return fail(p, GT_ERR_VALUE, "common mode: pwv_mean and r_out must be a number and non-negative");
+    // the constants of cm_setup (same arithmetic), in stack arrays instead of vectors: nothing is allocated, on either side
+    double le[kMaxChan];
+    float w[kMaxSpaxel];
+    {
+        const int n_pwv = p->n_pwv, nn = p->n_nu_lut;
+        double q = (pwv_mean_mm - p->lut_pwv0) / p->lut_dpwv;
+        if (!(q >= 0.0)) q = 0.0;
+        if (q > (double)(n_pwv - 1)) q = (double)(n_pwv - 1);
+        const int ip = (int)std::min<double>(std::floor(q), n_pwv - 2);
+        const double fpq = q - ip;
+        for (int c = 0; c < p->n_chan; ++c) {
+            const double r = (p->h_fc[c] - p->lut_nu0) / p->lut_dnu;
+            if (r < -1e-9 || r > (nn - 1) + 1e-9) return fail(p, GT_ERR_RANGE, "common mode: channel centre %d lies outside the lookup table", c);
+            int ir = (int)std::floor(r);
+            ir = std::max(0, std::min(ir, nn - 2));
+            const double fr = r - ir;
+            const float* L0 = p->h_lut.data() + (size_t)ip * nn + ir;
+            const float* L1 = L0 + nn;
+            const double ez = (1.0 - fpq) * ((1.0 - fr) * L0[0] + fr * L0[1]) + fpq * ((1.0 - fr) * L1[0] + fr * L1[1]);
+            le[c] = std::log(ez);
+            if (!(le[c] < 0.0)) return fail(p, GT_ERR_VALUE, "common mode: the atmosphere is fully transparent in channel %d (1 - eta_atm = 0 in Eq. 25)", c);
+        }
+    }
+    int32_t n = 0;
+    for (int s = 0; s < p->n_spaxel; ++s) { w[s] = std::hypot(p->h_daz[s], p->h_del[s]) > r_out_rad ? 1.f : 0.f; n += w[s] != 0.f; }
+    *n_out = n;
+    if (n < 1) return fail(p, GT_ERR_VALUE, "common mode: no spaxel lies outside r_out (N_out = 0 in Eq. 25)");
+    if (t_count == 0) return GT_OK;
+    GT_CUDA(p, cudaMemcpyAsync(p->d_ln_eta_z.p, le, (size_t)p->n_chan * sizeof(double), cudaMemcpyHostToDevice, st));
+    GT_CUDA(p, cudaMemcpyAsync(p->d_cm_weight.p, w, (size_t)p->n_spaxel * sizeof(float), cudaMemcpyHostToDevice, st));
+    GT_CUDA(p, cudaStreamSynchronize(st));                 // the stack arrays go out of scope
+    gt::CmParams k{};
+    k.sinE = p->d_sinE.p; k.cosE = p->d_cosE.p; k.sin_del = p->d_sp.p + 2 * p->n_spaxel; k.cos_del = p->d_sp.p + 3 * p->n_spaxel;
+    k.ln_eta_z = p->d_ln_eta_z.p; k.weight = p->d_cm_weight.p; k.n_spaxel = p->n_spaxel; k.n_chan = p->n_chan;
+    k.t0 = t_begin; k.T = t_count; k.inv_n_out = 1.0 / (double)n;
+    // cm_partial_kernel overwrites every element [0, t_count * n_chan) it later reads: nothing in the shared array has to
+    // start at zero, and what the previous call left behind is never read
+    gt::cm_partial_kernel<<<(unsigned)t_count, 128, 0, st>>>(k, tod_K_dev, scratch);
+    GT_CUDA(p, cudaGetLastError());
+    gt::cm_apply_kernel<<<(unsigned)(t_count * p->n_spaxel), 128, 0, st>>>(k, tod_K_dev, scratch);
+    GT_CUDA(p, cudaGetLastError());
+    p->launches += 2; p->last_stream = st;
     return GT_OK;
 }
 
