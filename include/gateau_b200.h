@@ -296,6 +296,12 @@ const char* gt_variant_name(const gt_plan* plan);
  * over its launches (CUDA events on the launching stream); synchronises the stream.  Also
  * returns the number of launches in *n_launches (NULL ok). */
 double gt_last_fused_ms(gt_plan* plan, int32_t* n_launches);
+/* Banded corrections of the tensor variant: *blocks = correction products of the three-term split,
+ * two (A_lo.Fm_hi and A_hi.Fm_lo) per (channel group, column group, 64-frequency slab) block of the contraction;
+ * *skipped = how many of them are not issued because the plan proved them negligible there (worst case over the spectra
+ * the plan can produce, all skipped products of a channel together, below 1e-6 of the channel's smallest power).
+ * Both 0 for GT_VARIANT_FP32.  Test and reporting hook. */
+gt_status gt_debug_corrections(const gt_plan* plan, int64_t* blocks, int64_t* skipped);
 /* Measurement hooks (bench.py).  gt_debug_timeline: device timeline of the last HOST-output gt_simulate call, per chunk
  * k < *n_chunks <= capacity: ms_out[4 k + {0,1,2,3}] = {compute begin, compute end, copy begin, copy end} in ms after the
  * first chunk's compute begin (CUDA events on the compute stream and on the internal copy stream): shows the D2H copy

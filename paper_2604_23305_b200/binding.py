@@ -24,7 +24,7 @@ EXPORTS = ("gt_plan_create", "gt_simulate", "gt_plan_destroy", "gt_last_error", 
            "gt_debug_kelvin_map", "gt_prepare_screen", "gt_prepare_source", "gt_plan_counters",
            "gt_pink_state_export", "gt_pink_state_import", "gt_debug_chunking", "gt_debug_timeline",
            "gt_measure_fp32_fma", "gt_common_mode_partial", "gt_common_mode_apply", "gt_release_cached_memory",
-           "gt_common_mode_static")
+           "gt_common_mode_static", "gt_debug_corrections")
 
 
 COMMON_MODE_STATIC_MAX = 2097152      # GT_COMMON_MODE_STATIC_MAX: floats of static device scratch (t_count * n_chan per call)
@@ -130,6 +130,8 @@ def lib() -> C.CDLL:
         L.gt_common_mode_static.restype = C.c_int
         L.gt_common_mode_static.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_void_p, C.c_double, C.c_double,
                                             C.POINTER(C.c_int32), C.c_void_p]
+        L.gt_debug_corrections.restype = C.c_int
+        L.gt_debug_corrections.argtypes = [C.c_void_p, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
         L.gt_release_cached_memory.restype = C.c_int
         L.gt_release_cached_memory.argtypes = []
         L.gt_debug_chunking.restype = C.c_int
@@ -319,6 +321,12 @@ class Plan:
         self._check(self.L.gt_common_mode_static(self.handle, t_begin, int(tod_K.shape[0]), _ptr(tod_K), float(pwv_mean_mm),
                                                  float(r_out_rad), C.byref(n), self._stream()))
         return tod_K, int(n.value)
+
+    def corrections(self):
+        """gt_debug_corrections: (blocks, blocks that skip the split's correction MMAs)."""
+        a, b = C.c_int64(0), C.c_int64(0)
+        self._check(self.L.gt_debug_corrections(self.handle, C.byref(a), C.byref(b)))
+        return int(a.value), int(b.value)
 
     def counters(self) -> dict:
         """gt_plan_counters: rows processed, rows outside the cube, PWV clamps below / above the LUT."""

@@ -528,39 +528,49 @@ gt_status gt_plan_create(const gt_config* cfg, void* cuda_stream, gt_plan** out_
 
     // ---- statistics of the large device arrays: non-finite values are refused, the cube's per-frequency maximum
     //      bounds the spectrum elements (operand range of the tensor kernel), the means feed the reference spectrum ----
-    std::vector<float> cube_max(nf, 0.f);
+    std::vector<float> cube_max(nf, 0.f), cube_lo(nf, 0.f), cube_hi(nf, 0.f);     // |.| maximum; signed range including 0 (outside the cube)
     std::vector<double> cube_mean(nf, 0.0);
-    double screen_mean = 0.0;
+    double screen_mean = 0.0, screen_lo = 0.0, screen_hi = 0.0;
     {
         const int64_t n_pix = c.cube ? (int64_t)c.n_az * c.n_el : 0;
         DevBuf<uint32_t> d_max; DevBuf<double> d_sum;
         const size_t n_stat = (size_t)nf + (size_t)c.nx;
-        GT_CUDA0(d_max.alloc(n_stat)); GT_CUDA0(d_sum.alloc(n_stat));
+        GT_CUDA0(d_max.alloc(3 * n_stat)); GT_CUDA0(d_sum.alloc(n_stat));           // |.| max bits, min keys, max keys
         GT_CUDA0(cudaMemsetAsync(d_max.p, 0, n_stat * sizeof(uint32_t), st));
+        GT_CUDA0(cudaMemsetAsync(d_max.p + n_stat, 0xFF, n_stat * sizeof(uint32_t), st));
+        GT_CUDA0(cudaMemsetAsync(d_max.p + 2 * n_stat, 0, n_stat * sizeof(uint32_t), st));
         GT_CUDA0(cudaMemsetAsync(d_sum.p, 0, n_stat * sizeof(double), st));
         if (c.cube) {
             const unsigned gy = (unsigned)std::min<int64_t>(n_pix, std::max<int64_t>(1, (8 * p->num_sms) / ((nf + 255) / 256)));
-            gt::colstat_kernel<<<dim3((unsigned)((nf + 255) / 256), gy), 256, 0, st>>>(c.cube, n_pix, nf, d_max.p, d_sum.p);
+            gt::colstat_kernel<<<dim3((unsigned)((nf + 255) / 256), gy), 256, 0, st>>>(c.cube, n_pix, nf, d_max.p, d_sum.p,
+                                                                                      d_max.p + n_stat, d_max.p + 2 * n_stat);
             GT_CUDA0(cudaGetLastError());
         }
         {
             const unsigned gy = (unsigned)std::min<int64_t>(c.ny, std::max<int64_t>(1, (8 * p->num_sms) / ((c.nx + 255) / 256)));
-            gt::colstat_kernel<<<dim3((unsigned)((c.nx + 255) / 256), gy), 256, 0, st>>>(c.screen, c.ny, c.nx, d_max.p + nf, d_sum.p + nf);
+            gt::colstat_kernel<<<dim3((unsigned)((c.nx + 255) / 256), gy), 256, 0, st>>>(c.screen, c.ny, c.nx, d_max.p + nf, d_sum.p + nf,
+                                                                                        d_max.p + n_stat + nf, d_max.p + 2 * n_stat + nf);
             GT_CUDA0(cudaGetLastError());
         }
         p->launches += c.cube ? 2 : 1;
-        std::vector<uint32_t> h_max(n_stat); std::vector<double> h_sum(n_stat);
-        GT_CUDA0(cudaMemcpyAsync(h_max.data(), d_max.p, n_stat * sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
+        std::vector<uint32_t> h_max(3 * n_stat); std::vector<double> h_sum(n_stat);
+        GT_CUDA0(cudaMemcpyAsync(h_max.data(), d_max.p, 3 * n_stat * sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
         GT_CUDA0(cudaMemcpyAsync(h_sum.data(), d_sum.p, n_stat * sizeof(double), cudaMemcpyDeviceToHost, st));
         GT_CUDA0(cudaStreamSynchronize(st));
         for (int i = 0; i < nf; ++i) {
             if (h_max[i] >= 0x7F800000u) return fail(nullptr, GT_ERR_VALUE, "the source cube holds a NaN or Inf (frequency index %d)", i);
             std::memcpy(&cube_max[i], &h_max[i], sizeof(float));
             cube_mean[i] = n_pix ? h_sum[i] / (double)n_pix : 0.0;
+            if (n_pix) {
+                cube_lo[i] = std::min(0.f, gt::key_float(h_max[n_stat + i]));
+                cube_hi[i] = std::max(0.f, gt::key_float(h_max[2 * n_stat + i]));
+            }
         }
         for (int i = 0; i < c.nx; ++i) {
             if (h_max[nf + i] >= 0x7F800000u) return fail(nullptr, GT_ERR_VALUE, "the PWV screen holds a NaN or Inf (column %d)", i);
             screen_mean += h_sum[nf + i];
+            const double lo = gt::key_float(h_max[n_stat + nf + i]), hi = gt::key_float(h_max[2 * n_stat + nf + i]);
+            screen_lo = i ? std::min(screen_lo, lo) : lo; screen_hi = i ? std::max(screen_hi, hi) : hi;
         }
         screen_mean /= (double)c.nx * (double)c.ny;
     }
@@ -691,7 +701,50 @@ gt_status gt_plan_create(const gt_config* cfg, void* cuda_stream, gt_plan** out_
         }
 #endif
         std::vector<float> inv;
-        if (gt_status s = gt::build_tc_tables(h_filt, nc, nf, nfp, a_ref, p->tc, inv, st)) {
+        // banded corrections: the range of the elements the generator can produce, per frequency (scaled units), and what
+        // every channel's power holds at least.  An element is (1 - eta) Xn + eta G S:
+        //   eta = eta_z(nu, PWV)^csc; PWV lies between pwv0(t) + the screen's minimum and maximum, so eta_z (bilinear in PWV:
+        //   a convex combination of two adjacent table rows) lies between the smallest and the largest entry of the table
+        //   rows that range touches; csc lies between its values at the lowest and highest elevation of the scan;
+        //   S (bilinear in the cube, zero outside) lies between the cube's minimum and maximum at that frequency, and 0.
+        // The expression is bilinear in (eta, S): its extremes are at the corners of that box.  1e-3 of margin covers the
+        // kernel's fp32 arithmetic (MUFU ex2 / lg2: ~1e-6).
+        std::vector<double> v_hi(nf), v_lo(nf), floor_c(nc);
+        {
+            const double t_end = (double)(c.n_samples - 1) / c.f_sample_hz;
+            const double p0 = c.pwv0_a_mm, p1 = c.pwv0_a_mm + c.pwv0_b_mm_per_s * t_end;
+            auto row_of = [&](double pwv) {
+                double q = (pwv - c.lut_pwv0_mm) / c.lut_dpwv_mm;
+                if (!(q >= 0.0)) q = 0.0;
+                if (q > (double)(c.n_pwv - 1)) q = (double)(c.n_pwv - 1);
+                return q;
+            };
+            const int r0 = (int)std::floor(row_of(std::min(p0, p1) + screen_lo));
+            const int r1 = std::min(c.n_pwv - 1, (int)std::floor(row_of(std::max(p0, p1) + screen_hi)) + 1);
+            double e_lo = 1e300, e_hi = -1e300, d_lo = 1e300, d_hi = -1e300;
+            for (int64_t n = 0; n < c.n_samples; ++n) { e_lo = std::min(e_lo, c.el_rad[n]); e_hi = std::max(e_hi, c.el_rad[n]); }
+            for (int sidx = 0; sidx < ns; ++sidx) { d_lo = std::min(d_lo, c.del_rad[sidx]); d_hi = std::max(d_hi, c.del_rad[sidx]); }
+            const double E_lo = c.el0_rad + e_lo + d_lo, E_hi = c.el0_rad + e_hi + d_hi;
+            const bool el_ok = E_lo > 1e-3 && E_hi < kPi - 1e-3;
+            // csc is unimodal on (0, pi) with its minimum 1 at pi/2
+            const double csc_hi = el_ok ? std::max(1.0 / std::sin(E_lo), 1.0 / std::sin(E_hi)) * (1.0 + 1e-6) : 0.0;
+            const double csc_lo = el_ok ? ((E_lo <= 0.5 * kPi && E_hi >= 0.5 * kPi) ? 1.0 : std::min(1.0 / std::sin(E_lo), 1.0 / std::sin(E_hi)) * (1.0 - 1e-6)) : 1.0;
+            for (int i = 0; i < nf; ++i) {
+                float z_lo = 1.f, z_hi = 0.f;
+                for (int q = r0; q <= r1; ++q) { z_lo = std::min(z_lo, lut_r[(size_t)q * nfp + i]); z_hi = std::max(z_hi, lut_r[(size_t)q * nfp + i]); }
+                const double eta_hi = std::pow((double)z_hi, csc_lo), eta_lo = el_ok ? std::pow((double)z_lo, csc_hi) : 0.0;
+                const double x = Xd[i], gs_lo = Gd[i] * (double)(Gd[i] >= 0 ? cube_lo[i] : cube_hi[i]), gs_hi = Gd[i] * (double)(Gd[i] >= 0 ? cube_hi[i] : cube_lo[i]);
+                double hi = -1e300, lo = 1e300;
+                for (double eta : {eta_lo, eta_hi})
+                    for (double gs : {gs_lo, gs_hi}) { const double v = (1.0 - eta) * x + eta * gs; hi = std::max(hi, v); lo = std::min(lo, v); }
+                const double pad = 1e-3 * std::max(std::fabs(hi), std::fabs(lo));
+                v_hi[i] = (hi + pad) / kPref;
+                v_lo[i] = (lo - pad) / kPref;
+            }
+        }
+        for (int ch = 0; ch < nc; ++ch) floor_c[ch] = std::max(0.0, (double)bias[ch] / (double)p->scale);
+        const gt::TcSkipBounds sb{&v_lo, &v_hi, &floor_c};            // {v_min, v_max, floor}
+        if (gt_status s = gt::build_tc_tables(h_filt, nc, nf, nfp, a_ref, p->tc, inv, st, nullptr, &sb)) {
             return fail(nullptr, s, "tensor variant: %s", gt::tc_error());
         }
         for (int ch = 0; ch < nc; ++ch) cw[ch] = inv[ch];            // channel ch = column ch % nb_tot of channel group ch / nb_tot
@@ -1232,6 +1285,13 @@ gt_status gt_common_mode_static(gt_plan* plan, int64_t t_begin, int64_t t_count,
     gt::cm_apply_kernel<<<(unsigned)(t_count * p->n_spaxel), 128, 0, st>>>(k, tod_K_dev, scratch);
     GT_CUDA(p, cudaGetLastError());
     p->launches += 2; p->last_stream = st;
+    return GT_OK;
+}
+
+gt_status gt_debug_corrections(const gt_plan* plan, int64_t* blocks, int64_t* skipped) {
+    if (!plan || !blocks || !skipped) return GT_ERR_NULL;
+    *blocks = plan->variant == GT_VARIANT_TENSOR ? plan->tc.n_corr_blocks : 0;
+    *skipped = plan->variant == GT_VARIANT_TENSOR ? plan->tc.n_corr_skipped : 0;
     return GT_OK;
 }
 

@@ -38,6 +38,30 @@ __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_
     return make_uint4(c0, c1, c2, c3);
 }
 
+// The same with the ten round keys made by the caller (a loop that draws one block per iteration keeps them in registers
+// instead of re-deriving them every time).
+struct PhiloxKeys { uint32_t k0[10], k1[10]; };
+__device__ __forceinline__ PhiloxKeys philox_keys(uint32_t k0, uint32_t k1) {
+    PhiloxKeys K;
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        K.k0[r] = k0 + (uint32_t)r * kPhiloxW0; K.k1[r] = k1 + (uint32_t)r * kPhiloxW1;
+        asm volatile("" : "+r"(K.k0[r]), "+r"(K.k1[r]));          // opaque: not re-materialised inside the loop
+    }
+    return K;
+}
+__device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, const PhiloxKeys& K) {
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t hi0 = __umulhi(kPhiloxM0, c0), lo0 = kPhiloxM0 * c0;
+        const uint32_t hi1 = __umulhi(kPhiloxM1, c2), lo1 = kPhiloxM1 * c2;
+        const uint32_t n0 = hi1 ^ c1 ^ K.k0[r];
+        const uint32_t n2 = hi0 ^ c3 ^ K.k1[r];
+        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+    }
+    return make_uint4(c0, c1, c2, c3);
+}
+
 // W independent Philox4x32-10 blocks at once: the ten rounds of one block are a strictly serial
 // chain (~10 cycles per round), so a lone warp only fills its issue slots if it interleaves
 // several blocks.  Same arithmetic as philox4x32_10; counters differ in word 2 (the channel).

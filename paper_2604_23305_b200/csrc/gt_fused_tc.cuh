@@ -33,6 +33,7 @@
 #include <cstring>
 #include <algorithm>
 #include <cstdlib>
+#include <cstdio>
 #include <cmath>
 #include <atomic>
 #include <thread>
@@ -133,6 +134,15 @@ constexpr float kTcTruncUlp = GT_TC_TRUNC_ULP;      // overall factor on the tab
 #define GT_TC_MAX_B_STAGES 3
 #endif
 constexpr int kTcMaxBStages = GT_TC_MAX_B_STAGES;   // <= 4 (barrier slots)
+// Banded corrections (DESIGN.md section 6 "Banded corrections"): the two correction products of the split, A_lo.Fm_hi and
+// A_hi.Fm_lo, are each at most 2^-12 of the main product element by element.  For a (column group, slab) block in which every
+// channel of the group has so little of its filter that BOTH corrections of ALL skipped blocks together stay, in the worst
+// case over the spectra the plan can produce, below kTcSkipBudget of the channel's power, the MMA thread issues only
+// A_hi.Fm_hi (a third of the tensor work of that block).  0 switches the skipping off.
+#ifndef GT_TC_SKIP_BUDGET
+#define GT_TC_SKIP_BUDGET 1e-6
+#endif
+constexpr double kTcSkipBudget = GT_TC_SKIP_BUDGET;
 constexpr int kTcSmemLimit = 227 * 1024;
 
 struct TcTables {
@@ -148,6 +158,8 @@ struct TcTables {
     int32_t smem_bytes = 0;
     float* comp = nullptr;               // [group][n_seg][nb_tot] truncation compensation in ulp of the segment sum, times 2^-23
     int32_t n_seg = 0;                   // segments per tile (max over the column groups)
+    unsigned char* corr_on = nullptr;    // [group][n_kb] bit cg: A_lo.Fm_hi of column group cg is issued for this slab; bit 4 + cg: A_hi.Fm_lo
+    int64_t n_corr_blocks = 0, n_corr_skipped = 0;     // correction products per (group, column group, slab): 2 each; how many are skipped
 };
 
 // plan-time host loops over channels / samples are independent: a plain thread pool per call (plan creation is part of
@@ -193,9 +205,23 @@ inline double tc_ulp_ratio(double p) {
 // tc_ulp_ratio(accumulator after that MMA / final segment sum), in the order the MMA thread issues them.
 // filt1 != nullptr (the Eq. 17 pass): no split -- unit 0 = fp16(2^kb filt), unit 1 = fp16(2^kb filt1), one scale per
 // channel from the larger of the two maxima; one accumulation segment per tile and no compensation table (sigma needs 1e-3).
+// What the plan knows about the elements the generator can produce, for the banded corrections: per frequency the range
+// of the elements in the generator's scaled units, per channel the part of the channel's power that does not pass through
+// the contraction (the bias), in units of the contraction sum.  nullptr: no skipping.
+// Two masks per (column group, slab), each with half of kTcSkipBudget of the channel's smallest possible power:
+//   A_lo.Fm_hi: |A_lo| <= 2^-12 |element|, sign unknown: worst case 2^-12 sum |Fm| max|v| over the skipped slabs;
+//   A_hi.Fm_lo: Fm_lo is known, so the sum over the skipped slabs is bounded by |sum Fm_lo v_mid| + sum |Fm_lo| (v_rad +
+//               2^-12 max|v|) with v_mid, v_rad the centre and half width of the element's range (the signs of Fm_lo
+//               cancel as they do in the product itself).
+struct TcSkipBounds {
+    const std::vector<double>* v_min;    // [n_freq] smallest element (may be negative)
+    const std::vector<double>* v_max;    // [n_freq] largest element
+    const std::vector<double>* floor_c;  // [n_chan], >= 0
+};
+
 inline gt_status build_tc_tables(const std::vector<float>& filt, int n_chan, int n_freq, int n_freq_pad,
                                  const std::vector<double>& a_ref, TcTables& t, std::vector<float>& inv_scale,
-                                 cudaStream_t st, const std::vector<float>* filt1 = nullptr) {
+                                 cudaStream_t st, const std::vector<float>* filt1 = nullptr, const TcSkipBounds* sb = nullptr) {
     const int G = (n_chan + kTcMaxGroupChan - 1) / kTcMaxGroupChan;
     int per = (n_chan + G - 1) / G;
     // several groups: every group starts on a multiple of 128 channels, so that a finisher lane's quads of channels
@@ -234,44 +260,142 @@ inline gt_status build_tc_tables(const std::vector<float>& filt, int n_chan, int
     std::vector<float> comp((size_t)G * t.n_seg * nbt, 0.f);
     uint16_t* img16 = reinterpret_cast<uint16_t*>(img.data());
     std::atomic<int> bad{0};
+    // per (channel, 16-frequency K step): the step's share of the contraction for the reference spectrum (compensation
+    // table); per (channel, slab): the worst-case |correction| of the slab in units of its budget (banded corrections)
+    const size_t n_steps = (size_t)t.n_kb * kTcKSteps;
+    std::vector<double> part_all((size_t)G * nbt * n_steps, 0.0);
+    const bool skipping = sb != nullptr && !filt1 && kTcSkipBudget > 0.0;
+    const size_t n_cost = skipping ? (size_t)G * nbt * t.n_kb : 0;
+    std::vector<float> cost(n_cost, 0.f), flo_a(n_cost, 0.f), flo_r(n_cost, 0.f);   // in units of the channel's budget; INFINITY: no skipping
+    // ---- phase A, per channel: scale, shared-memory image, reference profile, correction bounds ----
+    host_parallel_for((int64_t)G * nbt, [&](int64_t gn) {
+        const int g = (int)(gn / nbt), n = (int)(gn % nbt);
+        const int ch = g * nbt + n;
+        if (ch >= n_chan) return;
+        double* part = part_all.data() + (size_t)gn * n_steps;
+        const float* frow = filt.data() + (size_t)ch * n_freq;
+        const float* frow1 = filt1 ? filt1->data() + (size_t)ch * n_freq : nullptr;
+        float amax = 0.f;
+        bool negative = false;
+        for (int i = 0; i < n_freq; ++i) {
+            if (!std::isfinite(frow[i]) || (frow1 && !std::isfinite(frow1[i]))) { bad = 1; return; }
+            amax = std::max(amax, std::fabs(frow[i]));
+            negative |= frow[i] < 0.f;
+            if (frow1) amax = std::max(amax, std::fabs(frow1[i]));
+        }
+        int kb_c = 0;
+        if (amax > 0.f) { int e; std::frexp(amax, &e); kb_c = std::max(-100, std::min(100, kTcBMaxLog2 - e)); }
+        inv_scale[(size_t)g * nbt + n] = std::ldexp(1.0f, -kb_c);
+        // which CTA holds row n, and where inside its unit
+        const int cg = n / kTcBufCols, col0 = cg * kTcBufCols, w = std::min(kTcBufCols, nbt - col0);
+        const int rk = kTcPair ? (n - col0) / (w / 2) : 0;
+        const int nl = kTcPair ? col0 / 2 + (n - col0) - rk * (w / 2) : n;        // local row
+        double lo_sum = 0.0;                                                     // smallest contraction sum, scaled filter
+        for (int i = 0; i < n_freq; ++i) {
+            const float f = std::ldexp(frow[i], kb_c);
+            const __half fh = __float2half_rn(f);
+            const __half fl = __float2half_rn(frow1 ? std::ldexp(frow1[i], kb_c) : f - __half2float(fh));
+            const int kb = i / kTcBK, kk = i % kTcBK;
+            // element index of (group tile, slab, unit, rank): units are laid out [g][kb][unit][rank]
+            const size_t unit0 = ((size_t)((g * t.n_kb + kb) * 2 + 0) * kRanks + rk) * (t.unit_bytes / 2);
+            const size_t unit1 = ((size_t)((g * t.n_kb + kb) * 2 + 1) * kRanks + rk) * (t.unit_bytes / 2);
+            // K-major SWIZZLE_128B row of 64 fp16: 16-byte chunk (kk / 8) XOR (row % 8)
+            const size_t off = (size_t)nl * 64 + (size_t)(((kk >> 3) ^ (nl & 7)) << 3) + (kk & 7);
+            img16[unit0 + off] = __half_as_ushort(fh);         // unit 0: Fm_hi
+            img16[unit1 + off] = __half_as_ushort(fl);         // unit 1: Fm_lo
+            part[(size_t)kb * kTcKSteps + kk / 16] += (double)f * a_ref[i];
+            if (skipping) {
+                const double vmin = (*sb->v_min)[i], vmax = (*sb->v_max)[i], vabs = std::max(std::fabs(vmin), std::fabs(vmax));
+                const double flo = (double)__half2float(fl);
+                cost[(size_t)gn * t.n_kb + kb] += (float)(std::fabs((double)f) * vabs);
+                flo_a[(size_t)gn * t.n_kb + kb] += (float)(flo * 0.5 * (vmax + vmin));
+                flo_r[(size_t)gn * t.n_kb + kb] += (float)(std::fabs(flo) * (0.5 * (vmax - vmin) + std::ldexp(vabs, -12)));
+                lo_sum += (double)f * std::max(0.0, vmin);
+            }
+        }
+        if (skipping) {
+            // the channel's power is at least floor + sum Fm max(0, v_min) (all in units of the scaled contraction sum);
+            // each of the two corrections gets half of the budget
+            const double denom = 0.5 * kTcSkipBudget * ((*sb->floor_c)[ch] * std::ldexp(1.0, kb_c) + lo_sum);
+            const bool never = negative || !(denom > 0.0) || !std::isfinite(denom);
+            for (int kb = 0; kb < t.n_kb; ++kb) {
+                const size_t k = (size_t)gn * t.n_kb + kb;
+                cost[k] = never ? INFINITY : (float)(std::ldexp((double)cost[k], -12) / denom);
+                flo_a[k] = never ? INFINITY : (float)((double)flo_a[k] / denom);
+                flo_r[k] = never ? INFINITY : (float)((double)flo_r[k] / denom);
+            }
+        }
+    });
+    if (bad) { tc_error_ref() = "the filter holds a NaN or Inf"; return GT_ERR_VALUE; }
+    // ---- phase B, per (group, column group): the slabs whose corrections are skipped.  Slabs are tried in the order of
+    //      their largest cost over the group's channels; one is taken while every channel's total stays within its budget
+    //      (1 in these units).  Bit cg of corr_on: A_lo.Fm_hi issued; bit 4 + cg: A_hi.Fm_lo issued. ----
+    std::vector<unsigned char> corr_on((size_t)G * t.n_kb, 0xFF);
+    t.n_corr_blocks = 2 * (int64_t)G * t.n_cg * t.n_kb; t.n_corr_skipped = 0;
+    if (skipping) {
+        for (int g = 0; g < G; ++g)
+            for (int cg = 0; cg < t.n_cg; ++cg) {
+                const int n0 = cg * kTcBufCols, n1 = std::min({nbt, n0 + kTcBufCols, n_chan - g * nbt});
+                if (n1 <= n0) continue;
+                auto at = [&](const std::vector<float>& a, int n, int kb) { return a[((size_t)g * nbt + n) * t.n_kb + kb]; };
+                std::vector<std::pair<float, int>> order(t.n_kb);
+                // A_lo.Fm_hi: additive worst case
+                for (int kb = 0; kb < t.n_kb; ++kb) {
+                    float m = 0.f;
+                    for (int n = n0; n < n1; ++n) m = std::max(m, at(cost, n, kb));
+                    order[kb] = {m, kb};
+                }
+                std::sort(order.begin(), order.end());
+                std::vector<double> used(n1 - n0, 0.0), sum_a(n1 - n0, 0.0);
+                for (const auto& o : order) {
+                    if (!(o.first <= 1.f)) break;
+                    bool fits = true;
+                    for (int n = n0; n < n1 && fits; ++n) fits = used[n - n0] + at(cost, n, o.second) <= 1.0;
+                    if (!fits) break;
+                    for (int n = n0; n < n1; ++n) used[n - n0] += at(cost, n, o.second);
+                    corr_on[(size_t)g * t.n_kb + o.second] &= (unsigned char)~(1u << cg);
+                    ++t.n_corr_skipped;
+                }
+                // A_hi.Fm_lo: |signed sum| + radius
+                for (int kb = 0; kb < t.n_kb; ++kb) {
+                    float m = 0.f;
+                    for (int n = n0; n < n1; ++n) m = std::max(m, std::fabs(at(flo_a, n, kb)) + at(flo_r, n, kb));
+                    order[kb] = {m, kb};
+                }
+                std::sort(order.begin(), order.end());
+                std::fill(used.begin(), used.end(), 0.0);
+                for (const auto& o : order) {
+                    if (!(o.first <= 1.f)) break;
+                    bool fits = true;
+                    for (int n = n0; n < n1 && fits; ++n)
+                        fits = std::fabs(sum_a[n - n0] + at(flo_a, n, o.second)) + used[n - n0] + at(flo_r, n, o.second) <= 1.0;
+                    if (!fits) continue;                             // a later slab may still fit (the signed sums cancel)
+                    for (int n = n0; n < n1; ++n) { sum_a[n - n0] += at(flo_a, n, o.second); used[n - n0] += at(flo_r, n, o.second); }
+                    corr_on[(size_t)g * t.n_kb + o.second] &= (unsigned char)~(16u << cg);
+                    ++t.n_corr_skipped;
+                }
+            }
+    }
+#ifdef GT_TC_DIAG
+    if (skipping && std::getenv("GATEAU_TC_PRINT_MASK")) {           // tuning builds only
+        for (int g = 0; g < G; ++g) {
+            std::fprintf(stderr, "corr_on group %d:", g);
+            for (int kb = 0; kb < t.n_kb; ++kb) std::fprintf(stderr, " %02x", corr_on[(size_t)g * t.n_kb + kb]);
+            std::fprintf(stderr, "\n");
+        }
+    }
+#endif
+    // ---- phase C, per channel: truncation compensation ----
     host_parallel_for((int64_t)G * nbt, [&](int64_t gn) {
         {
             const int g = (int)(gn / nbt), n = (int)(gn % nbt);
             const int ch = g * nbt + n;
             if (ch >= n_chan) return;
-            std::vector<double> part((size_t)t.n_kb * kTcKSteps);
-            const float* frow = filt.data() + (size_t)ch * n_freq;
-            const float* frow1 = filt1 ? filt1->data() + (size_t)ch * n_freq : nullptr;
-            float amax = 0.f;
-            for (int i = 0; i < n_freq; ++i) {
-                if (!std::isfinite(frow[i]) || (frow1 && !std::isfinite(frow1[i]))) { bad = 1; return; }
-                amax = std::max(amax, std::fabs(frow[i]));
-                if (frow1) amax = std::max(amax, std::fabs(frow1[i]));
-            }
-            int kb_c = 0;
-            if (amax > 0.f) { int e; std::frexp(amax, &e); kb_c = std::max(-100, std::min(100, kTcBMaxLog2 - e)); }
-            inv_scale[(size_t)g * nbt + n] = std::ldexp(1.0f, -kb_c);
-            // which CTA holds row n, and where inside its unit
-            const int cg = n / kTcBufCols, col0 = cg * kTcBufCols, w = std::min(kTcBufCols, nbt - col0);
-            const int rk = kTcPair ? (n - col0) / (w / 2) : 0;
-            const int nl = kTcPair ? col0 / 2 + (n - col0) - rk * (w / 2) : n;        // local row
-            std::fill(part.begin(), part.end(), 0.0);
-            for (int i = 0; i < n_freq; ++i) {
-                const float f = std::ldexp(frow[i], kb_c);
-                const __half fh = __float2half_rn(f);
-                const __half fl = __float2half_rn(frow1 ? std::ldexp(frow1[i], kb_c) : f - __half2float(fh));
-                const int kb = i / kTcBK, kk = i % kTcBK;
-                // element index of (group tile, slab, unit, rank): units are laid out [g][kb][unit][rank]
-                const size_t unit0 = ((size_t)((g * t.n_kb + kb) * 2 + 0) * kRanks + rk) * (t.unit_bytes / 2);
-                const size_t unit1 = ((size_t)((g * t.n_kb + kb) * 2 + 1) * kRanks + rk) * (t.unit_bytes / 2);
-                // K-major SWIZZLE_128B row of 64 fp16: 16-byte chunk (kk / 8) XOR (row % 8)
-                const size_t off = (size_t)nl * 64 + (size_t)(((kk >> 3) ^ (nl & 7)) << 3) + (kk & 7);
-                img16[unit0 + off] = __half_as_ushort(fh);         // unit 0: Fm_hi
-                img16[unit1 + off] = __half_as_ushort(fl);         // unit 1: Fm_lo
-                part[(size_t)kb * kTcKSteps + kk / 16] += (double)f * a_ref[i];
-            }
-            // truncation compensation: walk the MMAs of every segment in issue order.  Per slab the MMA thread issues,
-            // for k = 0..3, A_hi.Fm_hi (moves the accumulator by part[kb][k]) and A_lo.Fm_hi, then for k = 0..3 A_hi.Fm_lo.
+            const double* part = part_all.data() + (size_t)gn * n_steps;
+            const int cg = n / kTcBufCols;
+            // walk the MMAs of every segment in issue order.  Per slab the MMA thread issues,
+            // for k = 0..3, A_hi.Fm_hi (moves the accumulator by part[kb][k]) and A_lo.Fm_hi, then for k = 0..3 A_hi.Fm_lo
+            // (the two corrections only where corr_on says so).
             for (int s0 = 0, kb0 = 0; kb0 < t.n_kb; ++s0) {
                 int kb1 = kb0;
                 while (kb1 < t.n_kb && seg_of[(size_t)cg * t.n_kb + kb1] == s0) ++kb1;
@@ -286,14 +410,15 @@ inline gt_status build_tc_tables(const std::vector<float>& filt, int n_chan, int
                     auto loss_corr = [&](double x) { return 0.5 * std::min(1.0, x * std::ldexp(1.0, -12) / 1.4142 / kTcTruncGrain); };
                     double acc = 0.0;
                     for (int kb = kb0; kb < kb1; ++kb) {
+                        const bool corr_lo = (corr_on[(size_t)g * t.n_kb + kb] >> cg) & 1u, corr_flo = (corr_on[(size_t)g * t.n_kb + kb] >> (4 + cg)) & 1u;
                         for (int k = 0; k < kTcKSteps; ++k) {
                             const double pk = part[(size_t)kb * kTcKSteps + k];
                             acc += pk;
                             const double r = tc_ulp_ratio(acc / S), x = step_x(pk, std::fabs(r));
-                            W += r * (loss_main(x) + loss_corr(x));
+                            W += r * (loss_main(x) + (corr_lo ? loss_corr(x) : 0.0));
                         }
                         const double r = tc_ulp_ratio(acc / S);
-                        for (int k = 0; k < kTcKSteps; ++k) W += r * loss_corr(step_x(part[(size_t)kb * kTcKSteps + k], std::fabs(r)));
+                        if (corr_flo) for (int k = 0; k < kTcKSteps; ++k) W += r * loss_corr(step_x(part[(size_t)kb * kTcKSteps + k], std::fabs(r)));
                     }
                     // a profile that overshoots or changes sign (filters with negative lobes) is not a profile the
                     // row's own sums need follow: keep the compensation inside what a one-signed sum can lose
@@ -308,11 +433,13 @@ inline gt_status build_tc_tables(const std::vector<float>& filt, int n_chan, int
     });
     if (bad) { tc_error_ref() = "the filter holds a NaN or Inf"; return GT_ERR_VALUE; }
     if (tc_alloc_fn()(reinterpret_cast<void**>(&t.filt_img), total) != cudaSuccess ||
+        tc_alloc_fn()(reinterpret_cast<void**>(&t.corr_on), corr_on.size()) != cudaSuccess ||
         tc_alloc_fn()(reinterpret_cast<void**>(&t.comp), comp.size() * sizeof(float)) != cudaSuccess) {
         cudaGetLastError(); tc_error_ref() = "cudaMalloc of the filter image failed"; return GT_ERR_OOM;
     }
     if (cudaMemcpyAsync(t.filt_img, img.data(), total, cudaMemcpyHostToDevice, st) != cudaSuccess ||
         cudaMemcpyAsync(t.comp, comp.data(), comp.size() * sizeof(float), cudaMemcpyHostToDevice, st) != cudaSuccess ||
+        cudaMemcpyAsync(t.corr_on, corr_on.data(), corr_on.size(), cudaMemcpyHostToDevice, st) != cudaSuccess ||
         cudaStreamSynchronize(st) != cudaSuccess) {
         cudaGetLastError(); tc_error_ref() = "upload of the filter image failed"; return GT_ERR_CUDA;
     }
@@ -331,7 +458,8 @@ inline void free_tc_tables(TcTables& t) {
     if (t.filt_img) tc_free_fn()(t.filt_img);
     if (t.scratch) tc_free_fn()(t.scratch);
     if (t.comp) tc_free_fn()(t.comp);
-    t.filt_img = nullptr; t.scratch = nullptr; t.comp = nullptr;
+    if (t.corr_on) tc_free_fn()(t.corr_on);
+    t.filt_img = nullptr; t.scratch = nullptr; t.comp = nullptr; t.corr_on = nullptr;
 }
 
 struct TcParams {
@@ -339,6 +467,7 @@ struct TcParams {
     const unsigned char* filt_img;
     float* scratch;
     const float* comp;          // [group][n_seg][nb_tot] truncation compensation (build_tc_tables)
+    const unsigned char* corr_on;   // [group][n_kb] bit cg: column group cg gets A_lo.Fm_hi in this slab, bit 4 + cg: A_hi.Fm_lo (banded corrections)
     int32_t n_seg;
     int32_t n_groups, nb_tot, n_cg, seg, n_kb, unit_bytes, b_stages;
     int32_t n_row_tiles;
@@ -813,8 +942,12 @@ fused_tc_kernel(const TcParams p) {
             constexpr int kGroupDesc = (kTcBufCols * 128 >> 4) / (kTcPair ? 2 : 1);   // descriptor step between column groups (pair: half the rows)
             uint32_t a_st = 0, a_ph = 0, bs = 0, bph = 0;
             for (int64_t tl = worker; tl < n_tiles; tl += n_workers) {
+                const unsigned char* const corr_t = p.corr_on + (size_t)(tl % p.n_groups) * p.n_kb;
                 for (int kb = 0; kb < p.n_kb; ++kb, a_ph ^= (++a_st == kTcAStages), a_st = a_st == kTcAStages ? 0u : a_st) {
                     const uint32_t stage = a_st, ph = a_ph;
+                    // banded corrections: bit g = column group g gets A_lo.Fm_hi in this slab, bit 4 + g = A_hi.Fm_lo (fetched
+                    // before the waits below: an L1/L2 hit whose latency they cover)
+                    const uint32_t corr = NEP ? 0xFFu : (uint32_t)__ldg(corr_t + kb);
                     uint32_t d[kTcMaxCg];
                     // a group that has just moved to another buffer waits until the epilogue has drained it
 #pragma unroll
@@ -840,7 +973,7 @@ fused_tc_kernel(const TcParams p) {
                                     if (g < p.n_cg) {
                                         const uint64_t bd = bd0 + (uint64_t)(g * kGroupDesc + k * 2);
                                         mma_f16(d[g], ad_hi + (uint64_t)(k * 2), bd, idesc[g], (k != 0 || !(fresh >> g & 1u)) ? 1u : 0u);
-                                        if constexpr (!NEP) mma_f16(d[g], ad_lo + (uint64_t)(k * 2), bd, idesc[g], 1u);
+                                        if constexpr (!NEP) if (corr >> g & 1u) mma_f16(d[g], ad_lo + (uint64_t)(k * 2), bd, idesc[g], 1u);
                                     }
                         }
                         __syncwarp();
@@ -857,7 +990,7 @@ fused_tc_kernel(const TcParams p) {
                             for (int k = 0; k < kTcKSteps; ++k)
 #pragma unroll
                                 for (int g = 0; g < kTcMaxCg; ++g)
-                                    if (g < p.n_cg)
+                                    if (g < p.n_cg && (corr >> (4 + g) & 1u))
                                         mma_f16(d[g], (NEP ? ad_lo : ad_hi) + (uint64_t)(k * 2),
                                                         bd0 + (uint64_t)(g * kGroupDesc + k * 2), idesc[g], 1u);
                         }
@@ -978,8 +1111,7 @@ fused_tc_kernel(const TcParams p) {
     } else {
         // ============ epilogue: segment flushes of the accumulators into the scratch tile =======
         ptx::setmaxnreg_dec<kTcRegsFlush>();
-        const int q = warp;                                    // tensor-memory lane quarter
-        const int trow = 32 * q + lane;                        // tile row = tensor-memory lane
+        const int q = warp;                                    // tensor-memory lane quarter (tile row = tensor-memory lane 32 q + lane)
         TcRotation rot(p.n_cg, p.seg, p.n_kb);
         uint32_t fulls = 0u;                                   // bit b: parity of buffer b's flush count
         uint32_t ti = 0;
@@ -1089,7 +1221,7 @@ inline cudaError_t launch_fused_tc(const FusedParams& fp, const TcTables& t, int
     TcParams p{};
     p.f = fp; p.filt_img = t.filt_img;
     // FusedParams::scale carries the spectrum scale of the plan; the per-channel filter scale is chan4.w
-    p.scratch = t.scratch; p.comp = t.comp; p.n_seg = t.n_seg;
+    p.scratch = t.scratch; p.comp = t.comp; p.corr_on = t.corr_on; p.n_seg = t.n_seg;
     p.n_groups = t.n_groups; p.nb_tot = t.nb_tot; p.n_cg = t.n_cg; p.seg = t.seg > 0 ? t.seg : kTcSegDefault; p.n_kb = t.n_kb;
     p.unit_bytes = t.unit_bytes; p.b_stages = t.b_stages;
     p.n_row_tiles = (int32_t)(((fp.n_rows / fp.n_spaxel + kTcBM - 1) / kTcBM) * fp.n_spaxel);      // time-major: blocks of 128 samples x spaxels

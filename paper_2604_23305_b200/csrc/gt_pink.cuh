@@ -100,15 +100,16 @@ pink_chain_kernel(PinkParams p, int64_t t0, int64_t T, float* __restrict__ tod) 
     }
     if (valid) {
         const uint32_t s = p.spaxel_base + (uint32_t)(d / p.n_chan), c = (uint32_t)(d % p.n_chan);
+        const PhiloxKeys keys = philox_keys(p.seed_lo, p.seed_hi);      // the ten round keys, once per thread (21.6 -> 21.2 ms per C4 step)
         for (int m = 0; m < len; ++m) {
             uint32_t w[JM];
             {
-                const uint4 a = philox4x32_10((uint32_t)(t0 + m0 + m), s, c, kStreamPinkLo, p.seed_lo, p.seed_hi);
+                const uint4 a = philox4x32_10((uint32_t)(t0 + m0 + m), s, c, kStreamPinkLo, keys);
                 w[0] = a.x; w[1] = a.y; w[2] = a.z; w[3] = a.w;
             }
             if constexpr (JM > 4) {
                 if (p.J > 4) {
-                    const uint4 b = philox4x32_10((uint32_t)(t0 + m0 + m), s, c, kStreamPinkHi, p.seed_lo, p.seed_hi);
+                    const uint4 b = philox4x32_10((uint32_t)(t0 + m0 + m), s, c, kStreamPinkHi, keys);
                     w[4] = b.x; w[5] = b.y; w[6] = b.z; w[7] = b.w;
                 } else {
                     w[4] = w[5] = w[6] = w[7] = 0u;       // stages 4-7 carry zero gains and zero states

@@ -264,6 +264,41 @@ def test_narrow_channels_on_the_edges_of_accumulation_segments():
     assert np.abs(err).max() <= 0.6 * TOL_PKID, "the per-segment compensation is off: recalibrate kTcTruncUlp"
 
 
+def test_banded_corrections_skip_only_what_the_plan_can_bound():
+    """Tensor kernel, DESIGN.md section 6 "Banded corrections": the correction products A_lo.Fm_hi and A_hi.Fm_lo of a
+    (column group, slab) block are not issued where the plan bounds them -- worst case over the spectra it can produce,
+    all skipped products of a channel together -- below 1e-6 of the channel's power.  On the C4 shape (R = 500
+    Lorentzians, a quiet sky) about half of them go; with a PWV screen 40 x rougher (rows spread over several table
+    rows: a wider range of spectra) fewer; with filter rows that change sign none; parity holds in every case."""
+    w = W.make_workload("C4", n_samples=256)
+    n_kb = -(-w.n_freq // 64)
+    rows_t, rows_s = [0, 77, 131, 255], [0, 20, 41, 60]
+    counts = []
+    for rough in (1.0, 40.0):
+        scr = np.asarray(w.screen, dtype=np.float64)
+        wr = w if rough == 1.0 else w.replace(screen=(scr.mean() + rough * (scr - scr.mean())).astype(np.float32))
+        assert wr.screen.min() + wr.pwv0_a_mm > wr.lut_pwv0_mm
+        ref = O.Oracle(wr).simulate_rows(rows_t, rows_s, noise=False)
+        with _plan(wr, B.VARIANT_TENSOR) as p:
+            products, skipped = p.corrections()
+            got = p.pkid().cpu().numpy()[rows_t, rows_s]
+        assert products == 2 * 3 * n_kb                      # one channel group of three column groups, two products each
+        assert rel_err(got, ref) <= TOL_PKID
+        counts.append(skipped)
+    print("correction products skipped (quiet, rough) of", 2 * 3 * n_kb, ":", counts)
+    assert 0.35 * 6 * n_kb <= counts[0] <= 0.75 * 6 * n_kb
+    assert 0 < counts[1] < counts[0]
+    with _plan(w, B.VARIANT_FP32) as p:
+        assert p.corrections() == (0, 0)
+    # filter rows that change sign (Eq. 7): a share of the channel's power bounds nothing
+    w7 = W.random_workload(78, n_samples=40, n_spaxel=2, n_chan=64, n_freq=600)
+    fc = w7.nu_hz[40] * (1 + 1 / 120.0) ** np.arange(64)
+    F = W.filterbank_upstream_absorption(w7.nu_hz, fc, 40.0, np.where(np.arange(64) % 2 == 0, 0.3, 0.05))
+    with _plan(w7.replace(filt=F, f_center_hz=fc, dnu_eff_hz=None), B.VARIANT_TENSOR) as p:
+        products, skipped = p.corrections()
+    assert products > 0 and skipped == 0
+
+
 def test_non_finite_inputs_and_lines_of_sight_below_the_horizon_are_refused():
     w = W.random_workload(26, n_samples=20)
     bad_cube = np.array(w.cube, copy=True); bad_cube[2, 3, 7] = np.nan
