@@ -267,6 +267,15 @@ inline gt_status build_tc_tables(const std::vector<float>& filt, int n_chan, int
     const bool skipping = sb != nullptr && !filt1 && kTcSkipBudget > 0.0;
     const size_t n_cost = skipping ? (size_t)G * nbt * t.n_kb : 0;
     std::vector<float> cost(n_cost, 0.f), flo_a(n_cost, 0.f), flo_r(n_cost, 0.f);   // in units of the channel's budget; INFINITY: no skipping
+    // per frequency, for the correction bounds: max |v|, centre of the bracket, half width + 2^-12 max |v|, max(0, v_min)
+    std::vector<double> b_abs(skipping ? n_freq : 0), b_mid(b_abs.size()), b_rad(b_abs.size()), b_pos(b_abs.size());
+    for (size_t i = 0; i < b_abs.size(); ++i) {
+        const double vmin = (*sb->v_min)[i], vmax = (*sb->v_max)[i];
+        b_abs[i] = std::max(std::fabs(vmin), std::fabs(vmax));
+        b_mid[i] = 0.5 * (vmax + vmin);
+        b_rad[i] = 0.5 * (vmax - vmin) + std::ldexp(b_abs[i], -12);
+        b_pos[i] = std::max(0.0, vmin);
+    }
     // ---- phase A, per channel: scale, shared-memory image, reference profile, correction bounds ----
     host_parallel_for((int64_t)G * nbt, [&](int64_t gn) {
         const int g = (int)(gn / nbt), n = (int)(gn % nbt);
@@ -291,10 +300,11 @@ inline gt_status build_tc_tables(const std::vector<float>& filt, int n_chan, int
         const int rk = kTcPair ? (n - col0) / (w / 2) : 0;
         const int nl = kTcPair ? col0 / 2 + (n - col0) - rk * (w / 2) : n;        // local row
         double lo_sum = 0.0;                                                     // smallest contraction sum, scaled filter
+        const float two_kb = std::ldexp(1.0f, kb_c);                             // a power of two: the products below are exact
         for (int i = 0; i < n_freq; ++i) {
-            const float f = std::ldexp(frow[i], kb_c);
+            const float f = frow[i] * two_kb;
             const __half fh = __float2half_rn(f);
-            const __half fl = __float2half_rn(frow1 ? std::ldexp(frow1[i], kb_c) : f - __half2float(fh));
+            const __half fl = __float2half_rn(frow1 ? frow1[i] * two_kb : f - __half2float(fh));
             const int kb = i / kTcBK, kk = i % kTcBK;
             // element index of (group tile, slab, unit, rank): units are laid out [g][kb][unit][rank]
             const size_t unit0 = ((size_t)((g * t.n_kb + kb) * 2 + 0) * kRanks + rk) * (t.unit_bytes / 2);
@@ -305,12 +315,11 @@ inline gt_status build_tc_tables(const std::vector<float>& filt, int n_chan, int
             img16[unit1 + off] = __half_as_ushort(fl);         // unit 1: Fm_lo
             part[(size_t)kb * kTcKSteps + kk / 16] += (double)f * a_ref[i];
             if (skipping) {
-                const double vmin = (*sb->v_min)[i], vmax = (*sb->v_max)[i], vabs = std::max(std::fabs(vmin), std::fabs(vmax));
                 const double flo = (double)__half2float(fl);
-                cost[(size_t)gn * t.n_kb + kb] += (float)(std::fabs((double)f) * vabs);
-                flo_a[(size_t)gn * t.n_kb + kb] += (float)(flo * 0.5 * (vmax + vmin));
-                flo_r[(size_t)gn * t.n_kb + kb] += (float)(std::fabs(flo) * (0.5 * (vmax - vmin) + std::ldexp(vabs, -12)));
-                lo_sum += (double)f * std::max(0.0, vmin);
+                cost[(size_t)gn * t.n_kb + kb] += (float)(std::fabs((double)f) * b_abs[i]);
+                flo_a[(size_t)gn * t.n_kb + kb] += (float)(flo * b_mid[i]);
+                flo_r[(size_t)gn * t.n_kb + kb] += (float)(std::fabs(flo) * b_rad[i]);
+                lo_sum += (double)f * b_pos[i];
             }
         }
         if (skipping) {
