@@ -267,11 +267,12 @@ inline gt_status build_tc_tables(const std::vector<float>& filt, int n_chan, int
     const bool skipping = sb != nullptr && !filt1 && kTcSkipBudget > 0.0;
     const size_t n_cost = skipping ? (size_t)G * nbt * t.n_kb : 0;
     std::vector<float> cost(n_cost, 0.f), flo_a(n_cost, 0.f), flo_r(n_cost, 0.f);   // in units of the channel's budget; INFINITY: no skipping
-    // per frequency, for the correction bounds: max |v|, centre of the bracket, half width + 2^-12 max |v|, max(0, v_min)
+    // per frequency, for the correction bounds: 2^12 x the largest |A_lo| = |v - fp16(v)| (2^-12 |v| in fp16's normal range,
+    // half a subnormal step 2^-25 below it), centre of the bracket, half width + the largest |A_hi - v|, max(0, v_min)
     std::vector<double> b_abs(skipping ? n_freq : 0), b_mid(b_abs.size()), b_rad(b_abs.size()), b_pos(b_abs.size());
     for (size_t i = 0; i < b_abs.size(); ++i) {
         const double vmin = (*sb->v_min)[i], vmax = (*sb->v_max)[i];
-        b_abs[i] = std::max(std::fabs(vmin), std::fabs(vmax));
+        b_abs[i] = std::max(std::fabs(vmin), std::fabs(vmax)) + std::ldexp(1.0, -13);
         b_mid[i] = 0.5 * (vmax + vmin);
         b_rad[i] = 0.5 * (vmax - vmin) + std::ldexp(b_abs[i], -12);
         b_pos[i] = std::max(0.0, vmin);
