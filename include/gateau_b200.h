@@ -62,7 +62,9 @@ typedef struct {
 enum {
     GT_VARIANT_DEFAULT = 0,   /* tcgen05 tensor-core kernel, three-term split of the fp32 operands */
     GT_VARIANT_FP32    = 1,   /* FP32 CUDA-core kernel (the measured alternative of north_star)  */
-    GT_VARIANT_TENSOR  = 2    /* tcgen05 kernel, explicitly                                      */
+    GT_VARIANT_TENSOR  = 2,   /* tcgen05 kernel, explicitly                                      */
+    GT_VARIANT_TENSOR_FULL = 3 /* tcgen05 kernel issuing EVERY correction product of the split: no banded corrections
+                                  (DESIGN.md section 6.1).  The reference the banded kernel is tested against; ~10 % slower. */
 };
 
 typedef struct {

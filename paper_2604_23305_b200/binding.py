@@ -17,7 +17,7 @@ from . import build as _build
 GT_OK = 0
 STATUS_NAMES = {0: "GT_OK", 1: "GT_ERR_NULL", 2: "GT_ERR_SHAPE", 3: "GT_ERR_VALUE", 4: "GT_ERR_RANGE",
                 5: "GT_ERR_OOM", 6: "GT_ERR_CUDA", 7: "GT_ERR_UNSUPPORTED"}
-VARIANT_DEFAULT, VARIANT_FP32, VARIANT_TENSOR = 0, 1, 2
+VARIANT_DEFAULT, VARIANT_FP32, VARIANT_TENSOR, VARIANT_TENSOR_FULL = 0, 1, 2, 3
 
 EXPORTS = ("gt_plan_create", "gt_simulate", "gt_plan_destroy", "gt_last_error", "gt_debug_geometry",
            "gt_debug_philox", "gt_debug_pkid", "gt_launch_count", "gt_variant_name", "gt_last_fused_ms",

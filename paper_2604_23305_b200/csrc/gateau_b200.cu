@@ -148,6 +148,7 @@ struct gt_plan {
     int32_t n_freq = 0, n_freq_pad = 0, n_chan = 0, n_chan_pad = 0, n_spaxel = 0, n_pwv = 0, J = 0;
     int64_t n_samples = 0, chunk_samples = 0, chunk_dev = 0;      // samples per launch: host-output chunks / device output
     int32_t photon_noise = 0, pink_noise = 0, variant = GT_VARIANT_FP32;
+    bool tc_full = false;             // GT_VARIANT_TENSOR_FULL: every correction product of the split is issued
     int32_t spaxel_base = 0;         // global index of spaxel 0 of this plan (Philox counter word 1)
     int device = 0;
     uint64_t seed = 0;
@@ -289,7 +290,7 @@ gt_status validate(const gt_config* c) {
     }
     if (c->pink_noise && c->pink_method == 1 && (!c->pink_A || !c->pink_alpha))
         return fail(nullptr, GT_ERR_NULL, "pink noise arrays are NULL");
-    if (c->variant != GT_VARIANT_DEFAULT && c->variant != GT_VARIANT_FP32 && c->variant != GT_VARIANT_TENSOR)
+    if (c->variant != GT_VARIANT_DEFAULT && c->variant != GT_VARIANT_FP32 && c->variant != GT_VARIANT_TENSOR && c->variant != GT_VARIANT_TENSOR_FULL)
         return fail(nullptr, GT_ERR_VALUE, "unknown variant %d", c->variant);
     // LUT must cover the frequency grid (R13)
     const double r_lo = (c->nu0_hz - c->lut_nu0_hz) / c->lut_dnu_hz;
@@ -524,6 +525,7 @@ gt_status gt_plan_create(const gt_config* cfg, void* cuda_stream, gt_plan** out_
     p->n_freq = nf; p->n_freq_pad = nfp; p->n_chan = nc; p->n_spaxel = ns; p->n_pwv = c.n_pwv;
     p->n_samples = c.n_samples; p->photon_noise = c.photon_noise != 0; p->pink_noise = c.pink_noise != 0;
     p->seed = c.seed; p->cube = c.cube; p->n_az = c.n_az; p->n_el = c.n_el; p->spaxel_base = c.spaxel_index_base;
+    p->tc_full = c.variant == GT_VARIANT_TENSOR_FULL;
     p->variant = (c.variant == GT_VARIANT_FP32) ? GT_VARIANT_FP32 : GT_VARIANT_TENSOR;   // DEFAULT -> tensor: measured 8x faster than the FP32 kernel on C4
 
     // ---- statistics of the large device arrays: non-finite values are refused, the cube's per-frequency maximum
@@ -744,7 +746,7 @@ gt_status gt_plan_create(const gt_config* cfg, void* cuda_stream, gt_plan** out_
         }
         for (int ch = 0; ch < nc; ++ch) floor_c[ch] = std::max(0.0, (double)bias[ch] / (double)p->scale);
         const gt::TcSkipBounds sb{&v_lo, &v_hi, &floor_c};            // {v_min, v_max, floor}
-        if (gt_status s = gt::build_tc_tables(h_filt, nc, nf, nfp, a_ref, p->tc, inv, st, nullptr, &sb)) {
+        if (gt_status s = gt::build_tc_tables(h_filt, nc, nf, nfp, a_ref, p->tc, inv, st, nullptr, c.variant == GT_VARIANT_TENSOR_FULL ? nullptr : &sb)) {
             return fail(nullptr, s, "tensor variant: %s", gt::tc_error());
         }
         for (int ch = 0; ch < nc; ++ch) cw[ch] = inv[ch];            // channel ch = column ch % nb_tot of channel group ch / nb_tot
@@ -1136,7 +1138,7 @@ gt_status gt_debug_chunking(const gt_plan* plan, int64_t* host_chunk, int64_t* d
 
 const char* gt_variant_name(const gt_plan* plan) {
     if (!plan) return "";
-    return plan->variant == GT_VARIANT_FP32 ? "fp32-ffma" : "tcgen05-3xf16-split";
+    return plan->variant == GT_VARIANT_FP32 ? "fp32-ffma" : plan->tc_full ? "tcgen05-3xf16-split-full" : "tcgen05-3xf16-split";
 }
 
 gt_status gt_debug_kelvin_map(gt_plan* plan, double* a_out, double* b_out) {

@@ -281,13 +281,30 @@ def test_banded_corrections_skip_only_what_the_plan_can_bound():
         ref = O.Oracle(wr).simulate_rows(rows_t, rows_s, noise=False)
         with _plan(wr, B.VARIANT_TENSOR) as p:
             products, skipped = p.corrections()
-            got = p.pkid().cpu().numpy()[rows_t, rows_s]
+            banded = p.pkid()
+        with _plan(wr, B.VARIANT_TENSOR_FULL) as p:          # the same kernel issuing every correction product
+            assert p.corrections() == (products, 0) and p.variant_name.endswith("-full")
+            full = p.pkid()
         assert products == 2 * 3 * n_kb                      # one channel group of three column groups, two products each
-        assert rel_err(got, ref) <= TOL_PKID
+        assert rel_err(banded.cpu().numpy()[rows_t, rows_s], ref) <= TOL_PKID
+        # the claim itself, on every element of the window (5.4e6 values): what the skipped products were worth is inside
+        # the plan's worst-case budget (measured 4-5e-7 at most, 7e-8 rms, truncation-path differences included)
+        d = ((banded.double() - full.double()) / full.double()).abs()
+        print(f"screen x {rough:g}: {skipped} of {products} skipped, max |banded/full - 1| = {float(d.max()):.2e}")
+        assert float(d.max()) <= 1e-6
         counts.append(skipped)
-    print("correction products skipped (quiet, rough) of", 2 * 3 * n_kb, ":", counts)
     assert 0.35 * 6 * n_kb <= counts[0] <= 0.75 * 6 * n_kb
     assert 0 < counts[1] < counts[0]
+    # a source 1e3 x brighter (its spectrum dominates some rows and not others: a wide bracket per frequency)
+    wb = w.replace(cube=(np.asarray(w.cube, dtype=np.float64) * 1e3).astype(np.float32))
+    with _plan(wb, B.VARIANT_TENSOR) as p:
+        skipped_b = p.corrections()[1]
+        banded = p.pkid(0, 128)
+    with _plan(wb, B.VARIANT_TENSOR_FULL) as p:
+        full = p.pkid(0, 128)
+    d = ((banded.double() - full.double()) / full.double()).abs()
+    print(f"cube x 1e3: {skipped_b} skipped, max |banded/full - 1| = {float(d.max()):.2e}")
+    assert float(d.max()) <= 1e-6 and skipped_b <= counts[0]
     with _plan(w, B.VARIANT_FP32) as p:
         assert p.corrections() == (0, 0)
     # filter rows that change sign (Eq. 7): a share of the channel's power bounds nothing
