@@ -1,4 +1,4 @@
-// gt_fused_tc.cuh -- steps 2-6a as ONE tcgen05 tensor-core kernel (GT_VARIANT_TENSOR).
+// gt_fused_tc.cuh -- steps 2-6a as ONE tcgen05 tensor-core kernel (GT_VARIANT_TENSOR, GT_VARIANT_TENSOR_FULL).
 //
 //   P_KID[row][c] = dnu * sum_nu Fm[c][nu] * P[row][nu]                       (Eq. 16)
 // is a dense [rows x n_freq] . [n_freq x n_chan] contraction whose left operand is GENERATED
@@ -6,13 +6,19 @@
 // (one per SM) and per tile of 128 rows:
 //
 //   generator warps (16)  : 64-frequency slab of the spectrum for 128 rows -> fp16 pair (hi, lo) of the
-//                           scaled value (22 mantissa bits) -> shared memory, UMMA K-major SWIZZLE_128B
+//                           scaled value (22 mantissa bits) -> shared memory, UMMA K-major SWIZZLE_128B.
+//                           A warp works on two rows x the whole slab (a thread walks four rows), on packed
+//                           fp32 pairs (FFMA2 / FMUL2 / FADD2); the L1's LSU data pipe (the 16-byte cube taps)
+//                           sets the cycles of the kernel (profiles/r02e_fused_tc.md)
 //   loader warp (1 lane)  : filter slab images (hi, lo; pre-split, pre-swizzled at plan time; CTA pair:
 //                           this CTA's half) global -> shared by cp.async.bulk, mbarrier complete_tx
 //   MMA warp (1 lane)     : tcgen05.mma.cta_group::2.kind::f16, M = 256 per CTA pair, N <= 128 per column
 //                           group, K = 16:  acc += A_hi.B_hi + A_lo.B_hi + A_hi.B_lo  (the three-term split
 //                           of north_star with fp16 pieces: every product of two 11-bit pieces is exact in
-//                           the fp32 accumulate, the dropped A_lo.B_lo term is 2^-22 relative)
+//                           the fp32 accumulate, the dropped A_lo.B_lo term is 2^-22 relative).  BANDED
+//                           CORRECTIONS: the two correction products of a (column group, slab) block are
+//                           issued only where the plan could not bound them below 1e-6 of the channel's
+//                           power in the worst case (corr_on): 54 % fewer on C4
 //   flush warps (4)       : SEGMENTED ACCUMULATION.  The tensor core's fp32 accumulate truncates
 //                           (measured: -2.7e-5 relative after 500 chained MMAs of positive terms,
 //                           DESIGN.md "Accumulation in tensor memory"), so no accumulator lives
@@ -22,8 +28,9 @@
 //                           group moves to the spare buffer and the epilogue warps add the
 //                           finished partial sums (tcgen05.ld) into a per-CTA, L2-resident fp32
 //                           scratch tile [column][row] with round-to-nearest FADDs.  After the
-//                           last segment the finisher warps (4) transpose the scratch tile into the TOD:
-//                           P = sum*scale + bias[c], photon noise (Eq. 18-19), coalesced stores.
+//                           last segment the finisher warps (8) transpose the scratch tile into the TOD:
+//                           P = sum*scale + bias[c], photon noise (Eq. 18-19; one Philox block per four
+//                           channels, R19), coalesced stores.
 //
 // Pipelines: A ring (2 stages, generators of both CTAs -> leader's MMA thread), B ring (loader -> MMA, the
 // peer's halves relayed by a forwarder), accumulator buffers flush_full / buf_free (MMA <-> flush), scratch
