@@ -510,12 +510,16 @@ gt_status gt_plan_create(const gt_config* cfg, void* cuda_stream, gt_plan** out_
          if (e_ != cudaSuccess) return fail(nullptr, e_ == cudaErrorMemoryAllocation ? GT_ERR_OOM : GT_ERR_CUDA, \
                                             "%s: %s", #expr, cudaGetErrorString(e_)); } while (0)
     {
-        int dev = 0; cudaDeviceProp prop{};
+        // single attributes, not cudaGetDeviceProperties: that call fills every field through the driver and was measured
+        // at 14 ms and more per plan whenever something else (nvidia-smi sampling the clocks) held the driver
+        int dev = 0, sms = 0, major = 0, minor = 0;
         GT_CUDA0(cudaGetDevice(&dev));
-        GT_CUDA0(cudaGetDeviceProperties(&prop, dev));
+        GT_CUDA0(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+        GT_CUDA0(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+        GT_CUDA0(cudaDeviceGetAttribute(&minor, cudaDevAttrComputeCapabilityMinor, dev));
         p->device = dev;
-        p->num_sms = prop.multiProcessorCount;
-        if (prop.major != 10) return fail(nullptr, GT_ERR_UNSUPPORTED, "built for sm_100a, device is sm_%d%d", prop.major, prop.minor);
+        p->num_sms = sms;
+        if (major != 10) return fail(nullptr, GT_ERR_UNSUPPORTED, "built for sm_100a, device is sm_%d%d", major, minor);
     }
     GT_CUDA0(cudaStreamSynchronize(st));
     gt::tc_alloc_fn() = pool_alloc_raw; gt::tc_free_fn() = pool_free_raw;
@@ -1313,10 +1317,10 @@ gt_status gt_debug_timeline(gt_plan* plan, int32_t capacity, int32_t* n_chunks, 
 gt_status gt_measure_fp32_fma(void* cuda_stream, double* tflops_out) {
     if (!tflops_out) return fail(nullptr, GT_ERR_NULL, "gt_measure_fp32_fma: NULL argument");
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    int dev = 0; cudaDeviceProp prop{};
+    int dev = 0, sm_count = 0;
     GT_CUDA(nullptr, cudaGetDevice(&dev));
-    GT_CUDA(nullptr, cudaGetDeviceProperties(&prop, dev));
-    const int blocks = 2 * prop.multiProcessorCount, iters = 1 << 14;     // 2 CTAs of 1024 threads per SM = every resident thread slot
+    GT_CUDA(nullptr, cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev));
+    const int blocks = 2 * sm_count, iters = 1 << 14;     // 2 CTAs of 1024 threads per SM = every resident thread slot
     DevBuf<float> out;
     GT_CUDA(nullptr, out.alloc((size_t)blocks * 1024));
     cudaEvent_t e0, e1;
