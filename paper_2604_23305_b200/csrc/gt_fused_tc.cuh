@@ -309,25 +309,33 @@ inline gt_status build_tc_tables(const std::vector<float>& filt, int n_chan, int
         const int nl = kTcPair ? col0 / 2 + (n - col0) - rk * (w / 2) : n;        // local row
         double lo_sum = 0.0;                                                     // smallest contraction sum, scaled filter
         const float two_kb = std::ldexp(1.0f, kb_c);                             // a power of two: the products below are exact
-        for (int i = 0; i < n_freq; ++i) {
-            const float f = frow[i] * two_kb;
-            const __half fh = __float2half_rn(f);
-            const __half fl = __float2half_rn(frow1 ? frow1[i] * two_kb : f - __half2float(fh));
-            const int kb = i / kTcBK, kk = i % kTcBK;
-            // element index of (group tile, slab, unit, rank): units are laid out [g][kb][unit][rank]
-            const size_t unit0 = ((size_t)((g * t.n_kb + kb) * 2 + 0) * kRanks + rk) * (t.unit_bytes / 2);
-            const size_t unit1 = ((size_t)((g * t.n_kb + kb) * 2 + 1) * kRanks + rk) * (t.unit_bytes / 2);
-            // K-major SWIZZLE_128B row of 64 fp16: 16-byte chunk (kk / 8) XOR (row % 8)
-            const size_t off = (size_t)nl * 64 + (size_t)(((kk >> 3) ^ (nl & 7)) << 3) + (kk & 7);
-            img16[unit0 + off] = __half_as_ushort(fh);         // unit 0: Fm_hi
-            img16[unit1 + off] = __half_as_ushort(fl);         // unit 1: Fm_lo
-            part[(size_t)kb * kTcKSteps + kk / 16] += (double)f * a_ref[i];
+        for (int kb = 0; kb < t.n_kb; ++kb) {
+            // (group tile, slab, unit, rank): units are laid out [g][kb][unit][rank]; inside, K-major SWIZZLE_128B rows of
+            // 64 fp16: 16-byte chunk (kk / 8) XOR (row % 8)
+            uint16_t* const u0 = img16 + ((size_t)((g * t.n_kb + kb) * 2 + 0) * kRanks + rk) * (t.unit_bytes / 2) + (size_t)nl * 64;
+            uint16_t* const u1 = img16 + ((size_t)((g * t.n_kb + kb) * 2 + 1) * kRanks + rk) * (t.unit_bytes / 2) + (size_t)nl * 64;
+            const int i_lo = kb * kTcBK, i_hi = std::min(n_freq, i_lo + kTcBK);
+            double pk[kTcKSteps] = {}, c_s = 0.0, a_s = 0.0, r_s = 0.0;          // sums of this slab, in registers
+            for (int i = i_lo; i < i_hi; ++i) {
+                const int kk = i - i_lo;
+                const float f = frow[i] * two_kb;
+                const __half fh = __float2half_rn(f);
+                const __half fl = __float2half_rn(frow1 ? frow1[i] * two_kb : f - __half2float(fh));
+                const int off = (((kk >> 3) ^ (nl & 7)) << 3) + (kk & 7);
+                u0[off] = __half_as_ushort(fh);                // unit 0: Fm_hi
+                u1[off] = __half_as_ushort(fl);                // unit 1: Fm_lo
+                pk[kk >> 4] += (double)f * a_ref[i];
+                if (skipping) {
+                    const double flo = (double)__half2float(fl);
+                    c_s += std::fabs((double)f) * b_abs[i];
+                    a_s += flo * b_mid[i];
+                    r_s += std::fabs(flo) * b_rad[i];
+                    lo_sum += (double)f * b_pos[i];
+                }
+            }
+            for (int k = 0; k < kTcKSteps; ++k) part[(size_t)kb * kTcKSteps + k] = pk[k];
             if (skipping) {
-                const double flo = (double)__half2float(fl);
-                cost[(size_t)gn * t.n_kb + kb] += (float)(std::fabs((double)f) * b_abs[i]);
-                flo_a[(size_t)gn * t.n_kb + kb] += (float)(flo * b_mid[i]);
-                flo_r[(size_t)gn * t.n_kb + kb] += (float)(std::fabs(flo) * b_rad[i]);
-                lo_sum += (double)f * b_pos[i];
+                cost[(size_t)gn * t.n_kb + kb] = (float)c_s; flo_a[(size_t)gn * t.n_kb + kb] = (float)a_s; flo_r[(size_t)gn * t.n_kb + kb] = (float)r_s;
             }
         }
         if (skipping) {
