@@ -14,9 +14,6 @@
 
 namespace gt {
 
-// grid = (ceil(n_cols / 256), row blocks); thread = one column, strided over its block's rows (coalesced across the
-// warp).  |x| of a finite float orders like its bit pattern, and NaN / Inf patterns (>= 0x7F800000) order above every
-// finite value, so one atomicMax on the bits gives the maximum AND the non-finite flag.
 // order-preserving map float -> uint32 (finite values and infinities): atomicMin / atomicMax on the keys give min / max
 __host__ __device__ __forceinline__ uint32_t float_key(float v) {
 #ifdef __CUDA_ARCH__
@@ -35,7 +32,10 @@ __host__ __device__ __forceinline__ float key_float(uint32_t k) {
 #endif
 }
 
-// min_key must be initialised to 0xFFFFFFFF and max_key to 0 (both may be nullptr)
+// grid = (ceil(n_cols / 256), row blocks); thread = one column, strided over its block's rows (coalesced across the
+// warp).  |x| of a finite float orders like its bit pattern, and NaN / Inf patterns (>= 0x7F800000) order above every
+// finite value, so one atomicMax on the bits gives the maximum AND the non-finite flag.
+// min_key must be initialised to 0xFFFFFFFF and max_key to 0 (both may be nullptr).
 __global__ void __launch_bounds__(256)
 colstat_kernel(const float* __restrict__ a, int64_t n_rows, int32_t n_cols, uint32_t* __restrict__ absmax_bits,
                double* __restrict__ sum, uint32_t* __restrict__ min_key = nullptr, uint32_t* __restrict__ max_key = nullptr) {
