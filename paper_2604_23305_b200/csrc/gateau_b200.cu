@@ -511,7 +511,7 @@ gt_status gt_plan_create(const gt_config* cfg, void* cuda_stream, gt_plan** out_
                                             "%s: %s", #expr, cudaGetErrorString(e_)); } while (0)
     {
         // single attributes, not cudaGetDeviceProperties: that call fills every field through the driver and was measured
-        // at 14 ms and more per plan whenever something else (nvidia-smi sampling the clocks) held the driver
+        // at ~2 ms per plan normally and, intermittently, at 14 ms and more (outliers of 50-100 ms in the end-to-end leg)
         int dev = 0, sms = 0, major = 0, minor = 0;
         GT_CUDA0(cudaGetDevice(&dev));
         GT_CUDA0(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
