@@ -316,6 +316,26 @@ def test_banded_corrections_skip_only_what_the_plan_can_bound():
     assert products > 0 and skipped == 0
 
 
+@pytest.mark.parametrize("n_chan,n_freq,R,drift,gain", [(420, 1920, 500.0, 2.0, 0.0), (420, 4000, 150.0, 2.0, 1.0),
+                                                       (347, 4000, 500.0, 2.0, 1.0), (130, 1920, 2000.0, 0.05, 1e3)])
+def test_banded_corrections_stay_inside_their_budget_on_random_inputs(n_chan, n_freq, R, drift, gain):
+    """Random cascades, screens and cubes with Lorentzian filterbanks (two channel groups included, PWV drifting through
+    the whole table, a source 1e3 x brighter): the banded kernel against the one that issues every product, every element."""
+    w = W.random_workload(1003, n_samples=96, n_spaxel=3, n_chan=n_chan, n_freq=n_freq)
+    fc = np.linspace(w.nu_hz[8], w.nu_hz[-8], n_chan)
+    w = w.replace(filt=W.lorentzian_filterbank(w.nu_hz, fc, R, 0.3), f_center_hz=fc, dnu_eff_hz=None,
+                  pwv0_a_mm=0.2, pwv0_b_mm_per_s=drift, cube=(w.cube.astype(np.float64) * gain).astype(np.float32))
+    with _plan(w, B.VARIANT_TENSOR) as p:
+        products, skipped = p.corrections()
+        banded = p.pkid().double()
+    with _plan(w, B.VARIANT_TENSOR_FULL) as p:
+        full = p.pkid().double()
+    assert skipped > 0
+    assert float(((banded - full) / full).abs().max()) <= 1e-6
+    ref = O.Oracle(w).simulate(want=("pkid",))["pkid"]
+    assert rel_err(banded.cpu().numpy(), ref) <= TOL_PKID
+
+
 def test_non_finite_inputs_and_lines_of_sight_below_the_horizon_are_refused():
     w = W.random_workload(26, n_samples=20)
     bad_cube = np.array(w.cube, copy=True); bad_cube[2, 3, 7] = np.nan
