@@ -196,7 +196,8 @@ struct gt_plan {
     std::vector<float> h_lut;  int32_t n_nu_lut = 0;
     double lut_nu0 = 0, lut_dnu = 0, lut_pwv0 = 0, lut_dpwv = 0;
     std::vector<double> h_daz, h_del, h_fc;
-    DevBuf<double> d_ln_eta_z;  DevBuf<float> d_cm_weight;
+    DevBuf<double> d_ln_eta_z;  DevBuf<float> d_cm_weight;      // common mode: [4][n_chan] le, eta0, 1 - eta0, 1 / eta0; [n_spaxel] S_j
+    double cm_csc0 = 1.0;                                      // reference airmass of the common-mode kernels (boresight)
     // diagnostics (SURVEY section 5 "Metrics"): rows seen by the geometry kernel, rows outside the cube, PWV clamps
     DevBuf<unsigned long long> d_counters;   // [3] outside cube, PWV below / above the LUT
     int64_t rows_done = 0;
@@ -796,7 +797,8 @@ gt_status gt_plan_create(const gt_config* cfg, void* cuda_stream, gt_plan** out_
     p->lut_pwv0 = c.lut_pwv0_mm; p->lut_dpwv = c.lut_dpwv_mm;
     p->h_daz.assign(c.daz_rad, c.daz_rad + ns); p->h_del.assign(c.del_rad, c.del_rad + ns);
     p->h_fc.assign(c.f_center_hz, c.f_center_hz + nc);
-    GT_CUDA0(p->d_ln_eta_z.alloc((size_t)nc)); GT_CUDA0(p->d_cm_weight.alloc((size_t)ns));
+    GT_CUDA0(p->d_ln_eta_z.alloc((size_t)4 * nc)); GT_CUDA0(p->d_cm_weight.alloc((size_t)ns));
+    { const double s0 = std::sin(c.el0_rad); p->cm_csc0 = s0 > 1e-3 ? 1.0 / s0 : 1.0; }
     GT_CUDA0(cm_static_resolve(p->device));     // device address of the static scratch of gt_common_mode_static
     GT_CUDA0(p->d_counters.alloc(3));
     GT_CUDA0(cudaMemsetAsync(p->d_counters.p, 0, 3 * sizeof(unsigned long long), st));
@@ -1184,9 +1186,12 @@ gt_status cm_setup(gt_plan* p, double pwv_mean_mm, double r_out_rad, gt::CmParam
     for (int s = 0; s < p->n_spaxel; ++s) { w[s] = std::hypot(p->h_daz[s], p->h_del[s]) > r_out_rad ? 1.f : 0.f; n += w[s] != 0.f; }
     GT_CUDA(p, cudaMemcpyAsync(p->d_ln_eta_z.p, le.data(), le.size() * sizeof(double), cudaMemcpyHostToDevice, st));
     GT_CUDA(p, cudaMemcpyAsync(p->d_cm_weight.p, w.data(), w.size() * sizeof(float), cudaMemcpyHostToDevice, st));
+    gt::cm_ref_kernel<<<(unsigned)((p->n_chan + 127) / 128), 128, 0, st>>>(p->d_ln_eta_z.p, p->n_chan, p->cm_csc0);   // eta0, 1 - eta0 at the reference airmass
+    GT_CUDA(p, cudaGetLastError());
     GT_CUDA(p, cudaStreamSynchronize(st));                 // the host vectors go out of scope
     k.sinE = p->d_sinE.p; k.cosE = p->d_cosE.p; k.sin_del = p->d_sp.p + 2 * p->n_spaxel; k.cos_del = p->d_sp.p + 3 * p->n_spaxel;
     k.ln_eta_z = p->d_ln_eta_z.p; k.weight = p->d_cm_weight.p; k.n_spaxel = p->n_spaxel; k.n_chan = p->n_chan;
+    k.csc0 = p->cm_csc0;
     if (n_out) *n_out = n;
     return GT_OK;
 }
@@ -1201,9 +1206,9 @@ gt_status gt_common_mode_partial(gt_plan* plan, int64_t t_begin, int64_t t_count
     if (gt_status s = cm_setup(plan, pwv_mean_mm, r_out_rad, k, n_out, st)) return s;
     if (t_count == 0) return GT_OK;
     k.t0 = t_begin; k.T = t_count;
-    gt::cm_partial_kernel<<<(unsigned)t_count, 128, 0, st>>>(k, tod_K_dev, partial_dev);
+    gt::cm_partial_kernel<<<(unsigned)t_count, 128, gt::cm_smem_bytes(plan->n_spaxel), st>>>(k, tod_K_dev, partial_dev);
     GT_CUDA(plan, cudaGetLastError());
-    plan->launches++; plan->last_stream = st;
+    plan->launches += 2; plan->last_stream = st;          // cm_ref_kernel (cm_setup) + this pass
     return GT_OK;
 }
 
@@ -1217,10 +1222,10 @@ gt_status gt_common_mode_apply(gt_plan* plan, int64_t t_begin, int64_t t_count, 
     if (gt_status s = cm_setup(plan, pwv_mean_mm, 0.0, k, nullptr, st)) return s;
     if (t_count == 0) return GT_OK;
     k.t0 = t_begin; k.T = t_count; k.inv_n_out = 1.0 / (double)n_out_total;
-    if (t_count * plan->n_spaxel > 0x7fffffffLL) return fail(plan, GT_ERR_SHAPE, "common mode: more than 2^31 rows in one call");
-    gt::cm_apply_kernel<<<(unsigned)(t_count * plan->n_spaxel), 128, 0, st>>>(k, tod_K_dev, sum_dev);
+    if (t_count > 0x7fffffffLL) return fail(plan, GT_ERR_SHAPE, "common mode: more than 2^31 samples in one call");
+    gt::cm_apply_kernel<<<(unsigned)t_count, 128, gt::cm_smem_bytes(plan->n_spaxel), st>>>(k, tod_K_dev, sum_dev);
     GT_CUDA(plan, cudaGetLastError());
-    plan->launches++; plan->last_stream = st;
+    plan->launches += 2; plan->last_stream = st;          // cm_ref_kernel (cm_setup) + this pass
     return GT_OK;
 }
 
@@ -1279,18 +1284,20 @@ gt_status gt_common_mode_static(gt_plan* plan, int64_t t_begin, int64_t t_count,
     if (t_count == 0) return GT_OK;
     GT_CUDA(p, cudaMemcpyAsync(p->d_ln_eta_z.p, le, (size_t)p->n_chan * sizeof(double), cudaMemcpyHostToDevice, st));
     GT_CUDA(p, cudaMemcpyAsync(p->d_cm_weight.p, w, (size_t)p->n_spaxel * sizeof(float), cudaMemcpyHostToDevice, st));
+    gt::cm_ref_kernel<<<(unsigned)((p->n_chan + 127) / 128), 128, 0, st>>>(p->d_ln_eta_z.p, p->n_chan, p->cm_csc0);   // eta0, 1 - eta0 at the reference airmass
+    GT_CUDA(p, cudaGetLastError());
     GT_CUDA(p, cudaStreamSynchronize(st));                 // the stack arrays go out of scope
     gt::CmParams k{};
     k.sinE = p->d_sinE.p; k.cosE = p->d_cosE.p; k.sin_del = p->d_sp.p + 2 * p->n_spaxel; k.cos_del = p->d_sp.p + 3 * p->n_spaxel;
     k.ln_eta_z = p->d_ln_eta_z.p; k.weight = p->d_cm_weight.p; k.n_spaxel = p->n_spaxel; k.n_chan = p->n_chan;
-    k.t0 = t_begin; k.T = t_count; k.inv_n_out = 1.0 / (double)n;
+    k.t0 = t_begin; k.T = t_count; k.inv_n_out = 1.0 / (double)n; k.csc0 = p->cm_csc0;
     // cm_partial_kernel overwrites every element [0, t_count * n_chan) it later reads: nothing in the shared array has to
     // start at zero, and what the previous call left behind is never read
-    gt::cm_partial_kernel<<<(unsigned)t_count, 128, 0, st>>>(k, tod_K_dev, scratch);
+    gt::cm_partial_kernel<<<(unsigned)t_count, 128, gt::cm_smem_bytes(p->n_spaxel), st>>>(k, tod_K_dev, scratch);
     GT_CUDA(p, cudaGetLastError());
-    gt::cm_apply_kernel<<<(unsigned)(t_count * p->n_spaxel), 128, 0, st>>>(k, tod_K_dev, scratch);
+    gt::cm_apply_kernel<<<(unsigned)t_count, 128, gt::cm_smem_bytes(p->n_spaxel), st>>>(k, tod_K_dev, scratch);
     GT_CUDA(p, cudaGetLastError());
-    p->launches += 2; p->last_stream = st;
+    p->launches += 3; p->last_stream = st;
     return GT_OK;
 }
 

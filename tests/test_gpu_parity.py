@@ -958,6 +958,34 @@ def test_common_mode_subtraction_sharded_and_single_plan_against_the_oracle():
         assert e.value.status == 3
 
 
+def test_common_mode_subtraction_over_a_wide_elevation_range():
+    """The common-mode kernels form eta = eta_z^csc from its value at the boresight airmass and a short fp32 polynomial
+    in x = (csc - csc0) ln eta_z, with the library functions beyond |x| = 0.05 (csrc/gt_common_mode.cuh).  A scan over
+    +-9 degrees of elevation puts |x| on both sides of that switch (0 ... 0.3); same oracle, same 3e-7."""
+    w = W.random_workload(122, n_samples=200, n_spaxel=5, n_chan=33, n_freq=80, photon_noise=True)
+    w = w.replace(output_unit=1, skydip_n=10, skydip_pwv_lo_mm=0.6, skydip_pwv_hi_mm=1.7,
+                  el_rad=np.linspace(-0.16, 0.16, 200))
+    r_out = 8 * np.pi / 180 / 3600
+    o = O.Oracle(w)
+    with B.Plan(w) as p:
+        tod, pwv = p.simulate(want_pwv=True)
+        pwv_mean = float(pwv.double().mean().item())
+        partial, n_out = p.common_mode_partial(tod, pwv_mean, r_out)
+        got = p.common_mode_apply(tod.clone(), pwv_mean, partial, n_out).cpu().numpy().astype(np.float64)
+        got_static, n_static = p.common_mode_static(tod.clone(), pwv_mean, r_out)
+        tod_np = tod.cpu().numpy()
+    eta_z = O.eta_zenith_at(w, w.f_center_hz, pwv_mean)
+    csc = o.geometry()["csc"]
+    x = (csc - 1.0 / np.sin(w.el0_rad))[:, :, None] * np.log(eta_z)[None, None, :]
+    assert np.abs(x).min() < 1e-3 and (np.abs(x) > 0.05).mean() > 0.2 and (np.abs(x) < 0.05).mean() > 0.2
+    ref, S, common = O.common_mode_subtract(tod_np.astype(np.float64), eta_z, csc, w.daz_rad, w.del_rad, r_out)
+    assert 0 < S.sum() and n_out == int(S.sum()) == n_static
+    scale = np.max(np.abs(tod_np / (eta_z[None, None, :] ** csc[:, :, None])))
+    assert np.max(np.abs(partial.cpu().numpy() - common)) <= 3e-7 * np.max(np.abs(common))
+    assert np.max(np.abs(got - ref)) <= 3e-7 * scale
+    assert np.array_equal(got_static.cpu().numpy(), got.astype(np.float32))
+
+
 def test_measurement_hooks_and_plan_pool():
     """gt_debug_timeline (per-chunk compute / copy events of a host-output call: every copy starts after its chunk's
     kernels and ends after it started), gt_measure_fp32_fma (tens of TFLOP/s on a B200), gt_release_cached_memory
