@@ -379,8 +379,13 @@ gt_status run_chunk(gt_plan* p, int64_t t0, int64_t T, float* dst, float* pwv_ds
     p->launches++;
     p->n_fused_last = fused_slot + 1;
 
+    // brightness-temperature output (the gt_simulate path; gt_debug_pkid stays in W): the map T = a_c + b_c (total of Eq. 21)
+    // rides on the last kernel that writes the TOD -- the pink-noise kernels -- and is a pass of its own only without them
+    const bool kelvin = noise && p->output_unit == 1;
+    bool kelvin_done = false;
     if (noise && p->pink_noise && p->pink_method == 1) {
         dim3 grid((unsigned)((T + 31) / 32), (unsigned)((p->tk.n_det + 31) / 32));
+        p->tk.kelvin_ab = kelvin ? p->d_kelvin_abf.p : nullptr; kelvin_done = kelvin;
         gt::tk_add_kernel<<<grid, 256, 0, st>>>(p->tk, t0, T, dst);
         GT_CUDA(p, cudaGetLastError());
         p->launches += 1;
@@ -394,6 +399,7 @@ gt_status run_chunk(gt_plan* p, int64_t t0, int64_t T, float* dst, float* pwv_ds
         if (n_flags > p->d_pink_sync.n) GT_CUDA(p, p->d_pink_sync.alloc(n_flags));
         GT_CUDA(p, cudaMemsetAsync(p->d_pink_sync.p, 0, n_flags * sizeof(uint32_t), st));
         p->pink.flags = p->d_pink_sync.p + 1; p->pink.ticket = p->d_pink_sync.p;
+        p->pink.kelvin_ab = kelvin ? p->d_kelvin_abf.p : nullptr; kelvin_done = kelvin;
         const size_t smem = (size_t)gt::kPinkSeg * 256 * sizeof(float);
         GT_CUDA(p, cudaFuncSetAttribute(gt::pink_chain_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         GT_CUDA(p, cudaFuncSetAttribute(gt::pink_chain_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -402,7 +408,7 @@ gt_status run_chunk(gt_plan* p, int64_t t0, int64_t T, float* dst, float* pwv_ds
         GT_CUDA(p, cudaGetLastError());
         p->launches += 1;
     }
-    if (noise && p->output_unit == 1) {          // the gt_simulate path; gt_debug_pkid stays in W
+    if (kelvin && !kelvin_done) {
         const int64_t n_span = (n_rows + gt::kKelvinRows - 1) / gt::kKelvinRows;
         gt::kelvin_kernel<<<(unsigned)std::min<int64_t>(n_span, 16 * p->num_sms), 256, 0, st>>>(dst, n_rows, p->n_chan, p->d_kelvin_abf.p);
         GT_CUDA(p, cudaGetLastError());

@@ -32,6 +32,8 @@ struct PinkParams {
     uint32_t* ticket;              // block ticket counter; zeroed before every launch
     uint32_t seed_lo, seed_hi;
     uint32_t spaxel_base;          // global index of the plan's spaxel 0 (Philox counter word 1)
+    const float2* kelvin_ab;       // [n_chan] (a, b) of the brightness-temperature map T = a + b P, applied to the total of
+                                   // Eq. 21 in the same write (nullptr: output in W, or applied elsewhere)
 };
 
 __device__ __forceinline__ void pink_normals(const PinkParams& p, uint32_t c0, uint32_t s, uint32_t c,
@@ -172,6 +174,7 @@ pink_chain_kernel(PinkParams p, int64_t t0, int64_t T, float* __restrict__ tod) 
 #pragma unroll
         for (int i = 0; i < JM / 2; ++i) a2[i] = mul2(g2[i], pk2(cin[2 * i], cin[2 * i + 1]));
         float* col = tod + m0 * p.n_det + d;
+        const float2 kab = p.kelvin_ab ? __ldg(p.kelvin_ab + d % p.n_chan) : make_float2(0.f, 1.f);
         for (int mb = 0; mb < len; mb += kPinkBatch) {
             float cur[kPinkBatch];
 #pragma unroll
@@ -184,7 +187,8 @@ pink_chain_kernel(PinkParams p, int64_t t0, int64_t T, float* __restrict__ tod) 
 #pragma unroll
                     for (int i = 0; i < JM / 2; ++i) { a2[i] = mul2(a2[i], phi2[i]); add2v = add2(add2v, a2[i]); }
                     const float2 add = upk2(add2v);
-                    col[(int64_t)m * p.n_det] = cur[b] + (s_pn[m * 256 + tid] + (add.x + add.y));
+                    const float total = cur[b] + (s_pn[m * 256 + tid] + (add.x + add.y));
+                    col[(int64_t)m * p.n_det] = p.kelvin_ab ? fmaf(kab.y, total, kab.x) : total;
                 }
             }
         }

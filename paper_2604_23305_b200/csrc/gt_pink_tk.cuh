@@ -25,6 +25,7 @@ struct TkParams {
     int64_t ld;
     uint32_t seed_lo, seed_hi;
     uint32_t spaxel_base;    // global index of the plan's spaxel 0 (Philox counter word 1)
+    const float2* kelvin_ab; // [n_chan] (a, b) of T = a + b P, applied to the total in tk_add_kernel's write (nullptr: none)
 };
 
 // thread = (detector, frequency index k), k fastest
@@ -62,7 +63,11 @@ __global__ void __launch_bounds__(256) tk_add_kernel(TkParams p, int64_t t0, int
 #pragma unroll
     for (int i = 0; i < 32; i += 8) {
         const int64_t t = tb + ty + i, d = db + tx;
-        if (d < p.n_det && t < T) tod[t * p.n_det + d] += tile[tx][ty + i];
+        if (d < p.n_det && t < T) {
+            const float total = tod[t * p.n_det + d] + tile[tx][ty + i];
+            if (p.kelvin_ab) { const float2 ab = __ldg(p.kelvin_ab + d % p.n_chan); tod[t * p.n_det + d] = fmaf(ab.y, total, ab.x); }
+            else tod[t * p.n_det + d] = total;
+        }
     }
 }
 
