@@ -39,12 +39,13 @@ __device__ __forceinline__ double cm_csc(const CmParams& p, int64_t t, int s) {
 // eta = exp(csc le) and 1 - eta = -expm1(csc le) to double accuracy, from the per-channel values at the reference airmass:
 //   eta = eta0 (1 + u),  1 - eta = om0 - eta0 u,  1 / eta = (1 + w) / eta0,   u = expm1(x),  w = expm1(-x),  x = (csc - csc0) le.
 // Over a scan the airmass moves by 1e-3 or so of csc0, so |x| << 1 and u, w are SMALL CORRECTIONS: they are evaluated in
-// fp32 (Taylor polynomial of degree 6, x^7 / 5040 < 2e-13 for |x| <= 0.05; the fp32 rounding of u, 6e-8 |x|, is below 3e-9 of
-// eta) and only folded into the double values eta0, om0 = -expm1(csc0 le) (no cancellation) and 1 / eta0 with one DFMA each.
+// fp32 (Taylor polynomial of degree 4: x^5 / 120 < 2.6e-9 for |x| <= 0.05 and 3e-16 for the |x| ~ 1e-3 of a scan; the fp32
+// rounding of u, 6e-8 |x|, is below 3e-9 of eta) and only folded into the double values eta0, om0 = -expm1(csc0 le) (no
+// cancellation) and 1 / eta0 with one DFMA each.
 // Beyond |x| = 0.05 the library functions in double.  The double-precision exp, expm1 and divisions per element were what
 // bound these kernels (15 ms each per C4 step: FP64 is a narrow pipe on this GPU).
 __device__ __forceinline__ float cm_expm1_small(float x) {
-    return x * fmaf(x, fmaf(x, fmaf(x, fmaf(x, fmaf(x, 1.0f / 720, 1.0f / 120), 1.0f / 24), 1.0f / 6), 0.5f), 1.0f);
+    return x * fmaf(x, fmaf(x, fmaf(x, 1.0f / 24, 1.0f / 6), 0.5f), 1.0f);
 }
 // 1 / d for d in the normal fp32 range: fp32 reciprocal (2^-23) and one Newton step in double (2^-46)
 __device__ __forceinline__ double cm_rcp(double d) {
