@@ -449,6 +449,22 @@ def run_extras(torch, B, w, local, tod):
         e1.record(); e1.synchronize()
         ms = e0.elapsed_time(e1) / 2
         out[name] = {"ms_per_step": ms, "value": w.detector_samples() / (ms * 1e-3), "unit": UNIT, "plan_create_ms": create_ms}
+        if name == "f2_kelvin_output" and w.n_spaxel > 1:
+            # row f4 on one GPU: the same Kelvin step followed by the common-mode subtraction of Eq. 25-26 (partial sums over
+            # the spaxels outside 0.6 of the array radius, then the apply pass); bench.py --shard spaxel is the N > 1 form
+            r_out = 0.6 * float(np.max(np.hypot(w.daz_rad, w.del_rad)))
+
+            def cm_step():
+                p.simulate(out=tod)
+                partial, n_out = p.common_mode_partial(tod, 1.0, r_out)
+                p.common_mode_apply(tod, 1.0, partial, n_out)
+            cm_step()
+            e0.record()
+            for _ in range(2):
+                cm_step()
+            e1.record(); e1.synchronize()
+            ms4 = e0.elapsed_time(e1) / 2
+            out["f4_kelvin_common_mode"] = {"ms_per_step": ms4, "value": w.detector_samples() / (ms4 * 1e-3), "unit": UNIT}
         p.destroy()
         torch.cuda.empty_cache()
     return out
