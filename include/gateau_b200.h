@@ -96,7 +96,9 @@ typedef struct {
     int32_t n_chan;  const float* filt;
     const double* f_center_hz;    /* HOST [n_chan] channel centre (photon noise h nu)            */
     const double* dnu_eff_hz;     /* HOST [n_chan] effective bandwidth, NULL => derived from filt */
-    /* noise: Philox4x32-10 keyed by seed, counter (n, spaxel, chan, stream) (R19) */
+    /* noise: Philox4x32-10 keyed by seed, counter (n, spaxel, chan, stream) (R19).  Photon noise (stream 0)
+       uses all four normals of a block: channel c takes normal (c / 32) % 4 of the block with counter word 2 =
+       32 (c / 128) + c % 32; pink noise (streams 1, 2) takes the four normals of block (n, spaxel, c) for its four stages */
     uint64_t seed;  int32_t photon_noise, pink_noise;
     const double *pink_A, *pink_alpha;     /* HOST [n_spaxel*n_chan] PSD level A and slope alpha */
     int32_t pink_n_stage;  const double* pink_f_corner_hz;   /* HOST [J] corner frequencies, J <= 8 */
